@@ -1,0 +1,139 @@
+/*
+ * zippel.h -- C-ABI of libzippel.so: one Zippel lifting step k-1 -> k variables over Z/pZ on a
+ * B200 (sm_100a).  Method: arXiv 2505.24256, "GPU Implementation of Zippel Method for Feynman
+ * Integral Reconstruction" (PAPER.md below = /root/reference/PAPER.md; Gn = readings in DESIGN.md).
+ *
+ * Conventions for every entry point
+ *   - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every
+ *     buffer; the library allocates nothing and keeps no state between calls.  Scratch comes from
+ *     the caller's `workspace` (device, 256-byte aligned, zippel_workspace_bytes() bytes).
+ *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *   - Residues are canonical, in [0, p); p is an odd prime, 3 <= p < 2^63 (primality is the caller's
+ *     contract; reading G14, G22).
+ *   - Batch layout: F functions, function f owns the terms [h_offsets[f], h_offsets[f+1]);
+ *     T_tot = h_offsets[F].  A "[B x T_tot]" array holds row b at x + b*T_tot; inside a row the
+ *     entries of function f start at h_offsets[f].
+ *   - Return value: ZP_OK, or an error found on the host before anything was enqueued.
+ *     Data-dependent failures are written to status[f] (device int32): 0 = ok, else
+ *     (index << 8) | code with the smallest offending index.  Outputs of a failed function are
+ *     unspecified; the other functions of the batch are unaffected.  No exceptions, no printing.
+ *   - There is no CPU fallback: without a CUDA device every call returns ZP_ERR_CUDA.
+ */
+#ifndef ZIPPEL_H
+#define ZIPPEL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* host return codes */
+#define ZP_OK 0
+#define ZP_ERR_ARG 1       /* null pointer, size <= 0, p even / < 3 / >= 2^63, nv > ZP_MAX_NV, B > ZP_MAX_B */
+#define ZP_ERR_WORKSPACE 2 /* workspace too small or misaligned */
+#define ZP_ERR_CUDA 3      /* launch / configuration error, or no device */
+
+/* per-function status codes (low byte of status[f]) */
+#define ZP_ST_DUPLICATE_NODE 16   /* den_i == 0: two terms map to one node (G24); or m_i == 0 with s0 = 1 (G25) */
+#define ZP_ST_DUPLICATE_SAMPLE 17 /* c_j == c_j' for some j' < j in Newton (index = j) */
+#define ZP_ST_ZERO_PIVOT 18       /* u_{0,s} == 0 in balancing (index = s) */
+
+#define ZP_MAX_NV 32 /* skeleton variables */
+#define ZP_MAX_B 64  /* sample values of x_k (D + 1) */
+
+/* basis of the Newton output */
+#define ZP_BASIS_NEWTON 0   /* a_0..a_D of eq. (1): f = a_0 + (x-c_0)[a_1 + (x-c_1)[a_2 + ...]]  (0-based, G16) */
+#define ZP_BASIS_MONOMIAL 1 /* coefficients of x_k^0..x_k^D */
+
+const char* zippel_strerror(int code);
+
+/* Scratch needed by an entry point for a batch with these term offsets and B sample values.
+ * h_offsets: host [F+1].  flags: ZP_WS_BALANCED adds the [B x T_tot] balanced-value buffer that
+ * balanced_zippel_lift_step needs (pass the larger part's offsets).  Returns 0 on bad arguments. */
+#define ZP_WS_BALANCED 1
+size_t zippel_workspace_bytes(const int64_t* h_offsets, int F, int B, int flags);
+
+/* (a1) Nodes, eq. (3) and L60 (G1, G2): the s-th Zippel probe is (y_1^s .. y_nv^s), so
+ * skeleton term i takes the value m_i^s there, with  m_i = prod_j y_j^{e_ij} mod p.
+ *   exps    [T_tot x nv] row-major uint16 exponents e_ij
+ *   anchors [nv] y_j
+ *   nodes   out [T_tot] m_i */
+int zippel_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t* anchors, uint64_t p,
+                      uint64_t* nodes, void* stream);
+
+/* (a2)-(a4) Batched transposed Vandermonde solve, PAPER.md L60 and section 2.2:
+ * for every function f and every right-hand side b find c with
+ *     sum_i c_{b,i} m_i^(s+s0) = v_{b,s},  s = 0 .. t_f-1,
+ * by the master polynomial M(z) = prod_i (z - m_i), per-node synthetic division
+ * Q_i = M/(z - m_i) (Horner), c_{b,i} = (sum_s q_{i,s} v_{b,s}) / Q_i(m_i) [/ m_i if s0 = 1] (G15).
+ *   nodes  [T_tot]; vals [B x T_tot]; coefs out [B x T_tot] (may alias vals: NO);
+ *   s0     first power, 0 or 1 (G1);  status out [F]. */
+int vandermonde_solve_batch(const uint64_t* nodes, const int64_t* h_offsets, int F, const uint64_t* vals, int B,
+                            int s0, uint64_t p, uint64_t* coefs, int32_t* status, void* workspace,
+                            size_t workspace_bytes, void* stream);
+
+/* (a5) Batched Newton interpolation in x_k, eq. (1), one lane per coefficient:
+ * column i of vals holds the values of coefficient i at samples c_0..c_D (row j at vals + j*ld);
+ * column i of out receives its B coefficients in `basis` (row d at out + d*ld).  out may alias vals.
+ * The samples are never reordered (G16).  status out [1]. */
+int newton_interp_batch(const uint64_t* samples, int B, const uint64_t* vals, int64_t n, int64_t ld, uint64_t p,
+                        int basis, uint64_t* out, int32_t* status, void* workspace, size_t workspace_bytes,
+                        void* stream);
+
+/* One lifting step = (a1) + (a2)-(a4) + (a5), section 1 L47-60.
+ *   vals [B x T_tot] probe values f(y^(s+s0), c_j): row j, function f, entry s;
+ *   out  [B x T_tot] row d = coefficient d (in `basis`) of every skeleton coefficient;
+ *   nodes_out optional [T_tot] (NULL to skip).
+ * status[f]: the solve's code if the solve failed, else DUPLICATE_SAMPLE for every function. */
+int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* anchors,
+                     const uint64_t* samples, int B, int s0, const uint64_t* vals, uint64_t p, int basis,
+                     uint64_t* out, uint64_t* nodes_out, int32_t* status, void* workspace, size_t workspace_bytes,
+                     void* stream);
+
+/* Host-buffer form of zippel_lift_step (the end-to-end call): every data pointer is a HOST pointer
+ * (pinned memory makes the copies asynchronous).  The library enqueues on `stream`: H2D of exps,
+ * anchors, samples and vals into staging carved from `workspace` (device,
+ * zippel_host_workspace_bytes() bytes), the lifting step, D2H of out [B x T_tot] and status [F].
+ * Nothing is synchronised: the caller waits on the stream before reading h_out / h_status. */
+size_t zippel_host_workspace_bytes(const int64_t* h_offsets, int F, int nv, int B);
+int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int F, int nv,
+                          const uint64_t* h_anchors, const uint64_t* h_samples, int B, int s0,
+                          const uint64_t* h_vals, uint64_t p, int basis, uint64_t* h_out, int32_t* h_status,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* (a6) forward evaluation used by the balanced step: power sums
+ *     out[b, off_f + s] = sum_i coef[b, off_f + i] * m_i^(s+s0),  s = 0 .. t_f-1
+ * (the skeleton evaluated at the Zippel probe points).  coef, out: [B x T_tot]. */
+int zippel_power_sums(const uint64_t* nodes, const int64_t* h_offsets, int F, const uint64_t* coef, int B, int s0,
+                      uint64_t p, uint64_t* out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* One part (numerator or denominator) of a batch of F rational functions. */
+typedef struct {
+  const uint16_t* exps;     /* [T_tot x nv] skeleton of this part */
+  const int64_t* h_offsets; /* host [F+1] */
+  const uint64_t* skel;     /* [T_tot] skeleton coefficients a'_i (the reconstruction at x_k = c_0) */
+  const uint64_t* uvals;    /* [B x T_tot] normalised univariate values u_{j,s}, s < t_f */
+  uint64_t* out;            /* [B x T_tot] */
+} zp_part;
+
+/* (a6) Balanced lifting step for rational functions, eq. (4) (G3, G20): for the
+ * numerator and the denominator separately, with R_s = sum_i a'_i m_i^(s+s0) the skeleton's value
+ * at probe s,  V_{j,s} = u_{j,s} * R_s / u_{0,s};  then (a2)-(a5) on V.  samples[0] = c_0.
+ * workspace must cover the larger part.  status [2F]: numerator codes, then denominator codes;
+ * precedence ZERO_PIVOT, then the solve's, then DUPLICATE_SAMPLE. */
+int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int nv, const uint64_t* anchors,
+                              const uint64_t* samples, int B, int s0, uint64_t p, int basis, int32_t* status,
+                              void* workspace, size_t workspace_bytes, void* stream);
+
+/* Self-test hook for the arithmetic substrate (a0), section 2.1: out[i] = op(a[i], b[i]) mod p,
+ * op: 0 mul, 1 add, 2 sub, 3 pow (b = exponent), 4 inverse of a (0 -> 0),
+ *     5 deferred dot: out[0] = sum_i a[i]*b[i] mod p through the 160-bit accumulator. */
+int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
+                             void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,383 @@
+// kernels.cuh -- device kernels of the Zippel lifting step.
+// Notation follows the paper: t terms, nodes m_i, master polynomial M, right-hand sides v_{b,s},
+// B = D+1 samples c_j of x_k.  "~" marks Montgomery form (modarith.cuh).
+#pragma once
+#include "modarith.cuh"
+
+#define ZP_ST_DUPLICATE_NODE 16
+#define ZP_ST_DUPLICATE_SAMPLE 17
+#define ZP_ST_ZERO_PIVOT 18
+#define ZP_ST_NONE 0x7fffffff
+
+// ------------------------------------------------------------------------------------------------
+// (a1) K1 eval_nodes: one lane per term.  m_i = prod_j y_j^{e_ij}  (eq. (3)).
+// The CTA first builds Y[j][k] = (y_j^(2^k))~ for k < 16 in shared memory (powers
+// from precomputed powers); each lane then multiplies the table entries its exponent bits select.
+// HBM-bound: 2*nv bytes in, 8 (or 16) bytes out per term.
+// ------------------------------------------------------------------------------------------------
+#define ZP_K1_THREADS 256
+__global__ void __launch_bounds__(ZP_K1_THREADS)
+k_eval_nodes(const uint16_t* __restrict__ exps, int64_t T_tot, int nv, const uint64_t* __restrict__ anchors,
+             ZpMod k, uint64_t* __restrict__ nodes) {
+  __shared__ uint64_t Y[32 * 16];
+  if (threadIdx.x < nv) {
+    uint64_t y = to_mont(anchors[threadIdx.x] % k.p, k);
+    for (int b = 0; b < 16; ++b) {
+      Y[threadIdx.x * 16 + b] = y;
+      y = mont_mul(y, y, k);
+    }
+  }
+  __syncthreads();
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < T_tot; i += (int64_t)gridDim.x * blockDim.x) {
+    const uint16_t* e = exps + i * nv;
+    uint64_t m = k.r1;
+    for (int j = 0; j < nv; ++j) {
+      uint32_t ej = e[j];
+      for (int b = 0; ej; ++b, ej >>= 1)
+        if (ej & 1) m = mont_mul(m, Y[j * 16 + b], k);
+    }
+    nodes[i] = from_mont(m, k);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// (a2) K2 master polynomial M(z) = prod_i (z - m_i), as a product tree.
+// A monic polynomial of degree n is stored WITHOUT its leading 1, as n Montgomery coefficients, in
+// the slots of the nodes it covers: the block of nodes [lo, hi) of a function owns buf[off+lo .. off+hi).
+// Merging the monic A (degree a) and B (degree b):  C' = A' * B' + z^a B' + z^b A'   (a + b slots).
+// Convolutions are deferred sums, one reduction per output coefficient.
+//
+// k_tree_leaf: one CTA builds the product of up to LEAF consecutive nodes of one function in shared
+// memory (all levels up to LEAF).  k_tree_level: one merge level in global memory for blocks > LEAF.
+// ------------------------------------------------------------------------------------------------
+#define ZP_LEAF 1024
+#define ZP_K2_THREADS 256
+
+// conv + shifts for output slot c of the merged block (A' = src[0..a), B' = src[a..a+b))
+template <typename SrcPtr>
+ZP_DEV uint64_t tree_merge_coef(SrcPtr src, int a, int b, int c, const ZpMod& k) {
+  // sum_{j} A'_j B'_{c-j},  max(0, c-b+1) <= j <= min(a-1, c)
+  const int jlo = c - b + 1 > 0 ? c - b + 1 : 0;
+  const int jhi = c < a - 1 ? c : a - 1;
+  uint64_t r = 0;
+  if (jhi >= jlo) {
+    Acc acc;
+    acc_zero(acc);
+    for (int j = jlo; j <= jhi; ++j) acc_mac(acc, src[j], src[a + c - j]);
+    r = mont_mul(acc_redc160(acc, k), k.c160, k);
+  }
+  if (c >= a) r = mod_add(r, src[a + (c - a)], k.p);  // z^a B'
+  if (c >= b) r = mod_add(r, src[c - b], k.p);        // z^b A'
+  return r;
+}
+
+__global__ void __launch_bounds__(ZP_K2_THREADS)
+k_tree_leaf(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offsets, int F, ZpMod k,
+            uint64_t* __restrict__ out) {
+  __shared__ uint64_t buf[2][ZP_LEAF];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int64_t t = offsets[f + 1] - off;
+    const int64_t lo = (int64_t)blockIdx.x * ZP_LEAF;
+    if (lo >= t) continue;  // uniform per CTA
+    const int n = (int)((t - lo < ZP_LEAF) ? (t - lo) : ZP_LEAF);
+    for (int i = threadIdx.x; i < n; i += blockDim.x)
+      buf[0][i] = mod_neg(to_mont(nodes[off + lo + i] % k.p, k), k.p);  // (z - m_i)' = -m_i~
+    __syncthreads();
+    int cur = 0;
+    for (int a = 1; a < n; a <<= 1) {  // merge blocks [2j a, 2j a + a) and [2j a + a, 2j a + 2a)
+      const uint64_t* src = buf[cur];
+      uint64_t* dst = buf[cur ^ 1];
+      for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int base = i & ~(2 * a - 1);
+        const int b = (n - base - a) < a ? (n - base - a) : a;  // right block length (may be <= 0)
+        dst[i] = (b <= 0) ? src[i] : tree_merge_coef(src + base, a, b, i - base, k);
+      }
+      __syncthreads();
+      cur ^= 1;
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) out[off + lo + i] = buf[cur][i];
+    __syncthreads();
+  }
+}
+
+// one level: left block length a (multiple of LEAF), thread per output slot
+__global__ void __launch_bounds__(ZP_K2_THREADS)
+k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offsets, int F, int64_t a, ZpMod k,
+             uint64_t* __restrict__ dst) {
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int64_t t = offsets[f + 1] - off;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < t; i += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t base = i - (i % (2 * a));
+      const int64_t b = (t - base - a) < a ? (t - base - a) : a;
+      dst[off + i] = (b <= 0) ? src[off + i] : tree_merge_coef(src + off + base, (int)a, (int)b, (int)(i - base), k);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// (a3)+(a4) K3 node_solve: the hot loop (PAPER.md L189-197 ZippelMultiplePrime(), L203-213).
+// One lane per node i of one function; the CTA streams tiles of M and of the NB right-hand sides
+// through shared memory (every lane needs the same M_l, v_{b,l}: warp-uniform broadcast reads).
+// Per lane, l = t-1 .. 0 with q = q_l (q_{t-1} = 1):
+//     acc_b += q * v_{b,l}                    NB deferred MACs   (L194-195 "vector of powers" x "values")
+//     q <- M_l + m q ; d <- d m + q   (l >= 1)   2 Montgomery products (L193 Horner / synthetic division)
+// then  c_{b,i} = acc_b / d  [ / m if s0 = 1 ]   (L196), d = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15).
+// Nothing of length t is stored per lane (reading G7).
+// Template NB = right-hand sides handled per pass; FIRST = this pass computes d and writes scale.
+// ------------------------------------------------------------------------------------------------
+#define ZP_K3_THREADS 128
+#define ZP_K3_TILE 64
+
+template <int NB, bool FIRST>
+__global__ void __launch_bounds__(ZP_K3_THREADS)
+k_node_solve(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ M, const int64_t* __restrict__ offsets,
+             int F, const uint64_t* __restrict__ vals, int64_t T_tot, int b0, int s0, ZpMod k,
+             uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
+  constexpr int NBP = (NB + 1) & ~1;  // row stride (even: 16-byte aligned pairs)
+  __shared__ __align__(16) uint64_t sM[ZP_K3_TILE];
+  __shared__ __align__(16) uint64_t sV[ZP_K3_TILE * NBP];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int t = (int)(offsets[f + 1] - off);
+    const int i0 = blockIdx.x * ZP_K3_THREADS;
+    if (i0 >= t) continue;  // uniform per CTA
+    const int i = i0 + threadIdx.x;
+    const bool live = i < t;
+    const uint64_t m = live ? to_mont(nodes[off + i] % k.p, k) : 0;
+    uint64_t q = k.r1, d = k.r1;
+    Acc acc[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) acc_zero(acc[b]);
+    const uint64_t* Mf = M + off;
+    for (int l1 = t; l1 > 0; l1 -= ZP_K3_TILE) {  // tile covers l in [l0, l1)
+      const int l0 = l1 - ZP_K3_TILE > 0 ? l1 - ZP_K3_TILE : 0;
+      const int n = l1 - l0;
+      __syncthreads();
+      for (int x = threadIdx.x; x < n; x += ZP_K3_THREADS) sM[x] = Mf[l0 + x];
+      for (int x = threadIdx.x; x < n * NB; x += ZP_K3_THREADS) {
+        const int b = x / n, s = x - b * n;
+        sV[s * NBP + b] = vals[(int64_t)(b0 + b) * T_tot + off + l0 + s];
+      }
+      __syncthreads();
+      for (int s = n - 1; s >= 0; --s) {
+#pragma unroll
+        for (int b = 0; b < NB; b += 2) {
+          if (b + 1 < NB) {
+            const ulonglong2 v2 = *reinterpret_cast<const ulonglong2*>(&sV[s * NBP + b]);
+            acc_mac(acc[b], q, v2.x);
+            acc_mac(acc[b + 1], q, v2.y);
+          } else {
+            acc_mac(acc[b], q, sV[s * NBP + b]);
+          }
+        }
+        if (l0 + s >= 1) {
+          q = mod_add(mont_mul(m, q, k), sM[s], k.p);
+          if (FIRST) d = mod_add(mont_mul(d, m, k), q, k.p);
+        }
+      }
+    }
+    if (live) {
+      uint64_t sc;
+      if (FIRST) {
+        const uint64_t dd = s0 ? mont_mul(d, m, k) : d;
+        if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
+        sc = mont_mul(mont_inv(dd, k), k.c160, k);  // plain d^-1 * 2^160
+        if (scale) scale[off + i] = sc;
+      } else {
+        sc = scale[off + i];
+      }
+#pragma unroll
+      for (int b = 0; b < NB; ++b)
+        coefs[(int64_t)(b0 + b) * T_tot + off + i] = mont_mul(acc_redc160(acc[b], k), sc, k);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// (a5) K5 Newton interpolation in x_k, one lane per coefficient (eq. (1)).
+// k_newton_prep: invd[j*B + jj] = (1/(c_j - c_jj))~ for jj < j, samples~, duplicate check.
+// k_newton: divided differences in shared memory (column per lane), optional monomial expansion.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_newton_prep(const uint64_t* __restrict__ samples, int B, ZpMod k, uint64_t* __restrict__ invd,
+                              uint64_t* __restrict__ smont, int32_t* __restrict__ nstatus) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= B * B) return;
+  const int j = idx / B, jj = idx % B;
+  const uint64_t cj = samples[j] % k.p, cjj = samples[jj] % k.p;
+  if (jj == 0) smont[j] = to_mont(cj, k);
+  if (jj < j) {
+    const uint64_t diff = mod_sub(cj, cjj, k.p);
+    if (diff == 0) atomicMin(nstatus, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
+    invd[idx] = mont_inv(to_mont(diff, k), k);
+  }
+}
+
+#define ZP_K5_THREADS 128
+__global__ void __launch_bounds__(ZP_K5_THREADS)
+k_newton(const uint64_t* __restrict__ invd, const uint64_t* __restrict__ smont, int B, const uint64_t* vals, int64_t n,
+         int64_t ld, ZpMod k, int basis, uint64_t* out) {
+  extern __shared__ uint64_t sh[];
+  uint64_t* sInv = sh;                                 // [B*B]
+  uint64_t* sC = sh + B * B;                           // [B] samples~
+  uint64_t* col = sC + B + threadIdx.x;                // column of this lane: col[j*TH]
+  uint64_t* pol = sC + B + (size_t)B * ZP_K5_THREADS + threadIdx.x;  // second column (monomial expansion)
+  constexpr int TH = ZP_K5_THREADS;
+  for (int x = threadIdx.x; x < B * B; x += TH) sInv[x] = invd[x];
+  for (int x = threadIdx.x; x < B; x += TH) sC[x] = smont[x];
+  __syncthreads();
+  const int D = B - 1;
+  for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
+    // the product by the Montgomery inverse difference keeps plain values plain
+    for (int j = 0; j < B; ++j) col[j * TH] = vals[j * ld + i] % k.p;
+    for (int l = 1; l <= D; ++l) {
+      uint64_t hiv = col[D * TH];
+      for (int j = D; j >= l; --j) {
+        const uint64_t lov = col[(j - 1) * TH];
+        col[j * TH] = mont_mul(mod_sub(hiv, lov, k.p), sInv[j * B + (j - l)], k);
+        hiv = lov;
+      }
+    }
+    if (basis == 0) {
+      for (int j = 0; j < B; ++j) out[j * ld + i] = col[j * TH];
+    } else {
+      // P <- [a_D]; for j = D-1 .. 0: P <- P (x - c_j) + a_j
+      int deg = 0;
+      pol[0] = col[D * TH];
+      for (int j = D - 1; j >= 0; --j) {
+        const uint64_t cj = sC[j];
+        uint64_t up = pol[deg * TH];
+        pol[(deg + 1) * TH] = up;
+        for (int x = deg; x >= 1; --x) {
+          const uint64_t below = pol[(x - 1) * TH];
+          pol[x * TH] = mod_sub(below, mont_mul(cj, pol[x * TH], k), k.p);
+        }
+        pol[0] = mod_sub(col[j * TH], mont_mul(cj, pol[0], k), k.p);
+        ++deg;
+      }
+      for (int j = 0; j < B; ++j) out[j * ld + i] = pol[j * TH];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// status plumbing
+// ------------------------------------------------------------------------------------------------
+__global__ void k_fill_i32(int32_t* x, int n, int32_t v) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) x[i] = v;
+}
+// final[f] = first non-NONE of (pre[f], solve[f], newton[0]) ; NONE -> 0
+__global__ void k_status_finish(const int32_t* pre, const int32_t* solve, const int32_t* newton, int F, int32_t* fin) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= F) return;
+  int32_t s = ZP_ST_NONE;
+  if (pre && pre[f] != ZP_ST_NONE) s = pre[f];
+  else if (solve && solve[f] != ZP_ST_NONE) s = solve[f];
+  else if (newton && newton[0] != ZP_ST_NONE) s = newton[0];
+  fin[f] = (s == ZP_ST_NONE) ? 0 : s;
+}
+
+// ------------------------------------------------------------------------------------------------
+// (a6) K6 power sums R_{b,s} = sum_i a_{b,i} m_i^(s+s0)  ("raise base variable
+// values to various powers and substitute them into the polynomial"; strided power tables, A21).
+// CTA = (function f, block of 256 consecutive s); node tiles of 128 in shared memory with
+//   base_i = a_i~ m_i^(sb0+s0),  lo_i[x] = m_i^x,  hi_i[x] = m_i^(16x)   (x < 16),
+// lane s: m_i^(s-sb0) = lo_i[s & 15] * hi_i[s >> 4]; deferred sum over i.
+// ------------------------------------------------------------------------------------------------
+#define ZP_K6_THREADS 256
+#define ZP_K6_NODES 128
+__global__ void __launch_bounds__(ZP_K6_THREADS)
+k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offsets, int F,
+             const uint64_t* __restrict__ coef, int64_t T_tot, int B, int s0, ZpMod k, uint64_t* __restrict__ out) {
+  __shared__ uint64_t sBase[ZP_K6_NODES];
+  __shared__ uint64_t sLo[ZP_K6_NODES * 16];
+  __shared__ uint64_t sHi[ZP_K6_NODES * 16];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int t = (int)(offsets[f + 1] - off);
+    const int sb0 = blockIdx.x * ZP_K6_THREADS;
+    if (sb0 >= t) continue;
+    const int s = sb0 + threadIdx.x;
+    for (int b = 0; b < B; ++b) {
+      Acc acc;
+      acc_zero(acc);
+      for (int i0 = 0; i0 < t; i0 += ZP_K6_NODES) {
+        const int n = t - i0 < ZP_K6_NODES ? t - i0 : ZP_K6_NODES;
+        __syncthreads();
+        if (threadIdx.x < n) {
+          const int i = i0 + threadIdx.x;
+          const uint64_t m = to_mont(nodes[off + i] % k.p, k);
+          const uint64_t a = to_mont(coef[(int64_t)b * T_tot + off + i] % k.p, k);
+          sBase[threadIdx.x] = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);
+          uint64_t pw = k.r1;
+          for (int x = 0; x < 16; ++x) {
+            sLo[threadIdx.x * 16 + x] = pw;
+            pw = mont_mul(pw, m, k);
+          }
+          const uint64_t m16 = pw;
+          pw = k.r1;
+          for (int x = 0; x < 16; ++x) {
+            sHi[threadIdx.x * 16 + x] = pw;
+            pw = mont_mul(pw, m16, k);
+          }
+        }
+        __syncthreads();
+        const int lo = threadIdx.x & 15, hi = threadIdx.x >> 4;
+        for (int x = 0; x < n; ++x)
+          acc_mac(acc, mont_mul(sLo[x * 16 + lo], sHi[x * 16 + hi], k), sBase[x]);
+      }
+      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c96, k);
+    }
+  }
+}
+
+// (a6) K7 balance: V_{j,s} = u_{j,s} * R_s / u_{0,s}   (eq. (4), readings G3, G20).
+__global__ void k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R,
+                          const int64_t* __restrict__ offsets, int F, int64_t T_tot, int B, ZpMod k,
+                          uint64_t* __restrict__ V, int32_t* __restrict__ pre) {
+  for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < T_tot; x += (int64_t)gridDim.x * blockDim.x) {
+    const uint64_t u0 = u[x] % k.p;
+    uint64_t sc = 0;
+    if (u0 == 0) {
+      int lo = 0, hi = F;  // function of slot x: offsets[lo] <= x < offsets[lo+1]
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (offsets[mid] <= x) lo = mid; else hi = mid;
+      }
+      atomicMin(&pre[lo], (int32_t)(((uint32_t)(x - offsets[lo]) << 8) | ZP_ST_ZERO_PIVOT));
+    } else {
+      sc = mont_mul(to_mont(R[x], k), mont_inv(to_mont(u0, k), k), k);  // (R_s / u_{0,s})~
+    }
+    for (int j = 0; j < B; ++j) V[(int64_t)j * T_tot + x] = mont_mul(u[(int64_t)j * T_tot + x] % k.p, sc, k);
+  }
+}
+
+// (a0) self-test kernel for the substrate
+__global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, ZpMod k, uint64_t* out) {
+  if (op == 5) {  // deferred dot through the wide accumulator, one CTA
+    __shared__ uint64_t part[256];
+    Acc acc;
+    acc_zero(acc);
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) acc_mac(acc, to_mont(a[i] % k.p, k), b[i]);
+    part[threadIdx.x] = mont_mul(acc_redc160(acc, k), k.c160, k);  // mont * plain -> plain
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      uint64_t r = 0;
+      for (int x = 0; x < (int)blockDim.x; ++x) r = mod_add(r, part[x], k.p);
+      out[0] = r;
+    }
+    return;
+  }
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const uint64_t x = a[i] % k.p, y = b ? b[i] : 0;
+    uint64_t r = 0;
+    if (op == 0) r = from_mont(mont_mul(to_mont(x, k), to_mont(y % k.p, k), k), k);
+    if (op == 1) r = mod_add(x, y % k.p, k.p);
+    if (op == 2) r = mod_sub(x, y % k.p, k.p);
+    if (op == 3) r = from_mont(mont_pow(to_mont(x, k), y, k), k);
+    if (op == 4) r = from_mont(mont_inv(to_mont(x, k), k), k);
+    out[i] = r;
+  }
+}

@@ -1,0 +1,166 @@
+// modarith.cuh -- (a0) arithmetic substrate: 63-bit Montgomery arithmetic on the sm_100a integer pipes.
+//
+// What the paper does here (section 2.1): 64-bit a*b mod n on the GPU; the FLINT
+// port (precomputed inverse, no division) won.  What this build does instead: Montgomery form with
+// R = 2^64 in 32-bit limbs.  Measured on B200 (profiles/r01_ubench.md): IMAD.WIDE.U32 (32x32+64->64)
+// issues at the full IMAD rate (64 lanes/clk/SM), IMAD.HI at well under half of it, and IMAD + IADD3
+// co-issue up to the scheduler's 128 lanes/clk/SM -- so everything is built from mul.wide/mad.wide and
+// the carries ride on predicates (ptxas turns add.cc/addc on mad.wide results into IMAD.WIDE[.X]).
+//
+// Forms:  plain x in [0,p);  Montgomery x~ = x * 2^64 mod p in [0,p).
+//   mont_mul(a,b) = a*b*2^-64 mod p            (10 multiplier instructions: 8 IMAD.WIDE + 2 IMAD.LO)
+//   Acc           = deferred 160-bit accumulator of 64x64 products ("emulating a
+//                   192-bit integer"; 160 bits suffice: < 2^31 products of < 2^128)   4 IMAD.WIDE / MAC
+//   acc_redc160   = T * 2^-160 mod p for a 160-bit T, any odd p < 2^63 (five 32-bit REDC rounds)
+#pragma once
+#include <cstdint>
+
+struct ZpMod {
+  uint64_t p;
+  uint32_t p0, p1;  // p = p1:p0
+  uint32_t pinv;    // -p^{-1} mod 2^32
+  uint64_t r1;      // 2^64  mod p : Montgomery form of 1
+  uint64_t r2;      // 2^128 mod p : to_mont multiplier
+  uint64_t c96;     // 2^96  mod p : mont_mul(acc_redc160(sum of mont*mont), c96)  -> plain
+  uint64_t c160;    // 2^160 mod p : mont_mul(acc_redc160(sum of mont*mont), c160) -> Montgomery
+                    //               mont_mul(acc_redc160(sum of mont*plain), c160) -> plain
+  uint64_t c224;    // 2^224 mod p : mont_mul(acc_redc160(sum of mont*plain), c224) -> Montgomery
+};
+
+#if defined(__CUDACC__)
+#define ZP_DEV __device__ __forceinline__
+
+ZP_DEV uint64_t zp_mulw(uint32_t a, uint32_t b) {
+  uint64_t r;
+  asm("mul.wide.u32 %0, %1, %2;" : "=l"(r) : "r"(a), "r"(b));
+  return r;
+}
+ZP_DEV uint64_t zp_madw(uint32_t a, uint32_t b, uint64_t c) {
+  uint64_t r;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
+  return r;
+}
+
+ZP_DEV uint64_t mod_add(uint64_t a, uint64_t b, uint64_t p) {  // a, b < p < 2^63: no overflow
+  uint64_t r = a + b, s = r - p;
+  return (r >= p) ? s : r;
+}
+ZP_DEV uint64_t mod_sub(uint64_t a, uint64_t b, uint64_t p) {
+  uint64_t r = a - b;
+  return (a >= b) ? r : r + p;
+}
+ZP_DEV uint64_t mod_neg(uint64_t a, uint64_t p) { return a ? p - a : 0; }
+
+// Montgomery product, column form.  Requires a*b < p*2^64 (true for a < 2^64, b < p); a_hi, b_hi < 2^31
+// is NOT required.  With T = a*b and two 32-bit REDC rounds:
+//   T + m0*p + m1*p*2^32 = (P00 + Q0) + (P01 + P10 + Q1 + S0)*2^32 + (P11 + S1)*2^64,  divisible by 2^64.
+// Column 0: the low words of P00 and Q0 cancel, its carry is c0 = hi(P00) + hi(Q0) + (lo(P00) != 0) < 2^33.
+// Column 1: P01 + P10 + Q1 + S0 + c0 may exceed 64 bits; `carry` counts the overflows (weight 2^64).
+// Result (T + ...)/2^64 < p + p = 2p < 2^64, then one conditional subtraction.
+ZP_DEV uint64_t mont_mul(uint64_t a, uint64_t b, const ZpMod& k) {
+  const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32), b0 = (uint32_t)b, b1 = (uint32_t)(b >> 32);
+  const uint64_t P00 = zp_mulw(a0, b0);
+  const uint64_t P01 = zp_mulw(a0, b1);
+  const uint64_t P10 = zp_mulw(a1, b0);
+  const uint64_t P11 = zp_mulw(a1, b1);
+  const uint32_t m0 = (uint32_t)P00 * k.pinv;
+  const uint64_t Q0 = zp_mulw(m0, k.p0), Q1 = zp_mulw(m0, k.p1);
+  const uint64_t c0 = (P00 >> 32) + (Q0 >> 32) + ((uint32_t)P00 != 0);
+  uint64_t col1;
+  uint32_t carry;
+  asm("{\n\t"
+      ".reg .u64 t;\n\t"
+      "add.cc.u64 t, %2, %3;\n\t"
+      "addc.u32 %1, 0, 0;\n\t"
+      "add.cc.u64 t, t, %4;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, t, %5;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "}"
+      : "=l"(col1), "=r"(carry)
+      : "l"(P01), "l"(P10), "l"(Q1), "l"(c0));
+  const uint32_t m1 = (uint32_t)col1 * k.pinv;
+  const uint64_t S0 = zp_mulw(m1, k.p0);
+  const uint64_t c1 = (col1 >> 32) + (S0 >> 32) + ((uint32_t)col1 != 0) + ((uint64_t)carry << 32);
+  // P11 + S1 + c1 = exact quotient < 2p + 1 <= 2^64 - ... : no overflow
+  const uint64_t r = zp_madw(m1, k.p1, P11 + c1);
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+
+ZP_DEV uint64_t to_mont(uint64_t x, const ZpMod& k) { return mont_mul(x, k.r2, k); }
+ZP_DEV uint64_t from_mont(uint64_t x, const ZpMod& k) { return mont_mul(x, 1, k); }
+
+// x~^e (Montgomery in, Montgomery out), right-to-left square and multiply.
+ZP_DEV uint64_t mont_pow(uint64_t x, uint64_t e, const ZpMod& k) {
+  uint64_t r = k.r1;
+  while (e) {
+    if (e & 1) r = mont_mul(r, x, k);
+    x = mont_mul(x, x, k);
+    e >>= 1;
+  }
+  return r;
+}
+// Inverse by Fermat, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.
+ZP_DEV uint64_t mont_inv(uint64_t x, const ZpMod& k) { return mont_pow(x, k.p - 2, k); }
+
+// Deferred accumulator.  value = E + O * 2^32 with
+//   E = e0 + e1*2^64 + e2*2^128  (takes x0*y0 at bit 0 and x1*y1 at bit 64),
+//   O = o0 + o1*2^64             (takes x0*y1 + x1*y0).
+// Per MAC: 4 IMAD.WIDE with the accumulate folded in, the carries leave through predicates into the
+// two 32-bit counters: 2 IADD3.X.  The split keeps every multiply 64-bit aligned so that no shifted
+// add is needed (8 registers instead of 5; the 5-register form costs 4 IADD3 per MAC).
+struct Acc {
+  uint64_t e0, e1, o0;
+  uint32_t e2, o1;
+};
+ZP_DEV void acc_zero(Acc& a) { a.e0 = a.e1 = a.o0 = 0; a.e2 = a.o1 = 0; }
+ZP_DEV void acc_mac(Acc& a, uint64_t x, uint64_t y) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0);
+  asm("add.cc.u64 %0, %0, %3;\n\t"
+      "addc.cc.u64 %1, %1, %4;\n\t"
+      "addc.u32 %2, %2, 0;"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi));
+  asm("add.cc.u64 %0, %0, %2;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %3;\n\t"
+      "addc.u32 %1, %1, 0;"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1));
+}
+
+// T * 2^-160 mod p, canonical, for the 160-bit T held in the accumulator (five REDC rounds of 32 bits:
+// T_{k+1} = (T_k + m p)/2^32 < T_k/2^32 + p, so T_5 < T_0/2^160 + p(1 + 2^-32 + ...) <= p + 1).
+ZP_DEV uint64_t acc_redc160(const Acc& a, const ZpMod& k) {
+  // fold E + O*2^32 into five words
+  uint32_t w0 = (uint32_t)a.e0, w1 = (uint32_t)(a.e0 >> 32), w2 = (uint32_t)a.e1, w3 = (uint32_t)(a.e1 >> 32), w4 = a.e2;
+  {
+    uint64_t c = (uint64_t)w1 + (uint32_t)a.o0;
+    w1 = (uint32_t)c;
+    c = (uint64_t)w2 + (uint32_t)(a.o0 >> 32) + (c >> 32);
+    w2 = (uint32_t)c;
+    c = (uint64_t)w3 + a.o1 + (c >> 32);
+    w3 = (uint32_t)c;
+    w4 += (uint32_t)(c >> 32);
+  }
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {
+    const uint32_t m = w0 * k.pinv;
+    uint64_t c = zp_madw(m, k.p0, (uint64_t)w0);      // low word cancels
+    c = zp_madw(m, k.p1, (uint64_t)w1 + (c >> 32));   // (2^32-1)(2^31-1) + 2*2^32 < 2^64
+    w0 = (uint32_t)c;
+    c = (uint64_t)w2 + (c >> 32);
+    w1 = (uint32_t)c;
+    c = (uint64_t)w3 + (c >> 32);
+    w2 = (uint32_t)c;
+    c = (uint64_t)w4 + (c >> 32);
+    w3 = (uint32_t)c;
+    w4 = (uint32_t)(c >> 32);
+  }
+  const uint64_t r = ((uint64_t)w1 << 32) | w0;  // w2 = w3 = w4 = 0 here
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+#endif  // __CUDACC__

@@ -1,0 +1,389 @@
+// zippel_capi.cu -- the C-ABI boundary (include/zippel.h): argument checks, Montgomery constants,
+// workspace carving and kernel launches.  No torch types, no allocation, no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstring>
+
+#include "../../include/zippel.h"
+#include "kernels.cuh"
+
+namespace {
+
+typedef unsigned __int128 u128;
+
+// ---- host: Montgomery constants for an odd p < 2^63 -------------------------------------------
+bool make_mod(uint64_t p, ZpMod* k) {
+  if (p < 3 || (p & 1) == 0 || (p >> 63)) return false;
+  k->p = p;
+  k->p0 = (uint32_t)p;
+  k->p1 = (uint32_t)(p >> 32);
+  uint32_t inv = 1;  // Newton: inv = p^-1 mod 2^32
+  for (int i = 0; i < 5; ++i) inv *= 2u - (uint32_t)p * inv;
+  k->pinv = 0u - inv;
+  auto pow2 = [&](int e) {  // 2^e mod p
+    uint64_t r = 1 % p;
+    for (int i = 0; i < e; ++i) r = (uint64_t)(((u128)r * 2) % p);
+    return r;
+  };
+  k->r1 = pow2(64);
+  k->r2 = pow2(128);
+  k->c96 = pow2(96);
+  k->c160 = pow2(160);
+  k->c224 = pow2(224);
+  return true;
+}
+
+// ---- workspace ----------------------------------------------------------------------------------
+struct Ws {
+  int64_t* d_offsets;
+  int32_t *st_pre, *st_solve, *st_newton;
+  uint64_t *nodes, *M0, *M1, *scale, *invd, *smont, *R, *V;
+  size_t bytes;
+};
+
+inline size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
+  Ws w;
+  size_t o = 0;
+  auto take = [&](size_t n) {
+    char* p = base ? (char*)base + o : nullptr;
+    o += al(n);
+    return (void*)p;
+  };
+  w.d_offsets = (int64_t*)take(sizeof(int64_t) * (size_t)(F + 1));
+  w.st_pre = (int32_t*)take(sizeof(int32_t) * (size_t)F);
+  w.st_solve = (int32_t*)take(sizeof(int32_t) * (size_t)F);
+  w.st_newton = (int32_t*)take(sizeof(int32_t) * 4);
+  w.nodes = (uint64_t*)take(8 * (size_t)T_tot);
+  w.M0 = (uint64_t*)take(8 * (size_t)T_tot);
+  w.M1 = (uint64_t*)take(8 * (size_t)T_tot);
+  w.scale = (uint64_t*)take(8 * (size_t)T_tot);
+  w.invd = (uint64_t*)take(8 * (size_t)B * B);
+  w.smont = (uint64_t*)take(8 * (size_t)B);
+  w.R = (uint64_t*)take(8 * (size_t)T_tot);
+  w.V = (flags & ZP_WS_BALANCED) ? (uint64_t*)take(8 * (size_t)T_tot * B) : nullptr;
+  w.bytes = o;
+  return w;
+}
+
+bool check_offsets(const int64_t* h, int F, int64_t* T_tot, int64_t* tmax) {
+  if (!h || F <= 0 || h[0] != 0) return false;
+  int64_t mx = 0;
+  for (int f = 0; f < F; ++f) {
+    const int64_t t = h[f + 1] - h[f];
+    if (t <= 0 || t >= ((int64_t)1 << 31)) return false;
+    if (t > mx) mx = t;
+  }
+  if (h[F] >= ((int64_t)1 << 31)) return false;
+  *T_tot = h[F];
+  *tmax = mx;
+  return true;
+}
+
+inline int cuda_ok() { return cudaGetLastError() == cudaSuccess ? ZP_OK : ZP_ERR_CUDA; }
+inline unsigned grid_y(int F) { return (unsigned)(F < 65535 ? F : 65535); }
+
+// ---- K3 dispatch ----------------------------------------------------------------------------------
+#define ZP_NB_MAX 25
+
+template <int NB>
+void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const uint64_t* M,
+                       const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k,
+                       uint64_t* scale, uint64_t* coefs, int32_t* status) {
+  if (first)
+    k_node_solve<NB, true><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+  else
+    k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+}
+
+void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const uint64_t* M,
+                         const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0,
+                         const ZpMod& k, uint64_t* scale, uint64_t* coefs, int32_t* status) {
+#define ZP_CASE(N) \
+  case N: launch_node_solve<N>(first, grid, st, nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status); break;
+  switch (nb) {
+    ZP_CASE(1) ZP_CASE(2) ZP_CASE(3) ZP_CASE(4) ZP_CASE(5) ZP_CASE(6) ZP_CASE(7) ZP_CASE(8) ZP_CASE(9)
+    ZP_CASE(10) ZP_CASE(11) ZP_CASE(12) ZP_CASE(13) ZP_CASE(14) ZP_CASE(15) ZP_CASE(16) ZP_CASE(17)
+    ZP_CASE(18) ZP_CASE(19) ZP_CASE(20) ZP_CASE(21) ZP_CASE(22) ZP_CASE(23) ZP_CASE(24) ZP_CASE(25)
+    default: break;
+  }
+#undef ZP_CASE
+}
+
+// ---- stages (device offsets already in w.d_offsets) ---------------------------------------------
+// (a2) master polynomial of every function -> returns the buffer holding M' (Montgomery)
+const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64_t tmax, const ZpMod& k,
+                                cudaStream_t st) {
+  dim3 g((unsigned)((tmax + ZP_LEAF - 1) / ZP_LEAF), grid_y(F));
+  k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes, w.d_offsets, F, k, w.M0);
+  uint64_t *src = w.M0, *dst = w.M1;
+  for (int64_t a = ZP_LEAF; a < tmax; a <<= 1) {
+    dim3 gl((unsigned)((tmax + ZP_K2_THREADS - 1) / ZP_K2_THREADS), grid_y(F));
+    k_tree_level<<<gl, ZP_K2_THREADS, 0, st>>>(src, w.d_offsets, F, a, k, dst);
+    uint64_t* tmp = src;
+    src = dst;
+    dst = tmp;
+  }
+  return src;
+}
+
+// (a2)-(a4): solve into coefs; per-function codes into w.st_solve (NONE = ok)
+void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
+               int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
+  k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
+  const uint64_t* M = run_master_poly(w, nodes, F, tmax, k, st);
+  const int passes = (B + ZP_NB_MAX - 1) / ZP_NB_MAX;
+  const int per = (B + passes - 1) / passes;
+  dim3 g((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
+  for (int b0 = 0, pass = 0; b0 < B; b0 += per, ++pass) {
+    const int nb = (B - b0 < per) ? (B - b0) : per;
+    dispatch_node_solve(nb, pass == 0, g, st, nodes, M, w.d_offsets, F, vals, T_tot, b0, s0, k, w.scale, coefs,
+                        w.st_solve);
+  }
+}
+
+// (a5): Newton on [B x n] with leading dimension ld; code into w.st_newton[0]
+void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* vals, int64_t n, int64_t ld,
+                const ZpMod& k, int basis, uint64_t* out, cudaStream_t st) {
+  k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
+  k_newton_prep<<<(B * B + 127) / 128, 128, 0, st>>>(samples, B, k, w.invd, w.smont, w.st_newton);
+  const size_t smem = 8 * ((size_t)B * B + B + 2 * (size_t)B * ZP_K5_THREADS);
+  cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
+  if (blocks > 148 * 64) blocks = 148 * 64;
+  k_newton<<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
+}
+
+void upload_offsets(const Ws& w, const int64_t* h_offsets, int F, cudaStream_t st) {
+  cudaMemcpyAsync(w.d_offsets, h_offsets, sizeof(int64_t) * (size_t)(F + 1), cudaMemcpyHostToDevice, st);
+}
+
+void run_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t* anchors, const ZpMod& k,
+                    uint64_t* nodes, cudaStream_t st) {
+  int64_t blocks = (T_tot + ZP_K1_THREADS - 1) / ZP_K1_THREADS;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_eval_nodes<<<(unsigned)blocks, ZP_K1_THREADS, 0, st>>>(exps, T_tot, nv, anchors, k, nodes);
+}
+
+void run_power_sums(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* coef,
+                    int B, int s0, const ZpMod& k, uint64_t* out, cudaStream_t st) {
+  dim3 g((unsigned)((tmax + ZP_K6_THREADS - 1) / ZP_K6_THREADS), grid_y(F));
+  k_power_sums<<<g, ZP_K6_THREADS, 0, st>>>(nodes, w.d_offsets, F, coef, T_tot, B, s0, k, out);
+}
+
+bool ws_ok(const void* ws, size_t have, size_t need) {
+  return ws && ((uintptr_t)ws & 255) == 0 && have >= need;
+}
+
+// staging of the host-buffer entry: [exps | anchors | samples | vals | out | status | inner workspace]
+struct HostWs {
+  uint16_t* exps;
+  uint64_t *anchors, *samples, *vals, *out;
+  int32_t* status;
+  void* inner;
+  size_t inner_bytes, bytes;
+};
+HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B) {
+  HostWs h;
+  size_t o = 0;
+  auto take = [&](size_t n) {
+    char* p = base ? (char*)base + o : nullptr;
+    o += al(n);
+    return (void*)p;
+  };
+  h.exps = (uint16_t*)take(2 * (size_t)T_tot * nv);
+  h.anchors = (uint64_t*)take(8 * (size_t)nv);
+  h.samples = (uint64_t*)take(8 * (size_t)B);
+  h.vals = (uint64_t*)take(8 * (size_t)T_tot * B);
+  h.out = (uint64_t*)take(8 * (size_t)T_tot * B);
+  h.status = (int32_t*)take(4 * (size_t)F);
+  h.inner_bytes = carve(nullptr, T_tot, F, B, 0).bytes;
+  h.inner = take(h.inner_bytes);
+  h.bytes = o;
+  return h;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* zippel_strerror(int code) {
+  switch (code) {
+    case ZP_OK: return "ok";
+    case ZP_ERR_ARG: return "bad argument";
+    case ZP_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case ZP_ERR_CUDA: return "CUDA error";
+    case ZP_ST_DUPLICATE_NODE: return "duplicate (or zero) node";
+    case ZP_ST_DUPLICATE_SAMPLE: return "duplicate sample";
+    case ZP_ST_ZERO_PIVOT: return "zero pivot in balancing";
+    default: return "unknown";
+  }
+}
+
+size_t zippel_workspace_bytes(const int64_t* h_offsets, int F, int B, int flags) {
+  int64_t T_tot, tmax;
+  if (!check_offsets(h_offsets, F, &T_tot, &tmax) || B <= 0 || B > ZP_MAX_B) return 0;
+  return carve(nullptr, T_tot, F, B, flags).bytes;
+}
+
+int zippel_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t* anchors, uint64_t p,
+                      uint64_t* nodes, void* stream) {
+  ZpMod k;
+  if (!exps || !anchors || !nodes || T_tot <= 0 || T_tot >= ((int64_t)1 << 31) || nv <= 0 || nv > ZP_MAX_NV ||
+      !make_mod(p, &k))
+    return ZP_ERR_ARG;
+  run_eval_nodes(exps, T_tot, nv, anchors, k, nodes, (cudaStream_t)stream);
+  return cuda_ok();
+}
+
+int vandermonde_solve_batch(const uint64_t* nodes, const int64_t* h_offsets, int F, const uint64_t* vals, int B,
+                            int s0, uint64_t p, uint64_t* coefs, int32_t* status, void* workspace,
+                            size_t workspace_bytes, void* stream) {
+  ZpMod k;
+  int64_t T_tot, tmax;
+  if (!nodes || !vals || !coefs || !status || B <= 0 || B > ZP_MAX_B || (s0 != 0 && s0 != 1) || !make_mod(p, &k) ||
+      !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0);
+  cudaStream_t st = (cudaStream_t)stream;
+  upload_offsets(w, h_offsets, F, st);
+  run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
+  k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, nullptr, F, status);
+  return cuda_ok();
+}
+
+int newton_interp_batch(const uint64_t* samples, int B, const uint64_t* vals, int64_t n, int64_t ld, uint64_t p,
+                        int basis, uint64_t* out, int32_t* status, void* workspace, size_t workspace_bytes,
+                        void* stream) {
+  ZpMod k;
+  if (!samples || !vals || !out || !status || B <= 0 || B > ZP_MAX_B || n <= 0 || ld < n || (basis != 0 && basis != 1) ||
+      !make_mod(p, &k))
+    return ZP_ERR_ARG;
+  const int64_t one[2] = {0, 1};
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, 1, 1, B, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, 1, 1, B, 0);
+  (void)one;
+  cudaStream_t st = (cudaStream_t)stream;
+  run_newton(w, samples, B, vals, n, ld, k, basis, out, st);
+  k_status_finish<<<1, 32, 0, st>>>(nullptr, nullptr, w.st_newton, 1, status);
+  return cuda_ok();
+}
+
+int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* anchors,
+                     const uint64_t* samples, int B, int s0, const uint64_t* vals, uint64_t p, int basis,
+                     uint64_t* out, uint64_t* nodes_out, int32_t* status, void* workspace, size_t workspace_bytes,
+                     void* stream) {
+  ZpMod k;
+  int64_t T_tot, tmax;
+  if (!exps || !anchors || !samples || !vals || !out || !status || nv <= 0 || nv > ZP_MAX_NV || B <= 0 ||
+      B > ZP_MAX_B || (s0 != 0 && s0 != 1) || (basis != 0 && basis != 1) || !make_mod(p, &k) ||
+      !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0);
+  cudaStream_t st = (cudaStream_t)stream;
+  uint64_t* nodes = nodes_out ? nodes_out : w.nodes;
+  upload_offsets(w, h_offsets, F, st);
+  run_eval_nodes(exps, T_tot, nv, anchors, k, nodes, st);
+  run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, out, st);
+  run_newton(w, samples, B, out, T_tot, T_tot, k, basis, out, st);
+  k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, w.st_newton, F, status);
+  return cuda_ok();
+}
+
+size_t zippel_host_workspace_bytes(const int64_t* h_offsets, int F, int nv, int B) {
+  int64_t T_tot, tmax;
+  if (!check_offsets(h_offsets, F, &T_tot, &tmax) || B <= 0 || B > ZP_MAX_B || nv <= 0 || nv > ZP_MAX_NV) return 0;
+  return carve_host(nullptr, T_tot, F, nv, B).bytes;
+}
+
+int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int F, int nv,
+                          const uint64_t* h_anchors, const uint64_t* h_samples, int B, int s0,
+                          const uint64_t* h_vals, uint64_t p, int basis, uint64_t* h_out, int32_t* h_status,
+                          void* workspace, size_t workspace_bytes, void* stream) {
+  int64_t T_tot, tmax;
+  if (!h_exps || !h_anchors || !h_samples || !h_vals || !h_out || !h_status || nv <= 0 || nv > ZP_MAX_NV ||
+      B <= 0 || B > ZP_MAX_B || !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve_host(nullptr, T_tot, F, nv, B).bytes)) return ZP_ERR_WORKSPACE;
+  const HostWs h = carve_host(workspace, T_tot, F, nv, B);
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaMemcpyAsync(h.exps, h_exps, 2 * (size_t)T_tot * nv, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(h.anchors, h_anchors, 8 * (size_t)nv, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(h.samples, h_samples, 8 * (size_t)B, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(h.vals, h_vals, 8 * (size_t)T_tot * B, cudaMemcpyHostToDevice, st);
+  const int rc = zippel_lift_step(h.exps, h_offsets, F, nv, h.anchors, h.samples, B, s0, h.vals, p, basis, h.out,
+                                  nullptr, h.status, h.inner, h.inner_bytes, stream);
+  if (rc != ZP_OK) return rc;
+  cudaMemcpyAsync(h_out, h.out, 8 * (size_t)T_tot * B, cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(h_status, h.status, 4 * (size_t)F, cudaMemcpyDeviceToHost, st);
+  return cuda_ok();
+}
+
+int zippel_power_sums(const uint64_t* nodes, const int64_t* h_offsets, int F, const uint64_t* coef, int B, int s0,
+                      uint64_t p, uint64_t* out, void* workspace, size_t workspace_bytes, void* stream) {
+  ZpMod k;
+  int64_t T_tot, tmax;
+  if (!nodes || !coef || !out || B <= 0 || B > ZP_MAX_B || (s0 != 0 && s0 != 1) || !make_mod(p, &k) ||
+      !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0);
+  cudaStream_t st = (cudaStream_t)stream;
+  upload_offsets(w, h_offsets, F, st);
+  run_power_sums(w, nodes, F, T_tot, tmax, coef, B, s0, k, out, st);
+  return cuda_ok();
+}
+
+int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int nv, const uint64_t* anchors,
+                              const uint64_t* samples, int B, int s0, uint64_t p, int basis, int32_t* status,
+                              void* workspace, size_t workspace_bytes, void* stream) {
+  ZpMod k;
+  if (!num || !den || !anchors || !samples || !status || nv <= 0 || nv > ZP_MAX_NV || B <= 0 || B > ZP_MAX_B ||
+      (s0 != 0 && s0 != 1) || (basis != 0 && basis != 1) || !make_mod(p, &k))
+    return ZP_ERR_ARG;
+  const zp_part* parts[2] = {num, den};
+  int64_t T_tot[2], tmax[2];
+  for (int x = 0; x < 2; ++x) {
+    const zp_part* q = parts[x];
+    if (!q->exps || !q->skel || !q->uvals || !q->out || !check_offsets(q->h_offsets, F, &T_tot[x], &tmax[x]))
+      return ZP_ERR_ARG;
+    if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot[x], F, B, ZP_WS_BALANCED).bytes)) return ZP_ERR_WORKSPACE;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int x = 0; x < 2; ++x) {  // the two parts run back to back on the stream and reuse the workspace
+    const zp_part* q = parts[x];
+    const Ws w = carve(workspace, T_tot[x], F, B, ZP_WS_BALANCED);
+    upload_offsets(w, q->h_offsets, F, st);
+    k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
+    run_eval_nodes(q->exps, T_tot[x], nv, anchors, k, w.nodes, st);
+    run_power_sums(w, w.nodes, F, T_tot[x], tmax[x], q->skel, 1, s0, k, w.R, st);
+    int64_t blocks = (T_tot[x] + 255) / 256;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
+    run_solve(w, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
+    run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st);
+    k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
+  }
+  return cuda_ok();
+}
+
+int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
+                             void* stream) {
+  ZpMod k;
+  if (!a || !out || n <= 0 || op < 0 || op > 5 || !make_mod(p, &k) || ((op <= 3 || op == 5) && !b)) return ZP_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (op == 5) {
+    k_modarith_selftest<<<1, 256, 0, st>>>(op, a, b, n, k, out);
+  } else {
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_modarith_selftest<<<(unsigned)blocks, 256, 0, st>>>(op, a, b, n, k, out);
+  }
+  return cuda_ok();
+}
+
+}  // extern "C"
