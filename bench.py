@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input resident in HBM:
+  config 2 (default; BASELINE.json configs[1], the batched 4 -> 5 variable lift: F = 4096 functions,
+            t = 1000 terms, B = D+1 = 21 samples): zippel_lift_step = nodes, master polynomials,
+            per-node synthetic division + 21 dot products, inversion/scaling, Newton in x_5;
+  config 3 / 5: the single large skeletons (eval_nodes + vandermonde_solve_batch [+ Newton]);
+  config 4: balanced_zippel_lift_step on F = 1024 rational functions.
+metric = Vandermonde terms solved per second = B * T_tot / time, whole job.
+N > 1 (torchrun): functions are independent, every rank lifts its own batch of the same shape (weak
+scaling, no data-path collective); time = max over ranks.
+
+--impl reference times the CPU oracle (oracle/, as it stands, single thread) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "vandermonde_terms_solved_per_s"
+UNIT = "terms/s"
+# IMAD-derived peak: 148 SMs x 64 lanes/clk of the 32-bit multiplier (fma) pipe x
+# 1.965 GHz max SM clock; the micro-benchmark in profiles/r01_ubench.md reached 60.8-63 of the 64.
+IMAD_PEAK_TOPS = 148 * 64 * 1.965e9 / 1e12
+C_MM, C_MAC = 10, 4  # multiplier instructions per Montgomery product / per deferred MAC
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------- workloads
+def load_workload(idx: int, seed_shift: int, F_override):
+    from paper_2505_24256_b200 import workloads as wl
+
+    kw = {}
+    if F_override:
+        kw["F"] = F_override
+    if idx == 4:
+        rw = wl.make_rational_workload("C4", wl.SEED_BASE + 4 + 1000 * seed_shift, kw.get("F", 1024), 6, 500, 200, 24, 25)
+        return rw
+    sh = dict(wl.CONFIG_SHAPES[idx])
+    sh.update(kw)
+    return wl.make_box_workload(f"C{idx}", wl.SEED_BASE + idx + 1000 * seed_shift, sh["F"], sh["nv"], sh["t"],
+                                sh["emax"], sh["B"], with_planted=False)
+
+
+def work_model(ts, B, nv, newton=True, balanced=False):
+    """Algorithmic multiplier-pipe instructions, total and for the node-solve kernel."""
+    t2 = float(sum(int(t) * int(t) for t in ts))
+    T = float(sum(int(t) for t in ts))
+    node_solve = t2 * (2 * C_MM + B * C_MAC)
+    total = node_solve + C_MAC * t2 / 2 + C_MM * ((nv - 1) * T + (3 + B) * T)
+    if newton:
+        total += C_MM * T * B * (B - 1) / 2
+    if balanced:
+        total += C_MM * t2
+    return total, node_solve
+
+
+# ---------------------------------------------------------------------------------------- ours
+def run_ours(args):
+    import torch
+
+    from paper_2505_24256_b200 import api
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    api.lib()
+    idx = args.config
+    w = load_workload(idx, rank, args.F)
+    stream = torch.cuda.Stream()
+    K, W = args.steps, args.warmup
+
+    # ---- resident inputs and the step closure --------------------------------------------------
+    if idx == 4:
+        parts = [w.num, w.den]
+        B, nv, F = w.num.B, w.num.nv, w.num.F
+        ts = [500] * F + [200] * F
+        dev = []
+        for q in parts:
+            dev.append(dict(exps=api.to_dev(q.exps), offsets=q.offsets, skel=api.to_dev(q.meta["skel_standin"]),
+                            uvals=api.to_dev(q.vals), out=torch.empty(q.vals.shape, dtype=torch.int64, device="cuda")))
+        anchors, samples = api.to_dev(w.num.anchors), api.to_dev(w.num.samples)
+        ws = api.alloc_workspace(w.num.offsets, B, api.WS_BALANCED)
+        status = torch.empty(2 * F, dtype=torch.int32, device="cuda")
+        T_tot = w.num.T_tot + w.den.T_tot
+        p = w.num.p
+
+        def step():
+            api.balanced_zippel_lift_step(dev[0], dev[1], anchors, samples, p, 0, 1, status=status, workspace=ws,
+                                          stream=stream)
+        total_ops, ns_ops = work_model(ts, B, nv, True, True)
+        workload = f"C4 balanced lift 5->6 vars: F={F} rational functions, t_N=500, t_D=200, B=25"
+        in_bytes = sum(q.exps.nbytes + q.vals.nbytes + q.meta["skel_standin"].nbytes for q in parts)
+        out_bytes = sum(q.vals.nbytes for q in parts)
+    else:
+        B, nv, F, T_tot, p = w.B, w.nv, w.F, w.T_tot, w.p
+        ts = np.diff(w.offsets)
+        exps, anchors, samples, vals = (api.to_dev(x) for x in (w.exps, w.anchors, w.samples, w.vals))
+        out = torch.empty_like(vals)
+        status = torch.empty(F, dtype=torch.int32, device="cuda")
+        ws = api.alloc_workspace(w.offsets, B)
+        newton = idx != 5
+        if newton:
+            def step():
+                api.zippel_lift_step(exps, w.offsets, anchors, samples, vals, p, 0, 1, out=out, status=status,
+                                     workspace=ws, stream=stream)
+        else:
+            nodes = torch.empty(T_tot, dtype=torch.int64, device="cuda")
+
+            def step():
+                api.zippel_eval_nodes(exps, anchors, p, out=nodes, stream=stream)
+                api.vandermonde_solve_batch(nodes, w.offsets, vals, p, 0, out=out, status=status, workspace=ws,
+                                            stream=stream)
+        total_ops, ns_ops = work_model(ts, B, nv, newton, False)
+        workload = (f"C{idx} {'lift' if newton else 'solve'}: F={F}, t={int(ts.max())}, nv={nv}, B={B}"
+                    + (" (BASELINE.json configs[1])" if idx == 2 and not args.F else ""))
+        in_bytes = w.exps.nbytes + w.vals.nbytes + w.anchors.nbytes + w.samples.nbytes
+        out_bytes = w.vals.nbytes + 4 * F
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+
+            dist.barrier()
+
+    # ---- warm-up, then K timed steps (device-resident) ----------------------------------------
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            step()
+        torch.cuda.synchronize()
+        st_host = status.cpu().numpy()
+        assert not st_host.any(), f"data-dependent failure in the synthetic batch: {st_host[st_host != 0][:4]}"
+        ev_k = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        for a, b in ev_k:
+            a.record(stream); b.record(stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(local) if rank == 0 else None
+        time.sleep(0.3 if sampler else 0.0)
+        barrier()
+        torch.cuda.synchronize()
+        n0 = api.zippel_launch_count()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for i in range(K):
+            api.zippel_profile_events(api.K_NODE_SOLVE, ev_k[i][0], ev_k[i][1])
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        t1 = time.perf_counter()
+        api.zippel_profile_events(0)
+        launches = api.zippel_launch_count() - n0
+        clocks = sampler.stop(t0, t1) if sampler else None
+        ms = e0.elapsed_time(e1)
+        ns_ms = sum(a.elapsed_time(b) for a, b in ev_k) / K
+    if world > 1:
+        import torch.distributed as dist
+
+        tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    ms_per_step = ms / K
+    terms = B * T_tot * world
+    value = terms / (ms_per_step * 1e-3)
+
+    # ---- e2e: host (pinned) buffers through the host-buffer C-ABI call ---------------------------
+    e2e = None
+    if not args.no_e2e and idx != 4 and idx != 5:
+        pin = lambda a: torch.from_numpy(a.view(np.int64) if a.dtype == np.uint64 else a.view(np.int16)).pin_memory()
+        h_exps, h_anch, h_samp, h_vals = pin(w.exps), pin(w.anchors), pin(w.samples), pin(w.vals)
+        h_out = torch.empty(w.vals.shape, dtype=torch.int64).pin_memory()
+        h_st = torch.empty(F, dtype=torch.int32).pin_memory()
+        hws = torch.empty(api.host_workspace_bytes(w.offsets, nv, B), dtype=torch.uint8, device="cuda")
+
+        def estep():
+            api.zippel_lift_step_host(h_exps, w.offsets, h_anch, h_samp, h_vals, p, h_out, h_st, hws, 0, 1, stream=stream)
+            stream.synchronize()  # the user reads the result of every step
+
+        for _ in range(max(1, min(W, 2))):
+            estep()
+        barrier()
+        torch.cuda.synchronize()
+        ta = time.perf_counter()
+        for _ in range(K):
+            estep()
+        torch.cuda.synchronize()
+        tb = time.perf_counter()
+        ems = (tb - ta) * 1e3
+        if world > 1:
+            import torch.distributed as dist
+
+            tt = torch.tensor([ems], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            ems = float(tt.item())
+        assert not h_st.numpy().any()
+        e2e = {"value": terms / (ems / K * 1e-3), "unit": UNIT, "ms_per_step": ems / K,
+               "h2d_bytes_per_step": int(in_bytes), "d2h_bytes_per_step": int(out_bytes),
+               "call": "zippel_lift_step_host (pinned host buffers; H2D + step + D2H + stream sync per step)"}
+
+    if rank != 0:
+        if world > 1:
+            import torch.distributed as dist
+
+            dist.destroy_process_group()
+        return
+
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) -------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_sample(idx, steps=1)
+
+    achieved = ns_ops / (ns_ms * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u64", "data": "synthetic",
+        "config": {"workload": workload, "p": "2^63-25", "basis": "monomial", "functions_per_gpu": int(F),
+                   "terms_per_gpu": int(T_tot), "l2": "inputs larger than L2 (688 MB of values per step)" if idx == 2
+                   else "inputs smaller than L2; compute-bound kernels (see DESIGN.md)", "parallelism": f"dp{world}"},
+        "lift_steps_per_s": F * world / (ms_per_step * 1e-3),
+        "credited_modmuls_per_s": B * float(sum(int(t) ** 2 for t in ts)) * world / (ms_per_step * 1e-3),
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {
+            "bound": "alu", "kernel": "k_node_solve", "achieved": achieved, "peak": IMAD_PEAK_TOPS,
+            "unit": "T 32-bit multiplier instr/s (lane-ops)", "frac": achieved / IMAD_PEAK_TOPS, "traffic": None,
+            "peak_source": "derived: 148 SM x 64 IMAD lanes/clk x 1.965 GHz (DESIGN.md); micro-benchmark reached 95-98% of it",
+            "algorithmic_ops_per_launch": ns_ops, "ms_per_launch": ns_ms,
+            "whole_step_frac": total_ops / (ms_per_step * 1e-3) / 1e12 / IMAD_PEAK_TOPS,
+        },
+        "e2e": e2e,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------- oracle legs
+SAMPLE = {1: dict(), 2: dict(F=32), 3: dict(t=6000), 4: dict(F=24), 5: dict(t=1 << 14)}
+
+
+def oracle_step(idx, w):
+    from oracle import ref
+
+    if idx == 4:
+        parts = {n: dict(exps=q.exps, offsets=q.offsets, skel=q.meta["skel_standin"], uvals=q.vals)
+                 for n, q in (("num", w.num), ("den", w.den))}
+        ref.balanced_zippel_lift_step(parts["num"], parts["den"], w.num.anchors, w.num.samples, w.num.p, 0, 1)
+        return w.num.B * (w.num.T_tot + w.den.T_tot), w.num.F
+    if idx == 5:
+        nodes = ref.eval_nodes(w.exps, w.anchors, w.p)
+        ref.vandermonde_solve_batch(nodes, w.offsets, w.vals, w.p, 0)
+    else:
+        ref.zippel_lift_step(w.exps, w.offsets, w.anchors, w.samples, w.vals, w.p, 0, 1)
+    return w.B * w.T_tot, w.F
+
+
+def oracle_sample(idx, steps=1, warmup=0):
+    """Time the oracle, as it stands (single thread, unsigned __int128 mulmod), on a bounded sample of the
+    bench workload.  The metric is terms/s AT THE SAMPLE'S t; for configs 3 and 5 the sample has a shorter
+    skeleton, so the value is also given scaled by (t_sample / t_full) (cost per term is linear in t)."""
+    from oracle import ref
+    from paper_2505_24256_b200 import workloads as wl
+
+    ref.lib()
+    w = wl.config(idx, **SAMPLE[idx])
+    for _ in range(warmup):
+        oracle_step(idx, w)
+    ta = time.perf_counter()
+    for _ in range(steps):
+        terms, F = oracle_step(idx, w)
+    dt = (time.perf_counter() - ta) / steps
+    full_t = wl.CONFIG_SHAPES[idx].get("t")
+    samp_t = SAMPLE[idx].get("t")
+    scale = (samp_t / full_t) if (samp_t and full_t) else 1.0
+    desc = {2: "first 32 of the 4096 functions (same t = 1000, B = 21)", 4: "first 24 of the 1024 functions",
+            3: "6000-term prefix as a complete problem, value scaled by 6000/100000",
+            5: "2^14-term prefix as a complete problem (BASELINE.json), value scaled by 2^14/2^19",
+            1: "the whole config"}[idx]
+    return {"value": terms / dt * scale, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+            "seconds_per_sample_step": dt, "lift_steps_per_s": F / dt * (scale * scale if scale != 1.0 else 1.0)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cpu = oracle_sample(args.config, steps=args.steps, warmup=min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": cpu["seconds_per_sample_step"] * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+        "config": {"workload": f"C{args.config} via the CPU oracle; each step = {cpu['sample']}", "p": "2^63-25"},
+        "cpu_baseline": cpu,
+        "e2e": {"value": cpu["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

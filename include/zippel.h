@@ -127,6 +127,20 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
                               const uint64_t* samples, int B, int s0, uint64_t p, int basis, int32_t* status,
                               void* workspace, size_t workspace_bytes, void* stream);
 
+/* Measurement hook (bench.py's roofline leg): when kernel != 0, every later call records the CUDA event
+ * `ev_start` on its stream right before the first launch of that kernel and `ev_stop` right after the
+ * last one (cudaEvent_t passed as void*; the caller owns them).  kernel: ZP_K_* below; 0 switches the
+ * hook off.  The only process-wide state in the library; not thread-safe; nothing else changes. */
+#define ZP_K_EVAL_NODES 1
+#define ZP_K_MASTER_POLY 2
+#define ZP_K_NODE_SOLVE 3
+#define ZP_K_NEWTON 5
+#define ZP_K_POWER_SUMS 6
+#define ZP_K_BALANCE 7
+int zippel_profile_events(int kernel, void* ev_start, void* ev_stop);
+/* Number of kernels this library has enqueued in this process so far (bench.py's gpu_launches). */
+unsigned long long zippel_launch_count(void);
+
 /* Self-test hook for the arithmetic substrate (a0), section 2.1: out[i] = op(a[i], b[i]) mod p,
  * op: 0 mul, 1 add, 2 sub, 3 pow (b = exponent), 4 inverse of a (0 -> 0),
  *     5 deferred dot: out[0] = sum_i a[i]*b[i] mod p through the 160-bit accumulator. */

@@ -27,8 +27,10 @@ MAX_NV, MAX_B = 32, 64
 EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
-    "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes",
+    "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
+    "zippel_launch_count",
 )
+K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
 
 class ZippelError(RuntimeError):
@@ -67,6 +69,9 @@ def lib() -> C.CDLL:
         L.balanced_zippel_lift_step.argtypes = [C.POINTER(_Part), C.POINTER(_Part), i32, i32, vp, vp, i32, i32,
                                                 u64, i32, vp, vp, sz, vp]
         L.zippel_modarith_selftest.argtypes = [i32, vp, vp, i64, u64, vp, vp]
+        L.zippel_profile_events.argtypes = [i32, vp, vp]
+        L.zippel_launch_count.restype = C.c_ulonglong
+        L.zippel_launch_count.argtypes = []
         _lib = L
     return _lib
 
@@ -285,3 +290,21 @@ def zippel_lift_step_host(h_exps: torch.Tensor, offsets, h_anchors: torch.Tensor
                                        h_out.data_ptr(), h_status.data_ptr(), _ptr(workspace), workspace.numel(),
                                        _stream(stream)), "zippel_lift_step_host")
     return h_out, h_status
+
+
+def zippel_profile_events(kernel: int, ev_start: Optional[torch.cuda.Event] = None,
+                          ev_stop: Optional[torch.cuda.Event] = None):
+    """Measurement hook: later calls record ev_start / ev_stop around the launches of `kernel` (K_* above);
+    kernel = 0 switches it off.  The events must be created with enable_timing=True."""
+    if kernel:
+        for ev in (ev_start, ev_stop):
+            if not ev.cuda_event:  # torch creates the CUDA event lazily
+                ev.record()
+        _check(lib().zippel_profile_events(kernel, ev_start.cuda_event, ev_stop.cuda_event), "zippel_profile_events")
+    else:
+        _check(lib().zippel_profile_events(0, None, None), "zippel_profile_events")
+
+
+def zippel_launch_count() -> int:
+    """Kernels enqueued by the library in this process so far."""
+    return int(lib().zippel_launch_count())

@@ -82,6 +82,21 @@ bool check_offsets(const int64_t* h, int F, int64_t* T_tot, int64_t* tmax) {
   return true;
 }
 
+// ---- measurement hook (zippel_profile_events) ----------------------------------------------------
+unsigned long long g_launches = 0;  // kernels enqueued by this library in this process
+int g_prof_kernel = 0;
+cudaEvent_t g_prof_start = nullptr, g_prof_stop = nullptr;
+struct ProfScope {  // records start at construction and stop at destruction when `kernel` is the hooked one
+  bool on;
+  cudaStream_t st;
+  ProfScope(int kernel, cudaStream_t s) : on(kernel == g_prof_kernel && g_prof_start && g_prof_stop), st(s) {
+    if (on) cudaEventRecord(g_prof_start, st);
+  }
+  ~ProfScope() {
+    if (on) cudaEventRecord(g_prof_stop, st);
+  }
+};
+
 inline int cuda_ok() { return cudaGetLastError() == cudaSuccess ? ZP_OK : ZP_ERR_CUDA; }
 inline unsigned grid_y(int F) { return (unsigned)(F < 65535 ? F : 65535); }
 
@@ -93,9 +108,9 @@ void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* n
                        const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k,
                        uint64_t* scale, uint64_t* coefs, int32_t* status) {
   if (first)
-    k_node_solve<NB, true><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+    ++g_launches, k_node_solve<NB, true><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
   else
-    k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+    ++g_launches, k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
 }
 
 void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const uint64_t* M,
@@ -116,12 +131,13 @@ void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const u
 // (a2) master polynomial of every function -> returns the buffer holding M' (Montgomery)
 const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64_t tmax, const ZpMod& k,
                                 cudaStream_t st) {
+  ProfScope prof(ZP_K_MASTER_POLY, st);
   dim3 g((unsigned)((tmax + ZP_LEAF - 1) / ZP_LEAF), grid_y(F));
-  k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes, w.d_offsets, F, k, w.M0);
+  ++g_launches, k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes, w.d_offsets, F, k, w.M0);
   uint64_t *src = w.M0, *dst = w.M1;
   for (int64_t a = ZP_LEAF; a < tmax; a <<= 1) {
     dim3 gl((unsigned)((tmax + ZP_K2_THREADS - 1) / ZP_K2_THREADS), grid_y(F));
-    k_tree_level<<<gl, ZP_K2_THREADS, 0, st>>>(src, w.d_offsets, F, a, k, dst);
+    ++g_launches, k_tree_level<<<gl, ZP_K2_THREADS, 0, st>>>(src, w.d_offsets, F, a, k, dst);
     uint64_t* tmp = src;
     src = dst;
     dst = tmp;
@@ -132,10 +148,11 @@ const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64
 // (a2)-(a4): solve into coefs; per-function codes into w.st_solve (NONE = ok)
 void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
                int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
-  k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
+  ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
   const uint64_t* M = run_master_poly(w, nodes, F, tmax, k, st);
   const int passes = (B + ZP_NB_MAX - 1) / ZP_NB_MAX;
   const int per = (B + passes - 1) / passes;
+  ProfScope prof(ZP_K_NODE_SOLVE, st);
   dim3 g((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
   for (int b0 = 0, pass = 0; b0 < B; b0 += per, ++pass) {
     const int nb = (B - b0 < per) ? (B - b0) : per;
@@ -147,13 +164,14 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
 // (a5): Newton on [B x n] with leading dimension ld; code into w.st_newton[0]
 void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* vals, int64_t n, int64_t ld,
                 const ZpMod& k, int basis, uint64_t* out, cudaStream_t st) {
-  k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
-  k_newton_prep<<<(B * B + 127) / 128, 128, 0, st>>>(samples, B, k, w.invd, w.smont, w.st_newton);
+  ++g_launches, k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
+  ++g_launches, k_newton_prep<<<(B * B + 127) / 128, 128, 0, st>>>(samples, B, k, w.invd, w.smont, w.st_newton);
+  ProfScope prof(ZP_K_NEWTON, st);
   const size_t smem = 8 * ((size_t)B * B + B + 2 * (size_t)B * ZP_K5_THREADS);
   cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
   if (blocks > 148 * 64) blocks = 148 * 64;
-  k_newton<<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
+  ++g_launches, k_newton<<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
 }
 
 void upload_offsets(const Ws& w, const int64_t* h_offsets, int F, cudaStream_t st) {
@@ -162,15 +180,17 @@ void upload_offsets(const Ws& w, const int64_t* h_offsets, int F, cudaStream_t s
 
 void run_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t* anchors, const ZpMod& k,
                     uint64_t* nodes, cudaStream_t st) {
+  ProfScope prof(ZP_K_EVAL_NODES, st);
   int64_t blocks = (T_tot + ZP_K1_THREADS - 1) / ZP_K1_THREADS;
   if (blocks > 148 * 16) blocks = 148 * 16;
-  k_eval_nodes<<<(unsigned)blocks, ZP_K1_THREADS, 0, st>>>(exps, T_tot, nv, anchors, k, nodes);
+  ++g_launches, k_eval_nodes<<<(unsigned)blocks, ZP_K1_THREADS, 0, st>>>(exps, T_tot, nv, anchors, k, nodes);
 }
 
 void run_power_sums(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* coef,
                     int B, int s0, const ZpMod& k, uint64_t* out, cudaStream_t st) {
+  ProfScope prof(ZP_K_POWER_SUMS, st);
   dim3 g((unsigned)((tmax + ZP_K6_THREADS - 1) / ZP_K6_THREADS), grid_y(F));
-  k_power_sums<<<g, ZP_K6_THREADS, 0, st>>>(nodes, w.d_offsets, F, coef, T_tot, B, s0, k, out);
+  ++g_launches, k_power_sums<<<g, ZP_K6_THREADS, 0, st>>>(nodes, w.d_offsets, F, coef, T_tot, B, s0, k, out);
 }
 
 bool ws_ok(const void* ws, size_t have, size_t need) {
@@ -251,7 +271,7 @@ int vandermonde_solve_batch(const uint64_t* nodes, const int64_t* h_offsets, int
   cudaStream_t st = (cudaStream_t)stream;
   upload_offsets(w, h_offsets, F, st);
   run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
-  k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, nullptr, F, status);
+  ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, nullptr, F, status);
   return cuda_ok();
 }
 
@@ -268,7 +288,7 @@ int newton_interp_batch(const uint64_t* samples, int B, const uint64_t* vals, in
   (void)one;
   cudaStream_t st = (cudaStream_t)stream;
   run_newton(w, samples, B, vals, n, ld, k, basis, out, st);
-  k_status_finish<<<1, 32, 0, st>>>(nullptr, nullptr, w.st_newton, 1, status);
+  ++g_launches, k_status_finish<<<1, 32, 0, st>>>(nullptr, nullptr, w.st_newton, 1, status);
   return cuda_ok();
 }
 
@@ -290,7 +310,7 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
   run_eval_nodes(exps, T_tot, nv, anchors, k, nodes, st);
   run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, out, st);
   run_newton(w, samples, B, out, T_tot, T_tot, k, basis, out, st);
-  k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, w.st_newton, F, status);
+  ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, w.st_newton, F, status);
   return cuda_ok();
 }
 
@@ -358,17 +378,30 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
     const zp_part* q = parts[x];
     const Ws w = carve(workspace, T_tot[x], F, B, ZP_WS_BALANCED);
     upload_offsets(w, q->h_offsets, F, st);
-    k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
+    ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
     run_eval_nodes(q->exps, T_tot[x], nv, anchors, k, w.nodes, st);
     run_power_sums(w, w.nodes, F, T_tot[x], tmax[x], q->skel, 1, s0, k, w.R, st);
     int64_t blocks = (T_tot[x] + 255) / 256;
     if (blocks > 148 * 32) blocks = 148 * 32;
-    k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
+    {
+      ProfScope prof(ZP_K_BALANCE, st);
+      ++g_launches, k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
+    }
     run_solve(w, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
     run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st);
-    k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
+    ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
   }
   return cuda_ok();
+}
+
+unsigned long long zippel_launch_count(void) { return g_launches; }
+
+int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
+  if (kernel < 0 || kernel > 7 || (kernel != 0 && (!ev_start || !ev_stop))) return ZP_ERR_ARG;
+  g_prof_kernel = kernel;
+  g_prof_start = kernel ? (cudaEvent_t)ev_start : nullptr;
+  g_prof_stop = kernel ? (cudaEvent_t)ev_stop : nullptr;
+  return ZP_OK;
 }
 
 int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
@@ -377,11 +410,11 @@ int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64
   if (!a || !out || n <= 0 || op < 0 || op > 5 || !make_mod(p, &k) || ((op <= 3 || op == 5) && !b)) return ZP_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (op == 5) {
-    k_modarith_selftest<<<1, 256, 0, st>>>(op, a, b, n, k, out);
+    ++g_launches, k_modarith_selftest<<<1, 256, 0, st>>>(op, a, b, n, k, out);
   } else {
     int64_t blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    k_modarith_selftest<<<(unsigned)blocks, 256, 0, st>>>(op, a, b, n, k, out);
+    ++g_launches, k_modarith_selftest<<<(unsigned)blocks, 256, 0, st>>>(op, a, b, n, k, out);
   }
   return cuda_ok();
 }
