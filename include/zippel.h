@@ -143,9 +143,17 @@ unsigned long long zippel_launch_count(void);
 
 /* Self-test hook for the arithmetic substrate (a0), section 2.1: out[i] = op(a[i], b[i]) mod p,
  * op: 0 mul, 1 add, 2 sub, 3 pow (b = exponent), 4 inverse of a (0 -> 0),
- *     5 deferred dot: out[0] = sum_i a[i]*b[i] mod p through the 160-bit accumulator. */
+ *     5 deferred dot: out[0] = sum_i a[i]*b[i] mod p through the 160-bit accumulator,
+ *     6 Horner step: out[i] = (b[i] * a[i] + a[(i+1) % n]) mod p, where the multiplicand a[i] is taken as a
+ *       LAZY value (any 64-bit number, not reduced first) -- the hot recurrence of (a3). */
 int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
                              void* stream);
+
+/* Roofline micro-benchmarks of the integer multiplier pipe:
+ * launches `blocks` CTAs of 256 lanes, each running `iters` x 64 statements of `kind` per chain group
+ * (kinds: csrc/ubench.cuh).  out: device scratch [blocks * 256].  *h_chain_steps (host, optional)
+ * receives the number of lane-statements executed, for the caller to divide by its event time. */
+int zippel_ubench(int kind, int iters, int blocks, uint64_t p, uint64_t* out, double* h_chain_steps, void* stream);
 
 #ifdef __cplusplus
 }

@@ -28,7 +28,7 @@ EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
     "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
-    "zippel_launch_count",
+    "zippel_launch_count", "zippel_ubench",
 )
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
                                                 u64, i32, vp, vp, sz, vp]
         L.zippel_modarith_selftest.argtypes = [i32, vp, vp, i64, u64, vp, vp]
         L.zippel_profile_events.argtypes = [i32, vp, vp]
+        L.zippel_ubench.argtypes = [i32, i32, i32, u64, vp, C.POINTER(C.c_double), vp]
         L.zippel_launch_count.restype = C.c_ulonglong
         L.zippel_launch_count.argtypes = []
         _lib = L
@@ -308,3 +309,11 @@ def zippel_profile_events(kernel: int, ev_start: Optional[torch.cuda.Event] = No
 def zippel_launch_count() -> int:
     """Kernels enqueued by the library in this process so far."""
     return int(lib().zippel_launch_count())
+
+
+def zippel_ubench(kind: int, iters: int, blocks: int, p: int, out: torch.Tensor, stream=None) -> float:
+    """Enqueue one micro-benchmark launch (csrc/ubench.cuh); returns the lane-statements it executes."""
+    _need_cuda()
+    n = C.c_double(0.0)
+    _check(lib().zippel_ubench(kind, iters, blocks, p, _ptr(out), C.byref(n), _stream(stream)), "zippel_ubench")
+    return n.value

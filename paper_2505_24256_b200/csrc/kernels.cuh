@@ -117,14 +117,41 @@ k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offse
 }
 
 // ------------------------------------------------------------------------------------------------
+// (a3) prologue k_solve_table: per coefficient l of every master polynomial, the 32-byte record the hot
+// loop broadcasts:  { M_l, M_l', D_l, D_l' }  with D_l = l M_l (coefficient of M'(z) at z^(l-1)) and
+// w' = floor(w 2^64 / p) the Shoup companion (modarith.cuh).  Input: the product tree's M~ (Montgomery).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F, ZpMod k,
+              ulonglong4* __restrict__ tab) {
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int64_t t = offsets[f + 1] - off;
+    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < t; l += (int64_t)gridDim.x * blockDim.x) {
+      const uint64_t Mm = Mt[off + l];
+      const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)l % k.p, k), k);  // (l M_l)~
+      ulonglong4 r;
+      r.x = from_mont(Mm, k);
+      r.y = shoup_companion(Mm, k);
+      r.z = from_mont(Dm, k);
+      r.w = shoup_companion(Dm, k);
+      tab[off + l] = r;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // (a3)+(a4) K3 node_solve: the hot loop (PAPER.md L189-197 ZippelMultiplePrime(), L203-213).
-// One lane per node i of one function; the CTA streams tiles of M and of the NB right-hand sides
-// through shared memory (every lane needs the same M_l, v_{b,l}: warp-uniform broadcast reads).
-// Per lane, l = t-1 .. 0 with q = q_l (q_{t-1} = 1):
-//     acc_b += q * v_{b,l}                    NB deferred MACs   (L194-195 "vector of powers" x "values")
-//     q <- M_l + m q ; d <- d m + q   (l >= 1)   2 Montgomery products (L193 Horner / synthetic division)
-// then  c_{b,i} = acc_b / d  [ / m if s0 = 1 ]   (L196), d = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15).
-// Nothing of length t is stored per lane (reading G7).
+// One lane per node i of one function; the CTA streams tiles of the table above and of the NB right-hand
+// sides through shared memory (every lane needs the same M_l, v_{b,l}: warp-uniform broadcast reads).
+// Per lane, l = t-1 .. 0 with q = q_l (q_{t-1} = 1) and d (= t at the start):
+//     acc_b += q * v_{b,l}                       NB deferred MACs (L194-195 "vector of powers" x "values", L205-209)
+//     q <- M_l + m q ;  d <- D_l + m d   (l >= 1)   2 Horner steps (L193: synthetic division; Horner of M')
+// then  c_{b,i} = acc_b / d  [ / m if s0 = 1 ]   (L196).  d = M'(m_i) = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15):
+// the paper's "polynomial value computed via Horner's method"; running Horner on M' instead of on the
+// quotient gives the same number and keeps the two chains independent (twice the ILP).
+// All values are plain residues; q and d stay lazy in [0, 2p) (horner_step), nothing of length t is
+// stored per lane (reading G7).
 // Template NB = right-hand sides handled per pass; FIRST = this pass computes d and writes scale.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K3_THREADS 128
@@ -132,11 +159,11 @@ k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offse
 
 template <int NB, bool FIRST>
 __global__ void __launch_bounds__(ZP_K3_THREADS)
-k_node_solve(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ M, const int64_t* __restrict__ offsets,
+k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
              int F, const uint64_t* __restrict__ vals, int64_t T_tot, int b0, int s0, ZpMod k,
              uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
   constexpr int NBP = (NB + 1) & ~1;  // row stride (even: 16-byte aligned pairs)
-  __shared__ __align__(16) uint64_t sM[ZP_K3_TILE];
+  __shared__ __align__(16) ulonglong4 sT[ZP_K3_TILE];
   __shared__ __align__(16) uint64_t sV[ZP_K3_TILE * NBP];
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
@@ -145,22 +172,25 @@ k_node_solve(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ M,
     if (i0 >= t) continue;  // uniform per CTA
     const int i = i0 + threadIdx.x;
     const bool live = i < t;
-    const uint64_t m = live ? to_mont(nodes[off + i] % k.p, k) : 0;
-    uint64_t q = k.r1, d = k.r1;
+    const uint64_t m = live ? nodes[off + i] % k.p : 0;
+    const uint64_t mm = to_mont(m, k);
+    const uint64_t mp = shoup_companion(mm, k);
+    uint64_t q = 1 % k.p, d = (uint64_t)t % k.p;
     Acc acc[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) acc_zero(acc[b]);
-    const uint64_t* Mf = M + off;
+    const ulonglong4* Tf = tab + off;
     for (int l1 = t; l1 > 0; l1 -= ZP_K3_TILE) {  // tile covers l in [l0, l1)
       const int l0 = l1 - ZP_K3_TILE > 0 ? l1 - ZP_K3_TILE : 0;
       const int n = l1 - l0;
       __syncthreads();
-      for (int x = threadIdx.x; x < n; x += ZP_K3_THREADS) sM[x] = Mf[l0 + x];
+      for (int x = threadIdx.x; x < n; x += ZP_K3_THREADS) sT[x] = Tf[l0 + x];
       for (int x = threadIdx.x; x < n * NB; x += ZP_K3_THREADS) {
         const int b = x / n, s = x - b * n;
         sV[s * NBP + b] = vals[(int64_t)(b0 + b) * T_tot + off + l0 + s];
       }
       __syncthreads();
+#pragma unroll 2
       for (int s = n - 1; s >= 0; --s) {
 #pragma unroll
         for (int b = 0; b < NB; b += 2) {
@@ -173,17 +203,22 @@ k_node_solve(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ M,
           }
         }
         if (l0 + s >= 1) {
-          q = mod_add(mont_mul(m, q, k), sM[s], k.p);
-          if (FIRST) d = mod_add(mont_mul(d, m, k), q, k.p);
+          const ulonglong2 tq = *reinterpret_cast<const ulonglong2*>(&sT[s].x);
+          q = horner_step(q, m, mp, tq.x, tq.y, k);
+          if (FIRST) {
+            const ulonglong2 td = *reinterpret_cast<const ulonglong2*>(&sT[s].z);
+            d = horner_step(d, m, mp, td.x, td.y, k);
+          }
         }
       }
     }
     if (live) {
       uint64_t sc;
       if (FIRST) {
-        const uint64_t dd = s0 ? mont_mul(d, m, k) : d;
+        const uint64_t dm = to_mont(lazy_canon(d, k.p), k);
+        const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
         if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-        sc = mont_mul(mont_inv(dd, k), k.c160, k);  // plain d^-1 * 2^160
+        sc = mont_mul(mont_inv(dd, k), k.c224, k);  // plain d^-1 * 2^224: acc_redc160 (x 2^-160) and mont_mul (x 2^-64) undo it
         if (scale) scale[off + i] = sc;
       } else {
         sc = scale[off + i];
@@ -378,6 +413,10 @@ __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b
     if (op == 2) r = mod_sub(x, y % k.p, k.p);
     if (op == 3) r = from_mont(mont_pow(to_mont(x, k), y, k), k);
     if (op == 4) r = from_mont(mont_inv(to_mont(x, k), k), k);
+    if (op == 6) {  // Horner step on a LAZY x (any 64-bit value): (y x + a[(i+1) % n]) mod p
+      const uint64_t m = y % k.p, ad = a[(i + 1) % n] % k.p;
+      r = lazy_canon(horner_step(a[i], m, shoup_companion(to_mont(m, k), k), ad, shoup_companion(to_mont(ad, k), k), k), k.p);
+    }
     out[i] = r;
   }
 }

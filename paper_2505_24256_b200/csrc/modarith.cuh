@@ -25,6 +25,8 @@ struct ZpMod {
   uint64_t c160;    // 2^160 mod p : mont_mul(acc_redc160(sum of mont*mont), c160) -> Montgomery
                     //               mont_mul(acc_redc160(sum of mont*plain), c160) -> plain
   uint64_t c224;    // 2^224 mod p : mont_mul(acc_redc160(sum of mont*plain), c224) -> Montgomery
+  uint64_t np;      // 2^64 - p          : x + q*np = x - q*p  (mod 2^64)
+  uint64_t ninv64;  // -p^{-1} mod 2^64  : shoup_companion
 };
 
 #if defined(__CUDACC__)
@@ -38,6 +40,12 @@ ZP_DEV uint64_t zp_mulw(uint32_t a, uint32_t b) {
 ZP_DEV uint64_t zp_madw(uint32_t a, uint32_t b, uint64_t c) {
   uint64_t r;
   asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
+  return r;
+}
+
+ZP_DEV uint32_t zp_madlo(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t r;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
   return r;
 }
 
@@ -103,6 +111,56 @@ ZP_DEV uint64_t mont_pow(uint64_t x, uint64_t e, const ZpMod& k) {
 }
 // Inverse by Fermat, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.
 ZP_DEV uint64_t mont_inv(uint64_t x, const ZpMod& k) { return mont_pow(x, k.p - 2, k); }
+
+// ---- Horner step with Shoup companions (the hot recurrence of (a3): q <- M_l + m q, d <- M'_l + m d) ----
+// For w in [0,p) its companion is w' = floor(w 2^64 / p) < 2^64.  Since w 2^64 - w~ = w' p with
+// w~ = w 2^64 mod p (the Montgomery form), w' = -w~ p^{-1} mod 2^64: one 64-bit low product.
+ZP_DEV uint64_t shoup_companion(uint64_t w_mont, const ZpMod& k) { return w_mont * k.ninv64; }
+
+// x <- m x + a (mod p), lazily: ANY x < 2^64 in, result in [0, 2p) (< 2^64 because p < 2^63).
+// With qq = floor((m' x + a') / 2^64):  (m x + a)/p = (m' x + a')/2^64 + (e1 x + e3)/2^64 with
+// e1, e3 in [0,1), so  u = m x + a - qq p = p (frac + (e1 x + e3)/2^64)  lies in [0, 2p) and is computed
+// exactly modulo 2^64.  No conditional correction and no Montgomery form: 10 multiplier instructions
+// (4 wide for the exact high half of m' x + a', 2 wide + 4 low for u) and 3 carry instructions.
+ZP_DEV uint64_t horner_step(uint64_t x, uint64_t m, uint64_t mp, uint64_t a, uint64_t ap, const ZpMod& k) {
+  const uint32_t w0 = (uint32_t)mp, w1 = (uint32_t)(mp >> 32), x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32);
+  const uint32_t m0 = (uint32_t)m, m1 = (uint32_t)(m >> 32);
+  const uint32_t np0 = (uint32_t)k.np, np1 = (uint32_t)(k.np >> 32);
+  const uint64_t Bm = zp_mulw(w0, x1);
+  uint32_t tlo, thi;
+  asm("{\n\t"
+      ".reg .u64 d, s;\n\t"
+      ".reg .u32 dlo, dhi, slo, shi, c0, c1, dummy;\n\t"
+      "mul.wide.u32 d, %2, %3;\n\t"
+      "add.cc.u64 d, d, %4;\n\t"  // D = w0 x0 + a'            carry c0 (weight 2^64)
+      "addc.u32 c0, 0, 0;\n\t"
+      "mul.wide.u32 s, %5, %3;\n\t"
+      "add.cc.u64 s, s, %6;\n\t"  // S = w1 x0 + w0 x1         carry c1 (weight 2^96)
+      "addc.u32 c1, 0, 0;\n\t"
+      "mov.b64 {dlo, dhi}, d;\n\t"
+      "mov.b64 {slo, shi}, s;\n\t"
+      "add.cc.u32 dummy, slo, dhi;\n\t"
+      "addc.cc.u32 %0, shi, c0;\n\t"
+      "addc.u32 %1, c1, 0;\n\t"
+      "}"
+      : "=r"(tlo), "=r"(thi)
+      : "r"(w0), "r"(x0), "l"(ap), "r"(w1), "l"(Bm));
+  const uint64_t qq = zp_madw(w1, x1, ((uint64_t)thi << 32) | tlo);
+  const uint32_t q0 = (uint32_t)qq, q1 = (uint32_t)(qq >> 32);
+  uint32_t uh = (uint32_t)(a >> 32);  // u = m x + a + qq np  (mod 2^64)
+  uh = zp_madlo(m0, x1, uh);
+  uh = zp_madlo(m1, x0, uh);
+  uh = zp_madlo(q0, np1, uh);
+  uh = zp_madlo(q1, np0, uh);
+  uint64_t u = ((uint64_t)uh << 32) | (uint32_t)a;
+  u = zp_madw(m0, x0, u);
+  u = zp_madw(q0, np0, u);
+  return u;
+}
+ZP_DEV uint64_t lazy_canon(uint64_t x, uint64_t p) {  // [0,2p) -> [0,p)
+  const uint64_t s = x - p;
+  return (x >= p) ? s : x;
+}
 
 // Deferred accumulator.  value = E + O * 2^32 with
 //   E = e0 + e1*2^64 + e2*2^128  (takes x0*y0 at bit 0 and x1*y1 at bit 64),

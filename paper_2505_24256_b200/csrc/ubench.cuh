@@ -1,0 +1,101 @@
+// ubench.cuh -- roofline micro-benchmarks for the 32-bit integer multiplier (fma-heavy) pipe of sm_100a.
+// the denominator of every reported fraction is measured, not assumed.  Each kernel
+// keeps CH independent chains per lane in registers, no memory traffic; the host (bench side) divides
+// lane-ops by elapsed time.  Kinds (ZP_UB_*):
+//   0 mad.lo.u32          IMAD            32x32+32 -> 32
+//   1 mad.wide.u32        IMAD.WIDE.U32   32x32+64 -> 64
+//   2 mad.hi.u32          IMAD.HI.U32     hi32(32x32)+32
+//   3 mad.wide + add.cc / addc chain (IMAD.WIDE with carry-out + IADD3.X): the deferred MAC (4 wide / MAC)
+//   4 add + xor           IADD3 + LOP3    (alu pipe; 2 per statement)
+//   5 mad.wide.u32 and IADD3 interleaved 1:1 (co-issue check)
+//   6 mad.lo.u32 and mad.wide.u32 interleaved 2:1
+//   7 the library's Horner step (horner_step, modarith.cuh): modular x <- m x + a with Shoup companions
+//   8 the library's Montgomery product (mont_mul)
+//   9 fma.rn.f64          DFMA            (fp64 pipe)
+//  10 DFMA and IMAD.WIDE interleaved 1:1 (do the fp64 and fma-heavy pipes overlap?)
+#pragma once
+#include "modarith.cuh"
+
+#define ZP_UB_THREADS 256
+#define ZP_UB_CH 8
+
+template <int KIND>
+__global__ void __launch_bounds__(ZP_UB_THREADS)
+k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
+  const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+  uint32_t a = tid * 2654435761u + 12345u, b = (tid ^ 0x9e3779b9u) | 1u;
+  uint64_t acc[ZP_UB_CH];
+  uint32_t car[ZP_UB_CH];
+#pragma unroll
+  for (int c = 0; c < ZP_UB_CH; ++c) {
+    acc[c] = ((uint64_t)(tid + c) << 32) | (a + c);
+    car[c] = c;
+  }
+  if (KIND == 7 || KIND == 8) {
+#pragma unroll
+    for (int c = 0; c < ZP_UB_CH; ++c) acc[c] %= k.p;
+  }
+  const double dk1 = 1.0 + 1e-9 * (double)(tid & 7), dk2 = 1e-3 * (double)(tid & 3);
+  uint64_t wacc[ZP_UB_CH];
+#pragma unroll
+  for (int c = 0; c < ZP_UB_CH; ++c) wacc[c] = acc[c] ^ 0x5555;
+  if (KIND == 9 || KIND == 10) {
+#pragma unroll
+    for (int c = 0; c < ZP_UB_CH; ++c) acc[c] = (uint64_t)__double_as_longlong(1.0 + (double)c);
+  }
+  const uint64_t m = (((uint64_t)a << 32) | b) % k.p;
+  const uint64_t mp = shoup_companion(to_mont(m, k), k);
+  const uint64_t ad = (((uint64_t)b << 32) | a) % k.p;
+  const uint64_t adp = shoup_companion(to_mont(ad, k), k);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int c = 0; c < ZP_UB_CH; ++c) {
+        // every multiplicand comes from the chain itself, so that nothing can be hoisted out of the loop
+        uint32_t lo = (uint32_t)acc[c];
+        const uint32_t nb = (uint32_t)(acc[(c + 1) % ZP_UB_CH] >> 32);  // neighbour chain's high word
+        if (KIND == 0) {
+          asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(lo) : "r"(b), "r"(a));
+          acc[c] = (acc[c] & 0xffffffff00000000ull) | lo;
+        } else if (KIND == 1) {
+          asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[c]) : "r"(nb), "r"(b));
+        } else if (KIND == 2) {
+          asm volatile("mad.hi.u32 %0, %0, %1, %2;" : "+r"(lo) : "r"(b), "r"(a));
+          acc[c] = (acc[c] & 0xffffffff00000000ull) | lo;
+        } else if (KIND == 3) {
+          asm volatile("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tadd.cc.u64 %0, %0, t;\n\taddc.u32 %1, %1, 0;\n\t}"
+                       : "+l"(acc[c]), "+r"(car[c]) : "r"(nb), "r"(b));
+        } else if (KIND == 4) {
+          asm volatile("add.u32 %0, %0, %1;" : "+r"(car[c]) : "r"(lo));
+          asm volatile("xor.b32 %0, %0, %1;" : "+r"(lo) : "r"(car[c]));
+          acc[c] = (acc[c] & 0xffffffff00000000ull) | lo;
+        } else if (KIND == 5) {
+          asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[c]) : "r"(nb), "r"(b));
+          asm volatile("add.u32 %0, %0, %1;" : "+r"(car[c]) : "r"(nb));
+        } else if (KIND == 6) {
+          asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[c]) : "r"(nb), "r"(b));
+          asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(car[c]) : "r"(b), "r"(lo));
+          asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(car[c]) : "r"(a), "r"(lo));
+        } else if (KIND == 9) {
+          double x = __longlong_as_double((long long)acc[c]);
+          asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x) : "d"(dk1), "d"(dk2));
+          acc[c] = (uint64_t)__double_as_longlong(x);
+        } else if (KIND == 10) {
+          double x = __longlong_as_double((long long)acc[c]);
+          asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x) : "d"(dk1), "d"(dk2));
+          acc[c] = (uint64_t)__double_as_longlong(x);
+          asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(wacc[c]) : "r"((uint32_t)(wacc[(c + 1) % ZP_UB_CH] >> 32)), "r"(b));
+        } else if (KIND == 7) {
+          acc[c] = horner_step(acc[c], m, mp, ad, adp, k);
+        } else if (KIND == 8) {
+          acc[c] = mont_mul(acc[c], m, k);
+        }
+      }
+    }
+  }
+  uint64_t s = 0;
+#pragma unroll
+  for (int c = 0; c < ZP_UB_CH; ++c) s += acc[c] + car[c] + (KIND == 10 ? wacc[c] : 0);
+  if (s == 0x123456789abcdefull) out[tid] = s;  // keeps the chains alive, practically never taken
+}

@@ -7,6 +7,7 @@
 
 #include "../../include/zippel.h"
 #include "kernels.cuh"
+#include "ubench.cuh"
 
 namespace {
 
@@ -31,6 +32,10 @@ bool make_mod(uint64_t p, ZpMod* k) {
   k->c96 = pow2(96);
   k->c160 = pow2(160);
   k->c224 = pow2(224);
+  k->np = 0ull - p;
+  uint64_t inv64 = 1;  // Newton: inv64 = p^-1 mod 2^64
+  for (int i = 0; i < 6; ++i) inv64 *= 2ull - p * inv64;
+  k->ninv64 = 0ull - inv64;
   return true;
 }
 
@@ -39,6 +44,7 @@ struct Ws {
   int64_t* d_offsets;
   int32_t *st_pre, *st_solve, *st_newton;
   uint64_t *nodes, *M0, *M1, *scale, *invd, *smont, *R, *V;
+  ulonglong4* tab;
   size_t bytes;
 };
 
@@ -60,6 +66,7 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
   w.M0 = (uint64_t*)take(8 * (size_t)T_tot);
   w.M1 = (uint64_t*)take(8 * (size_t)T_tot);
   w.scale = (uint64_t*)take(8 * (size_t)T_tot);
+  w.tab = (ulonglong4*)take(32 * (size_t)T_tot);
   w.invd = (uint64_t*)take(8 * (size_t)B * B);
   w.smont = (uint64_t*)take(8 * (size_t)B);
   w.R = (uint64_t*)take(8 * (size_t)T_tot);
@@ -104,7 +111,7 @@ inline unsigned grid_y(int F) { return (unsigned)(F < 65535 ? F : 65535); }
 #define ZP_NB_MAX 25
 
 template <int NB>
-void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const uint64_t* M,
+void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
                        const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k,
                        uint64_t* scale, uint64_t* coefs, int32_t* status) {
   if (first)
@@ -113,7 +120,7 @@ void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* n
     ++g_launches, k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
 }
 
-void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const uint64_t* M,
+void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
                          const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0,
                          const ZpMod& k, uint64_t* scale, uint64_t* coefs, int32_t* status) {
 #define ZP_CASE(N) \
@@ -149,7 +156,12 @@ const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64
 void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
                int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
   ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
-  const uint64_t* M = run_master_poly(w, nodes, F, tmax, k, st);
+  const uint64_t* Mt = run_master_poly(w, nodes, F, tmax, k, st);
+  {
+    dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
+    ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(Mt, w.d_offsets, F, k, w.tab);
+  }
+  const ulonglong4* M = w.tab;
   const int passes = (B + ZP_NB_MAX - 1) / ZP_NB_MAX;
   const int per = (B + passes - 1) / passes;
   ProfScope prof(ZP_K_NODE_SOLVE, st);
@@ -407,7 +419,7 @@ int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
 int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
                              void* stream) {
   ZpMod k;
-  if (!a || !out || n <= 0 || op < 0 || op > 5 || !make_mod(p, &k) || ((op <= 3 || op == 5) && !b)) return ZP_ERR_ARG;
+  if (!a || !out || n <= 0 || op < 0 || op > 6 || !make_mod(p, &k) || ((op <= 3 || op >= 5) && !b)) return ZP_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   if (op == 5) {
     ++g_launches, k_modarith_selftest<<<1, 256, 0, st>>>(op, a, b, n, k, out);
@@ -416,6 +428,17 @@ int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64
     if (blocks > 148 * 8) blocks = 148 * 8;
     ++g_launches, k_modarith_selftest<<<(unsigned)blocks, 256, 0, st>>>(op, a, b, n, k, out);
   }
+  return cuda_ok();
+}
+
+int zippel_ubench(int kind, int iters, int blocks, uint64_t p, uint64_t* out, double* h_chain_steps, void* stream) {
+  ZpMod k;
+  if (kind < 0 || kind > 10 || iters <= 0 || blocks <= 0 || !out || !make_mod(p, &k)) return ZP_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+#define ZP_UB(K) case K: ++g_launches, k_ubench<K><<<blocks, ZP_UB_THREADS, 0, st>>>(iters, k, out); break;
+  switch (kind) { ZP_UB(0) ZP_UB(1) ZP_UB(2) ZP_UB(3) ZP_UB(4) ZP_UB(5) ZP_UB(6) ZP_UB(7) ZP_UB(8) ZP_UB(9) ZP_UB(10) }
+#undef ZP_UB
+  if (h_chain_steps) *h_chain_steps = (double)blocks * ZP_UB_THREADS * (double)iters * 8.0 * ZP_UB_CH;
   return cuda_ok();
 }
 

@@ -72,6 +72,27 @@ def test_modarith_fuzz_vs_python(zp, p):
     assert [int(x) for x in got] == [pow(int(x), p - 2, p) for x in a[:m]]
 
 
+@pytest.mark.parametrize("p", PRIMES)
+def test_horner_step_lazy_operand_vs_python(zp, p):
+    """The hot recurrence x <- m x + a of (a3) (PAPER.md L193 Horner / synthetic division), with x a LAZY
+    value: any 64-bit number, in particular the extremes 2p-1, 2^64-1, and m, a at 0, 1, p-1."""
+    r = np.random.Generator(np.random.Philox(key=[11, p & 0xFFFF]))
+    n = 500_000
+    ex = sorted({0, 1, p - 1, p, p + 1, 2 * p - 1, 2 * p, (1 << 64) - 1, (1 << 64) - 2, 1 << 63, (1 << 63) - 1,
+                 (1 << 32) - 1, 1 << 32, 0xFFFFFFFF00000000, 0x00000000FFFFFFFF})
+    ev = edge_values(p)
+    xs = [x for x in ex for _ in ev]
+    ms = [m for _ in ex for m in ev]
+    x = np.concatenate([u64(xs), r.integers(0, 1 << 64, n, dtype=np.uint64)])
+    m = np.concatenate([u64(ms), r.integers(0, p, n, dtype=np.uint64)])
+    x[-8:] = u64([p - 1, 0, 1, p - 1, (1 << 64) - 1, p - 1, 2 * p - 1, p - 1])  # addend a[(i+1) % n] at its extremes too
+    m[-8:] = p - 1
+    got = zp.to_host(zp.zippel_modarith_selftest(6, zp.to_dev(x), zp.to_dev(m), p))
+    xo, mo = x.astype(object), m.astype(object)
+    ao = np.roll(xo, -1) % p
+    assert (got.astype(object) == (mo * xo + ao) % p).all()
+
+
 @pytest.mark.parametrize("p", [65537, P63])
 @pytest.mark.parametrize("n", [1, 255, 100_000])
 def test_deferred_dot_identity_L208(zp, p, n):
