@@ -117,9 +117,11 @@ k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offse
 }
 
 // ------------------------------------------------------------------------------------------------
-// (a3) prologue k_solve_table: per coefficient l of every master polynomial, the 32-byte record the hot
-// loop broadcasts:  { M_l, M_l', D_l, D_l' }  with D_l = l M_l (coefficient of M'(z) at z^(l-1)) and
-// w' = floor(w 2^64 / p) the Shoup companion (modarith.cuh).  Input: the product tree's M~ (Montgomery).
+// (a3) prologue k_solve_table: the 32-byte record the hot loop broadcasts for the Horner step from stage l
+// to stage l-1 (q_{l-1} = M_l + m q_l), stored at slot l-1, l = 1 .. t:
+//     { M_l, M_l', D_l, D_l' },  D_l = l M_l (coefficient of z^(l-1) in M'(z)),  M_t = 1,
+// w' = floor(w 2^64 / p) the Shoup companion (modarith.cuh).  Input: the product tree's M~ (Montgomery,
+// coefficients 0 .. t-1).
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F, ZpMod k,
@@ -127,15 +129,15 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int64_t t = offsets[f + 1] - off;
-    for (int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l < t; l += (int64_t)gridDim.x * blockDim.x) {
-      const uint64_t Mm = Mt[off + l];
+    for (int64_t l = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l <= t; l += (int64_t)gridDim.x * blockDim.x) {
+      const uint64_t Mm = (l < t) ? Mt[off + l] : k.r1;
       const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)l % k.p, k), k);  // (l M_l)~
       ulonglong4 r;
       r.x = from_mont(Mm, k);
       r.y = shoup_companion(Mm, k);
       r.z = from_mont(Dm, k);
       r.w = shoup_companion(Dm, k);
-      tab[off + l] = r;
+      tab[off + l - 1] = r;
     }
   }
 }
@@ -144,27 +146,29 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 // (a3)+(a4) K3 node_solve: the hot loop (PAPER.md L189-197 ZippelMultiplePrime(), L203-213).
 // One lane per node i of one function; the CTA streams tiles of the table above and of the NB right-hand
 // sides through shared memory (every lane needs the same M_l, v_{b,l}: warp-uniform broadcast reads).
-// Per lane, l = t-1 .. 0 with q = q_l (q_{t-1} = 1) and d (= t at the start):
-//     acc_b += q * v_{b,l}                       NB deferred MACs (L194-195 "vector of powers" x "values", L205-209)
-//     q <- M_l + m q ;  d <- D_l + m d   (l >= 1)   2 Horner steps (L193: synthetic division; Horner of M')
+// Per lane, stages l = t-1 .. 0 with q = q_l (q_{t-1} = 1) and d:
+//     acc_b += q_l * v_{b,l}                       NB deferred MACs (L194-195 "vector of powers" x "values", L205-209)
+//     q_{l-1} = M_l + m q_l ;  d <- D_l + m d   (l >= 1)   2 Horner steps (L193: synthetic division; Horner of M')
 // then  c_{b,i} = acc_b / d  [ / m if s0 = 1 ]   (L196).  d = M'(m_i) = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15):
 // the paper's "polynomial value computed via Horner's method"; running Horner on M' instead of on the
-// quotient gives the same number and keeps the two chains independent (twice the ILP).
-// All values are plain residues; q and d stay lazy in [0, 2p) (horner_step), nothing of length t is
+// quotient gives the same number and keeps the two chains independent.
+// Stages are taken in pairs (2j+1, 2j), j = J-1 .. 0, J = t/2 + 1, starting from q = d = 0 at a stage >= t
+// (records beyond t and values v_{b,l}, l >= t, are zero; record t carries M_t = 1): the two MACs of a
+// pair go into the accumulator together (acc_mac2).
+// All values are plain residues; q and d stay lazy in [0, 2p) (horner_step); nothing of length t is
 // stored per lane (reading G7).
 // Template NB = right-hand sides handled per pass; FIRST = this pass computes d and writes scale.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K3_THREADS 128
-#define ZP_K3_TILE 64
+#define ZP_K3_PAIRS 32
 
 template <int NB, bool FIRST>
 __global__ void __launch_bounds__(ZP_K3_THREADS)
 k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
              int F, const uint64_t* __restrict__ vals, int64_t T_tot, int b0, int s0, ZpMod k,
              uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
-  constexpr int NBP = (NB + 1) & ~1;  // row stride (even: 16-byte aligned pairs)
-  __shared__ __align__(16) ulonglong4 sT[ZP_K3_TILE];
-  __shared__ __align__(16) uint64_t sV[ZP_K3_TILE * NBP];
+  __shared__ __align__(16) ulonglong4 sT[2 * ZP_K3_PAIRS];      // record of stage l = 2 j0 + x
+  __shared__ __align__(16) ulonglong2 sV[ZP_K3_PAIRS * NB];     // [pair][b] = { v_{b,2j}, v_{b,2j+1} }
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -175,40 +179,41 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
     const uint64_t m = live ? nodes[off + i] % k.p : 0;
     const uint64_t mm = to_mont(m, k);
     const uint64_t mp = shoup_companion(mm, k);
-    uint64_t q = 1 % k.p, d = (uint64_t)t % k.p;
+    uint64_t q = 0, d = 0;
     Acc acc[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) acc_zero(acc[b]);
     const ulonglong4* Tf = tab + off;
-    for (int l1 = t; l1 > 0; l1 -= ZP_K3_TILE) {  // tile covers l in [l0, l1)
-      const int l0 = l1 - ZP_K3_TILE > 0 ? l1 - ZP_K3_TILE : 0;
-      const int n = l1 - l0;
+    const int J = t / 2 + 1;
+    for (int j1 = J; j1 > 0; j1 -= ZP_K3_PAIRS) {  // tile covers pairs [j0, j1)
+      const int j0 = j1 - ZP_K3_PAIRS > 0 ? j1 - ZP_K3_PAIRS : 0;
+      const int np = j1 - j0;
       __syncthreads();
-      for (int x = threadIdx.x; x < n; x += ZP_K3_THREADS) sT[x] = Tf[l0 + x];
-      for (int x = threadIdx.x; x < n * NB; x += ZP_K3_THREADS) {
-        const int b = x / n, s = x - b * n;
-        sV[s * NBP + b] = vals[(int64_t)(b0 + b) * T_tot + off + l0 + s];
+      for (int x = threadIdx.x; x < 2 * np; x += ZP_K3_THREADS) {
+        const int l = 2 * j0 + x;
+        sT[x] = (l >= 1 && l <= t) ? Tf[l - 1] : make_ulonglong4(0, 0, 0, 0);
+      }
+      for (int x = threadIdx.x; x < 2 * np * NB; x += ZP_K3_THREADS) {
+        const int b = x / (2 * np), r = x - b * (2 * np);  // r = stage offset inside the tile
+        const int l = 2 * j0 + r;
+        reinterpret_cast<uint64_t*>(sV)[((r >> 1) * NB + b) * 2 + (r & 1)] =
+            (l < t) ? vals[(int64_t)(b0 + b) * T_tot + off + l] : 0;
       }
       __syncthreads();
-#pragma unroll 2
-      for (int s = n - 1; s >= 0; --s) {
+      for (int jj = np - 1; jj >= 0; --jj) {
+        const ulonglong4 r1 = sT[2 * jj + 1];
+        const uint64_t qa = q;
+        const uint64_t qb = horner_step(qa, m, mp, r1.x, r1.y, k);
+        if (FIRST) d = horner_step(d, m, mp, r1.z, r1.w, k);
 #pragma unroll
-        for (int b = 0; b < NB; b += 2) {
-          if (b + 1 < NB) {
-            const ulonglong2 v2 = *reinterpret_cast<const ulonglong2*>(&sV[s * NBP + b]);
-            acc_mac(acc[b], q, v2.x);
-            acc_mac(acc[b + 1], q, v2.y);
-          } else {
-            acc_mac(acc[b], q, sV[s * NBP + b]);
-          }
+        for (int b = 0; b < NB; ++b) {
+          const ulonglong2 v2 = sV[jj * NB + b];
+          acc_mac2(acc[b], qa, v2.y, qb, v2.x);
         }
-        if (l0 + s >= 1) {
-          const ulonglong2 tq = *reinterpret_cast<const ulonglong2*>(&sT[s].x);
-          q = horner_step(q, m, mp, tq.x, tq.y, k);
-          if (FIRST) {
-            const ulonglong2 td = *reinterpret_cast<const ulonglong2*>(&sT[s].z);
-            d = horner_step(d, m, mp, td.x, td.y, k);
-          }
+        if (j0 + jj > 0) {
+          const ulonglong4 r0 = sT[2 * jj];
+          q = horner_step(qb, m, mp, r0.x, r0.y, k);
+          if (FIRST) d = horner_step(d, m, mp, r0.z, r0.w, k);
         }
       }
     }

@@ -189,6 +189,34 @@ ZP_DEV void acc_mac(Acc& a, uint64_t x, uint64_t y) {
       : "l"(m0), "l"(m1));
 }
 
+// Two MACs into the same accumulator, a += x*y + u*w, written so that carries of equal weight are adjacent:
+// ptxas then folds each pair of carries into ONE IADD3.X with two carry-ins (alu pipe) instead of IMAD.X
+// (which would take a slot of the multiplier pipe, the bound of the hot loop): 8 IMAD.WIDE + 3 IADD3.X.
+ZP_DEV void acc_mac2(Acc& a, uint64_t x, uint64_t y, uint64_t u, uint64_t w) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint32_t u0 = (uint32_t)u, u1 = (uint32_t)(u >> 32), w0 = (uint32_t)w, w1 = (uint32_t)(w >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), lo2 = zp_mulw(u0, w0), hi2 = zp_mulw(u1, w1);
+  asm("add.cc.u64 %0, %0, %3;\n\t"
+      "addc.cc.u64 %1, %1, %4;\n\t"
+      "addc.u32 %2, %2, 0;\n\t"
+      "add.cc.u64 %0, %0, %5;\n\t"
+      "addc.cc.u64 %1, %1, %6;\n\t"
+      "addc.u32 %2, %2, 0;"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi), "l"(lo2), "l"(hi2));
+  const uint64_t m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0), m2 = zp_mulw(u0, w1), m3 = zp_mulw(u1, w0);
+  asm("add.cc.u64 %0, %0, %2;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %3;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %4;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %5;\n\t"
+      "addc.u32 %1, %1, 0;"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1), "l"(m2), "l"(m3));
+}
+
 // T * 2^-160 mod p, canonical, for the 160-bit T held in the accumulator (five REDC rounds of 32 bits:
 // T_{k+1} = (T_k + m p)/2^32 < T_k/2^32 + p, so T_5 < T_0/2^160 + p(1 + 2^-32 + ...) <= p + 1).
 ZP_DEV uint64_t acc_redc160(const Acc& a, const ZpMod& k) {

@@ -13,6 +13,7 @@
 //   8 the library's Montgomery product (mont_mul)
 //   9 fma.rn.f64          DFMA            (fp64 pipe)
 //  10 DFMA and IMAD.WIDE interleaved 1:1 (do the fp64 and fma-heavy pipes overlap?)
+//  11 mul.wide.u32        IMAD.WIDE.U32 with a zero addend (the bare 32x32 -> 64 product)
 #pragma once
 #include "modarith.cuh"
 
@@ -77,6 +78,8 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
           asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc[c]) : "r"(nb), "r"(b));
           asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(car[c]) : "r"(b), "r"(lo));
           asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(car[c]) : "r"(a), "r"(lo));
+        } else if (KIND == 11) {
+          asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(acc[c]) : "r"(nb), "r"(b));
         } else if (KIND == 9) {
           double x = __longlong_as_double((long long)acc[c]);
           asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x) : "d"(dk1), "d"(dk2));

@@ -21,6 +21,7 @@ KINDS = [
     (3, "IMAD.WIDE + carry-out + IADD3.X (deferred MAC quarter)", 1), (4, "add + xor (alu)", 2),
     (5, "IMAD.WIDE + IADD3 1:1", 1), (6, "IMAD.WIDE + 2 IMAD", 3), (7, "horner_step (10 mult instr)", 10),
     (8, "mont_mul (10 mult instr)", 10), (9, "DFMA (fma.rn.f64)", 1), (10, "DFMA + IMAD.WIDE 1:1", 1),
+    (11, "IMAD.WIDE.U32 zero addend (mul.wide.u32)", 1),
 ]
 
 
