@@ -34,10 +34,16 @@ import numpy as np  # noqa: E402
 
 METRIC = "vandermonde_terms_solved_per_s"
 UNIT = "terms/s"
-# IMAD-derived peak: 148 SMs x 64 lanes/clk of the 32-bit multiplier (fma) pipe x
-# 1.965 GHz max SM clock; the micro-benchmark in profiles/r01_ubench.md reached 60.8-63 of the 64.
+# Multiplier-pipe roofline (profiles/r01_baseline.md): the fma-heavy pipe issues
+# 64 lanes/clk/SM of the 32-bit low multiply-add (IMAD) and 32 lanes/clk/SM of anything that needs the
+# 64-bit product (IMAD.WIDE, IMAD.HI).  Unit = one lane-cycle of that pipe's 64-lane issue rate:
+# IMAD = 1 unit, a 32x32->64 product = 2 units.  peak = 148 SMs x 64 units/clk x 1.965 GHz.
 IMAD_PEAK_TOPS = 148 * 64 * 1.965e9 / 1e12
-C_MM, C_MAC = 10, 4  # multiplier instructions per Montgomery product / per deferred MAC
+# algorithmic cost of the method's two primitives in those units (cheapest known generic-p forms):
+#   modular multiply-add x <- m x + a : 6 wide + 4 low = 16 ; deferred 64x64 MAC : 4 wide = 8
+C_MM, C_MAC = 16, 8
+# the instruction-count accounting of SURVEY.md 8(d).4 (10 / 4 multiplier instructions), kept as a second figure
+C_MM_INSTR, C_MAC_INSTR = 10, 4
 
 
 def parse():
@@ -117,16 +123,16 @@ def load_workload(idx: int, seed_shift: int, F_override):
                                 sh["emax"], sh["B"], with_planted=False)
 
 
-def work_model(ts, B, nv, newton=True, balanced=False):
-    """Algorithmic multiplier-pipe instructions, total and for the node-solve kernel."""
+def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
+    """Algorithmic multiplier-pipe units (SURVEY.md 8(d).4 formula), total and for the node-solve kernel."""
     t2 = float(sum(int(t) * int(t) for t in ts))
     T = float(sum(int(t) for t in ts))
-    node_solve = t2 * (2 * C_MM + B * C_MAC)
-    total = node_solve + C_MAC * t2 / 2 + C_MM * ((nv - 1) * T + (3 + B) * T)
+    node_solve = t2 * (2 * c_mm + B * c_mac)
+    total = node_solve + c_mac * t2 / 2 + c_mm * ((nv - 1) * T + (3 + B) * T)
     if newton:
-        total += C_MM * T * B * (B - 1) / 2
+        total += c_mm * T * B * (B - 1) / 2
     if balanced:
-        total += C_MM * t2
+        total += c_mm * t2
     return total, node_solve
 
 
@@ -169,7 +175,8 @@ def run_ours(args):
         def step():
             api.balanced_zippel_lift_step(dev[0], dev[1], anchors, samples, p, 0, 1, status=status, workspace=ws,
                                           stream=stream)
-        total_ops, ns_ops = work_model(ts, B, nv, True, True)
+        total_ops, _ = work_model(ts, B, nv, True, True)
+        _, ns_ops = work_model([500] * F, B, nv, True, True)  # the hook times the numerator part's node solve
         workload = f"C4 balanced lift 5->6 vars: F={F} rational functions, t_N=500, t_D=200, B=25"
         in_bytes = sum(q.exps.nbytes + q.vals.nbytes + q.meta["skel_standin"].nbytes for q in parts)
         out_bytes = sum(q.vals.nbytes for q in parts)
@@ -223,7 +230,7 @@ def run_ours(args):
         t0 = time.perf_counter()
         e0.record(stream)
         for i in range(K):
-            api.zippel_profile_events(api.K_NODE_SOLVE, ev_k[i][0], ev_k[i][1])
+            api.zippel_profile_events(api.K_NODE_SOLVE | (1 << 8), ev_k[i][0], ev_k[i][1])  # 1st node solve of the step
             step()
         e1.record(stream)
         torch.cuda.synchronize()
@@ -291,6 +298,7 @@ def run_ours(args):
         cpu = oracle_sample(idx, steps=1)
 
     achieved = ns_ops / (ns_ms * 1e-3) / 1e12
+    ns_ops_instr = ns_ops * (2 * C_MM_INSTR + B * C_MAC_INSTR) / (2 * C_MM + B * C_MAC)  # SURVEY.md 8(d).4 accounting
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -303,11 +311,16 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {
-            "bound": "alu", "kernel": "k_node_solve", "achieved": achieved, "peak": IMAD_PEAK_TOPS,
-            "unit": "T 32-bit multiplier instr/s (lane-ops)", "frac": achieved / IMAD_PEAK_TOPS, "traffic": None,
-            "peak_source": "derived: 148 SM x 64 IMAD lanes/clk x 1.965 GHz (DESIGN.md); micro-benchmark reached 95-98% of it",
+            "bound": "alu", "kernel": "k_node_solve" + (" (numerator part)" if idx == 4 else ""),
+            "achieved": achieved, "peak": IMAD_PEAK_TOPS,
+            "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
+            "traffic": None,
+            "peak_source": "derived (DESIGN.md Roofline): 148 SM x 64 lanes/clk of the fma-heavy pipe x 1.965 GHz; "
+                           "profiles/r01_baseline.md measures IMAD at 63.5 and IMAD.WIDE at 31.8 lanes/clk/SM",
             "algorithmic_ops_per_launch": ns_ops, "ms_per_launch": ns_ms,
+            "algorithmic_cost": "modular multiply-add = 16 units (6 wide + 4 low), deferred 64x64 MAC = 8 units (4 wide)",
             "whole_step_frac": total_ops / (ms_per_step * 1e-3) / 1e12 / IMAD_PEAK_TOPS,
+            "frac_instr_count_10_4": ns_ops_instr / (ns_ms * 1e-3) / 1e12 / IMAD_PEAK_TOPS,
         },
         "e2e": e2e,
         "cpu_baseline": cpu,

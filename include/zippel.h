@@ -129,8 +129,11 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
 
 /* Measurement hook (bench.py's roofline leg): when kernel != 0, every later call records the CUDA event
  * `ev_start` on its stream right before the first launch of that kernel and `ev_stop` right after the
- * last one (cudaEvent_t passed as void*; the caller owns them).  kernel: ZP_K_* below; 0 switches the
- * hook off.  The only process-wide state in the library; not thread-safe; nothing else changes. */
+ * last one (cudaEvent_t passed as void*; the caller owns them).  kernel: ZP_K_* below in the low byte; 0
+ * switches the hook off.  Bits 8.. select an occurrence: 0 = every stage of that kind re-records the
+ * events (the last one wins), n >= 1 = only the n-th such stage enqueued after this call (a balanced step
+ * runs every stage twice: numerator = 1, denominator = 2).  The only process-wide state in the library;
+ * not thread-safe; nothing else changes. */
 #define ZP_K_EVAL_NODES 1
 #define ZP_K_MASTER_POLY 2
 #define ZP_K_NODE_SOLVE 3

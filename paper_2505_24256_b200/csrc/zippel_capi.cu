@@ -91,12 +91,16 @@ bool check_offsets(const int64_t* h, int F, int64_t* T_tot, int64_t* tmax) {
 
 // ---- measurement hook (zippel_profile_events) ----------------------------------------------------
 unsigned long long g_launches = 0;  // kernels enqueued by this library in this process
-int g_prof_kernel = 0;
+int g_prof_kernel = 0, g_prof_ordinal = -1, g_prof_seen = 0;
 cudaEvent_t g_prof_start = nullptr, g_prof_stop = nullptr;
 struct ProfScope {  // records start at construction and stop at destruction when `kernel` is the hooked one
   bool on;
   cudaStream_t st;
-  ProfScope(int kernel, cudaStream_t s) : on(kernel == g_prof_kernel && g_prof_start && g_prof_stop), st(s) {
+  ProfScope(int kernel, cudaStream_t s) : on(false), st(s) {
+    if (kernel == g_prof_kernel && g_prof_start && g_prof_stop) {
+      on = g_prof_ordinal < 0 || g_prof_seen == g_prof_ordinal;  // ordinal: n-th occurrence since the hook was set
+      ++g_prof_seen;
+    }
     if (on) cudaEventRecord(g_prof_start, st);
   }
   ~ProfScope() {
@@ -409,7 +413,10 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
 unsigned long long zippel_launch_count(void) { return g_launches; }
 
 int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
-  if (kernel < 0 || kernel > 7 || (kernel != 0 && (!ev_start || !ev_stop))) return ZP_ERR_ARG;
+  if (kernel < 0 || (kernel & 0xff) > 7 || (kernel != 0 && (!ev_start || !ev_stop))) return ZP_ERR_ARG;
+  g_prof_ordinal = (kernel >> 8) - 1;  // bits 8.. : 0 = every occurrence, n = only the n-th (1-based) after this call
+  g_prof_seen = 0;
+  kernel &= 0xff;
   g_prof_kernel = kernel;
   g_prof_start = kernel ? (cudaEvent_t)ev_start : nullptr;
   g_prof_stop = kernel ? (cudaEvent_t)ev_stop : nullptr;
