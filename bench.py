@@ -115,11 +115,11 @@ def load_workload(idx: int, seed_shift: int, F_override):
     if F_override:
         kw["F"] = F_override
     if idx == 4:
-        rw = wl.make_rational_workload("C4", wl.SEED_BASE + 4 + 1000 * seed_shift, kw.get("F", 1024), 6, 500, 200, 24, 25)
+        rw = wl.make_rational_workload("C4", wl.SEED_BASE + 4 + seed_shift, kw.get("F", 1024), 6, 500, 200, 24, 25)
         return rw
     sh = dict(wl.CONFIG_SHAPES[idx])
     sh.update(kw)
-    return wl.make_box_workload(f"C{idx}", wl.SEED_BASE + idx + 1000 * seed_shift, sh["F"], sh["nv"], sh["t"],
+    return wl.make_box_workload(f"C{idx}", wl.SEED_BASE + idx + seed_shift, sh["F"], sh["nv"], sh["t"],
                                 sh["emax"], sh["B"], with_planted=False)
 
 
@@ -140,7 +140,7 @@ def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
 def run_ours(args):
     import torch
 
-    from paper_2505_24256_b200 import api
+    from paper_2505_24256_b200 import api, sharding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -153,7 +153,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     api.lib()
     idx = args.config
-    w = load_workload(idx, rank, args.F)
+    w = load_workload(idx, sharding.rank_seed_shift(rank), args.F)
     stream = torch.cuda.Stream()
     K, W = args.steps, args.warmup
 
@@ -241,12 +241,7 @@ def run_ours(args):
         clocks = sampler.stop(t0, t1) if sampler else None
         ms = e0.elapsed_time(e1)
         ns_ms = sum(a.elapsed_time(b) for a, b in ev_k) / K
-    if world > 1:
-        import torch.distributed as dist
-
-        tt = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = sharding.max_over_ranks(ms, "cuda")
     ms_per_step = ms / K
     terms = B * T_tot * world
     value = terms / (ms_per_step * 1e-3)
@@ -274,12 +269,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         tb = time.perf_counter()
         ems = (tb - ta) * 1e3
-        if world > 1:
-            import torch.distributed as dist
-
-            tt = torch.tensor([ems], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ems = float(tt.item())
+        ems = sharding.max_over_ranks(ems, "cuda")
         assert not h_st.numpy().any()
         e2e = {"value": terms / (ems / K * 1e-3), "unit": UNIT, "ms_per_step": ems / K,
                "h2d_bytes_per_step": int(in_bytes), "d2h_bytes_per_step": int(out_bytes),
