@@ -217,6 +217,46 @@ ZP_DEV void acc_mac2(Acc& a, uint64_t x, uint64_t y, uint64_t u, uint64_t w) {
       : "l"(m0), "l"(m1), "l"(m2), "l"(m3));
 }
 
+// Alternative forms of the same MAC, for the pipe-balance micro-benchmarks (zippel_ubench kinds 12-16).
+// acc_mac_split: every product is a bare IMAD.WIDE (zero addend, 4 pipe cycles instead of the > 5 of the
+// accumulating form, profiles/r01_baseline.md); the 160-bit additions run on the alu pipe as 32-bit carry chains.
+ZP_DEV void acc_mac_split(Acc& a, uint64_t x, uint64_t y) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0);
+  asm("{\n\t.reg .u32 a0, a1, a2, a3, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {a2, a3}, %1;\n\tmov.b64 {l0, l1}, %3;\n\tmov.b64 {h0, h1}, %4;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.cc.u32 a2, a2, h0;\n\taddc.cc.u32 a3, a3, h1;\n\t"
+      "addc.u32 %2, %2, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\tmov.b64 %1, {a2, a3};\n\t}"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi));
+  asm("{\n\t.reg .u32 a0, a1, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {l0, l1}, %2;\n\tmov.b64 {h0, h1}, %3;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "add.cc.u32 a0, a0, h0;\n\taddc.cc.u32 a1, a1, h1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\t}"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1));
+}
+// acc_mac_hyb: the two 64-bit aligned products of the even lattice accumulate inside IMAD.WIDE (as acc_mac),
+// the two middle products are bare and are added on the alu pipe.
+ZP_DEV void acc_mac_hyb(Acc& a, uint64_t x, uint64_t y) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0);
+  asm("add.cc.u64 %0, %0, %3;\n\t"
+      "addc.cc.u64 %1, %1, %4;\n\t"
+      "addc.u32 %2, %2, 0;"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi));
+  asm("{\n\t.reg .u32 a0, a1, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {l0, l1}, %2;\n\tmov.b64 {h0, h1}, %3;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "add.cc.u32 a0, a0, h0;\n\taddc.cc.u32 a1, a1, h1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\t}"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1));
+}
+
 // T * 2^-160 mod p, canonical, for the 160-bit T held in the accumulator (five REDC rounds of 32 bits:
 // T_{k+1} = (T_k + m p)/2^32 < T_k/2^32 + p, so T_5 < T_0/2^160 + p(1 + 2^-32 + ...) <= p + 1).
 ZP_DEV uint64_t acc_redc160(const Acc& a, const ZpMod& k) {

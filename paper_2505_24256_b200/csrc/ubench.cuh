@@ -14,6 +14,10 @@
 //   9 fma.rn.f64          DFMA            (fp64 pipe)
 //  10 DFMA and IMAD.WIDE interleaved 1:1 (do the fp64 and fma-heavy pipes overlap?)
 //  11 mul.wide.u32        IMAD.WIDE.U32 with a zero addend (the bare 32x32 -> 64 product)
+//  12 acc_mac             deferred MAC, products accumulate inside IMAD.WIDE (4 wide + carries)
+//  13 acc_mac2            two such MACs with merged carries (the node-solve loop's form; counts 2 MACs)
+//  14 acc_mac_split       bare products, all additions on the alu pipe
+//  15 acc_mac_hyb         even lattice inside IMAD.WIDE, middle products bare + alu
 #pragma once
 #include "modarith.cuh"
 
@@ -48,9 +52,17 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
   const uint64_t mp = shoup_companion(to_mont(m, k), k);
   const uint64_t ad = (((uint64_t)b << 32) | a) % k.p;
   const uint64_t adp = shoup_companion(to_mont(ad, k), k);
+  Acc macc[ZP_UB_CH];
+#pragma unroll
+  for (int c = 0; c < ZP_UB_CH; ++c) acc_zero(macc[c]);
+  uint64_t xw = m, xw2 = ad;
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
+      if (KIND >= 12 && KIND <= 15) {
+        xw ^= xw << 13; xw ^= xw >> 7;     // alu-only walk of the per-lane operand
+        xw2 ^= xw2 << 11; xw2 ^= xw2 >> 5;
+      }
 #pragma unroll
       for (int c = 0; c < ZP_UB_CH; ++c) {
         // every multiplicand comes from the chain itself, so that nothing can be hoisted out of the loop
@@ -89,6 +101,15 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
           asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(x) : "d"(dk1), "d"(dk2));
           acc[c] = (uint64_t)__double_as_longlong(x);
           asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(wacc[c]) : "r"((uint32_t)(wacc[(c + 1) % ZP_UB_CH] >> 32)), "r"(b));
+        } else if (KIND >= 12 && KIND <= 15) {
+          // deferred MAC forms: 8 accumulators per lane, the per-lane operand x walks (alu only), the other
+          // operand is a per-chain constant (as the broadcast v of the node-solve loop)
+          Acc& A = macc[c];
+          const uint64_t yv = ad + (uint64_t)c * 0x9e3779b97f4a7c15ull;
+          if (KIND == 12) acc_mac(A, xw, yv);
+          if (KIND == 13) acc_mac2(A, xw, yv, xw2, yv ^ mp);
+          if (KIND == 14) acc_mac_split(A, xw, yv);
+          if (KIND == 15) acc_mac_hyb(A, xw, yv);
         } else if (KIND == 7) {
           acc[c] = horner_step(acc[c], m, mp, ad, adp, k);
         } else if (KIND == 8) {
@@ -100,5 +121,9 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
   uint64_t s = 0;
 #pragma unroll
   for (int c = 0; c < ZP_UB_CH; ++c) s += acc[c] + car[c] + (KIND == 10 ? wacc[c] : 0);
+  if (KIND >= 12 && KIND <= 15) {
+#pragma unroll
+    for (int c = 0; c < ZP_UB_CH; ++c) s += macc[c].e0 + macc[c].e1 + macc[c].o0 + macc[c].e2 + macc[c].o1;
+  }
   if (s == 0x123456789abcdefull) out[tid] = s;  // keeps the chains alive, practically never taken
 }

@@ -22,6 +22,8 @@ KINDS = [
     (5, "IMAD.WIDE + IADD3 1:1", 1), (6, "IMAD.WIDE + 2 IMAD", 3), (7, "horner_step (10 mult instr)", 10),
     (8, "mont_mul (10 mult instr)", 10), (9, "DFMA (fma.rn.f64)", 1), (10, "DFMA + IMAD.WIDE 1:1", 1),
     (11, "IMAD.WIDE.U32 zero addend (mul.wide.u32)", 1),
+    (12, "acc_mac (4 accumulating wide)", 4), (13, "acc_mac2 (2 MACs, 8 accumulating wide)", 8),
+    (14, "acc_mac_split (4 bare wide + alu chains)", 4), (15, "acc_mac_hyb (2 accumulating + 2 bare wide)", 4),
 ]
 
 

@@ -155,10 +155,10 @@ def test_solve_small_ragged_batch(zp, ref, p, s0):
     assert (zp.to_host(got) == want).all()
 
 
-@pytest.mark.parametrize("B", [1, 2, 3, 8, 11, 21, 25, 26, 33, 64])
+@pytest.mark.parametrize("B", list(range(1, 28)) + [33, 52, 53, 64])
 def test_solve_every_rhs_count_path(zp, ref, B):
     """each B exercises another template instance / pass split of the node-solve kernel"""
-    nodes, offsets, vals = random_solve_case(100 + B, [127, 128, 129, 300], B, P63)
+    nodes, offsets, vals = random_solve_case(100 + B, [63, 64, 65, 129, 200], B, P63)
     want, _ = ref.vandermonde_solve_batch(nodes, offsets, vals, P63, 0)
     got, st = zp.vandermonde_solve_batch(zp.to_dev(nodes), offsets, zp.to_dev(vals), P63, 0)
     assert not zp.to_host(st).any()
