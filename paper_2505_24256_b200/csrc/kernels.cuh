@@ -162,13 +162,27 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 #define ZP_K3_THREADS 128
 #define ZP_K3_PAIRS 32
 
+// cp.async (LDGSTS) with zero fill: src-size 0 reads nothing and writes zeros
+ZP_DEV void cp_async8(void* smem, const void* g, bool ok) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g),
+               "r"(ok ? 8 : 0) : "memory");
+}
+ZP_DEV void cp_async16(void* smem, const void* g, bool ok) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g),
+               "r"(ok ? 16 : 0) : "memory");
+}
+ZP_DEV void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+ZP_DEV void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <int NB, bool FIRST>
 __global__ void __launch_bounds__(ZP_K3_THREADS)
 k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
              int F, const uint64_t* __restrict__ vals, int64_t T_tot, int b0, int s0, ZpMod k,
              uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
-  __shared__ __align__(16) ulonglong4 sT[2 * ZP_K3_PAIRS];      // record of stage l = 2 j0 + x
-  __shared__ __align__(16) ulonglong2 sV[ZP_K3_PAIRS * NB];     // [pair][b] = { v_{b,2j}, v_{b,2j+1} }
+  // two buffers: the tile after the current one is in flight (cp.async) while the current one is consumed
+  __shared__ __align__(16) ulonglong4 sT[2][2 * ZP_K3_PAIRS];      // record of stage l = 2 j0 + x
+  __shared__ __align__(16) ulonglong2 sV[2][ZP_K3_PAIRS * NB];     // [pair][b] = { v_{b,2j}, v_{b,2j+1} }
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -185,37 +199,57 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
     for (int b = 0; b < NB; ++b) acc_zero(acc[b]);
     const ulonglong4* Tf = tab + off;
     const int J = t / 2 + 1;
-    for (int j1 = J; j1 > 0; j1 -= ZP_K3_PAIRS) {  // tile covers pairs [j0, j1)
+    // tile = pairs [j0, j1), j0 = max(j1 - PAIRS, 0); out-of-range stages are zero-filled (src-size 0)
+    auto issue_tile = [&](int j1, int buf) {
       const int j0 = j1 - ZP_K3_PAIRS > 0 ? j1 - ZP_K3_PAIRS : 0;
       const int np = j1 - j0;
-      __syncthreads();
-      for (int x = threadIdx.x; x < 2 * np; x += ZP_K3_THREADS) {
-        const int l = 2 * j0 + x;
-        sT[x] = (l >= 1 && l <= t) ? Tf[l - 1] : make_ulonglong4(0, 0, 0, 0);
+      for (int x = threadIdx.x; x < 4 * np; x += ZP_K3_THREADS) {  // 16-byte halves of the 32-byte records
+        const int l = 2 * j0 + (x >> 1);
+        const bool ok = l >= 1 && l <= t;
+        cp_async16(reinterpret_cast<ulonglong2*>(&sT[buf][0]) + x,
+                   reinterpret_cast<const ulonglong2*>(Tf + (ok ? l - 1 : 0)) + (x & 1), ok);
       }
       for (int x = threadIdx.x; x < 2 * np * NB; x += ZP_K3_THREADS) {
         const int b = x / (2 * np), r = x - b * (2 * np);  // r = stage offset inside the tile
         const int l = 2 * j0 + r;
-        reinterpret_cast<uint64_t*>(sV)[((r >> 1) * NB + b) * 2 + (r & 1)] =
-            (l < t) ? vals[(int64_t)(b0 + b) * T_tot + off + l] : 0;
+        const bool ok = l < t;
+        cp_async8(reinterpret_cast<uint64_t*>(&sV[buf][0]) + ((r >> 1) * NB + b) * 2 + (r & 1),
+                  vals + (int64_t)(b0 + b) * T_tot + off + (ok ? l : 0), ok);
+      }
+      cp_async_commit();
+    };
+    __syncthreads();  // the previous function's last tile has been consumed
+    issue_tile(J, 0);
+    int buf = 0;
+    for (int j1 = J; j1 > 0; j1 -= ZP_K3_PAIRS, buf ^= 1) {  // tile covers pairs [j0, j1)
+      const int j0 = j1 - ZP_K3_PAIRS > 0 ? j1 - ZP_K3_PAIRS : 0;
+      const int np = j1 - j0;
+      if (j0 > 0) {
+        issue_tile(j0, buf ^ 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
       }
       __syncthreads();
+      const ulonglong4* cT = sT[buf];
+      const ulonglong2* cV = sV[buf];
       for (int jj = np - 1; jj >= 0; --jj) {
-        const ulonglong4 r1 = sT[2 * jj + 1];
+        const ulonglong4 r1 = cT[2 * jj + 1];
         const uint64_t qa = q;
         const uint64_t qb = horner_step(qa, m, mp, r1.x, r1.y, k);
         if (FIRST) d = horner_step(d, m, mp, r1.z, r1.w, k);
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-          const ulonglong2 v2 = sV[jj * NB + b];
+          const ulonglong2 v2 = cV[jj * NB + b];
           acc_mac2(acc[b], qa, v2.y, qb, v2.x);
         }
         if (j0 + jj > 0) {
-          const ulonglong4 r0 = sT[2 * jj];
+          const ulonglong4 r0 = cT[2 * jj];
           q = horner_step(qb, m, mp, r0.x, r0.y, k);
           if (FIRST) d = horner_step(d, m, mp, r0.z, r0.w, k);
         }
       }
+      __syncthreads();  // this buffer is refilled by the next iteration's prefetch
     }
     if (live) {
       uint64_t sc;
