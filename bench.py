@@ -273,7 +273,7 @@ def run_ours(args):
         assert not h_st.numpy().any()
         e2e = {"value": terms / (ems / K * 1e-3), "unit": UNIT, "ms_per_step": ems / K,
                "h2d_bytes_per_step": int(in_bytes), "d2h_bytes_per_step": int(out_bytes),
-               "call": "zippel_lift_step_host (pinned host buffers; H2D + step + D2H + stream sync per step)"}
+               "call": "zippel_lift_step_host (pinned host buffers; chunked H2D / step / D2H pipeline on 3 streams + stream sync per step)"}
 
     if rank != 0:
         if world > 1:

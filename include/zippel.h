@@ -93,10 +93,14 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
                      void* stream);
 
 /* Host-buffer form of zippel_lift_step (the end-to-end call): every data pointer is a HOST pointer
- * (pinned memory makes the copies asynchronous).  The library enqueues on `stream`: H2D of exps,
- * anchors, samples and vals into staging carved from `workspace` (device,
- * zippel_host_workspace_bytes() bytes), the lifting step, D2H of out [B x T_tot] and status [F].
- * Nothing is synchronised: the caller waits on the stream before reading h_out / h_status. */
+ * (pinned memory makes the copies asynchronous).  Staging is carved from `workspace` (device,
+ * zippel_host_workspace_bytes() bytes).  Batches above 8 MB of values are cut into up to 16 chunks of whole
+ * functions (functions are independent): the H2D copy of chunk c+1 and the D2H copy of
+ * chunk c-1 run on two copy streams of the library while the kernels of chunk c run on `stream`; the copy
+ * streams start after the work already queued on `stream`, and `stream` ends waiting for the last D2H copy.
+ * Nothing is synchronised: the caller waits on `stream` before reading h_out / h_status.  The two copy
+ * streams and their events are created on first use per device and kept for the process (with the profiling
+ * hook the only process-wide state; not thread-safe per device). */
 size_t zippel_host_workspace_bytes(const int64_t* h_offsets, int F, int nv, int B);
 int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int F, int nv,
                           const uint64_t* h_anchors, const uint64_t* h_samples, int B, int s0,

@@ -241,6 +241,52 @@ HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B) {
   return h;
 }
 
+// (a1)-(a5) on the functions [f0, f1) of a batch whose arrays are resident in full (row stride T_tot): the
+// kernels index by absolute term offsets, so a chunk is the same launch sequence on shifted offset/status
+// pointers.  The whole batch is the chunk [0, F).
+void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T_tot, int nv, const uint16_t* exps,
+                const uint64_t* anchors, const uint64_t* samples, int B, int s0, const uint64_t* vals, const ZpMod& k,
+                int basis, uint64_t* out, uint64_t* nodes, int32_t* status, cudaStream_t st) {
+  const int64_t a = h_offsets[f0], n = h_offsets[f1] - a;
+  int64_t tmax = 0;
+  for (int f = f0; f < f1; ++f) tmax = (h_offsets[f + 1] - h_offsets[f] > tmax) ? h_offsets[f + 1] - h_offsets[f] : tmax;
+  Ws wc = w;
+  wc.d_offsets += f0;
+  wc.st_solve += f0;
+  wc.st_pre += f0;
+  const int Fc = f1 - f0;
+  run_eval_nodes(exps + a * nv, n, nv, anchors, k, nodes + a, st);
+  run_solve(wc, nodes, Fc, T_tot, tmax, vals, B, s0, k, out, st);
+  run_newton(wc, samples, B, out + a, n, T_tot, k, basis, out + a, st);
+  ++g_launches, k_status_finish<<<(Fc + 255) / 256, 256, 0, st>>>(nullptr, wc.st_solve, wc.st_newton, Fc, status + f0);
+}
+
+// copy streams and events of the host-buffer entry (created once per device, kept for the process)
+#define ZP_PIPE_MAX_CHUNKS 16
+struct Pipe {
+  bool ready = false;
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_start = nullptr, ev_end = nullptr, ev_in[ZP_PIPE_MAX_CHUNKS], ev_done[ZP_PIPE_MAX_CHUNKS];
+};
+Pipe g_pipe[16];
+Pipe* get_pipe() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 16) return nullptr;
+  Pipe& P = g_pipe[dev];
+  if (!P.ready) {
+    bool ok = cudaStreamCreateWithFlags(&P.s_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&P.s_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&P.ev_start, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&P.ev_end, cudaEventDisableTiming) == cudaSuccess;
+    for (int c = 0; ok && c < ZP_PIPE_MAX_CHUNKS; ++c)
+      ok = cudaEventCreateWithFlags(&P.ev_in[c], cudaEventDisableTiming) == cudaSuccess &&
+           cudaEventCreateWithFlags(&P.ev_done[c], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) return nullptr;
+    P.ready = true;
+  }
+  return &P;
+}
+
 }  // namespace
 
 extern "C" {
@@ -321,12 +367,9 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
   if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
   const Ws w = carve(workspace, T_tot, F, B, 0);
   cudaStream_t st = (cudaStream_t)stream;
-  uint64_t* nodes = nodes_out ? nodes_out : w.nodes;
   upload_offsets(w, h_offsets, F, st);
-  run_eval_nodes(exps, T_tot, nv, anchors, k, nodes, st);
-  run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, out, st);
-  run_newton(w, samples, B, out, T_tot, T_tot, k, basis, out, st);
-  ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, w.st_newton, F, status);
+  lift_chunk(w, h_offsets, 0, F, T_tot, nv, exps, anchors, samples, B, s0, vals, k, basis, out,
+             nodes_out ? nodes_out : w.nodes, status, st);
   return cuda_ok();
 }
 
@@ -340,22 +383,52 @@ int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int 
                           const uint64_t* h_anchors, const uint64_t* h_samples, int B, int s0,
                           const uint64_t* h_vals, uint64_t p, int basis, uint64_t* h_out, int32_t* h_status,
                           void* workspace, size_t workspace_bytes, void* stream) {
+  ZpMod k;
   int64_t T_tot, tmax;
   if (!h_exps || !h_anchors || !h_samples || !h_vals || !h_out || !h_status || nv <= 0 || nv > ZP_MAX_NV ||
-      B <= 0 || B > ZP_MAX_B || !check_offsets(h_offsets, F, &T_tot, &tmax))
+      B <= 0 || B > ZP_MAX_B || (s0 != 0 && s0 != 1) || (basis != 0 && basis != 1) || !make_mod(p, &k) ||
+      !check_offsets(h_offsets, F, &T_tot, &tmax))
     return ZP_ERR_ARG;
   if (!ws_ok(workspace, workspace_bytes, carve_host(nullptr, T_tot, F, nv, B).bytes)) return ZP_ERR_WORKSPACE;
   const HostWs h = carve_host(workspace, T_tot, F, nv, B);
+  const Ws w = carve(h.inner, T_tot, F, B, 0);
   cudaStream_t st = (cudaStream_t)stream;
-  cudaMemcpyAsync(h.exps, h_exps, 2 * (size_t)T_tot * nv, cudaMemcpyHostToDevice, st);
+  Pipe* P = get_pipe();
+  if (!P) return ZP_ERR_CUDA;
+  // chunks of whole functions, equal in terms; small batches go in one piece
+  const size_t bytes = 8 * (size_t)T_tot * B;
+  int nch = bytes < ((size_t)8 << 20) ? 1 : (F < ZP_PIPE_MAX_CHUNKS ? F : ZP_PIPE_MAX_CHUNKS);
+  int cut[ZP_PIPE_MAX_CHUNKS + 1];
+  cut[0] = 0;
+  for (int c = 1, f = 0; c <= nch; ++c) {
+    const int64_t target = T_tot * c / nch;
+    while (f < F && h_offsets[f] < target) ++f;
+    cut[c] = (c == nch) ? F : f;
+  }
   cudaMemcpyAsync(h.anchors, h_anchors, 8 * (size_t)nv, cudaMemcpyHostToDevice, st);
   cudaMemcpyAsync(h.samples, h_samples, 8 * (size_t)B, cudaMemcpyHostToDevice, st);
-  cudaMemcpyAsync(h.vals, h_vals, 8 * (size_t)T_tot * B, cudaMemcpyHostToDevice, st);
-  const int rc = zippel_lift_step(h.exps, h_offsets, F, nv, h.anchors, h.samples, B, s0, h.vals, p, basis, h.out,
-                                  nullptr, h.status, h.inner, h.inner_bytes, stream);
-  if (rc != ZP_OK) return rc;
-  cudaMemcpyAsync(h_out, h.out, 8 * (size_t)T_tot * B, cudaMemcpyDeviceToHost, st);
-  cudaMemcpyAsync(h_status, h.status, 4 * (size_t)F, cudaMemcpyDeviceToHost, st);
+  upload_offsets(w, h_offsets, F, st);
+  cudaEventRecord(P->ev_start, st);  // the copy streams start after everything already queued on `stream`
+  cudaStreamWaitEvent(P->s_in, P->ev_start, 0);
+  cudaStreamWaitEvent(P->s_out, P->ev_start, 0);
+  const size_t pitch = 8 * (size_t)T_tot;
+  for (int c = 0; c < nch; ++c) {  // H2D of chunk c+1 and D2H of chunk c-1 overlap the kernels of chunk c
+    const int f0 = cut[c], f1 = cut[c + 1];
+    if (f1 <= f0) continue;
+    const int64_t a = h_offsets[f0], n = h_offsets[f1] - a;
+    cudaMemcpyAsync(h.exps + a * nv, h_exps + a * nv, 2 * (size_t)n * nv, cudaMemcpyHostToDevice, P->s_in);
+    cudaMemcpy2DAsync(h.vals + a, pitch, h_vals + a, pitch, 8 * (size_t)n, (size_t)B, cudaMemcpyHostToDevice, P->s_in);
+    cudaEventRecord(P->ev_in[c], P->s_in);
+    cudaStreamWaitEvent(st, P->ev_in[c], 0);
+    lift_chunk(w, h_offsets, f0, f1, T_tot, nv, h.exps, h.anchors, h.samples, B, s0, h.vals, k, basis, h.out, w.nodes,
+               h.status, st);
+    cudaEventRecord(P->ev_done[c], st);
+    cudaStreamWaitEvent(P->s_out, P->ev_done[c], 0);
+    cudaMemcpy2DAsync(h_out + a, pitch, h.out + a, pitch, 8 * (size_t)n, (size_t)B, cudaMemcpyDeviceToHost, P->s_out);
+    cudaMemcpyAsync(h_status + f0, h.status + f0, 4 * (size_t)(f1 - f0), cudaMemcpyDeviceToHost, P->s_out);
+  }
+  cudaEventRecord(P->ev_end, P->s_out);
+  cudaStreamWaitEvent(st, P->ev_end, 0);  // a synchronize on `stream` covers the result copies
   return cuda_ok();
 }
 
