@@ -101,17 +101,54 @@ k_tree_leaf(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offs
   }
 }
 
-// one level: left block length a (multiple of LEAF), thread per output slot
-__global__ void __launch_bounds__(ZP_K2_THREADS)
+// one level: left block length a (a multiple of LEAF, so a tile of TC output slots never straddles two
+// merges).  CTA = TC consecutive output slots of one function, one per lane; the convolution runs over
+// j-tiles of TJ coefficients of A' (broadcast reads) against a window of TC + TJ - 1 coefficients of B'
+// (unit-stride reads), both staged in shared memory and zero-padded outside their ranges, so the inner
+// loop is branch-free deferred MACs.
+#define ZP_K2_TC 256
+#define ZP_K2_TJ 64
+__global__ void __launch_bounds__(ZP_K2_TC)
 k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offsets, int F, int64_t a, ZpMod k,
              uint64_t* __restrict__ dst) {
+  __shared__ uint64_t sA[ZP_K2_TJ];
+  __shared__ uint64_t sB[ZP_K2_TC + ZP_K2_TJ];
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int64_t t = offsets[f + 1] - off;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < t; i += (int64_t)gridDim.x * blockDim.x) {
-      const int64_t base = i - (i % (2 * a));
-      const int64_t b = (t - base - a) < a ? (t - base - a) : a;
-      dst[off + i] = (b <= 0) ? src[off + i] : tree_merge_coef(src + off + base, (int)a, (int)b, (int)(i - base), k);
+    for (int64_t i0 = (int64_t)blockIdx.x * ZP_K2_TC; i0 < t; i0 += (int64_t)gridDim.x * ZP_K2_TC) {
+      const int64_t base = i0 - (i0 % (2 * a));
+      const int64_t b = (t - base - a) < a ? (t - base - a) : a;  // right block length (<= 0: nothing to merge)
+      const int64_t i = i0 + threadIdx.x;
+      if (b <= 0) {  // uniform per CTA
+        if (i < t) dst[off + i] = src[off + i];
+        continue;
+      }
+      const uint64_t* A = src + off + base;      // A'[0 .. a)
+      const uint64_t* Bp = src + off + base + a;  // B'[0 .. b)
+      const int64_t c0 = i0 - base, c = c0 + threadIdx.x;
+      const int64_t jlo = c0 - b + 1 > 0 ? c0 - b + 1 : 0;
+      const int64_t jhi = c0 + ZP_K2_TC - 1 < a - 1 ? c0 + ZP_K2_TC - 1 : a - 1;
+      Acc acc;
+      acc_zero(acc);
+      for (int64_t j0 = jlo; j0 <= jhi; j0 += ZP_K2_TJ) {
+        __syncthreads();
+        if (threadIdx.x < ZP_K2_TJ) sA[threadIdx.x] = (j0 + threadIdx.x < a) ? A[j0 + threadIdx.x] : 0;
+        for (int x = threadIdx.x; x < ZP_K2_TC + ZP_K2_TJ - 1; x += ZP_K2_TC) {
+          const int64_t kb = c0 - j0 - (ZP_K2_TJ - 1) + x;  // B' index of window slot x
+          sB[x] = (kb >= 0 && kb < b) ? Bp[kb] : 0;
+        }
+        __syncthreads();
+        const uint64_t* win = sB + threadIdx.x + (ZP_K2_TJ - 1);  // win[-jj] = B'[c - (j0 + jj)]
+#pragma unroll 8
+        for (int jj = 0; jj < ZP_K2_TJ; jj += 2) acc_mac2(acc, sA[jj], win[-jj], sA[jj + 1], win[-jj - 1]);
+      }
+      if (i < t) {
+        uint64_t r = mont_mul(acc_redc160(acc, k), k.c160, k);
+        if (c >= a) r = mod_add(r, Bp[c - a], k.p);  // z^a B'
+        if (c >= b) r = mod_add(r, A[c - b], k.p);   // z^b A'
+        dst[off + i] = r;
+      }
     }
   }
 }
@@ -271,47 +308,65 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 
 // ------------------------------------------------------------------------------------------------
 // (a5) K5 Newton interpolation in x_k, one lane per coefficient (eq. (1)).
-// k_newton_prep: invd[j*B + jj] = (1/(c_j - c_jj))~ for jj < j, samples~, duplicate check.
+// k_newton_prep: invd[j*B + jj] = {w, w'} with w = 1/(c_j - c_jj) for jj < j (plain, with its Shoup companion),
+// negc[j] = {-c_j, companion}, duplicate check.
 // k_newton: divided differences in shared memory (column per lane), optional monomial expansion.
 // ------------------------------------------------------------------------------------------------
-__global__ void k_newton_prep(const uint64_t* __restrict__ samples, int B, ZpMod k, uint64_t* __restrict__ invd,
-                              uint64_t* __restrict__ smont, int32_t* __restrict__ nstatus) {
+__global__ void k_newton_prep(const uint64_t* __restrict__ samples, int B, ZpMod k, ulonglong2* __restrict__ invd,
+                              ulonglong2* __restrict__ negc, int32_t* __restrict__ nstatus) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= B * B) return;
   const int j = idx / B, jj = idx % B;
   const uint64_t cj = samples[j] % k.p, cjj = samples[jj] % k.p;
-  if (jj == 0) smont[j] = to_mont(cj, k);
+  if (jj == 0) {  // multiplier -c_j of the monomial expansion, with its Shoup companion
+    const uint64_t nc = mod_neg(cj, k.p);
+    negc[j] = make_ulonglong2(nc, shoup_companion(to_mont(nc, k), k));
+  }
   if (jj < j) {
     const uint64_t diff = mod_sub(cj, cjj, k.p);
     if (diff == 0) atomicMin(nstatus, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
-    invd[idx] = mont_inv(to_mont(diff, k), k);
+    const uint64_t wm = mont_inv(to_mont(diff, k), k);  // (1/(c_j - c_jj))~
+    invd[idx] = make_ulonglong2(from_mont(wm, k), shoup_companion(wm, k));
   }
+}
+
+// x * w mod p for a fixed multiplier w with companion w' (horner_step with a zero addend), canonical result;
+// x may be any 64-bit value
+ZP_DEV uint64_t shoup_mul(uint64_t x, ulonglong2 w, const ZpMod& k) {
+  return lazy_canon(horner_step(x, w.x, w.y, 0, 0, k), k.p);
 }
 
 #define ZP_K5_THREADS 128
 __global__ void __launch_bounds__(ZP_K5_THREADS)
-k_newton(const uint64_t* __restrict__ invd, const uint64_t* __restrict__ smont, int B, const uint64_t* vals, int64_t n,
+k_newton(const ulonglong2* __restrict__ invd, const ulonglong2* __restrict__ negc, int B, const uint64_t* vals, int64_t n,
          int64_t ld, ZpMod k, int basis, uint64_t* out) {
-  extern __shared__ uint64_t sh[];
-  uint64_t* sInv = sh;                                 // [B*B]
-  uint64_t* sC = sh + B * B;                           // [B] samples~
-  uint64_t* col = sC + B + threadIdx.x;                // column of this lane: col[j*TH]
-  uint64_t* pol = sC + B + (size_t)B * ZP_K5_THREADS + threadIdx.x;  // second column (monomial expansion)
+  extern __shared__ __align__(16) uint64_t sh[];
+  ulonglong2* sInv = reinterpret_cast<ulonglong2*>(sh);  // [B*B] {w, w'}
+  ulonglong2* sC = sInv + B * B;                         // [B]   {-c_j, companion}
+  uint64_t* col = reinterpret_cast<uint64_t*>(sC + B) + threadIdx.x;  // column of this lane: col[j*TH]
+  uint64_t* pol = col + (size_t)B * ZP_K5_THREADS;                    // second column (monomial expansion)
   constexpr int TH = ZP_K5_THREADS;
   for (int x = threadIdx.x; x < B * B; x += TH) sInv[x] = invd[x];
-  for (int x = threadIdx.x; x < B; x += TH) sC[x] = smont[x];
+  for (int x = threadIdx.x; x < B; x += TH) sC[x] = negc[x];
   __syncthreads();
   const int D = B - 1;
   for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
-    // the product by the Montgomery inverse difference keeps plain values plain
     for (int j = 0; j < B; ++j) col[j * TH] = vals[j * ld + i] % k.p;
+    // a_j <- (a_j - a_{j-1}) / (c_j - c_{j-l}), j = D .. l; four independent steps at a time (all loads of a
+    // group precede its stores, so the group's products overlap in the pipe)
     for (int l = 1; l <= D; ++l) {
-      uint64_t hiv = col[D * TH];
-      for (int j = D; j >= l; --j) {
-        const uint64_t lov = col[(j - 1) * TH];
-        col[j * TH] = mont_mul(mod_sub(hiv, lov, k.p), sInv[j * B + (j - l)], k);
-        hiv = lov;
+      int j = D;
+      for (; j - 3 >= l; j -= 4) {
+        const uint64_t v0 = col[j * TH], v1 = col[(j - 1) * TH], v2 = col[(j - 2) * TH], v3 = col[(j - 3) * TH],
+                       v4 = col[(j - 4) * TH];
+        const ulonglong2* w = sInv + j * B + (j - l);  // row stride B, same column offset j - l
+        col[j * TH] = shoup_mul(v0 + k.p - v1, w[0], k);
+        col[(j - 1) * TH] = shoup_mul(v1 + k.p - v2, w[-B - 1], k);
+        col[(j - 2) * TH] = shoup_mul(v2 + k.p - v3, w[-2 * B - 2], k);
+        col[(j - 3) * TH] = shoup_mul(v3 + k.p - v4, w[-3 * B - 3], k);
       }
+      for (; j >= l; --j)
+        col[j * TH] = shoup_mul(col[j * TH] + k.p - col[(j - 1) * TH], sInv[j * B + (j - l)], k);
     }
     if (basis == 0) {
       for (int j = 0; j < B; ++j) out[j * ld + i] = col[j * TH];
@@ -320,14 +375,20 @@ k_newton(const uint64_t* __restrict__ invd, const uint64_t* __restrict__ smont, 
       int deg = 0;
       pol[0] = col[D * TH];
       for (int j = D - 1; j >= 0; --j) {
-        const uint64_t cj = sC[j];
+        const ulonglong2 nc = sC[j];
         uint64_t up = pol[deg * TH];
         pol[(deg + 1) * TH] = up;
-        for (int x = deg; x >= 1; --x) {
-          const uint64_t below = pol[(x - 1) * TH];
-          pol[x * TH] = mod_sub(below, mont_mul(cj, pol[x * TH], k), k.p);
+        int x = deg;
+        for (; x - 3 >= 1; x -= 4) {
+          const uint64_t v0 = pol[x * TH], v1 = pol[(x - 1) * TH], v2 = pol[(x - 2) * TH], v3 = pol[(x - 3) * TH],
+                         v4 = pol[(x - 4) * TH];
+          pol[x * TH] = mod_add(v1, shoup_mul(v0, nc, k), k.p);
+          pol[(x - 1) * TH] = mod_add(v2, shoup_mul(v1, nc, k), k.p);
+          pol[(x - 2) * TH] = mod_add(v3, shoup_mul(v2, nc, k), k.p);
+          pol[(x - 3) * TH] = mod_add(v4, shoup_mul(v3, nc, k), k.p);
         }
-        pol[0] = mod_sub(col[j * TH], mont_mul(cj, pol[0], k), k.p);
+        for (; x >= 1; --x) pol[x * TH] = mod_add(pol[(x - 1) * TH], shoup_mul(pol[x * TH], nc, k), k.p);
+        pol[0] = mod_add(col[j * TH], shoup_mul(pol[0], nc, k), k.p);
         ++deg;
       }
       for (int j = 0; j < B; ++j) out[j * ld + i] = pol[j * TH];
@@ -356,18 +417,18 @@ __global__ void k_status_finish(const int32_t* pre, const int32_t* solve, const 
 // ------------------------------------------------------------------------------------------------
 // (a6) K6 power sums R_{b,s} = sum_i a_{b,i} m_i^(s+s0)  ("raise base variable
 // values to various powers and substitute them into the polynomial"; strided power tables, A21).
-// CTA = (function f, block of 256 consecutive s); node tiles of 128 in shared memory with
+// CTA = (function f, block of 256 consecutive s); node tiles of 96 in shared memory with
 //   base_i = a_i~ m_i^(sb0+s0),  lo_i[x] = m_i^x,  hi_i[x] = m_i^(16x)   (x < 16),
 // lane s: m_i^(s-sb0) = lo_i[s & 15] * hi_i[s >> 4]; deferred sum over i.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K6_THREADS 256
-#define ZP_K6_NODES 128
+#define ZP_K6_NODES 96
 __global__ void __launch_bounds__(ZP_K6_THREADS)
 k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offsets, int F,
              const uint64_t* __restrict__ coef, int64_t T_tot, int B, int s0, ZpMod k, uint64_t* __restrict__ out) {
-  __shared__ uint64_t sBase[ZP_K6_NODES];
-  __shared__ uint64_t sLo[ZP_K6_NODES * 16];
-  __shared__ uint64_t sHi[ZP_K6_NODES * 16];
+  __shared__ uint64_t sBase[ZP_K6_NODES];                       // plain a_i m_i^(sb0+s0)
+  __shared__ __align__(16) ulonglong2 sLo[ZP_K6_NODES * 16];    // {w, w'}: plain m_i^x with its Shoup companion
+  __shared__ uint64_t sHi[ZP_K6_NODES * 16];                    // plain m_i^(16x)
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -383,26 +444,28 @@ k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ off
         if (threadIdx.x < n) {
           const int i = i0 + threadIdx.x;
           const uint64_t m = to_mont(nodes[off + i] % k.p, k);
-          const uint64_t a = to_mont(coef[(int64_t)b * T_tot + off + i] % k.p, k);
-          sBase[threadIdx.x] = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);
+          const uint64_t a = coef[(int64_t)b * T_tot + off + i] % k.p;
+          sBase[threadIdx.x] = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);  // plain * mont -> plain
           uint64_t pw = k.r1;
           for (int x = 0; x < 16; ++x) {
-            sLo[threadIdx.x * 16 + x] = pw;
+            sLo[threadIdx.x * 16 + x] = make_ulonglong2(from_mont(pw, k), shoup_companion(pw, k));
             pw = mont_mul(pw, m, k);
           }
           const uint64_t m16 = pw;
           pw = k.r1;
           for (int x = 0; x < 16; ++x) {
-            sHi[threadIdx.x * 16 + x] = pw;
+            sHi[threadIdx.x * 16 + x] = from_mont(pw, k);
             pw = mont_mul(pw, m16, k);
           }
         }
         __syncthreads();
         const int lo = threadIdx.x & 15, hi = threadIdx.x >> 4;
-        for (int x = 0; x < n; ++x)
-          acc_mac(acc, mont_mul(sLo[x * 16 + lo], sHi[x * 16 + hi], k), sBase[x]);
+        for (int x = 0; x < n; ++x) {
+          const ulonglong2 w = sLo[x * 16 + lo];
+          acc_mac(acc, horner_step(sHi[x * 16 + hi], w.x, w.y, 0, 0, k), sBase[x]);  // lazy m_i^(s-sb0) times base
+        }
       }
-      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c96, k);
+      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c224, k);  // plain*plain sums
     }
   }
 }

@@ -43,7 +43,8 @@ bool make_mod(uint64_t p, ZpMod* k) {
 struct Ws {
   int64_t* d_offsets;
   int32_t *st_pre, *st_solve, *st_newton;
-  uint64_t *nodes, *M0, *M1, *scale, *invd, *smont, *R, *V;
+  uint64_t *nodes, *M0, *M1, *scale, *R, *V;
+  ulonglong2 *invd, *smont;  // Newton: {w, w'} tables
   ulonglong4* tab;
   size_t bytes;
 };
@@ -67,8 +68,8 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
   w.M1 = (uint64_t*)take(8 * (size_t)T_tot);
   w.scale = (uint64_t*)take(8 * (size_t)T_tot);
   w.tab = (ulonglong4*)take(32 * (size_t)T_tot);
-  w.invd = (uint64_t*)take(8 * (size_t)B * B);
-  w.smont = (uint64_t*)take(8 * (size_t)B);
+  w.invd = (ulonglong2*)take(16 * (size_t)B * B);
+  w.smont = (ulonglong2*)take(16 * (size_t)B);
   w.R = (uint64_t*)take(8 * (size_t)T_tot);
   w.V = (flags & ZP_WS_BALANCED) ? (uint64_t*)take(8 * (size_t)T_tot * B) : nullptr;
   w.bytes = o;
@@ -147,8 +148,8 @@ const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64
   ++g_launches, k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes, w.d_offsets, F, k, w.M0);
   uint64_t *src = w.M0, *dst = w.M1;
   for (int64_t a = ZP_LEAF; a < tmax; a <<= 1) {
-    dim3 gl((unsigned)((tmax + ZP_K2_THREADS - 1) / ZP_K2_THREADS), grid_y(F));
-    ++g_launches, k_tree_level<<<gl, ZP_K2_THREADS, 0, st>>>(src, w.d_offsets, F, a, k, dst);
+    dim3 gl((unsigned)((tmax + ZP_K2_TC - 1) / ZP_K2_TC), grid_y(F));
+    ++g_launches, k_tree_level<<<gl, ZP_K2_TC, 0, st>>>(src, w.d_offsets, F, a, k, dst);
     uint64_t* tmp = src;
     src = dst;
     dst = tmp;
@@ -183,7 +184,7 @@ void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* val
   ++g_launches, k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
   ++g_launches, k_newton_prep<<<(B * B + 127) / 128, 128, 0, st>>>(samples, B, k, w.invd, w.smont, w.st_newton);
   ProfScope prof(ZP_K_NEWTON, st);
-  const size_t smem = 8 * ((size_t)B * B + B + 2 * (size_t)B * ZP_K5_THREADS);
+  const size_t smem = 16 * ((size_t)B * B + B) + 16 * (size_t)B * ZP_K5_THREADS;
   cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
   if (blocks > 148 * 64) blocks = 148 * 64;
