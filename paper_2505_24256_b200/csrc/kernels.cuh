@@ -337,6 +337,8 @@ ZP_DEV uint64_t shoup_mul(uint64_t x, ulonglong2 w, const ZpMod& k) {
 }
 
 #define ZP_K5_THREADS 128
+// CANON: the values are known to be canonical (the lifting step feeds the solve's output), skip the reduction
+template <bool CANON>
 __global__ void __launch_bounds__(ZP_K5_THREADS)
 k_newton(const ulonglong2* __restrict__ invd, const ulonglong2* __restrict__ negc, int B, const uint64_t* vals, int64_t n,
          int64_t ld, ZpMod k, int basis, uint64_t* out) {
@@ -344,14 +346,13 @@ k_newton(const ulonglong2* __restrict__ invd, const ulonglong2* __restrict__ neg
   ulonglong2* sInv = reinterpret_cast<ulonglong2*>(sh);  // [B*B] {w, w'}
   ulonglong2* sC = sInv + B * B;                         // [B]   {-c_j, companion}
   uint64_t* col = reinterpret_cast<uint64_t*>(sC + B) + threadIdx.x;  // column of this lane: col[j*TH]
-  uint64_t* pol = col + (size_t)B * ZP_K5_THREADS;                    // second column (monomial expansion)
   constexpr int TH = ZP_K5_THREADS;
   for (int x = threadIdx.x; x < B * B; x += TH) sInv[x] = invd[x];
   for (int x = threadIdx.x; x < B; x += TH) sC[x] = negc[x];
   __syncthreads();
   const int D = B - 1;
   for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
-    for (int j = 0; j < B; ++j) col[j * TH] = vals[j * ld + i] % k.p;
+    for (int j = 0; j < B; ++j) col[j * TH] = CANON ? vals[j * ld + i] : vals[j * ld + i] % k.p;
     // a_j <- (a_j - a_{j-1}) / (c_j - c_{j-l}), j = D .. l; four independent steps at a time (all loads of a
     // group precede its stores, so the group's products overlap in the pipe)
     for (int l = 1; l <= D; ++l) {
@@ -368,31 +369,26 @@ k_newton(const ulonglong2* __restrict__ invd, const ulonglong2* __restrict__ neg
       for (; j >= l; --j)
         col[j * TH] = shoup_mul(col[j * TH] + k.p - col[(j - 1) * TH], sInv[j * B + (j - l)], k);
     }
-    if (basis == 0) {
-      for (int j = 0; j < B; ++j) out[j * ld + i] = col[j * TH];
-    } else {
-      // P <- [a_D]; for j = D-1 .. 0: P <- P (x - c_j) + a_j
-      int deg = 0;
-      pol[0] = col[D * TH];
+    if (basis == 1) {
+      // P <- [a_D]; for j = D-1 .. 0: P <- P (x - c_j) + a_j, in place.  Before step j the polynomial P (degree
+      // D-j-1) sits in slots j+1 .. D (P_x in slot j+1+x); the step is slot[s] <- slot[s] - c_j slot[s+1] for
+      // s = j .. D-1 ascending (slot s holds a_j for s = j, else the old P_{s-j-1}; slot s+1 is still the old
+      // P_{s-j}); slot D stays.  After step 0 slot d holds the coefficient of x^d.
       for (int j = D - 1; j >= 0; --j) {
         const ulonglong2 nc = sC[j];
-        uint64_t up = pol[deg * TH];
-        pol[(deg + 1) * TH] = up;
-        int x = deg;
-        for (; x - 3 >= 1; x -= 4) {
-          const uint64_t v0 = pol[x * TH], v1 = pol[(x - 1) * TH], v2 = pol[(x - 2) * TH], v3 = pol[(x - 3) * TH],
-                         v4 = pol[(x - 4) * TH];
-          pol[x * TH] = mod_add(v1, shoup_mul(v0, nc, k), k.p);
-          pol[(x - 1) * TH] = mod_add(v2, shoup_mul(v1, nc, k), k.p);
-          pol[(x - 2) * TH] = mod_add(v3, shoup_mul(v2, nc, k), k.p);
-          pol[(x - 3) * TH] = mod_add(v4, shoup_mul(v3, nc, k), k.p);
+        int x = j;
+        for (; x + 3 < D; x += 4) {
+          const uint64_t v0 = col[x * TH], v1 = col[(x + 1) * TH], v2 = col[(x + 2) * TH], v3 = col[(x + 3) * TH],
+                         v4 = col[(x + 4) * TH];
+          col[x * TH] = mod_add(v0, shoup_mul(v1, nc, k), k.p);
+          col[(x + 1) * TH] = mod_add(v1, shoup_mul(v2, nc, k), k.p);
+          col[(x + 2) * TH] = mod_add(v2, shoup_mul(v3, nc, k), k.p);
+          col[(x + 3) * TH] = mod_add(v3, shoup_mul(v4, nc, k), k.p);
         }
-        for (; x >= 1; --x) pol[x * TH] = mod_add(pol[(x - 1) * TH], shoup_mul(pol[x * TH], nc, k), k.p);
-        pol[0] = mod_add(col[j * TH], shoup_mul(pol[0], nc, k), k.p);
-        ++deg;
+        for (; x < D; ++x) col[x * TH] = mod_add(col[x * TH], shoup_mul(col[(x + 1) * TH], nc, k), k.p);
       }
-      for (int j = 0; j < B; ++j) out[j * ld + i] = pol[j * TH];
     }
+    for (int j = 0; j < B; ++j) out[j * ld + i] = col[j * TH];
   }
 }
 

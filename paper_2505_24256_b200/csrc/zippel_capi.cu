@@ -180,15 +180,20 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
 
 // (a5): Newton on [B x n] with leading dimension ld; code into w.st_newton[0]
 void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* vals, int64_t n, int64_t ld,
-                const ZpMod& k, int basis, uint64_t* out, cudaStream_t st) {
+                const ZpMod& k, int basis, uint64_t* out, cudaStream_t st, bool canonical_in) {
   ++g_launches, k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
   ++g_launches, k_newton_prep<<<(B * B + 127) / 128, 128, 0, st>>>(samples, B, k, w.invd, w.smont, w.st_newton);
   ProfScope prof(ZP_K_NEWTON, st);
-  const size_t smem = 16 * ((size_t)B * B + B) + 16 * (size_t)B * ZP_K5_THREADS;
-  cudaFuncSetAttribute(k_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  const size_t smem = 16 * ((size_t)B * B + B) + 8 * (size_t)B * ZP_K5_THREADS;
   int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
   if (blocks > 148 * 64) blocks = 148 * 64;
-  ++g_launches, k_newton<<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
+  if (canonical_in) {
+    cudaFuncSetAttribute(k_newton<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ++g_launches, k_newton<true><<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
+  } else {
+    cudaFuncSetAttribute(k_newton<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ++g_launches, k_newton<false><<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);
+  }
 }
 
 void upload_offsets(const Ws& w, const int64_t* h_offsets, int F, cudaStream_t st) {
@@ -258,7 +263,7 @@ void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T
   const int Fc = f1 - f0;
   run_eval_nodes(exps + a * nv, n, nv, anchors, k, nodes + a, st);
   run_solve(wc, nodes, Fc, T_tot, tmax, vals, B, s0, k, out, st);
-  run_newton(wc, samples, B, out + a, n, T_tot, k, basis, out + a, st);
+  run_newton(wc, samples, B, out + a, n, T_tot, k, basis, out + a, st, true);
   ++g_launches, k_status_finish<<<(Fc + 255) / 256, 256, 0, st>>>(nullptr, wc.st_solve, wc.st_newton, Fc, status + f0);
 }
 
@@ -350,7 +355,7 @@ int newton_interp_batch(const uint64_t* samples, int B, const uint64_t* vals, in
   const Ws w = carve(workspace, 1, 1, B, 0);
   (void)one;
   cudaStream_t st = (cudaStream_t)stream;
-  run_newton(w, samples, B, vals, n, ld, k, basis, out, st);
+  run_newton(w, samples, B, vals, n, ld, k, basis, out, st, false);
   ++g_launches, k_status_finish<<<1, 32, 0, st>>>(nullptr, nullptr, w.st_newton, 1, status);
   return cuda_ok();
 }
@@ -478,7 +483,7 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
       ++g_launches, k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
     }
     run_solve(w, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
-    run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st);
+    run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st, true);
     ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
   }
   return cuda_ok();

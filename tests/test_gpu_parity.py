@@ -218,7 +218,7 @@ def test_solve_status_duplicate_and_zero_node(zp, ref):
 
 
 # ------------------------------------------------------------------------------ (a5) Newton
-@pytest.mark.parametrize("B", [1, 2, 3, 9, 21, 25, 64])
+@pytest.mark.parametrize("B", [1, 2, 3, 9, 16, 17, 21, 25, 32, 33, 64])
 @pytest.mark.parametrize("basis", [0, 1])
 def test_newton_parity(zp, ref, B, basis):
     p = P63
