@@ -18,6 +18,8 @@
 //  13 acc_mac2            two such MACs with merged carries (the node-solve loop's form; counts 2 MACs)
 //  14 acc_mac_split       bare products, all additions on the alu pipe
 //  15 acc_mac_hyb         even lattice inside IMAD.WIDE, middle products bare + alu
+//  16 as 3 with the multiplicand in an even register (register-bank experiment: 3 has both multiplicands odd)
+//  17/18/19 as 3 with multiplicands (lo, hi) / (lo, lo) / (hi, hi) halves of live 64-bit pairs: even+odd / even+even / odd+odd
 #pragma once
 #include "modarith.cuh"
 
@@ -79,6 +81,16 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
         } else if (KIND == 3) {
           asm volatile("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tadd.cc.u64 %0, %0, t;\n\taddc.u32 %1, %1, 0;\n\t}"
                        : "+l"(acc[c]), "+r"(car[c]) : "r"(nb), "r"(b));
+        } else if (KIND == 16) {  // as 3, multiplicand = the neighbour chain's LOW word (even register of its pair)
+          const uint32_t nl = (uint32_t)acc[(c + 1) % ZP_UB_CH];
+          asm volatile("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tadd.cc.u64 %0, %0, t;\n\taddc.u32 %1, %1, 0;\n\t}"
+                       : "+l"(acc[c]), "+r"(car[c]) : "r"(nl), "r"(b));
+        } else if (KIND >= 17 && KIND <= 19) {  // register-bank experiment: both multiplicands are halves of live pairs
+          const uint64_t n1 = acc[(c + 1) % ZP_UB_CH], n2 = acc[(c + 2) % ZP_UB_CH];
+          const uint32_t ma = (KIND == 19) ? (uint32_t)(n1 >> 32) : (uint32_t)n1;  // 17: lo, 18: lo, 19: hi
+          const uint32_t mb = (KIND == 18) ? (uint32_t)n2 : (uint32_t)(n2 >> 32);  // 17: hi, 18: lo, 19: hi
+          asm volatile("{\n\t.reg .u64 t;\n\tmul.wide.u32 t, %2, %3;\n\tadd.cc.u64 %0, %0, t;\n\taddc.u32 %1, %1, 0;\n\t}"
+                       : "+l"(acc[c]), "+r"(car[c]) : "r"(ma), "r"(mb));
         } else if (KIND == 4) {
           asm volatile("add.u32 %0, %0, %1;" : "+r"(car[c]) : "r"(lo));
           asm volatile("xor.b32 %0, %0, %1;" : "+r"(lo) : "r"(car[c]));

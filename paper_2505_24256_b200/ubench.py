@@ -24,6 +24,9 @@ KINDS = [
     (11, "IMAD.WIDE.U32 zero addend (mul.wide.u32)", 1),
     (12, "acc_mac (4 accumulating wide)", 4), (13, "acc_mac2 (2 MACs, 8 accumulating wide)", 8),
     (14, "acc_mac_split (4 bare wide + alu chains)", 4), (15, "acc_mac_hyb (2 accumulating + 2 bare wide)", 4),
+    (16, "as 3, one multiplicand in an even register", 1),
+    (17, "accumulating IMAD.WIDE, multiplicands even+odd", 1), (18, "accumulating IMAD.WIDE, multiplicands even+even", 1),
+    (19, "accumulating IMAD.WIDE, multiplicands odd+odd", 1),
 ]
 
 
