@@ -72,6 +72,7 @@ def lib():
         L.ref_balanced_zippel_lift_step.argtypes = [C.POINTER(_Part), C.POINTER(_Part), C.c_int, C.c_int,
                                                     u64p, u64p, C.c_int, C.c_int, u64, C.c_int, i32p]
         L.ref_poly_rows_eval.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p]
+        L.ref_thiele_reconstruct_batch.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p, u64p, i32p, u64p, i32p]
         L.ref_eval_sparse.restype = u64
         L.ref_eval_sparse.argtypes = [u16p, u64p, C.c_int64, C.c_int, u64p, u64]
         _lib = L
@@ -221,3 +222,15 @@ def eval_sparse(exps, coef, point, p):
     exps, coef, point = _a(exps, np.uint16), _a(coef, np.uint64), _a(point, np.uint64)
     return int(lib().ref_eval_sparse(_p(exps, u16p), _p(coef, u64p), exps.shape[0], exps.shape[1],
                                      _p(point, u64p), p))
+
+
+def thiele_reconstruct_batch(points, vals, p):
+    """(f2) eq. (2): vals [T, n] -> (num [T, n], den [T, n], degs [2, n], cf [T, n], status [n])."""
+    points, vals = _a(points, np.uint64), _a(vals, np.uint64)
+    T, n = vals.shape
+    num, den, cf = np.zeros_like(vals), np.zeros_like(vals), np.zeros_like(vals)
+    degs = np.zeros((2, n), dtype=np.int32)
+    status = np.zeros(n, dtype=np.int32)
+    _ok(lib().ref_thiele_reconstruct_batch(_p(points, u64p), T, _p(vals, u64p), n, n, p, _p(num, u64p), _p(den, u64p),
+                                           _p(degs, i32p), _p(cf, u64p), _p(status, i32p)), "thiele_reconstruct_batch")
+    return num, den, degs, cf, status

@@ -421,3 +421,98 @@ uint64_t ref_eval_sparse(const uint16_t* exps, const uint64_t* coef, int64_t t, 
   }
   return r;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * (f2) Thiele reconstruction, eq. (2); see zippel_ref.h for the statement.
+ * Literal form: one modular inverse per inverse difference, no batching.
+ * ---------------------------------------------------------------------------------------- */
+int ref_thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals, int64_t n, int64_t ld,
+                                 uint64_t p, uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf,
+                                 int32_t* status) {
+  if (!points || !vals || !num || !den || !degs || !status || T <= 0 || n <= 0 || ld < n) return REF_ERR_ARG;
+  int32_t dup = 0;
+  for (int j = 0; j < T && !dup; ++j)
+    for (int jj = 0; jj < j; ++jj)
+      if (points[j] % p == points[jj] % p) {
+        dup = (int32_t)(((uint32_t)j << 8) | REF_ST_DUPLICATE_SAMPLE);
+        break;
+      }
+  uint64_t* phi = (uint64_t*)malloc((size_t)T * sizeof(uint64_t));
+  uint64_t* b = (uint64_t*)malloc((size_t)T * sizeof(uint64_t));
+  uint64_t* N = (uint64_t*)calloc((size_t)T + 1, sizeof(uint64_t));
+  uint64_t* D = (uint64_t*)calloc((size_t)T + 1, sizeof(uint64_t));
+  uint64_t* Nn = (uint64_t*)calloc((size_t)T + 1, sizeof(uint64_t));
+  for (int64_t i = 0; i < n; ++i) {
+    for (int d = 0; d < T; ++d) {
+      num[(int64_t)d * ld + i] = 0;
+      den[(int64_t)d * ld + i] = 0;
+      if (cf) cf[(int64_t)d * ld + i] = 0;
+    }
+    degs[i] = -1;
+    degs[ld + i] = -1;
+    status[i] = dup;
+    if (dup) continue;
+    /* inverse differences */
+    for (int j = 0; j < T; ++j) phi[j] = vals[(int64_t)j * ld + i] % p;
+    int K = T, bad = 0;
+    b[0] = phi[0];
+    for (int k = 1; k < T; ++k) {
+      int zeros = 0;
+      for (int j = k; j < T; ++j) zeros += (phi[j] == phi[k - 1]);
+      if (zeros == T - k) {
+        K = k;
+        break;
+      }
+      if (zeros != 0) {
+        bad = k;
+        break;
+      }
+      for (int j = T - 1; j >= k; --j)
+        phi[j] = ref_mulmod(ref_submod(points[j] % p, points[k - 1] % p, p),
+                            ref_invmod(ref_submod(phi[j], phi[k - 1], p), p), p);
+      b[k] = phi[k];
+    }
+    if (bad) {
+      status[i] = (int32_t)(((uint32_t)bad << 8) | REF_ST_THIELE_DEGENERATE);
+      continue;
+    }
+    if (cf)
+      for (int k = 0; k < K; ++k) cf[(int64_t)k * ld + i] = b[k];
+    /* expansion from the tail: (N, D) <- (b_k N + (x - x_k) D, N) */
+    for (int d = 0; d <= T; ++d) N[d] = D[d] = 0;
+    N[0] = b[K - 1];
+    D[0] = 1 % p;
+    for (int k = K - 2; k >= 0; --k) {
+      const uint64_t xk = points[k] % p;
+      for (int d = 0; d <= T; ++d) {
+        uint64_t v = ref_mulmod(b[k], N[d], p);                       /* b_k N        */
+        if (d >= 1) v = ref_addmod(v, D[d - 1], p);                   /* + x D        */
+        v = ref_submod(v, ref_mulmod(xk, D[d], p), p);                /* - x_k D      */
+        Nn[d] = v;
+      }
+      for (int d = 0; d <= T; ++d) {
+        D[d] = N[d];
+        N[d] = Nn[d];
+      }
+    }
+    int dn = T, dd = T;
+    while (dn >= 0 && N[dn] == 0) --dn;
+    while (dd >= 0 && D[dd] == 0) --dd;
+    /* D = previous N is never the zero polynomial unless f has a pole at every point: treat as degenerate */
+    if (dd < 0) {
+      status[i] = (int32_t)(((uint32_t)0 << 8) | REF_ST_THIELE_DEGENERATE);
+      continue;
+    }
+    const uint64_t sc = ref_invmod(D[dd], p);
+    for (int d = 0; d <= dn; ++d) num[(int64_t)d * ld + i] = ref_mulmod(N[d], sc, p);
+    for (int d = 0; d <= dd; ++d) den[(int64_t)d * ld + i] = ref_mulmod(D[d], sc, p);
+    degs[i] = dn;
+    degs[ld + i] = dd;
+  }
+  free(phi);
+  free(b);
+  free(N);
+  free(D);
+  free(Nn);
+  return REF_OK;
+}

@@ -47,6 +47,7 @@ extern "C" {
 #define REF_ST_DUPLICATE_NODE 16   /* den_i == 0 (two terms map to one node) or m_i == 0 with s0 = 1 */
 #define REF_ST_DUPLICATE_SAMPLE 17 /* c_j == c_j' in Newton */
 #define REF_ST_ZERO_PIVOT 18       /* u_{0,s} == 0 in balancing */
+#define REF_ST_THIELE_DEGENERATE 20 /* an inverse difference of eq. (2) has a zero denominator at some but not all points */
 
 /* ---- arithmetic in Z/pZ (variant 1 is the definition) ---- */
 uint64_t ref_mulmod(uint64_t a, uint64_t b, uint64_t p);
@@ -121,6 +122,22 @@ int ref_poly_rows_eval(const uint64_t* samples, int B, const uint64_t* P, int64_
 /* ---- fresh probes: value of a sparse polynomial sum_i coef_i prod_j z_j^{e_ij} ---- */
 uint64_t ref_eval_sparse(const uint16_t* exps, const uint64_t* coef, int64_t t, int nv,
                          const uint64_t* point, uint64_t p);
+
+/* ---- (f2) univariate Thiele reconstruction, eq. (2), one column of values at a time:
+ *   f(x) = b_0 + (x - x_0) / ( b_1 + (x - x_1) / ( b_2 + ... + (x - x_{K-2}) / b_{K-1} ) )      (0-based)
+ * with the inverse differences  phi_0(x_i) = f(x_i),  phi_k(x_i) = (x_i - x_{k-1}) / (phi_{k-1}(x_i) - phi_{k-1}(x_{k-1})),
+ * i >= k, and b_k = phi_k(x_k).  The fraction ends at K = k terms when every phi_{k-1}(x_i), i >= k, equals
+ * phi_{k-1}(x_{k-1}) (the function is reproduced at all remaining points); K = T if that never happens.  If
+ * only some of them are equal the column gets status (k << 8) | REF_ST_THIELE_DEGENERATE and zero output.
+ * The fraction is then expanded from the tail, (N, D) <- (b_k N + (x - x_k) D, N), starting at (b_{K-1}, 1),
+ * trimmed to its true degrees and scaled so that D is monic.
+ *   points [T] pairwise distinct; vals [T x n] (row j = values at x_j, leading dimension ld)
+ *   num, den [T x n]: row d = coefficient of x^d (zero above the degree); degs [2 x n]: deg N, deg D (deg N = -1
+ *   for the zero function); cf [T x n]: b_0..b_{K-1} (zero above K), may be NULL; status [n].
+ * A duplicate point: every status = (j << 8) | REF_ST_DUPLICATE_SAMPLE. ---- */
+int ref_thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals, int64_t n, int64_t ld,
+                                 uint64_t p, uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf,
+                                 int32_t* status);
 
 #ifdef __cplusplus
 }
