@@ -51,7 +51,8 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6],
+                    help="1-5: BASELINE.json configs; 6: batched Thiele reconstruction (SURVEY.md row f2), C4's input side")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -381,9 +382,96 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ---------------------------------------------------------------------------------------- (f2) Thiele leg
+def thiele_inputs(n, T, seed):
+    """Arbitrary residues as values (every column runs the full T levels: the cost model's case) at T distinct
+    points; shaped like C4's input side: 1024 functions x 500 probes, degree <= 24 in x_6 -> T = 50 points."""
+    from paper_2505_24256_b200 import workloads as wl
+
+    pts = wl.distinct_residues(wl._rng(seed, 40), 2, wl.P63, T)
+    vals = wl.uniform_residues(wl._rng(seed, 41), 0, wl.P63, (T, n))
+    return pts, vals, wl.P63
+
+
+def run_thiele(args):
+    import torch
+
+    from paper_2505_24256_b200 import api, workloads as wl
+
+    T, n = 50, (args.F or 1024) * 500
+    K, W = args.steps, args.warmup
+    if args.impl == "reference":
+        from oracle import ref
+
+        pts, vals, p = thiele_inputs(4000, T, wl.SEED_BASE + 6)
+        ta = time.perf_counter()
+        for _ in range(K):
+            ref.thiele_reconstruct_batch(pts, vals, p)
+        dt = (time.perf_counter() - ta) / K
+        cpu = {"value": 4000 / dt, "unit": "reconstructions/s", "cores": 1, "kind": "oracle", "sample": "4000 columns, T = 50"}
+        print(json.dumps({"impl": "reference", "metric": "thiele_reconstructions_per_s", "value": 4000 / dt,
+                          "unit": "reconstructions/s", "n_gpus": 1, "steps": K, "warmup": 0, "ms_per_step": dt * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+                          "config": {"workload": "Thiele via the CPU oracle; each step = 4000 columns, T = 50"},
+                          "cpu_baseline": cpu, "gpu_launches": 0,
+                          "e2e": {"value": 4000 / dt, "unit": "reconstructions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+    torch.cuda.set_device(0)
+    api.lib()
+    pts, vals, p = thiele_inputs(n, T, wl.SEED_BASE + 6)
+    dp, dv = api.to_dev(pts), api.to_dev(vals)
+    ws = api.alloc_workspace([0, 1], T)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            out = api.thiele_reconstruct_batch(dp, dv, p, want_cf=False, workspace=ws, stream=stream)
+        torch.cuda.synchronize()
+        assert not api.to_host(out[4]).any()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(0)
+        time.sleep(0.3)
+        n0, t0 = api.zippel_launch_count(), time.perf_counter()
+        e0.record(stream)
+        for _ in range(K):
+            api.thiele_reconstruct_batch(dp, dv, p, want_cf=False, workspace=ws, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        ms = e0.elapsed_time(e1) / K
+    clocks = sampler.stop(t0, t1)
+    # algorithmic Montgomery products per column (DESIGN.md section 9), fraction form: 4 per point and level
+    # (2T^2 - 2T), one batched inversion of the b_k (3T + 93), expansion (T^2/2 + 2T), monic scaling (T + 94);
+    # 18 units each
+    units = n * 18.0 * (2.5 * T * T + 4 * T + 187)
+    achieved = units / (ms * 1e-3) / 1e12
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import ref
+
+        cp, cv, _ = thiele_inputs(4000, T, wl.SEED_BASE + 6)
+        ta = time.perf_counter()
+        ref.thiele_reconstruct_batch(cp, cv, p)
+        dt = time.perf_counter() - ta
+        cpu = {"value": 4000 / dt, "unit": "reconstructions/s", "cores": 1, "kind": "oracle", "sample": "4000 columns, T = 50"}
+    print(json.dumps({
+        "metric": "thiele_reconstructions_per_s", "value": n / (ms * 1e-3), "unit": "reconstructions/s", "n_gpus": 1,
+        "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u64", "data": "synthetic",
+        "config": {"workload": f"Thiele batch: n={n} columns (1024 functions x 500 probes), T={T} points, p=2^63-25",
+                   "l2": "inputs larger than L2 (205 MB of values per step)"},
+        "gpu_launches": int(api.zippel_launch_count() - n0), "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "k_thiele", "achieved": achieved, "peak": IMAD_PEAK_TOPS,
+                     "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
+                     "traffic": None, "algorithmic_ops_per_launch": units, "ms_per_launch": ms,
+                     "algorithmic_cost": "Montgomery product = 18 units; (2.5 T^2 + 4 T + 187) products per column"},
+        "e2e": None, "cpu_baseline": cpu}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.impl == "reference":
+    if a.config == 6:
+        run_thiele(a)
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_ours(a)

@@ -39,6 +39,8 @@ extern "C" {
 #define ZP_ST_DUPLICATE_NODE 16   /* den_i == 0: two terms map to one node (G24); or m_i == 0 with s0 = 1 (G25) */
 #define ZP_ST_DUPLICATE_SAMPLE 17 /* c_j == c_j' for some j' < j in Newton (index = j) */
 #define ZP_ST_ZERO_PIVOT 18       /* u_{0,s} == 0 in balancing (index = s) */
+#define ZP_ST_THIELE_DEGENERATE 20 /* Thiele: an inverse difference of level k has a zero denominator at some but
+                                      not all of the remaining points (index = k); or the denominator vanished */
 
 #define ZP_MAX_NV 32 /* skeleton variables */
 #define ZP_MAX_B 64  /* sample values of x_k (D + 1) */
@@ -130,6 +132,25 @@ typedef struct {
 int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int nv, const uint64_t* anchors,
                               const uint64_t* samples, int B, int s0, uint64_t p, int basis, int32_t* status,
                               void* workspace, size_t workspace_bytes, void* stream);
+
+/* (f2, SURVEY.md section 8 "next") Batched univariate Thiele reconstruction, eq. (2): for every
+ * column i of values f_i(x_j) at the T pairwise distinct points x_0..x_{T-1} (device, residues), the continued
+ * fraction   f(x) = b_0 + (x - x_0) / (b_1 + (x - x_1) / (b_2 + ... ))   with  b_k = phi_k(x_k),
+ * phi_0 = f,  phi_k(x_j) = (x_j - x_{k-1}) / (phi_{k-1}(x_j) - phi_{k-1}(x_{k-1}))  (j >= k).  The fraction ends at
+ * K = k terms when ALL differences of level k vanish (the function is reproduced at the remaining points);
+ * K = T otherwise.  It is then expanded to N(x) / D(x), trimmed to the true degrees and scaled so that D is
+ * monic: these are the normalised univariate numerator and denominator whose values at the samples feed
+ * balanced_zippel_lift_step (reading G3).  One lane per column.
+ *   vals [T x n], leading dimension ld >= n, row j = values at x_j (device);  T <= ZP_MAX_B
+ *   num, den [T x n] (ld): row d = coefficient of x^d, zero above the degree
+ *   degs [2 x ld] int32: degs[i] = deg N (-1 for the zero function), degs[ld + i] = deg D
+ *   cf   [T x n] (ld) or NULL: b_0 .. b_{K-1}, zero above K
+ *   status [n]: 0, (k << 8) | ZP_ST_THIELE_DEGENERATE (outputs of that column are zero, degs -1), or
+ *               (j << 8) | ZP_ST_DUPLICATE_SAMPLE for every column when x_j repeats an earlier point.
+ *   workspace: zippel_workspace_bytes({0,1}, 1, T, 0) bytes. */
+int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals, int64_t n, int64_t ld, uint64_t p,
+                             uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf, int32_t* status,
+                             void* workspace, size_t workspace_bytes, void* stream);
 
 /* Measurement hook (bench.py's roofline leg): when kernel != 0, every later call records the CUDA event
  * `ev_start` on its stream right before the first launch of that kernel and `ev_stop` right after the

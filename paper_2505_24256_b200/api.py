@@ -28,7 +28,7 @@ EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
     "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
-    "zippel_launch_count", "zippel_ubench",
+    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch",
 )
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
         L.zippel_modarith_selftest.argtypes = [i32, vp, vp, i64, u64, vp, vp]
         L.zippel_profile_events.argtypes = [i32, vp, vp]
         L.zippel_ubench.argtypes = [i32, i32, i32, u64, vp, C.POINTER(C.c_double), vp]
+        L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         L.zippel_launch_count.restype = C.c_ulonglong
         L.zippel_launch_count.argtypes = []
         _lib = L
@@ -317,3 +318,26 @@ def zippel_ubench(kind: int, iters: int, blocks: int, p: int, out: torch.Tensor,
     n = C.c_double(0.0)
     _check(lib().zippel_ubench(kind, iters, blocks, p, _ptr(out), C.byref(n), _stream(stream)), "zippel_ubench")
     return n.value
+
+
+ST_THIELE_DEGENERATE = 20
+
+
+def thiele_reconstruct_batch(points: torch.Tensor, vals: torch.Tensor, p: int, want_cf: bool = True,
+                             workspace: Optional[torch.Tensor] = None, stream=None):
+    """(f2) eq. (2): vals [T, n] -> (num [T, n], den [T, n], degs [2, n] int32, cf [T, n] or None, status [n])."""
+    _need_cuda()
+    T, n = vals.shape
+    assert vals.stride(1) == 1
+    ld = vals.stride(0) if T > 1 else n
+    mk = lambda: torch.empty((T, ld), dtype=vals.dtype, device=vals.device)  # outputs share the input's leading dimension
+    num, den = mk(), mk()
+    cf = mk() if want_cf else None
+    degs = torch.empty((2, ld), dtype=torch.int32, device=vals.device)
+    status = torch.empty(n, dtype=torch.int32, device=vals.device)
+    if workspace is None:
+        workspace = alloc_workspace([0, 1], T)
+    _check(lib().thiele_reconstruct_batch(points.data_ptr(), T, vals.data_ptr(), n, ld, p, num.data_ptr(), den.data_ptr(),
+                                          degs.data_ptr(), _ptr(cf), status.data_ptr(), _ptr(workspace),
+                                          workspace.numel(), _stream(stream)), "thiele_reconstruct_batch")
+    return num[:, :n], den[:, :n], degs[:, :n], None if cf is None else cf[:, :n], status

@@ -487,6 +487,151 @@ __global__ void k_balance(const uint64_t* __restrict__ u, const uint64_t* __rest
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// (f2) Thiele reconstruction in one variable, one lane per column of values (eq. (2)):
+//   f(x) = b_0 + (x - x_0) / (b_1 + (x - x_1) / (b_2 + ...)),   b_k = phi_k(x_k),
+//   phi_0(x_j) = f(x_j),  phi_k(x_j) = (x_j - x_{k-1}) / (phi_{k-1}(x_j) - phi_{k-1}(x_{k-1})),  j >= k.
+// Level k inverts its T - k differences with ONE modular inverse (prefix products, Montgomery's trick; the
+// batched inversion of SURVEY.md row a4).  The fraction ends at K = k when all differences of level k vanish;
+// some but not all vanishing -> ZP_ST_THIELE_DEGENERATE.  Expansion from the tail, in place in two columns:
+//   (N, D) <- (b_k N + (x - x_k) D, N),  then trim to the true degrees and scale D monic.
+// Columns live in shared memory (column stride = lanes per CTA); everything is in Montgomery form.
+// k_thiele_prep: xd[j*T + k] = (x_j - x_k)~, xm[j] = x_j~, duplicate check.
+// ------------------------------------------------------------------------------------------------
+#define ZP_ST_THIELE_DEGENERATE 20
+__global__ void k_thiele_prep(const uint64_t* __restrict__ points, int T, ZpMod k, uint64_t* __restrict__ xd,
+                              uint64_t* __restrict__ xm, int32_t* __restrict__ dup) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= T * T) return;
+  const int j = idx / T, kk = idx % T;
+  const uint64_t diff = mod_sub(points[j] % k.p, points[kk] % k.p, k.p);
+  if (kk < j && diff == 0) atomicMin(dup, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
+  xd[idx] = to_mont(diff, k);
+  if (kk == 0) xm[j] = to_mont(points[j] % k.p, k);
+}
+
+#define ZP_K8_THREADS 64
+// The inverse differences are carried as fractions phi_k(x_j) = A_j / B_j, so that a level is four independent
+// Montgomery products per point and no inversion:
+//   A_j <- (x_j - x_{k-1}) B_j B_p ,   B_j <- A_j B_p - A_p B_j      (p = k-1, the pivot; j = k .. T-1),
+// B_j = 0 <=> the oracle's zero denominator.  The b_k = A_k / B_k come from ONE batched inversion at the end
+// (prefix products, Montgomery's trick), the monic scaling from a second one: 2 inversions per column in all.
+__global__ void __launch_bounds__(ZP_K8_THREADS)
+k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const int32_t* __restrict__ dup, int T,
+         const uint64_t* __restrict__ vals, int64_t n, int64_t ld, ZpMod k, uint64_t* __restrict__ num,
+         uint64_t* __restrict__ den, int32_t* __restrict__ degs, uint64_t* __restrict__ cf, int32_t* __restrict__ status) {
+  extern __shared__ __align__(16) uint64_t sh[];
+  constexpr int TH = ZP_K8_THREADS;
+  uint64_t* Ac = sh + threadIdx.x;                 // column A_j (ends as b_0 .. b_{K-1}), stride TH
+  uint64_t* Bc = Ac + (size_t)(T + 2) * TH;        // column B_j; later N (slots 0 ..) and D (slots T/2+1 ..)
+  const int32_t dupst = dup[0];
+  for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
+    for (int d = 0; d < T; ++d) {
+      num[d * ld + i] = 0;
+      den[d * ld + i] = 0;
+      if (cf) cf[d * ld + i] = 0;
+    }
+    degs[i] = -1;
+    degs[ld + i] = -1;
+    if (dupst != ZP_ST_NONE) {
+      status[i] = dupst;
+      continue;
+    }
+    for (int j = 0; j < T; ++j) {
+      Ac[j * TH] = to_mont(vals[j * ld + i] % k.p, k);
+      Bc[j * TH] = k.r1;
+    }
+    int K = T, bad = 0;
+    for (int kk = 1; kk < T; ++kk) {
+      const uint64_t Ap = Ac[(kk - 1) * TH], Bp = Bc[(kk - 1) * TH];
+      const uint64_t* xrow = xd + (kk - 1);  // xd[j*T + kk-1] = (x_j - x_{kk-1})~
+      int zeros = 0;
+      int j = kk;
+      for (; j + 1 < T; j += 2) {  // two points at a time: eight independent products in flight
+        const uint64_t a0 = Ac[j * TH], b0 = Bc[j * TH], a1 = Ac[(j + 1) * TH], b1 = Bc[(j + 1) * TH];
+        const uint64_t nb0 = mod_sub(mont_mul(a0, Bp, k), mont_mul(Ap, b0, k), k.p);
+        const uint64_t nb1 = mod_sub(mont_mul(a1, Bp, k), mont_mul(Ap, b1, k), k.p);
+        const uint64_t na0 = mont_mul(mont_mul(b0, Bp, k), __ldg(xrow + (size_t)j * T), k);
+        const uint64_t na1 = mont_mul(mont_mul(b1, Bp, k), __ldg(xrow + (size_t)(j + 1) * T), k);
+        zeros += (nb0 == 0) + (nb1 == 0);
+        Ac[j * TH] = na0;
+        Bc[j * TH] = nb0;
+        Ac[(j + 1) * TH] = na1;
+        Bc[(j + 1) * TH] = nb1;
+      }
+      if (j < T) {
+        const uint64_t a0 = Ac[j * TH], b0 = Bc[j * TH];
+        const uint64_t nb0 = mod_sub(mont_mul(a0, Bp, k), mont_mul(Ap, b0, k), k.p);
+        Ac[j * TH] = mont_mul(mont_mul(b0, Bp, k), __ldg(xrow + (size_t)j * T), k);
+        Bc[j * TH] = nb0;
+        zeros += (nb0 == 0);
+      }
+      if (zeros == T - kk) {
+        K = kk;
+        break;
+      }
+      if (zeros != 0) {
+        bad = kk;
+        break;
+      }
+    }
+    if (bad) {
+      status[i] = (int32_t)(((uint32_t)bad << 8) | ZP_ST_THIELE_DEGENERATE);
+      continue;
+    }
+    // b_k = A_k / B_k, k < K, by one batched inversion; the prefix products are parked in this lane's own
+    // output column num[., i] (global, unit stride across lanes, overwritten with the result below)
+    {
+      uint64_t run = k.r1;
+      for (int kk = 0; kk < K; ++kk) {
+        run = mont_mul(run, Bc[kk * TH], k);
+        num[kk * ld + i] = run;  // scratch: prefix products (overwritten with zeros / results below)
+      }
+      uint64_t inv = mont_inv(run, k);
+      for (int kk = K - 1; kk >= 0; --kk) {
+        const uint64_t invk = (kk > 0) ? mont_mul(inv, num[(kk - 1) * ld + i], k) : inv;  // 1 / B_k
+        inv = mont_mul(inv, Bc[kk * TH], k);
+        Ac[kk * TH] = mont_mul(Ac[kk * TH], invk, k);  // b_k
+        num[kk * ld + i] = 0;
+      }
+    }
+    if (cf)
+      for (int kk = 0; kk < K; ++kk) cf[kk * ld + i] = from_mont(Ac[kk * TH], k);
+    // expansion from the tail, in place: after s steps deg N <= (s+1)/2, deg D <= s/2
+    uint64_t* Nc = Bc;
+    uint64_t* Dc = Bc + (size_t)(T / 2 + 1) * TH;
+    const int half = T / 2;
+    for (int d = 0; d <= half; ++d) Nc[d * TH] = Dc[d * TH] = 0;
+    Nc[0] = Ac[(K - 1) * TH];
+    Dc[0] = k.r1;
+    for (int kk = K - 2, s2 = 1; kk >= 0; --kk, ++s2) {
+      const uint64_t bk = Ac[kk * TH];
+      const uint64_t xk = __ldg(xm + kk);
+      for (int d = (s2 + 1) / 2; d >= 0; --d) {  // descending: D[d-1] is still the old one
+        const uint64_t Nd = Nc[d * TH], Dd = Dc[d * TH];
+        uint64_t v = mont_mul(bk, Nd, k);
+        if (d >= 1) v = mod_add(v, Dc[(d - 1) * TH], k.p);
+        v = mod_sub(v, mont_mul(xk, Dd, k), k.p);
+        Dc[d * TH] = Nd;
+        Nc[d * TH] = v;
+      }
+    }
+    int dn = (K - 1 + 1) / 2, dd = (K - 1) / 2;
+    while (dn >= 0 && Nc[dn * TH] == 0) --dn;
+    while (dd >= 0 && Dc[dd * TH] == 0) --dd;
+    if (dd < 0) {
+      status[i] = (int32_t)ZP_ST_THIELE_DEGENERATE;
+      continue;
+    }
+    const uint64_t sc = mont_inv(Dc[dd * TH], k);
+    for (int d = 0; d <= dn; ++d) num[d * ld + i] = from_mont(mont_mul(Nc[d * TH], sc, k), k);
+    for (int d = 0; d <= dd; ++d) den[d * ld + i] = from_mont(mont_mul(Dc[d * TH], sc, k), k);
+    degs[i] = dn;
+    degs[ld + i] = dd;
+    status[i] = 0;
+  }
+}
+
 // (a0) self-test kernel for the substrate
 __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, ZpMod k, uint64_t* out) {
   if (op == 5) {  // deferred dot through the wide accumulator, one CTA

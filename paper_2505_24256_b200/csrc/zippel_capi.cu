@@ -306,6 +306,7 @@ const char* zippel_strerror(int code) {
     case ZP_ST_DUPLICATE_NODE: return "duplicate (or zero) node";
     case ZP_ST_DUPLICATE_SAMPLE: return "duplicate sample";
     case ZP_ST_ZERO_PIVOT: return "zero pivot in balancing";
+    case ZP_ST_THIELE_DEGENERATE: return "degenerate inverse difference in Thiele reconstruction";
     default: return "unknown";
   }
 }
@@ -486,6 +487,29 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
     run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st, true);
     ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
   }
+  return cuda_ok();
+}
+
+int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals, int64_t n, int64_t ld, uint64_t p,
+                             uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf, int32_t* status,
+                             void* workspace, size_t workspace_bytes, void* stream) {
+  ZpMod k;
+  if (!points || !vals || !num || !den || !degs || !status || T <= 0 || T > ZP_MAX_B || n <= 0 || ld < n ||
+      !make_mod(p, &k))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, 1, 1, T, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, 1, 1, T, 0);
+  cudaStream_t st = (cudaStream_t)stream;
+  uint64_t* xd = reinterpret_cast<uint64_t*>(w.invd);   // [T*T] (the slice holds 16 T^2 bytes)
+  uint64_t* xm = reinterpret_cast<uint64_t*>(w.smont);  // [T]
+  ++g_launches, k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
+  ++g_launches, k_thiele_prep<<<(T * T + 127) / 128, 128, 0, st>>>(points, T, k, xd, xm, w.st_newton);
+  const size_t smem = 8 * 2 * (size_t)(T + 2) * ZP_K8_THREADS;  // two columns per lane
+  cudaFuncSetAttribute(k_thiele, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int64_t blocks = (n + ZP_K8_THREADS - 1) / ZP_K8_THREADS;
+  if (blocks > 148 * 64) blocks = 148 * 64;
+  ++g_launches, k_thiele<<<(unsigned)blocks, ZP_K8_THREADS, smem, st>>>(xd, xm, w.st_newton, T, vals, n, ld, k, num, den,
+                                                                         degs, cf, status);
   return cuda_ok();
 }
 
