@@ -21,7 +21,7 @@ k_eval_nodes(const uint16_t* __restrict__ exps, int64_t T_tot, int nv, const uin
              ZpMod k, uint64_t* __restrict__ nodes) {
   __shared__ uint64_t Y[32 * 16];
   if (threadIdx.x < nv) {
-    uint64_t y = to_mont(anchors[threadIdx.x] % k.p, k);
+    uint64_t y = to_mont(zp_canon(anchors[threadIdx.x], k.p), k);
     for (int b = 0; b < 16; ++b) {
       Y[threadIdx.x * 16 + b] = y;
       y = mont_mul(y, y, k);
@@ -82,7 +82,7 @@ k_tree_leaf(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offs
     if (lo >= t) continue;  // uniform per CTA
     const int n = (int)((t - lo < ZP_LEAF) ? (t - lo) : ZP_LEAF);
     for (int i = threadIdx.x; i < n; i += blockDim.x)
-      buf[0][i] = mod_neg(to_mont(nodes[off + lo + i] % k.p, k), k.p);  // (z - m_i)' = -m_i~
+      buf[0][i] = mod_neg(to_mont(zp_canon(nodes[off + lo + i], k.p), k), k.p);  // (z - m_i)' = -m_i~
     __syncthreads();
     int cur = 0;
     for (int a = 1; a < n; a <<= 1) {  // merge blocks [2j a, 2j a + a) and [2j a + a, 2j a + 2a)
@@ -168,7 +168,7 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
     const int64_t t = offsets[f + 1] - off;
     for (int64_t l = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l <= t; l += (int64_t)gridDim.x * blockDim.x) {
       const uint64_t Mm = (l < t) ? Mt[off + l] : k.r1;
-      const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)l % k.p, k), k);  // (l M_l)~
+      const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)zp_canon(l, k.p), k), k);  // (l M_l)~
       ulonglong4 r;
       r.x = from_mont(Mm, k);
       r.y = shoup_companion(Mm, k);
@@ -227,7 +227,7 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
     if (i0 >= t) continue;  // uniform per CTA
     const int i = i0 + threadIdx.x;
     const bool live = i < t;
-    const uint64_t m = live ? nodes[off + i] % k.p : 0;
+    const uint64_t m = live ? zp_canon(nodes[off + i], k.p) : 0;
     const uint64_t mm = to_mont(m, k);
     const uint64_t mp = shoup_companion(mm, k);
     uint64_t q = 0, d = 0;
@@ -317,7 +317,7 @@ __global__ void k_newton_prep(const uint64_t* __restrict__ samples, int B, ZpMod
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= B * B) return;
   const int j = idx / B, jj = idx % B;
-  const uint64_t cj = samples[j] % k.p, cjj = samples[jj] % k.p;
+  const uint64_t cj = zp_canon(samples[j], k.p), cjj = zp_canon(samples[jj], k.p);
   if (jj == 0) {  // multiplier -c_j of the monomial expansion, with its Shoup companion
     const uint64_t nc = mod_neg(cj, k.p);
     negc[j] = make_ulonglong2(nc, shoup_companion(to_mont(nc, k), k));
@@ -352,7 +352,7 @@ k_newton(const ulonglong2* __restrict__ invd, const ulonglong2* __restrict__ neg
   __syncthreads();
   const int D = B - 1;
   for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
-    for (int j = 0; j < B; ++j) col[j * TH] = CANON ? vals[j * ld + i] : vals[j * ld + i] % k.p;
+    for (int j = 0; j < B; ++j) col[j * TH] = CANON ? vals[j * ld + i] : zp_canon(vals[j * ld + i], k.p);
     // a_j <- (a_j - a_{j-1}) / (c_j - c_{j-l}), j = D .. l; four independent steps at a time (all loads of a
     // group precede its stores, so the group's products overlap in the pipe)
     for (int l = 1; l <= D; ++l) {
@@ -439,8 +439,8 @@ k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ off
         __syncthreads();
         if (threadIdx.x < n) {
           const int i = i0 + threadIdx.x;
-          const uint64_t m = to_mont(nodes[off + i] % k.p, k);
-          const uint64_t a = coef[(int64_t)b * T_tot + off + i] % k.p;
+          const uint64_t m = to_mont(zp_canon(nodes[off + i], k.p), k);
+          const uint64_t a = zp_canon(coef[(int64_t)b * T_tot + off + i], k.p);
           sBase[threadIdx.x] = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);  // plain * mont -> plain
           uint64_t pw = k.r1;
           for (int x = 0; x < 16; ++x) {
@@ -471,7 +471,7 @@ __global__ void k_balance(const uint64_t* __restrict__ u, const uint64_t* __rest
                           const int64_t* __restrict__ offsets, int F, int64_t T_tot, int B, ZpMod k,
                           uint64_t* __restrict__ V, int32_t* __restrict__ pre) {
   for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < T_tot; x += (int64_t)gridDim.x * blockDim.x) {
-    const uint64_t u0 = u[x] % k.p;
+    const uint64_t u0 = zp_canon(u[x], k.p);
     uint64_t sc = 0;
     if (u0 == 0) {
       int lo = 0, hi = F;  // function of slot x: offsets[lo] <= x < offsets[lo+1]
@@ -483,7 +483,7 @@ __global__ void k_balance(const uint64_t* __restrict__ u, const uint64_t* __rest
     } else {
       sc = mont_mul(to_mont(R[x], k), mont_inv(to_mont(u0, k), k), k);  // (R_s / u_{0,s})~
     }
-    for (int j = 0; j < B; ++j) V[(int64_t)j * T_tot + x] = mont_mul(u[(int64_t)j * T_tot + x] % k.p, sc, k);
+    for (int j = 0; j < B; ++j) V[(int64_t)j * T_tot + x] = mont_mul(zp_canon(u[(int64_t)j * T_tot + x], k.p), sc, k);
   }
 }
 
@@ -504,10 +504,10 @@ __global__ void k_thiele_prep(const uint64_t* __restrict__ points, int T, ZpMod 
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= T * T) return;
   const int j = idx / T, kk = idx % T;
-  const uint64_t diff = mod_sub(points[j] % k.p, points[kk] % k.p, k.p);
+  const uint64_t diff = mod_sub(zp_canon(points[j], k.p), zp_canon(points[kk], k.p), k.p);
   if (kk < j && diff == 0) atomicMin(dup, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
   xd[idx] = to_mont(diff, k);
-  if (kk == 0) xm[j] = to_mont(points[j] % k.p, k);
+  if (kk == 0) xm[j] = to_mont(zp_canon(points[j], k.p), k);
 }
 
 #define ZP_K8_THREADS 64
@@ -538,7 +538,7 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
       continue;
     }
     for (int j = 0; j < T; ++j) {
-      Ac[j * TH] = to_mont(vals[j * ld + i] % k.p, k);
+      Ac[j * TH] = to_mont(zp_canon(vals[j * ld + i], k.p), k);
       Bc[j * TH] = k.r1;
     }
     int K = T, bad = 0;
@@ -638,7 +638,7 @@ __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b
     __shared__ uint64_t part[256];
     Acc acc;
     acc_zero(acc);
-    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) acc_mac(acc, to_mont(a[i] % k.p, k), b[i]);
+    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) acc_mac(acc, to_mont(zp_canon(a[i], k.p), k), b[i]);
     part[threadIdx.x] = mont_mul(acc_redc160(acc, k), k.c160, k);  // mont * plain -> plain
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -649,15 +649,15 @@ __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b
     return;
   }
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    const uint64_t x = a[i] % k.p, y = b ? b[i] : 0;
+    const uint64_t x = zp_canon(a[i], k.p), y = b ? b[i] : 0;
     uint64_t r = 0;
-    if (op == 0) r = from_mont(mont_mul(to_mont(x, k), to_mont(y % k.p, k), k), k);
-    if (op == 1) r = mod_add(x, y % k.p, k.p);
-    if (op == 2) r = mod_sub(x, y % k.p, k.p);
+    if (op == 0) r = from_mont(mont_mul(to_mont(x, k), to_mont(zp_canon(y, k.p), k), k), k);
+    if (op == 1) r = mod_add(x, zp_canon(y, k.p), k.p);
+    if (op == 2) r = mod_sub(x, zp_canon(y, k.p), k.p);
     if (op == 3) r = from_mont(mont_pow(to_mont(x, k), y, k), k);
     if (op == 4) r = from_mont(mont_inv(to_mont(x, k), k), k);
     if (op == 6) {  // Horner step on a LAZY x (any 64-bit value): (y x + a[(i+1) % n]) mod p
-      const uint64_t m = y % k.p, ad = a[(i + 1) % n] % k.p;
+      const uint64_t m = zp_canon(y, k.p), ad = zp_canon(a[(i + 1) % n], k.p);
       r = lazy_canon(horner_step(a[i], m, shoup_companion(to_mont(m, k), k), ad, shoup_companion(to_mont(ad, k), k), k), k.p);
     }
     out[i] = r;

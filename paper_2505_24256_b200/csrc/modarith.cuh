@@ -58,6 +58,9 @@ ZP_DEV uint64_t mod_sub(uint64_t a, uint64_t b, uint64_t p) {
   return (a >= b) ? r : r + p;
 }
 ZP_DEV uint64_t mod_neg(uint64_t a, uint64_t p) { return a ? p - a : 0; }
+// input residue -> canonical.  Callers pass canonical residues (reading G22), so the 64-bit division (about a
+// hundred instructions) sits behind a branch that is practically never taken.
+ZP_DEV uint64_t zp_canon(uint64_t x, uint64_t p) { return x < p ? x : x % p; }
 
 // Montgomery product, column form.  Requires a*b < p*2^64 (true for a < 2^64, b < p); a_hi, b_hi < 2^31
 // is NOT required.  With T = a*b and two 32-bit REDC rounds:
