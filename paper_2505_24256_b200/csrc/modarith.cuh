@@ -62,13 +62,13 @@ ZP_DEV uint64_t mod_neg(uint64_t a, uint64_t p) { return a ? p - a : 0; }
 // hundred instructions) sits behind a branch that is practically never taken.
 ZP_DEV uint64_t zp_canon(uint64_t x, uint64_t p) { return x < p ? x : x % p; }
 
-// Montgomery product, column form.  Requires a*b < p*2^64 (true for a < 2^64, b < p); a_hi, b_hi < 2^31
+// Montgomery product, column form (mont_mul_v1: the first version, kept for the micro-benchmark).  Requires a*b < p*2^64 (true for a < 2^64, b < p); a_hi, b_hi < 2^31
 // is NOT required.  With T = a*b and two 32-bit REDC rounds:
 //   T + m0*p + m1*p*2^32 = (P00 + Q0) + (P01 + P10 + Q1 + S0)*2^32 + (P11 + S1)*2^64,  divisible by 2^64.
 // Column 0: the low words of P00 and Q0 cancel, its carry is c0 = hi(P00) + hi(Q0) + (lo(P00) != 0) < 2^33.
 // Column 1: P01 + P10 + Q1 + S0 + c0 may exceed 64 bits; `carry` counts the overflows (weight 2^64).
 // Result (T + ...)/2^64 < p + p = 2p < 2^64, then one conditional subtraction.
-ZP_DEV uint64_t mont_mul(uint64_t a, uint64_t b, const ZpMod& k) {
+ZP_DEV uint64_t mont_mul_v1(uint64_t a, uint64_t b, const ZpMod& k) {
   const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32), b0 = (uint32_t)b, b1 = (uint32_t)(b >> 32);
   const uint64_t P00 = zp_mulw(a0, b0);
   const uint64_t P01 = zp_mulw(a0, b1);
@@ -95,6 +95,48 @@ ZP_DEV uint64_t mont_mul(uint64_t a, uint64_t b, const ZpMod& k) {
   const uint64_t c1 = (col1 >> 32) + (S0 >> 32) + ((uint32_t)col1 != 0) + ((uint64_t)carry << 32);
   // P11 + S1 + c1 = exact quotient < 2p + 1 <= 2^64 - ... : no overflow
   const uint64_t r = zp_madw(m1, k.p1, P11 + c1);
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+
+// The form in use (54 pipe cycles against 62.5 for the column form above and 59.7 for v3 below, zippel_ubench kinds
+// 20 / 8 / 21, profiles/r01_final.md): one 64-bit REDC round, written with 64-bit operations (the compiler expands them):
+//     m = lo(T) * (-p^-1 mod 2^64);  (T + m p) / 2^64 = hi(T) + hi(m p) + (lo(T) != 0)  < 2p.
+ZP_DEV uint64_t mont_mul(uint64_t a, uint64_t b, const ZpMod& k) {
+  const uint64_t lo = a * b, hi = __umul64hi(a, b);
+  const uint64_t m = lo * k.ninv64;
+  const uint64_t r = hi + __umul64hi(m, k.p) + (lo != 0);
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+// v3: two 32-bit REDC rounds, every product a bare mul.wide, every addition a 32-bit carry chain (alu pipe).
+ZP_DEV uint64_t mont_mul_v3(uint64_t a, uint64_t b, const ZpMod& k) {
+  const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32), b0 = (uint32_t)b, b1 = (uint32_t)(b >> 32);
+  const uint64_t P00 = zp_mulw(a0, b0), P01 = zp_mulw(a0, b1), P10 = zp_mulw(a1, b0), P11 = zp_mulw(a1, b1);
+  uint32_t t0, t1, t2, t3;
+  asm("{\n\t.reg .u32 x1, y0, y1, z0, z1, w0, w1;\n\t"
+      "mov.b64 {%0, x1}, %4;\n\tmov.b64 {y0, y1}, %5;\n\tmov.b64 {z0, z1}, %6;\n\tmov.b64 {w0, w1}, %7;\n\t"
+      "add.cc.u32 %1, x1, y0;\n\taddc.cc.u32 %2, y1, w0;\n\taddc.u32 %3, w1, 0;\n\t"
+      "add.cc.u32 %1, %1, z0;\n\taddc.cc.u32 %2, %2, z1;\n\taddc.u32 %3, %3, 0;\n\t}"
+      : "=r"(t0), "=r"(t1), "=r"(t2), "=r"(t3)
+      : "l"(P00), "l"(P01), "l"(P10), "l"(P11));
+  const uint32_t m0 = t0 * k.pinv;
+  const uint64_t Q0 = zp_mulw(m0, k.p0), Q1 = zp_mulw(m0, k.p1);
+  asm("{\n\t.reg .u32 q0, q1, r0, r1, dummy;\n\t"
+      "mov.b64 {q0, q1}, %4;\n\tmov.b64 {r0, r1}, %5;\n\t"
+      "add.cc.u32 dummy, %3, q0;\n\taddc.cc.u32 %0, %0, q1;\n\taddc.cc.u32 %1, %1, r1;\n\taddc.u32 %2, %2, 0;\n\t"
+      "add.cc.u32 %0, %0, r0;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.u32 %2, %2, 0;\n\t}"
+      : "+r"(t1), "+r"(t2), "+r"(t3)
+      : "r"(t0), "l"(Q0), "l"(Q1));
+  const uint32_t m1 = t1 * k.pinv;
+  const uint64_t S0 = zp_mulw(m1, k.p0), S1 = zp_mulw(m1, k.p1);
+  asm("{\n\t.reg .u32 q0, q1, r0, r1, dummy;\n\t"
+      "mov.b64 {q0, q1}, %3;\n\tmov.b64 {r0, r1}, %4;\n\t"
+      "add.cc.u32 dummy, %2, q0;\n\taddc.cc.u32 %0, %0, q1;\n\taddc.u32 %1, %1, r1;\n\t"
+      "add.cc.u32 %0, %0, r0;\n\taddc.u32 %1, %1, 0;\n\t}"
+      : "+r"(t2), "+r"(t3)
+      : "r"(t1), "l"(S0), "l"(S1));
+  const uint64_t r = ((uint64_t)t3 << 32) | t2;
   const uint64_t s = r - k.p;
   return (r >= k.p) ? s : r;
 }

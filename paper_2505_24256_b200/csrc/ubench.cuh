@@ -19,6 +19,7 @@
 //  14 acc_mac_split       bare products, all additions on the alu pipe
 //  15 acc_mac_hyb         even lattice inside IMAD.WIDE, middle products bare + alu
 //  16 as 3 with the multiplicand in an even register (register-bank experiment: 3 has both multiplicands odd)
+//  8/20/21 forms of the Montgomery product (8 mont_mul_v1: columns; 20 mont_mul: 64-bit REDC, in use; 21 mont_mul_v3: bare products + 32-bit chains)
 //  17/18/19 as 3 with multiplicands (lo, hi) / (lo, lo) / (hi, hi) halves of live 64-bit pairs: even+odd / even+even / odd+odd
 #pragma once
 #include "modarith.cuh"
@@ -38,7 +39,7 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
     acc[c] = ((uint64_t)(tid + c) << 32) | (a + c);
     car[c] = c;
   }
-  if (KIND == 7 || KIND == 8) {
+  if (KIND == 7 || KIND == 8 || KIND == 20 || KIND == 21) {
 #pragma unroll
     for (int c = 0; c < ZP_UB_CH; ++c) acc[c] %= k.p;
   }
@@ -125,7 +126,11 @@ k_ubench(int iters, ZpMod k, uint64_t* __restrict__ out) {
         } else if (KIND == 7) {
           acc[c] = horner_step(acc[c], m, mp, ad, adp, k);
         } else if (KIND == 8) {
+          acc[c] = mont_mul_v1(acc[c], m, k);
+        } else if (KIND == 20) {
           acc[c] = mont_mul(acc[c], m, k);
+        } else if (KIND == 21) {
+          acc[c] = mont_mul_v3(acc[c], m, k);
         }
       }
     }

@@ -543,10 +543,10 @@ int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64
 
 int zippel_ubench(int kind, int iters, int blocks, uint64_t p, uint64_t* out, double* h_chain_steps, void* stream) {
   ZpMod k;
-  if (kind < 0 || kind > 19 || iters <= 0 || blocks <= 0 || !out || !make_mod(p, &k)) return ZP_ERR_ARG;
+  if (kind < 0 || kind > 21 || iters <= 0 || blocks <= 0 || !out || !make_mod(p, &k)) return ZP_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
 #define ZP_UB(K) case K: ++g_launches, k_ubench<K><<<blocks, ZP_UB_THREADS, 0, st>>>(iters, k, out); break;
-  switch (kind) { ZP_UB(0) ZP_UB(1) ZP_UB(2) ZP_UB(3) ZP_UB(4) ZP_UB(5) ZP_UB(6) ZP_UB(7) ZP_UB(8) ZP_UB(9) ZP_UB(10) ZP_UB(11) ZP_UB(12) ZP_UB(13) ZP_UB(14) ZP_UB(15) ZP_UB(16) ZP_UB(17) ZP_UB(18) ZP_UB(19) }
+  switch (kind) { ZP_UB(0) ZP_UB(1) ZP_UB(2) ZP_UB(3) ZP_UB(4) ZP_UB(5) ZP_UB(6) ZP_UB(7) ZP_UB(8) ZP_UB(9) ZP_UB(10) ZP_UB(11) ZP_UB(12) ZP_UB(13) ZP_UB(14) ZP_UB(15) ZP_UB(16) ZP_UB(17) ZP_UB(18) ZP_UB(19) ZP_UB(20) ZP_UB(21) }
 #undef ZP_UB
   if (h_chain_steps) *h_chain_steps = (double)blocks * ZP_UB_THREADS * (double)iters * 8.0 * ZP_UB_CH;
   return cuda_ok();

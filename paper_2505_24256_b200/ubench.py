@@ -20,13 +20,14 @@ KINDS = [
     (0, "IMAD (mad.lo.u32)", 1), (1, "IMAD.WIDE.U32 (mad.wide.u32)", 1), (2, "IMAD.HI.U32 (mad.hi.u32)", 1),
     (3, "IMAD.WIDE + carry-out + IADD3.X (deferred MAC quarter)", 1), (4, "add + xor (alu)", 2),
     (5, "IMAD.WIDE + IADD3 1:1", 1), (6, "IMAD.WIDE + 2 IMAD", 3), (7, "horner_step (10 mult instr)", 10),
-    (8, "mont_mul (10 mult instr)", 10), (9, "DFMA (fma.rn.f64)", 1), (10, "DFMA + IMAD.WIDE 1:1", 1),
+    (8, "mont_mul_v1 (column form, 8 wide + 2 low)", 10), (9, "DFMA (fma.rn.f64)", 1), (10, "DFMA + IMAD.WIDE 1:1", 1),
     (11, "IMAD.WIDE.U32 zero addend (mul.wide.u32)", 1),
     (12, "acc_mac (4 accumulating wide)", 4), (13, "acc_mac2 (2 MACs, 8 accumulating wide)", 8),
     (14, "acc_mac_split (4 bare wide + alu chains)", 4), (15, "acc_mac_hyb (2 accumulating + 2 bare wide)", 4),
     (16, "as 3, one multiplicand in an even register", 1),
     (17, "accumulating IMAD.WIDE, multiplicands even+odd", 1), (18, "accumulating IMAD.WIDE, multiplicands even+even", 1),
     (19, "accumulating IMAD.WIDE, multiplicands odd+odd", 1),
+    (20, "mont_mul (64-bit REDC, the form in use)", 10), (21, "mont_mul_v3 (bare products + 32-bit chains)", 10),
 ]
 
 
