@@ -73,6 +73,7 @@ def lib():
                                                     u64p, u64p, C.c_int, C.c_int, u64, C.c_int, i32p]
         L.ref_poly_rows_eval.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p]
         L.ref_thiele_reconstruct_batch.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p, u64p, i32p, u64p, i32p]
+        L.ref_extend_skeleton.argtypes = [u16p, i64p, C.c_int, C.c_int, u64p, C.c_int, u64, u16p, u64p, C.c_int64, i64p, i32p]
         L.ref_eval_sparse.restype = u64
         L.ref_eval_sparse.argtypes = [u16p, u64p, C.c_int64, C.c_int, u64p, u64]
         _lib = L
@@ -234,3 +235,19 @@ def thiele_reconstruct_batch(points, vals, p):
     _ok(lib().ref_thiele_reconstruct_batch(_p(points, u64p), T, _p(vals, u64p), n, n, p, _p(num, u64p), _p(den, u64p),
                                            _p(degs, i32p), _p(cf, u64p), _p(status, i32p)), "thiele_reconstruct_batch")
     return num, den, degs, cf, status
+
+
+def extend_skeleton(exps, offsets, coefs, p, cap=None):
+    """(f1): monomial coefficients [B, T_tot] -> (new_exps [T', nv+1], new_coefs [T'], new_offsets [F+1], degs [F])."""
+    exps, offsets, coefs = _a(exps, np.uint16), _a(offsets, np.int64), _a(coefs, np.uint64)
+    B, T_tot = coefs.shape
+    F, nv = len(offsets) - 1, exps.shape[1]
+    cap = B * T_tot if cap is None else cap
+    ne = np.zeros((max(cap, 1), nv + 1), dtype=np.uint16)
+    nc = np.zeros(max(cap, 1), dtype=np.uint64)
+    no = np.zeros(F + 1, dtype=np.int64)
+    degs = np.zeros(F, dtype=np.int32)
+    _ok(lib().ref_extend_skeleton(_p(exps, u16p), _p(offsets, i64p), F, nv, _p(coefs, u64p), B, p, _p(ne, u16p),
+                                  _p(nc, u64p), cap, _p(no, i64p), _p(degs, i32p)), "extend_skeleton")
+    n = min(int(no[-1]), cap)
+    return ne[:n], nc[:n], no, degs

@@ -516,3 +516,34 @@ int ref_thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* 
   free(Nn);
   return REF_OK;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * (f1) skeleton extension; see zippel_ref.h.
+ * ---------------------------------------------------------------------------------------- */
+int ref_extend_skeleton(const uint16_t* exps, const int64_t* offsets, int F, int nv, const uint64_t* coefs, int B,
+                        uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
+                        int32_t* degs) {
+  if (!exps || !offsets || !coefs || !new_exps || !new_coefs || !new_offsets || !degs || F <= 0 || nv <= 0 || B <= 0 ||
+      cap < 0)
+    return REF_ERR_ARG;
+  const int64_t T_tot = offsets[F];
+  int64_t pos = 0;
+  for (int f = 0; f < F; ++f) {
+    new_offsets[f] = pos;
+    degs[f] = -1;
+    for (int64_t i = offsets[f]; i < offsets[f + 1]; ++i)
+      for (int d = 0; d < B; ++d) {
+        const uint64_t v = coefs[(int64_t)d * T_tot + i] % p;
+        if (v == 0) continue;
+        if (pos < cap) {
+          for (int j = 0; j < nv; ++j) new_exps[pos * (nv + 1) + j] = exps[i * nv + j];
+          new_exps[pos * (nv + 1) + nv] = (uint16_t)d;
+          new_coefs[pos] = v;
+        }
+        if (d > degs[f]) degs[f] = d;
+        ++pos;
+      }
+  }
+  new_offsets[F] = pos;
+  return REF_OK;
+}

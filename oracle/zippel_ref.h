@@ -139,6 +139,18 @@ int ref_thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* 
                                  uint64_t p, uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf,
                                  int32_t* status);
 
+/* ---- (f1) skeleton extension between two lifting steps (the polynomial in k variables
+ *      reconstructed by one step is the skeleton of the next): from the monomial-in-x_k coefficients
+ *      coefs[d*T_tot + off_f + i] of every skeleton term i of function f, the terms of the new skeleton are the
+ *      pairs (i, d) with a non-zero coefficient, in the order i ascending, then d ascending:
+ *        new_exps row = (exps row of i, d)   [nv + 1 columns],   new_coefs = that coefficient,
+ *        new_offsets [F+1] term ranges,   degs[f] = largest d with a non-zero coefficient in f (-1: none;
+ *        the early-termination test: degs[f] < B-1 means fewer samples of x_k would have sufficed).
+ *      Returns the total number of new terms through new_offsets[F]; writes at most cap terms. ---- */
+int ref_extend_skeleton(const uint16_t* exps, const int64_t* offsets, int F, int nv, const uint64_t* coefs, int B,
+                        uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
+                        int32_t* degs);
+
 #ifdef __cplusplus
 }
 #endif
