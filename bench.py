@@ -51,8 +51,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6],
-                    help="1-5: BASELINE.json configs; 6: batched Thiele reconstruction (SURVEY.md row f2), C4's input side")
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6, 7],
+                    help="1-5: BASELINE.json configs; 6: batched Thiele reconstruction (row f2), C4's input side; "
+                         "7: skeleton extension (row f1) on C2's output")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -467,9 +468,89 @@ def run_thiele(args):
         "e2e": None, "cpu_baseline": cpu}))
 
 
+# ---------------------------------------------------------------------------------------- (f1) extension leg
+def run_extend(args):
+    """zippel_extend_skeleton on the output shape of C2 (4096 functions x 1000 terms, B = 21, the sparse law's one
+    non-zero degree per term): HBM-bound stream compaction, reported against the measured copy bandwidth."""
+    import torch
+
+    from paper_2505_24256_b200 import api, workloads as wl
+
+    K, W = args.steps, args.warmup
+    sh = dict(wl.CONFIG_SHAPES[2])
+    F = args.F or (64 if args.impl == "reference" else sh["F"])
+    w = wl.make_box_workload("C2out", wl.SEED_BASE + 2, F, sh["nv"], sh["t"], sh["emax"], sh["B"], with_vals=False)
+    T_tot, B, nv = w.T_tot, w.B, w.nv
+    if args.impl == "reference":
+        from oracle import ref
+
+        ta = time.perf_counter()
+        for _ in range(K):
+            ref.extend_skeleton(w.exps, w.offsets, w.planted, w.p)
+        dt = (time.perf_counter() - ta) / K
+        cpu = {"value": T_tot / dt, "unit": "terms/s", "cores": 1, "kind": "oracle", "sample": f"{F} functions of C2's shape"}
+        print(json.dumps({"impl": "reference", "metric": "skeleton_terms_extended_per_s", "value": T_tot / dt, "unit": "terms/s",
+                          "n_gpus": 1, "steps": K, "warmup": 0, "ms_per_step": dt * 1e3, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
+                          "config": {"workload": f"skeleton extension via the CPU oracle, {F} functions"}, "cpu_baseline": cpu,
+                          "gpu_launches": 0, "e2e": {"value": T_tot / dt, "unit": "terms/s", "h2d_bytes_per_step": 0,
+                                                     "d2h_bytes_per_step": 0}}))
+        return
+    torch.cuda.set_device(0)
+    api.lib()
+    de, dc = api.to_dev(w.exps), api.to_dev(w.planted)
+    ws = api.alloc_workspace(w.offsets, B)
+    stream = torch.cuda.Stream()
+    cap = T_tot  # one non-zero degree per term
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            ne, nc, no, dg = api.zippel_extend_skeleton(de, w.offsets, dc, w.p, cap, workspace=ws, stream=stream)
+        torch.cuda.synchronize()
+        assert int(no.cpu()[-1]) == T_tot
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(0)
+        time.sleep(0.3)
+        n0, t0 = api.zippel_launch_count(), time.perf_counter()
+        e0.record(stream)
+        for _ in range(K):
+            api.zippel_extend_skeleton(de, w.offsets, dc, w.p, cap, workspace=ws, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        ms = e0.elapsed_time(e1) / K
+    clocks = sampler.stop(t0, t1)
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    # algorithmic bytes: the coefficient matrix and the exponent rows in, the new rows and coefficients out
+    alg = 8.0 * B * T_tot + 2.0 * nv * T_tot + (2.0 * (nv + 1) + 8.0) * T_tot + 8.0 * (F + 1) + 4.0 * F
+    achieved = alg / (ms * 1e-3) / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import ref
+
+        ws_ = wl.make_box_workload("C2out", wl.SEED_BASE + 2, 64, sh["nv"], sh["t"], sh["emax"], sh["B"], with_vals=False)
+        ta = time.perf_counter()
+        ref.extend_skeleton(ws_.exps, ws_.offsets, ws_.planted, ws_.p)
+        dt = time.perf_counter() - ta
+        cpu = {"value": ws_.T_tot / dt, "unit": "terms/s", "cores": 1, "kind": "oracle", "sample": "first 64 functions"}
+    print(json.dumps({
+        "metric": "skeleton_terms_extended_per_s", "value": T_tot / (ms * 1e-3), "unit": "terms/s", "n_gpus": 1, "steps": K,
+        "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64",
+        "data": "synthetic",
+        "config": {"workload": f"skeleton extension on C2's output: F={F}, t=1000, nv={nv}, B={B}, one non-zero degree per term",
+                   "l2": "inputs larger than L2 (688 MB of coefficients per step)"},
+        "gpu_launches": int(api.zippel_launch_count() - n0), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "k_ext_count + k_ext_emit", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "algorithmic_bytes_per_launch": alg, "ms_per_launch": ms,
+                     "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy bandwidth)" if peaks else "fallback 6650 GB/s"},
+        "e2e": None, "cpu_baseline": cpu}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.config == 6:
+    if a.config == 7:
+        run_extend(a)
+    elif a.config == 6:
         run_thiele(a)
     elif a.impl == "reference":
         run_reference(a)

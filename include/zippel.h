@@ -152,6 +152,20 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
                              uint64_t* num, uint64_t* den, int32_t* degs, uint64_t* cf, int32_t* status,
                              void* workspace, size_t workspace_bytes, void* stream);
 
+/* (f1, SURVEY.md section 8 "next") Skeleton extension between two lifting steps (the polynomial in
+ * k variables that one step reconstructs is the skeleton of the next).  From the monomial-in-x_k coefficients
+ * coefs [B x T_tot] (the `out` of zippel_lift_step with basis = 1) the terms of the new skeleton are the pairs
+ * (term i, degree d) with a non-zero coefficient, ordered by i, then d:
+ *   new_exps  [cap x (nv+1)] uint16 row-major: (exps row of i, d);   new_coefs [cap]: that coefficient;
+ *   new_offsets [F+1] int64 (DEVICE; copy it back to call the next step): term ranges; new_offsets[F] is the
+ *   total even when it exceeds cap (then only the first cap terms are written);
+ *   degs [F] int32: largest d with a non-zero coefficient in function f, -1 if none (degs[f] < B-1: fewer
+ *   samples of x_k would have sufficed -- the early-termination test).
+ * nv < ZP_MAX_NV.  workspace: zippel_workspace_bytes(h_offsets, F, B, 0). */
+int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs, int B,
+                           uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
+                           int32_t* degs, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Measurement hook (bench.py's roofline leg): when kernel != 0, every later call records the CUDA event
  * `ev_start` on its stream right before the first launch of that kernel and `ev_stop` right after the
  * last one (cudaEvent_t passed as void*; the caller owns them).  kernel: ZP_K_* below in the low byte; 0

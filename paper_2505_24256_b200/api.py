@@ -28,7 +28,7 @@ EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
     "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
-    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch",
+    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch", "zippel_extend_skeleton",
 )
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
@@ -72,6 +72,7 @@ def lib() -> C.CDLL:
         L.zippel_profile_events.argtypes = [i32, vp, vp]
         L.zippel_ubench.argtypes = [i32, i32, i32, u64, vp, C.POINTER(C.c_double), vp]
         L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.zippel_extend_skeleton.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp, C.c_size_t, vp]
         L.zippel_launch_count.restype = C.c_ulonglong
         L.zippel_launch_count.argtypes = []
         _lib = L
@@ -341,3 +342,23 @@ def thiele_reconstruct_batch(points: torch.Tensor, vals: torch.Tensor, p: int, w
                                           degs.data_ptr(), _ptr(cf), status.data_ptr(), _ptr(workspace),
                                           workspace.numel(), _stream(stream)), "thiele_reconstruct_batch")
     return num[:, :n], den[:, :n], degs[:, :n], None if cf is None else cf[:, :n], status
+
+
+def zippel_extend_skeleton(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: int, cap: Optional[int] = None,
+                           workspace: Optional[torch.Tensor] = None, stream=None):
+    """(f1): coefs [B, T_tot] monomial in x_k -> (new_exps [cap, nv+1] int16, new_coefs [cap], new_offsets [F+1]
+    int64 on the device, degs [F] int32).  The caller trims to new_offsets[-1] after a synchronisation."""
+    _need_cuda()
+    o = _offs(offsets)
+    F, (B, T_tot), nv = len(o) - 1, coefs.shape, exps.shape[1]
+    cap = B * T_tot if cap is None else cap
+    ne = torch.empty((max(cap, 1), nv + 1), dtype=torch.int16, device=coefs.device)
+    nc = torch.empty(max(cap, 1), dtype=torch.int64, device=coefs.device)
+    no = torch.empty(F + 1, dtype=torch.int64, device=coefs.device)
+    degs = torch.empty(F, dtype=torch.int32, device=coefs.device)
+    if workspace is None:
+        workspace = alloc_workspace(o, B)
+    _check(lib().zippel_extend_skeleton(_ptr(exps), o.ctypes.data, F, nv, _ptr(coefs), B, p, _ptr(ne), _ptr(nc), cap,
+                                        _ptr(no), _ptr(degs), _ptr(workspace), workspace.numel(), _stream(stream)),
+           "zippel_extend_skeleton")
+    return ne, nc, no, degs

@@ -632,6 +632,121 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// (f1) skeleton extension between two lifting steps: the pairs (term i,
+// degree d) with a non-zero monomial coefficient become the terms of the next skeleton, in the order i
+// ascending, d ascending.  HBM-bound stream compaction in three launches:
+//   k_ext_count   one lane per term: 64-bit mask of its non-zero degrees (B <= 64), block-exclusive scan of the
+//                 popcounts, block totals; per-function maximum degree (early-termination test)
+//   k_ext_scan    exclusive scan of the block totals (one CTA)
+//   k_ext_emit    one lane per term: writes its rows (exps row, d) and coefficients, and the new offsets
+// The coefficient matrix is read once (the emit pass re-reads only the non-zero entries).
+// ------------------------------------------------------------------------------------------------
+#define ZP_K9_THREADS 256
+__global__ void __launch_bounds__(ZP_K9_THREADS)
+k_ext_count(const uint64_t* __restrict__ coefs, int64_t T_tot, int B, const int64_t* __restrict__ offsets, int F,
+            ZpMod k, uint64_t* __restrict__ mask, int32_t* __restrict__ lpos, int64_t* __restrict__ bsum,
+            int32_t* __restrict__ degs) {
+  __shared__ int32_t wsum[ZP_K9_THREADS / 32];
+  const int64_t i = (int64_t)blockIdx.x * ZP_K9_THREADS + threadIdx.x;
+  uint64_t m = 0;
+  if (i < T_tot) {
+    int d = 0;
+    for (; d + 8 <= B; d += 8) {  // eight independent loads in flight per lane (the pass is a pure HBM stream)
+      uint64_t v[8];
+#pragma unroll
+      for (int x = 0; x < 8; ++x) v[x] = __ldcs(coefs + (int64_t)(d + x) * T_tot + i);
+#pragma unroll
+      for (int x = 0; x < 8; ++x) m |= (uint64_t)(zp_canon(v[x], k.p) != 0) << (d + x);
+    }
+    for (; d < B; ++d) m |= (uint64_t)(zp_canon(__ldcs(coefs + (int64_t)d * T_tot + i), k.p) != 0) << d;
+    mask[i] = m;
+  }
+  {  // per-function maximum degree: one atomic per warp when the warp lies inside one function (the usual case)
+    int lo = 0;
+    if (i < T_tot) {  // function of term i: offsets[f] <= i < offsets[f+1]
+      int hi = F;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (offsets[mid] <= i) lo = mid; else hi = mid;
+      }
+    }
+    const int deg = m ? 63 - __clzll((long long)m) : -1;
+    const unsigned full = 0xffffffffu;
+    const int f0 = __shfl_sync(full, lo, 0);
+    if (__all_sync(full, lo == f0 || i >= T_tot)) {
+      const int wmax = __reduce_max_sync(full, deg);
+      if ((threadIdx.x & 31) == 0 && wmax >= 0) atomicMax(&degs[f0], wmax);
+    } else if (deg >= 0) {
+      atomicMax(&degs[lo], deg);
+    }
+  }
+  const int c = __popcll(m);
+  int incl = c;  // inclusive scan inside the warp
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if ((threadIdx.x & 31) >= o) incl += v;
+  }
+  if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = incl;
+  __syncthreads();
+  int base = 0;
+  for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) base += wsum[w];
+  if (i < T_tot) lpos[i] = base + incl - c;
+  if (threadIdx.x == ZP_K9_THREADS - 1) bsum[blockIdx.x] = base + incl;
+}
+
+__global__ void __launch_bounds__(1024)
+k_ext_scan(int64_t* __restrict__ bsum, int64_t nb) {  // in place: exclusive prefix; bsum[nb] = total
+  __shared__ int64_t part[1024];
+  const int64_t chunk = (nb + 1023) / 1024;
+  const int64_t lo = (int64_t)threadIdx.x * chunk, hi = (lo + chunk < nb) ? lo + chunk : nb;
+  int64_t s = 0;
+  for (int64_t x = lo; x < hi; ++x) s += bsum[x];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int64_t run = 0;
+    for (int x = 0; x < 1024; ++x) {
+      const int64_t v = part[x];
+      part[x] = run;
+      run += v;
+    }
+    bsum[nb] = run;
+  }
+  __syncthreads();
+  int64_t run = part[threadIdx.x];
+  for (int64_t x = lo; x < hi; ++x) {
+    const int64_t v = bsum[x];
+    bsum[x] = run;
+    run += v;
+  }
+}
+
+__global__ void __launch_bounds__(ZP_K9_THREADS)
+k_ext_emit(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restrict__ coefs, int64_t T_tot, ZpMod k,
+           const uint64_t* __restrict__ mask, const int32_t* __restrict__ lpos, const int64_t* __restrict__ bsum,
+           const int64_t* __restrict__ offsets, int F, uint16_t* __restrict__ new_exps, uint64_t* __restrict__ new_coefs,
+           int64_t cap, int64_t* __restrict__ new_offsets) {
+  const int64_t i = (int64_t)blockIdx.x * ZP_K9_THREADS + threadIdx.x;
+  if (i <= F) {  // the first F+1 lanes also translate the offsets
+    const int64_t o = offsets[i];
+    new_offsets[i] = (o < T_tot) ? bsum[o / ZP_K9_THREADS] + lpos[o] : bsum[(T_tot + ZP_K9_THREADS - 1) / ZP_K9_THREADS];
+  }
+  if (i >= T_tot) return;
+  uint64_t m = mask[i];
+  int64_t pos = bsum[blockIdx.x] + lpos[i];
+  while (m && pos < cap) {
+    const int d = __ffsll((long long)m) - 1;
+    m &= m - 1;
+    uint16_t* row = new_exps + pos * (nv + 1);
+    for (int j = 0; j < nv; ++j) row[j] = exps[i * nv + j];
+    row[nv] = (uint16_t)d;
+    new_coefs[pos] = zp_canon(coefs[(int64_t)d * T_tot + i], k.p);
+    ++pos;
+  }
+}
+
 // (a0) self-test kernel for the substrate
 __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, ZpMod k, uint64_t* out) {
   if (op == 5) {  // deferred dot through the wide accumulator, one CTA

@@ -513,6 +513,31 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
   return cuda_ok();
 }
 
+int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs, int B,
+                           uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
+                           int32_t* degs, void* workspace, size_t workspace_bytes, void* stream) {
+  ZpMod k;
+  int64_t T_tot, tmax;
+  if (!exps || !coefs || !new_exps || !new_coefs || !new_offsets || !degs || nv <= 0 || nv >= ZP_MAX_NV || B <= 0 ||
+      B > ZP_MAX_B || cap < 0 || !make_mod(p, &k) || !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0);
+  cudaStream_t st = (cudaStream_t)stream;
+  upload_offsets(w, h_offsets, F, st);
+  const int64_t nb = (T_tot + ZP_K9_THREADS - 1) / ZP_K9_THREADS;
+  uint64_t* mask = w.nodes;                                   // [T_tot]
+  int32_t* lpos = reinterpret_cast<int32_t*>(w.scale);        // [T_tot]
+  int64_t* bsum = reinterpret_cast<int64_t*>(w.tab);          // [nb + 1] (the slice holds 32 T_tot bytes)
+  ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(degs, F, -1);
+  ++g_launches, k_ext_count<<<(unsigned)nb, ZP_K9_THREADS, 0, st>>>(coefs, T_tot, B, w.d_offsets, F, k, mask, lpos, bsum, degs);
+  ++g_launches, k_ext_scan<<<1, 1024, 0, st>>>(bsum, nb);
+  const int64_t ne = (T_tot > F + 1 ? T_tot : F + 1);
+  ++g_launches, k_ext_emit<<<(unsigned)((ne + ZP_K9_THREADS - 1) / ZP_K9_THREADS), ZP_K9_THREADS, 0, st>>>(
+      exps, nv, coefs, T_tot, k, mask, lpos, bsum, w.d_offsets, F, new_exps, new_coefs, cap, new_offsets);
+  return cuda_ok();
+}
+
 unsigned long long zippel_launch_count(void) { return g_launches; }
 
 int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
