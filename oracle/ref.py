@@ -74,6 +74,7 @@ def lib():
         L.ref_poly_rows_eval.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p]
         L.ref_thiele_reconstruct_batch.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, u64p, u64p, i32p, u64p, i32p]
         L.ref_extend_skeleton.argtypes = [u16p, i64p, C.c_int, C.c_int, u64p, C.c_int, u64, u16p, u64p, C.c_int64, i64p, i32p]
+        L.ref_crt_rational_batch.argtypes = [u64p, u64p, C.c_int64, u64, u64, i64p, i64p, i32p]
         L.ref_eval_sparse.restype = u64
         L.ref_eval_sparse.argtypes = [u16p, u64p, C.c_int64, C.c_int, u64p, u64]
         _lib = L
@@ -251,3 +252,14 @@ def extend_skeleton(exps, offsets, coefs, p, cap=None):
                                   _p(nc, u64p), cap, _p(no, i64p), _p(degs, i32p)), "extend_skeleton")
     n = min(int(no[-1]), cap)
     return ne[:n], nc[:n], no, degs
+
+
+def crt_rational_batch(r1, r2, p1, p2):
+    """(f4): residues mod p1 and mod p2 -> (num int64 [n], den int64 [n], status [n])."""
+    r1, r2 = _a(r1, np.uint64), _a(r2, np.uint64)
+    n = len(r1)
+    num, den = np.zeros(n, dtype=np.int64), np.zeros(n, dtype=np.int64)
+    status = np.zeros(n, dtype=np.int32)
+    _ok(lib().ref_crt_rational_batch(_p(r1, u64p), _p(r2, u64p), n, p1, p2, _p(num, i64p), _p(den, i64p),
+                                     _p(status, i32p)), "crt_rational_batch")
+    return num, den, status

@@ -547,3 +547,62 @@ int ref_extend_skeleton(const uint16_t* exps, const int64_t* offsets, int F, int
   new_offsets[F] = pos;
   return REF_OK;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * (f4) CRT of two primes and rational reconstruction; see zippel_ref.h.  Plain unsigned __int128.
+ * ---------------------------------------------------------------------------------------- */
+typedef unsigned __int128 ref_u128;
+typedef __int128 ref_i128;
+
+static ref_u128 ref_isqrt128(ref_u128 v) { /* floor(sqrt(v)) by bisection on the bits */
+  ref_u128 r = 0;
+  for (int b = 63; b >= 0; --b) {
+    const ref_u128 c = r | ((ref_u128)1 << b);
+    if (c * c <= v) r = c;
+  }
+  return r;
+}
+
+int ref_crt_rational_batch(const uint64_t* r1, const uint64_t* r2, int64_t n, uint64_t p1, uint64_t p2, int64_t* num,
+                           int64_t* den, int32_t* status) {
+  if (!r1 || !r2 || !num || !den || !status || n <= 0 || p1 == p2 || p1 < 3 || p2 < 3 || (p1 >> 63) || (p2 >> 63))
+    return REF_ERR_ARG;
+  const ref_u128 m = (ref_u128)p1 * p2;
+  const ref_u128 N = ref_isqrt128((m - 1) / 2);
+  const uint64_t p1inv = ref_invmod(p1 % p2, p2);
+  for (int64_t i = 0; i < n; ++i) {
+    const uint64_t a1 = r1[i] % p1, a2 = r2[i] % p2;
+    const uint64_t h = ref_mulmod(ref_submod(a2, a1 % p2, p2), p1inv, p2);
+    const ref_u128 x = (ref_u128)a1 + (ref_u128)p1 * h;
+    ref_u128 ra = m, rb = x;
+    ref_i128 ta = 0, tb = 1;
+    while (rb > N) {
+      const ref_u128 q = ra / rb;
+      const ref_u128 rn = ra - q * rb;
+      const ref_i128 tn = ta - (ref_i128)q * tb;
+      ra = rb;
+      rb = rn;
+      ta = tb;
+      tb = tn;
+    }
+    ref_i128 a = (ref_i128)rb, b = tb;
+    if (b < 0) {
+      a = -a;
+      b = -b;
+    }
+    int ok = (b > 0) && ((ref_u128)b <= N);
+    if (ok) { /* gcd(|a|, b) */
+      uint64_t g0 = (uint64_t)(a < 0 ? -a : a), g1 = (uint64_t)b;
+      while (g1) {
+        const uint64_t tmp = g0 % g1;
+        g0 = g1;
+        g1 = tmp;
+      }
+      ok = (g0 == 1);
+    }
+    num[i] = ok ? (int64_t)a : 0;
+    den[i] = ok ? (int64_t)b : 0;
+    status[i] = ok ? 0 : REF_ST_NO_RATIONAL;
+  }
+  return REF_OK;
+}

@@ -47,6 +47,7 @@ extern "C" {
 #define REF_ST_DUPLICATE_NODE 16   /* den_i == 0 (two terms map to one node) or m_i == 0 with s0 = 1 */
 #define REF_ST_DUPLICATE_SAMPLE 17 /* c_j == c_j' in Newton */
 #define REF_ST_ZERO_PIVOT 18       /* u_{0,s} == 0 in balancing */
+#define REF_ST_NO_RATIONAL 21 /* rational reconstruction: no a/b within the bounds (or gcd(a, b) != 1) */
 #define REF_ST_THIELE_DEGENERATE 20 /* an inverse difference of eq. (2) has a zero denominator at some but not all points */
 
 /* ---- arithmetic in Z/pZ (variant 1 is the definition) ---- */
@@ -150,6 +151,17 @@ int ref_thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* 
 int ref_extend_skeleton(const uint16_t* exps, const int64_t* offsets, int F, int nv, const uint64_t* coefs, int B,
                         uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
                         int32_t* degs);
+
+/* ---- (f4) second prime + CRT + rational reconstruction (the reduction is run over several large
+ *      primes "fitting into 2^64" and "the final reconstruction to rational numbers is performed as a final step").
+ *      For every coefficient i with residues r1[i] mod p1 and r2[i] mod p2 (p1 != p2 odd primes < 2^63):
+ *        x = r1 + p1 * ((r2 - r1) * p1^-1 mod p2)  in [0, m),  m = p1 p2           (Chinese remainder theorem)
+ *        extended Euclid on (m, x):  (r, t) sequences with r_j = t_j x (mod m), stopped at the first r_j <= N,
+ *        N = D = floor(sqrt((m - 1) / 2))  (Wang's bounds: 2 N D < m makes the answer unique);
+ *        a = r_j, b = t_j, sign moved to a so that b > 0; valid iff b <= D and gcd(|a|, b) = 1.
+ *      num [n] int64 (signed), den [n] int64 (> 0), status [n]: 0 or REF_ST_NO_RATIONAL (num = den = 0). ---- */
+int ref_crt_rational_batch(const uint64_t* r1, const uint64_t* r2, int64_t n, uint64_t p1, uint64_t p2, int64_t* num,
+                           int64_t* den, int32_t* status);
 
 #ifdef __cplusplus
 }
