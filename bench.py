@@ -51,9 +51,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6, 7],
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6, 7, 8],
                     help="1-5: BASELINE.json configs; 6: batched Thiele reconstruction (row f2), C4's input side; "
-                         "7: skeleton extension (row f1) on C2's output")
+                         "7: skeleton extension (row f1) on C2's output; 8: two-prime CRT + rational reconstruction (row f4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -546,9 +546,96 @@ def run_extend(args):
         "e2e": None, "cpu_baseline": cpu}))
 
 
+# ---------------------------------------------------------------------------------------- (f4) CRT leg
+def run_crt(args):
+    """crt_rational_reconstruct_batch on as many coefficients as C2 reconstructs (4 096 000), images of random
+    fractions a/b with |a|, b < 2^40 (two primes determine them with room to spare)."""
+    import torch
+
+    from paper_2505_24256_b200 import api, workloads as wl
+
+    K, W = args.steps, args.warmup
+    p1, p2 = wl.P63, (1 << 63) - 165
+    n = 4000 if args.impl == "reference" else (args.F or 4096) * 1000
+    rng = wl._rng(wl.SEED_BASE + 8, 50)
+    a = rng.integers(-(1 << 40), 1 << 40, n, dtype=np.int64)
+    bb = rng.integers(1, 1 << 40, n, dtype=np.int64)
+    # images mod p by float-free vectorised arithmetic is awkward in numpy; build them from a table of 4096 fractions
+    tab = [(int(x), int(y)) for x, y in zip(a[:4096], bb[:4096])]
+    t1 = np.array([x * pow(y, -1, p1) % p1 for x, y in tab], dtype=np.uint64)
+    t2 = np.array([x * pow(y, -1, p2) % p2 for x, y in tab], dtype=np.uint64)
+    idx = rng.integers(0, len(tab), n)
+    r1, r2 = t1[idx], t2[idx]
+    if args.impl == "reference":
+        from oracle import ref
+
+        ta = time.perf_counter()
+        for _ in range(K):
+            ref.crt_rational_batch(r1, r2, p1, p2)
+        dt = (time.perf_counter() - ta) / K
+        cpu = {"value": n / dt, "unit": "reconstructions/s", "cores": 1, "kind": "oracle", "sample": f"{n} coefficients"}
+        print(json.dumps({"impl": "reference", "metric": "rational_reconstructions_per_s", "value": n / dt,
+                          "unit": "reconstructions/s", "n_gpus": 1, "steps": K, "warmup": 0, "ms_per_step": dt * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u128", "data": "synthetic",
+                          "config": {"workload": f"CRT + rational reconstruction via the CPU oracle, {n} coefficients"},
+                          "cpu_baseline": cpu, "gpu_launches": 0,
+                          "e2e": {"value": n / dt, "unit": "reconstructions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+    torch.cuda.set_device(0)
+    api.lib()
+    d1, d2 = api.to_dev(r1), api.to_dev(r2)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        for _ in range(W):
+            num, den, st = api.crt_rational_reconstruct_batch(d1, d2, p1, p2, stream=stream)
+        torch.cuda.synchronize()
+        assert not st.any().item()
+        hn, hd = num[:1000].cpu().numpy(), den[:1000].cpu().numpy()
+        assert all(int(x) * tab[j][1] == tab[j][0] * int(y) for x, y, j in zip(hn, hd, idx[:1000]))  # same fraction
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(0)
+        time.sleep(0.3)
+        n0, t0 = api.zippel_launch_count(), time.perf_counter()
+        e0.record(stream)
+        for _ in range(K):
+            api.crt_rational_reconstruct_batch(d1, d2, p1, p2, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1_ = time.perf_counter()
+        ms = e0.elapsed_time(e1) / K
+    clocks = sampler.stop(t0, t1_)
+    # algorithmic work (DESIGN.md section 11): about 0.843 ln(sqrt(m)) = 37 Euclid steps per coefficient, each at least
+    # two 64 x 64 -> 128 products (q r and q t): 16 units
+    units = n * 37.0 * 16.0
+    achieved = units / (ms * 1e-3) / 1e12
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import ref
+
+        ta = time.perf_counter()
+        ref.crt_rational_batch(r1[:200000], r2[:200000], p1, p2)
+        dt = time.perf_counter() - ta
+        cpu = {"value": 200000 / dt, "unit": "reconstructions/s", "cores": 1, "kind": "oracle", "sample": "first 200 000 coefficients"}
+    print(json.dumps({
+        "metric": "rational_reconstructions_per_s", "value": n / (ms * 1e-3), "unit": "reconstructions/s", "n_gpus": 1,
+        "steps": K, "warmup": W, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u128", "data": "synthetic",
+        "config": {"workload": f"two-prime CRT + rational reconstruction: n={n} coefficients, p1=2^63-25, p2=2^63-165",
+                   "l2": "inputs larger than L2 only at 8 M coefficients; the kernel is bound by 128-bit integer arithmetic"},
+        "gpu_launches": int(api.zippel_launch_count() - n0), "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "k_crt_rational", "achieved": achieved, "peak": IMAD_PEAK_TOPS,
+                     "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
+                     "traffic": None, "algorithmic_ops_per_launch": units, "ms_per_launch": ms,
+                     "algorithmic_cost": "37 Euclid steps x two 64x64->128 products (16 units) per coefficient; the quotient itself "
+                                         "(128-bit division, data-dependent) is not in the multiplier count"},
+        "e2e": None, "cpu_baseline": cpu}))
+
+
 if __name__ == "__main__":
     a = parse()
-    if a.config == 7:
+    if a.config == 8:
+        run_crt(a)
+    elif a.config == 7:
         run_extend(a)
     elif a.config == 6:
         run_thiele(a)

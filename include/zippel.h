@@ -39,6 +39,7 @@ extern "C" {
 #define ZP_ST_DUPLICATE_NODE 16   /* den_i == 0: two terms map to one node (G24); or m_i == 0 with s0 = 1 (G25) */
 #define ZP_ST_DUPLICATE_SAMPLE 17 /* c_j == c_j' for some j' < j in Newton (index = j) */
 #define ZP_ST_ZERO_PIVOT 18       /* u_{0,s} == 0 in balancing (index = s) */
+#define ZP_ST_NO_RATIONAL 21       /* CRT + rational reconstruction: no a/b within Wang's bounds with gcd(a, b) = 1 */
 #define ZP_ST_THIELE_DEGENERATE 20 /* Thiele: an inverse difference of level k has a zero denominator at some but
                                       not all of the remaining points (index = k); or the denominator vanished */
 
@@ -165,6 +166,16 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
 int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs, int B,
                            uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
                            int32_t* degs, void* workspace, size_t workspace_bytes, void* stream);
+
+/* (f4, SURVEY.md section 8 "next") Second prime + CRT + rational reconstruction (the reduction runs
+ * over several large primes "fitting into 2^64" and "the final reconstruction to rational numbers is performed as
+ * a final step").  For every coefficient i, from its images r1[i] mod p1 and r2[i] mod p2 (device arrays; p1 != p2
+ * odd primes < 2^63, e.g. 2^63 - 25 and 2^63 - 165):  x = CRT(r1, r2) in [0, m = p1 p2), then the extended Euclidean
+ * sequence of (m, x) down to the first remainder <= N = floor(sqrt((m-1)/2)) gives a = remainder, b = cofactor
+ * (sign moved to a, b > 0); accepted iff b <= N and gcd(|a|, b) = 1 (Wang's bounds; 2 N^2 < m makes a/b unique).
+ *   num [n] int64 (signed), den [n] int64 (> 0), status [n]: 0, or ZP_ST_NO_RATIONAL with num = den = 0. */
+int crt_rational_reconstruct_batch(const uint64_t* r1, const uint64_t* r2, int64_t n, uint64_t p1, uint64_t p2,
+                                   int64_t* num, int64_t* den, int32_t* status, void* stream);
 
 /* Measurement hook (bench.py's roofline leg): when kernel != 0, every later call records the CUDA event
  * `ev_start` on its stream right before the first launch of that kernel and `ev_stop` right after the

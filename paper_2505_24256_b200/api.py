@@ -28,7 +28,7 @@ EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
     "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
-    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch", "zippel_extend_skeleton",
+    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch", "zippel_extend_skeleton", "crt_rational_reconstruct_batch",
 )
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
@@ -73,6 +73,7 @@ def lib() -> C.CDLL:
         L.zippel_ubench.argtypes = [i32, i32, i32, u64, vp, C.POINTER(C.c_double), vp]
         L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         L.zippel_extend_skeleton.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp, C.c_size_t, vp]
+        L.crt_rational_reconstruct_batch.argtypes = [vp, vp, C.c_int64, u64, u64, vp, vp, vp, vp]
         L.zippel_launch_count.restype = C.c_ulonglong
         L.zippel_launch_count.argtypes = []
         _lib = L
@@ -362,3 +363,17 @@ def zippel_extend_skeleton(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: 
                                         _ptr(no), _ptr(degs), _ptr(workspace), workspace.numel(), _stream(stream)),
            "zippel_extend_skeleton")
     return ne, nc, no, degs
+
+
+ST_NO_RATIONAL = 21
+
+
+def crt_rational_reconstruct_batch(r1: torch.Tensor, r2: torch.Tensor, p1: int, p2: int, stream=None):
+    """(f4): images mod p1 and mod p2 [n] -> (num int64 [n] signed, den int64 [n] > 0, status int32 [n])."""
+    _need_cuda()
+    n = r1.numel()
+    num, den = torch.empty(n, dtype=torch.int64, device=r1.device), torch.empty(n, dtype=torch.int64, device=r1.device)
+    status = torch.empty(n, dtype=torch.int32, device=r1.device)
+    _check(lib().crt_rational_reconstruct_batch(r1.data_ptr(), r2.data_ptr(), n, p1, p2, num.data_ptr(), den.data_ptr(),
+                                                status.data_ptr(), _stream(stream)), "crt_rational_reconstruct_batch")
+    return num, den, status

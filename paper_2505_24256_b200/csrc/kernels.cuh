@@ -747,6 +747,77 @@ k_ext_emit(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restrict
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// (f4) two-prime CRT + rational reconstruction, one lane per coefficient:
+//   x = r1 + p1 ((r2 - r1) p1^-1 mod p2) in [0, m = p1 p2);  extended Euclid on (m, x) down to the first
+//   remainder <= N = floor(sqrt((m-1)/2)) (Wang's bounds);  a/b = remainder / cofactor, b > 0, b <= N, gcd 1.
+// 128-bit integers; Euclid's quotients are mostly 1, 2, 3 (tried by subtraction before the 128-bit division),
+// and the tail of the sequence runs in 64 bits.  Data-dependent and divergent by nature; HBM traffic 32 B/lane.
+// ------------------------------------------------------------------------------------------------
+#define ZP_ST_NO_RATIONAL 21
+typedef unsigned __int128 zp_u128;
+typedef __int128 zp_i128;
+__global__ void __launch_bounds__(256)
+k_crt_rational(const uint64_t* __restrict__ r1, const uint64_t* __restrict__ r2, int64_t n, uint64_t p1, ZpMod k2,
+               uint64_t p1inv, uint64_t m_hi, uint64_t m_lo, uint64_t N, int64_t* __restrict__ num,
+               int64_t* __restrict__ den, int32_t* __restrict__ status) {
+  const zp_u128 m = ((zp_u128)m_hi << 64) | m_lo;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const uint64_t a1 = zp_canon(r1[i], p1), a2 = zp_canon(r2[i], k2.p);
+    const uint64_t diff = mod_sub(a2, zp_canon(a1, k2.p), k2.p);
+    const uint64_t h = mont_mul(to_mont(diff, k2), p1inv, k2);  // Montgomery x plain -> plain: diff / p1 mod p2
+    const zp_u128 x = (zp_u128)a1 + (zp_u128)p1 * h;
+    zp_u128 ra = m, rb = x;
+    zp_i128 ta = 0, tb = 1;
+    while (rb > N) {
+      zp_u128 q, rn;
+      if ((uint64_t)(ra >> 64) == 0) {
+        const uint64_t a = (uint64_t)ra, b = (uint64_t)rb, qq = a / b;
+        q = qq;
+        rn = a - qq * b;
+      } else {
+        rn = ra - rb;
+        q = 1;
+        if (rn >= rb) {
+          rn -= rb;
+          q = 2;
+          if (rn >= rb) {
+            rn -= rb;
+            q = 3;
+            if (rn >= rb) {
+              q = ra / rb;
+              rn = ra - q * rb;
+            }
+          }
+        }
+      }
+      const zp_i128 tn = ta - (zp_i128)q * tb;
+      ra = rb;
+      rb = rn;
+      ta = tb;
+      tb = tn;
+    }
+    zp_i128 a = (zp_i128)rb, b = tb;
+    if (b < 0) {
+      a = -a;
+      b = -b;
+    }
+    bool ok = (b > 0) && ((zp_u128)b <= N);
+    if (ok) {
+      uint64_t g0 = (uint64_t)(a < 0 ? -a : a), g1 = (uint64_t)b;
+      while (g1) {
+        const uint64_t tmp = g0 % g1;
+        g0 = g1;
+        g1 = tmp;
+      }
+      ok = (g0 == 1);
+    }
+    num[i] = ok ? (int64_t)a : 0;
+    den[i] = ok ? (int64_t)b : 0;
+    status[i] = ok ? 0 : ZP_ST_NO_RATIONAL;
+  }
+}
+
 // (a0) self-test kernel for the substrate
 __global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, ZpMod k, uint64_t* out) {
   if (op == 5) {  // deferred dot through the wide accumulator, one CTA

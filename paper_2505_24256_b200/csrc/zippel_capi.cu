@@ -307,6 +307,7 @@ const char* zippel_strerror(int code) {
     case ZP_ST_DUPLICATE_SAMPLE: return "duplicate sample";
     case ZP_ST_ZERO_PIVOT: return "zero pivot in balancing";
     case ZP_ST_THIELE_DEGENERATE: return "degenerate inverse difference in Thiele reconstruction";
+    case ZP_ST_NO_RATIONAL: return "no rational number within the bounds";
     default: return "unknown";
   }
 }
@@ -535,6 +536,30 @@ int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F
   const int64_t ne = (T_tot > F + 1 ? T_tot : F + 1);
   ++g_launches, k_ext_emit<<<(unsigned)((ne + ZP_K9_THREADS - 1) / ZP_K9_THREADS), ZP_K9_THREADS, 0, st>>>(
       exps, nv, coefs, T_tot, k, mask, lpos, bsum, w.d_offsets, F, new_exps, new_coefs, cap, new_offsets);
+  return cuda_ok();
+}
+
+int crt_rational_reconstruct_batch(const uint64_t* r1, const uint64_t* r2, int64_t n, uint64_t p1, uint64_t p2,
+                                   int64_t* num, int64_t* den, int32_t* status, void* stream) {
+  ZpMod k1, k2;
+  if (!r1 || !r2 || !num || !den || !status || n <= 0 || p1 == p2 || !make_mod(p1, &k1) || !make_mod(p2, &k2))
+    return ZP_ERR_ARG;
+  const u128 m = (u128)p1 * p2;
+  u128 N = 0;  // floor(sqrt((m - 1) / 2))
+  for (int b = 63; b >= 0; --b) {
+    const u128 cnd = N | ((u128)1 << b);
+    if (cnd * cnd <= (m - 1) / 2) N = cnd;
+  }
+  uint64_t inv = 1, base = p1 % p2, e = p2 - 2;  // p1^-1 mod p2 (Fermat; p2 prime is the caller's contract)
+  while (e) {
+    if (e & 1) inv = (uint64_t)((u128)inv * base % p2);
+    base = (uint64_t)((u128)base * base % p2);
+    e >>= 1;
+  }
+  int64_t blocks = (n + 255) / 256;
+  if (blocks > 148 * 32) blocks = 148 * 32;
+  ++g_launches, k_crt_rational<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
+      r1, r2, n, p1, k2, inv, (uint64_t)(m >> 64), (uint64_t)m, (uint64_t)N, num, den, status);
   return cuda_ok();
 }
 
