@@ -204,6 +204,10 @@ ZP_DEV void cp_async8(void* smem, const void* g, bool ok) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g),
                "r"(ok ? 8 : 0) : "memory");
 }
+ZP_DEV void cp_async4(void* smem, const void* g, bool ok) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g),
+               "r"(ok ? 4 : 0) : "memory");
+}
 ZP_DEV void cp_async16(void* smem, const void* g, bool ok) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(g),
                "r"(ok ? 16 : 0) : "memory");
@@ -250,8 +254,11 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         const int b = x / (2 * np), r = x - b * (2 * np);  // r = stage offset inside the tile
         const int l = 2 * j0 + r;
         const bool ok = l < t;
-        cp_async8(reinterpret_cast<uint64_t*>(&sV[buf][0]) + ((r >> 1) * NB + b) * 2 + (r & 1),
-                  vals + (int64_t)(b0 + b) * T_tot + off + (ok ? l : 0), ok);
+        // 16-byte record of (pair, b): { v_odd.lo, v_even.lo, v_odd.hi, v_even.hi }  (odd stage pairs with qa)
+        uint32_t* rec = reinterpret_cast<uint32_t*>(&sV[buf][0]) + ((r >> 1) * NB + b) * 4 + ((r & 1) ^ 1);
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(vals + (int64_t)(b0 + b) * T_tot + off + (ok ? l : 0));
+        cp_async4(rec, src, ok);
+        cp_async4(rec + 2, src + 1, ok);
       }
       cp_async_commit();
     };
@@ -277,8 +284,8 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         if (FIRST) d = horner_step(d, m, mp, r1.z, r1.w, k);
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-          const ulonglong2 v2 = cV[jj * NB + b];
-          acc_mac2(acc[b], qa, v2.y, qb, v2.x);
+          const uint4 w = reinterpret_cast<const uint4*>(cV)[jj * NB + b];
+          acc_mac2_limbs(acc[b], (uint32_t)qa, (uint32_t)(qa >> 32), w.x, w.z, (uint32_t)qb, (uint32_t)(qb >> 32), w.y, w.w);
         }
         if (j0 + jj > 0) {
           const ulonglong4 r0 = cT[2 * jj];

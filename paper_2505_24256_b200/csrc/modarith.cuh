@@ -262,6 +262,33 @@ ZP_DEV void acc_mac2(Acc& a, uint64_t x, uint64_t y, uint64_t u, uint64_t w) {
       : "l"(m0), "l"(m1), "l"(m2), "l"(m3));
 }
 
+// acc_mac2 on limbs: a += (x1:x0)*(y1:y0) + (u1:u0)*(w1:w0), the caller supplies the 32-bit halves (the node-solve
+// loop loads the broadcast operands as {y0, w0, y1, w1} so that the two limbs of one operand sit in registers of
+// the same parity: profiles/r01_final.md, register banks).
+ZP_DEV void acc_mac2_limbs(Acc& a, uint32_t x0, uint32_t x1, uint32_t y0, uint32_t y1, uint32_t u0, uint32_t u1,
+                           uint32_t w0, uint32_t w1) {
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), lo2 = zp_mulw(u0, w0), hi2 = zp_mulw(u1, w1);
+  asm("add.cc.u64 %0, %0, %3;\n\t"
+      "addc.cc.u64 %1, %1, %4;\n\t"
+      "addc.u32 %2, %2, 0;\n\t"
+      "add.cc.u64 %0, %0, %5;\n\t"
+      "addc.cc.u64 %1, %1, %6;\n\t"
+      "addc.u32 %2, %2, 0;"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi), "l"(lo2), "l"(hi2));
+  const uint64_t m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0), m2 = zp_mulw(u0, w1), m3 = zp_mulw(u1, w0);
+  asm("add.cc.u64 %0, %0, %2;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %3;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %4;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, %0, %5;\n\t"
+      "addc.u32 %1, %1, 0;"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1), "l"(m2), "l"(m3));
+}
+
 // Alternative forms of the same MAC, for the pipe-balance micro-benchmarks (zippel_ubench kinds 12-16).
 // acc_mac_split: every product is a bare IMAD.WIDE (zero addend, 4 pipe cycles instead of the > 5 of the
 // accumulating form, profiles/r01_baseline.md); the 160-bit additions run on the alu pipe as 32-bit carry chains.
