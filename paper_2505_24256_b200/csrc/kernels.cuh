@@ -250,8 +250,9 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         cp_async16(reinterpret_cast<ulonglong2*>(&sT[buf][0]) + x,
                    reinterpret_cast<const ulonglong2*>(Tf + (ok ? l - 1 : 0)) + (x & 1), ok);
       }
-      for (int x = threadIdx.x; x < 2 * np * NB; x += ZP_K3_THREADS) {
-        const int b = x / (2 * np), r = x - b * (2 * np);  // r = stage offset inside the tile
+      for (int x = threadIdx.x; x < 2 * ZP_K3_PAIRS * NB; x += ZP_K3_THREADS) {
+        const int b = x / (2 * ZP_K3_PAIRS), r = x % (2 * ZP_K3_PAIRS);  // r = stage offset inside the tile (shifts)
+        if (r >= 2 * np) continue;  // only the lowest tile can be short
         const int l = 2 * j0 + r;
         const bool ok = l < t;
         // 16-byte record of (pair, b): { v_odd.lo, v_even.lo, v_odd.hi, v_even.hi }  (odd stage pairs with qa)
