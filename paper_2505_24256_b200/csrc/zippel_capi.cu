@@ -43,7 +43,7 @@ bool make_mod(uint64_t p, ZpMod* k) {
 struct Ws {
   int64_t* d_offsets;
   int32_t *st_pre, *st_solve, *st_newton;
-  uint64_t *nodes, *M0, *M1, *scale, *R, *V;
+  uint64_t *nodes, *M0, *M1, *scale, *R, *V, *newtI, *newtL;
   ulonglong2 *invd, *smont;  // Newton: {w, w'} tables
   ulonglong4* tab;
   size_t bytes;
@@ -70,6 +70,8 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
   w.tab = (ulonglong4*)take(32 * (size_t)T_tot);
   w.invd = (ulonglong2*)take(16 * (size_t)B * B);
   w.smont = (ulonglong2*)take(16 * (size_t)B);
+  w.newtI = (uint64_t*)take(8 * (size_t)B * B);  // identity, then L = k_newton(identity)
+  w.newtL = (uint64_t*)take(8 * (size_t)B * B);
   w.R = (uint64_t*)take(8 * (size_t)T_tot);
   w.V = (flags & ZP_WS_BALANCED) ? (uint64_t*)take(8 * (size_t)T_tot * B) : nullptr;
   w.bytes = o;
@@ -187,6 +189,21 @@ void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* val
   const size_t smem = 16 * ((size_t)B * B + B) + 8 * (size_t)B * ZP_K5_THREADS;
   int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
   if (blocks > 148 * 64) blocks = 148 * 64;
+  if (n >= 4 * (int64_t)B) {
+    // many coefficients: L = Newton(identity) once, then the batch is the product L x vals (k_newton_apply)
+    ++g_launches, k_set_identity<<<(B * B + 255) / 256, 256, 0, st>>>(w.newtI, B);
+    cudaFuncSetAttribute(k_newton<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ++g_launches, k_newton<true><<<1, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, w.newtI, B, B, k, basis, w.newtL);
+    const size_t smem2 = 8 * ((size_t)(B + 3) * B + (size_t)B * ZP_K5_THREADS);
+    if (canonical_in) {
+      cudaFuncSetAttribute(k_newton_apply<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+      ++g_launches, k_newton_apply<true><<<(unsigned)blocks, ZP_K5_THREADS, smem2, st>>>(w.newtL, B, vals, n, ld, k, basis, out);
+    } else {
+      cudaFuncSetAttribute(k_newton_apply<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+      ++g_launches, k_newton_apply<false><<<(unsigned)blocks, ZP_K5_THREADS, smem2, st>>>(w.newtL, B, vals, n, ld, k, basis, out);
+    }
+    return;
+  }
   if (canonical_in) {
     cudaFuncSetAttribute(k_newton<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     ++g_launches, k_newton<true><<<(unsigned)blocks, ZP_K5_THREADS, smem, st>>>(w.invd, w.smont, B, vals, n, ld, k, basis, out);

@@ -220,10 +220,10 @@ def test_solve_status_duplicate_and_zero_node(zp, ref):
 # ------------------------------------------------------------------------------ (a5) Newton
 @pytest.mark.parametrize("B", [1, 2, 3, 9, 16, 17, 21, 25, 32, 33, 64])
 @pytest.mark.parametrize("basis", [0, 1])
-def test_newton_parity(zp, ref, B, basis):
+@pytest.mark.parametrize("n", [5, 1000 + 37])  # few coefficients: per-column recurrences; many: the matrix form L x vals
+def test_newton_parity(zp, ref, B, basis, n):
     p = P63
     r = np.random.Generator(np.random.Philox(key=[11, B]))
-    n = 1000 + 37
     samples = wl.distinct_residues(r, 0, p, B)
     vals = r.integers(0, p, (B, n), dtype=np.uint64)
     want, wst = ref.newton_interp_batch(samples, vals, p, basis)
