@@ -198,6 +198,16 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 // ------------------------------------------------------------------------------------------------
 #define ZP_K3_THREADS 128
 #define ZP_K3_PAIRS 32
+// Orientation of the 16-byte value record per template instance.  Both orders put the two limbs of one operand
+// into registers of the same parity; which of the two ptxas's register allocation serves with fewer bank
+// conflicts differs from instance to instance, so it is read off the SASS (share of accumulating IMAD.WIDE whose
+// multiplicands have equal parity; profiles/r01_final.md) and tabulated: bit NB = 1 -> odd stage first.
+#ifdef ZP_K3_FORCE_ORIENT
+#define ZP_K3_ORIENT(NB) (ZP_K3_FORCE_ORIENT)
+#else
+#define ZP_K3_ORIENT_MASK 0x1e18108u
+#define ZP_K3_ORIENT(NB) ((ZP_K3_ORIENT_MASK >> (NB)) & 1u)
+#endif
 
 // cp.async (LDGSTS) with zero fill: src-size 0 reads nothing and writes zeros
 ZP_DEV void cp_async8(void* smem, const void* g, bool ok) {
@@ -223,7 +233,8 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
              uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
   // two buffers: the tile after the current one is in flight (cp.async) while the current one is consumed
   __shared__ __align__(16) ulonglong4 sT[2][2 * ZP_K3_PAIRS];      // record of stage l = 2 j0 + x
-  __shared__ __align__(16) ulonglong2 sV[2][ZP_K3_PAIRS * NB];     // [pair][b] = { v_{b,2j}, v_{b,2j+1} }
+  __shared__ __align__(16) ulonglong2 sV[2][ZP_K3_PAIRS * NB];     // [pair][b]: 16-byte record of limbs, see issue_tile
+  constexpr int ORIENT = ZP_K3_ORIENT(NB);
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -255,8 +266,9 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         if (r >= 2 * np) continue;  // only the lowest tile can be short
         const int l = 2 * j0 + r;
         const bool ok = l < t;
-        // 16-byte record of (pair, b): { v_odd.lo, v_even.lo, v_odd.hi, v_even.hi }  (odd stage pairs with qa)
-        uint32_t* rec = reinterpret_cast<uint32_t*>(&sV[buf][0]) + ((r >> 1) * NB + b) * 4 + ((r & 1) ^ 1);
+        // 16-byte record of (pair, b): ORIENT = 1: { v_odd.lo, v_even.lo, v_odd.hi, v_even.hi }, 0: even first
+        // (the odd stage pairs with qa)
+        uint32_t* rec = reinterpret_cast<uint32_t*>(&sV[buf][0]) + ((r >> 1) * NB + b) * 4 + ((r & 1) ^ ORIENT);
         const uint32_t* src = reinterpret_cast<const uint32_t*>(vals + (int64_t)(b0 + b) * T_tot + off + (ok ? l : 0));
         cp_async4(rec, src, ok);
         cp_async4(rec + 2, src + 1, ok);
@@ -286,7 +298,10 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
           const uint4 w = reinterpret_cast<const uint4*>(cV)[jj * NB + b];
-          acc_mac2_limbs(acc[b], (uint32_t)qa, (uint32_t)(qa >> 32), w.x, w.z, (uint32_t)qb, (uint32_t)(qb >> 32), w.y, w.w);
+          if (ORIENT)
+            acc_mac2_limbs(acc[b], (uint32_t)qa, (uint32_t)(qa >> 32), w.x, w.z, (uint32_t)qb, (uint32_t)(qb >> 32), w.y, w.w);
+          else
+            acc_mac2_limbs(acc[b], (uint32_t)qa, (uint32_t)(qa >> 32), w.y, w.w, (uint32_t)qb, (uint32_t)(qb >> 32), w.x, w.z);
         }
         if (j0 + jj > 0) {
           const ulonglong4 r0 = cT[2 * jj];
