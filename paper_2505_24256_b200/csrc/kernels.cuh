@@ -330,6 +330,127 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------------
+// (a3) for ONE right-hand side and a long skeleton (C5): with q_{i,l} = sum_{k>l} M_k m_i^(k-l-1),
+//     num_i = sum_l q_{i,l} v_l = sum_j W_j m_i^j = W(m_i),    W_j = sum_l v_l M_{l+j+1}   (M_t = 1),
+// so the per-node work is two Horner chains (W and M') instead of two chains and a MAC: 2 x 16 instead of
+// 2 x 16 + 8 units per (node, stage), for t^2/2 extra MACs once per function (k_corr_w, a tiled correlation like
+// k_tree_level).  Pays only for B = 1 (for B right-hand sides it would trade B MACs for B Horner steps).
+//   k_corr_w         W~_j (Montgomery) from the plain values v and the tree's M~
+//   k_solve_table_w  records { W_{l-1}, W_{l-1}', D_l, D_l' } at slot l-1
+//   k_node_eval2     one lane per node: q <- W_{l-1} + m q, d <- D_l + m d for l = t .. 1, then c_i = q / d [/ m]
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(ZP_K2_TC)
+k_corr_w(const uint64_t* __restrict__ vals, const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F,
+         ZpMod k, uint64_t* __restrict__ Wt) {
+  __shared__ uint64_t sA[ZP_K2_TJ];
+  __shared__ uint64_t sB[ZP_K2_TC + ZP_K2_TJ];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int64_t t = offsets[f + 1] - off;
+    const uint64_t* v = vals + off;
+    const uint64_t* M = Mt + off;
+    for (int64_t j0 = (int64_t)blockIdx.x * ZP_K2_TC; j0 < t; j0 += (int64_t)gridDim.x * ZP_K2_TC) {
+      const int64_t j = j0 + threadIdx.x;
+      Acc acc;
+      acc_zero(acc);
+      for (int64_t l0 = 0; l0 + j0 + 1 <= t - 1; l0 += ZP_K2_TJ) {  // some (l, j) of the tile has l + j + 1 <= t - 1
+        __syncthreads();
+        if (threadIdx.x < ZP_K2_TJ) sA[threadIdx.x] = (l0 + threadIdx.x < t) ? zp_canon(v[l0 + threadIdx.x], k.p) : 0;
+        for (int x = threadIdx.x; x < ZP_K2_TC + ZP_K2_TJ - 1; x += ZP_K2_TC) {
+          const int64_t kk = l0 + j0 + 1 + x;  // index into M of window slot x
+          sB[x] = (kk <= t - 1) ? M[kk] : 0;
+        }
+        __syncthreads();
+        const uint64_t* win = sB + threadIdx.x;  // win[jj] = M_{(l0 + jj) + j + 1}
+#pragma unroll 8
+        for (int jj = 0; jj < ZP_K2_TJ; jj += 2) acc_mac2(acc, sA[jj], win[jj], sA[jj + 1], win[jj + 1]);
+      }
+      if (j < t) {
+        const uint64_t r = mont_mul(acc_redc160(acc, k), k.c224, k);  // plain * Montgomery sums -> Montgomery
+        Wt[off + j] = mod_add(r, to_mont(zp_canon(v[t - 1 - j], k.p), k), k.p);  // + v_{t-1-j} M_t
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_solve_table_w(const uint64_t* __restrict__ Wt, const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets,
+                int F, ZpMod k, ulonglong4* __restrict__ tab) {
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int64_t t = offsets[f + 1] - off;
+    for (int64_t l = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l <= t; l += (int64_t)gridDim.x * blockDim.x) {
+      const uint64_t Wm = Wt[off + l - 1];
+      const uint64_t Mm = (l < t) ? Mt[off + l] : k.r1;
+      const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)zp_canon(l, k.p), k), k);  // (l M_l)~
+      ulonglong4 r;
+      r.x = from_mont(Wm, k);
+      r.y = shoup_companion(Wm, k);
+      r.z = from_mont(Dm, k);
+      r.w = shoup_companion(Dm, k);
+      tab[off + l - 1] = r;
+    }
+  }
+}
+
+#define ZP_K3E_STAGES 64
+__global__ void __launch_bounds__(ZP_K3_THREADS)
+k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
+             int F, int s0, ZpMod k, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
+  __shared__ __align__(16) ulonglong4 sT[2][ZP_K3E_STAGES];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int t = (int)(offsets[f + 1] - off);
+    const int i0 = blockIdx.x * ZP_K3_THREADS;
+    if (i0 >= t) continue;  // uniform per CTA
+    const int i = i0 + threadIdx.x;
+    const bool live = i < t;
+    const uint64_t m = live ? zp_canon(nodes[off + i], k.p) : 0;
+    const uint64_t mm = to_mont(m, k);
+    const uint64_t mp = shoup_companion(mm, k);
+    uint64_t q = 0, d = 0;
+    const ulonglong4* Tf = tab + off;
+    // tile = records l in (l1 - STAGES, l1], slot x holds record l1 - x (descending); records < 1 are zero and are
+    // consumed after the real ones: q <- 0 + m q would spoil the value, so the loop stops at l = 1
+    auto issue_tile = [&](int l1, int buf) {
+      for (int x = threadIdx.x; x < 2 * ZP_K3E_STAGES; x += ZP_K3_THREADS) {
+        const int l = l1 - (x >> 1);
+        const bool ok = l >= 1;
+        cp_async16(reinterpret_cast<ulonglong2*>(&sT[buf][0]) + x,
+                   reinterpret_cast<const ulonglong2*>(Tf + (ok ? l - 1 : 0)) + (x & 1), ok);
+      }
+      cp_async_commit();
+    };
+    __syncthreads();
+    issue_tile(t, 0);
+    int buf = 0;
+    for (int l1 = t; l1 >= 1; l1 -= ZP_K3E_STAGES, buf ^= 1) {
+      if (l1 - ZP_K3E_STAGES >= 1) {
+        issue_tile(l1 - ZP_K3E_STAGES, buf ^ 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
+      }
+      __syncthreads();
+      const int cnt = l1 < ZP_K3E_STAGES ? l1 : ZP_K3E_STAGES;
+#pragma unroll 4
+      for (int x = 0; x < cnt; ++x) {
+        const ulonglong4 r = sT[buf][x];
+        q = horner_step(q, m, mp, r.x, r.y, k);
+        d = horner_step(d, m, mp, r.z, r.w, k);
+      }
+      __syncthreads();
+    }
+    if (live) {
+      const uint64_t dm = to_mont(lazy_canon(d, k.p), k);
+      const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
+      if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
+      coefs[off + i] = mont_mul(lazy_canon(q, k.p), mont_inv(dd, k), k);  // plain * Montgomery -> plain
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // (a5) K5 Newton interpolation in x_k, one lane per coefficient (eq. (1)).
 // k_newton_prep: invd[j*B + jj] = {w, w'} with w = 1/(c_j - c_jj) for jj < j (plain, with its Shoup companion),
 // negc[j] = {-c_j, companion}, duplicate check.

@@ -141,6 +141,8 @@ void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const u
 #undef ZP_CASE
 }
 
+#define ZP_EVAL2_MIN_T 4096  // B = 1: from this skeleton length on the correlation + two-chain path is used
+
 // ---- stages (device offsets already in w.d_offsets) ---------------------------------------------
 // (a2) master polynomial of every function -> returns the buffer holding M' (Montgomery)
 const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64_t tmax, const ZpMod& k,
@@ -164,6 +166,18 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
                int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
   ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
   const uint64_t* Mt = run_master_poly(w, nodes, F, tmax, k, st);
+  if (B == 1 && tmax >= ZP_EVAL2_MIN_T) {
+    // one right-hand side, long skeleton: num_i = W(m_i) with W = correlation of v and M (kernels.cuh, k_corr_w)
+    uint64_t* Wt = (Mt == w.M0) ? w.M1 : w.M0;  // the tree's other buffer is free now
+    ProfScope prof(ZP_K_NODE_SOLVE, st);
+    dim3 gc((unsigned)((tmax + ZP_K2_TC - 1) / ZP_K2_TC), grid_y(F));
+    ++g_launches, k_corr_w<<<gc, ZP_K2_TC, 0, st>>>(vals, Mt, w.d_offsets, F, k, Wt);
+    dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
+    ++g_launches, k_solve_table_w<<<gt, 256, 0, st>>>(Wt, Mt, w.d_offsets, F, k, w.tab);
+    dim3 ge((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
+    ++g_launches, k_node_eval2<<<ge, ZP_K3_THREADS, 0, st>>>(nodes, w.tab, w.d_offsets, F, s0, k, coefs, w.st_solve);
+    return;
+  }
   {
     dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
     ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(Mt, w.d_offsets, F, k, w.tab);

@@ -175,6 +175,18 @@ def test_solve_tree_levels_and_tails(zp, ref, ts, B):
     assert (zp.to_host(got) == want).all()
 
 
+@pytest.mark.parametrize("ts", [[4095], [4096], [4097, 5000, 300]])
+@pytest.mark.parametrize("s0", [0, 1])
+def test_solve_single_rhs_both_paths(zp, ref, ts, s0):
+    """B = 1: below t = 4096 the per-node quotient form, from 4096 on W = corr(v, M) and two Horner chains per node
+    (k_corr_w, k_node_eval2); a batch mixes functions of both lengths under the longer one's path"""
+    nodes, offsets, vals = random_solve_case(40 + len(ts), ts, 1, P63)
+    want, wst = ref.vandermonde_solve_batch(nodes, offsets, vals, P63, s0)
+    got, st = zp.vandermonde_solve_batch(zp.to_dev(nodes), offsets, zp.to_dev(vals), P63, s0)
+    assert not wst.any() and not zp.to_host(st).any()
+    assert (zp.to_host(got) == want).all()
+
+
 def test_solve_residual_property_large(zp, ref):
     """size the oracle cannot finish in seconds: t = 40000; the unique solution is checked by the residual
     sum_i c_i m_i^s = v_s on sampled s through the oracle's power sums (one s costs O(t log s))."""
