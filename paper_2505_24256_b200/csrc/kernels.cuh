@@ -107,7 +107,7 @@ k_tree_leaf(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offs
 // (unit-stride reads), both staged in shared memory and zero-padded outside their ranges, so the inner
 // loop is branch-free deferred MACs.
 #define ZP_K2_TC 256
-#define ZP_K2_TJ 64
+#define ZP_K2_TJ 256
 __global__ void __launch_bounds__(ZP_K2_TC)
 k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offsets, int F, int64_t a, ZpMod k,
              uint64_t* __restrict__ dst) {
