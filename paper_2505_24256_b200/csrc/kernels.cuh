@@ -603,18 +603,19 @@ __global__ void k_status_finish(const int32_t* pre, const int32_t* solve, const 
 // ------------------------------------------------------------------------------------------------
 // (a6) K6 power sums R_{b,s} = sum_i a_{b,i} m_i^(s+s0)  ("raise base variable
 // values to various powers and substitute them into the polynomial"; strided power tables, A21).
-// CTA = (function f, block of 256 consecutive s); node tiles of 96 in shared memory with
-//   base_i = a_i~ m_i^(sb0+s0),  lo_i[x] = m_i^x,  hi_i[x] = m_i^(16x)   (x < 16),
-// lane s: m_i^(s-sb0) = lo_i[s & 15] * hi_i[s >> 4]; deferred sum over i.
+// CTA = (function f, block of 256 consecutive s); node tiles of 128 in shared memory with the strided power
+// tables  P_i[x] = a_i m_i^(sb0+s0) m_i^x,  H_i[x] = m_i^(16x)   (x < 16):  lane s adds P_i[s & 15] * H_i[s >> 4],
+// a deferred sum over i with no modular product in the inner loop.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K6_THREADS 256
-#define ZP_K6_NODES 96
+#define ZP_K6_NODES 128
 __global__ void __launch_bounds__(ZP_K6_THREADS)
 k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offsets, int F,
              const uint64_t* __restrict__ coef, int64_t T_tot, int B, int s0, ZpMod k, uint64_t* __restrict__ out) {
-  __shared__ uint64_t sBase[ZP_K6_NODES];                       // plain a_i m_i^(sb0+s0)
-  __shared__ __align__(16) ulonglong2 sLo[ZP_K6_NODES * 16];    // {w, w'}: plain m_i^x with its Shoup companion
-  __shared__ uint64_t sHi[ZP_K6_NODES * 16];                    // plain m_i^(16x)
+  // lane s = sb0 + 16 s2 + s1:  a_i m_i^(s+s0) = [a_i m_i^(sb0+s0) m_i^s1] * [(m_i^16)^s2] = P_i[s1] * H_i[s2],
+  // so with the two 16-entry tables of a node in shared memory the inner loop is one deferred MAC per (s, i)
+  __shared__ uint64_t sP[ZP_K6_NODES * 16];  // Montgomery
+  __shared__ uint64_t sH[ZP_K6_NODES * 16];  // plain
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -627,31 +628,36 @@ k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ off
       for (int i0 = 0; i0 < t; i0 += ZP_K6_NODES) {
         const int n = t - i0 < ZP_K6_NODES ? t - i0 : ZP_K6_NODES;
         __syncthreads();
-        if (threadIdx.x < n) {
-          const int i = i0 + threadIdx.x;
-          const uint64_t m = to_mont(zp_canon(nodes[off + i], k.p), k);
-          const uint64_t a = zp_canon(coef[(int64_t)b * T_tot + off + i], k.p);
-          sBase[threadIdx.x] = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);  // plain * mont -> plain
-          uint64_t pw = k.r1;
-          for (int x = 0; x < 16; ++x) {
-            sLo[threadIdx.x * 16 + x] = make_ulonglong2(from_mont(pw, k), shoup_companion(pw, k));
-            pw = mont_mul(pw, m, k);
-          }
-          const uint64_t m16 = pw;
-          pw = k.r1;
-          for (int x = 0; x < 16; ++x) {
-            sHi[threadIdx.x * 16 + x] = from_mont(pw, k);
-            pw = mont_mul(pw, m16, k);
+        {  // two builder lanes per node: lane (x, 0) fills P_x, lane (x, 1) fills H_x
+          const int x = threadIdx.x >> 1, which = threadIdx.x & 1;
+          if (x < n) {
+            const uint64_t m = to_mont(zp_canon(nodes[off + i0 + x], k.p), k);
+            if (which == 0) {
+              const uint64_t a = to_mont(zp_canon(coef[(int64_t)b * T_tot + off + i0 + x], k.p), k);
+              uint64_t pw = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);
+              for (int e = 0; e < 16; ++e) {
+                sP[x * 16 + e] = pw;
+                pw = mont_mul(pw, m, k);
+              }
+            } else {
+              uint64_t m16 = m;
+              for (int e = 0; e < 4; ++e) m16 = mont_mul(m16, m16, k);
+              uint64_t pw = 1 % k.p;  // plain; plain * Montgomery -> plain
+              for (int e = 0; e < 16; ++e) {
+                sH[x * 16 + e] = pw;
+                pw = mont_mul(pw, m16, k);
+              }
+            }
           }
         }
         __syncthreads();
-        const int lo = threadIdx.x & 15, hi = threadIdx.x >> 4;
-        for (int x = 0; x < n; ++x) {
-          const ulonglong2 w = sLo[x * 16 + lo];
-          acc_mac(acc, horner_step(sHi[x * 16 + hi], w.x, w.y, 0, 0, k), sBase[x]);  // lazy m_i^(s-sb0) times base
-        }
+        const uint64_t* pP = sP + (threadIdx.x & 15);
+        const uint64_t* pH = sH + (threadIdx.x >> 4);
+        int x = 0;
+        for (; x + 1 < n; x += 2) acc_mac2(acc, pP[x * 16], pH[x * 16], pP[x * 16 + 16], pH[x * 16 + 16]);
+        if (x < n) acc_mac(acc, pP[x * 16], pH[x * 16]);
       }
-      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c224, k);  // plain*plain sums
+      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c160, k);  // Montgomery * plain sums
     }
   }
 }
