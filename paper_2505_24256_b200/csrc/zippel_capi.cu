@@ -299,7 +299,7 @@ void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T
 }
 
 // copy streams and events of the host-buffer entry (created once per device, kept for the process)
-#define ZP_PIPE_MAX_CHUNKS 16
+#define ZP_PIPE_MAX_CHUNKS 24
 struct Pipe {
   bool ready = false;
   cudaStream_t s_in = nullptr, s_out = nullptr;
@@ -434,15 +434,22 @@ int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int 
   cudaStream_t st = (cudaStream_t)stream;
   Pipe* P = get_pipe();
   if (!P) return ZP_ERR_CUDA;
-  // chunks of whole functions, equal in terms; small batches go in one piece
+  // chunks of whole functions; small batches go in one piece.  The first and the last chunks are small (1/64,
+  // 2/64, 4/64 of the terms ...) because the first H2D copy and the last D2H copy cannot overlap with anything.
+  static const int kCut64[] = {0, 1, 3, 7, 12, 16, 20, 24, 28, 32, 36, 40, 44, 48, 52, 57, 61, 63, 64};
   const size_t bytes = 8 * (size_t)T_tot * B;
-  int nch = bytes < ((size_t)8 << 20) ? 1 : (F < ZP_PIPE_MAX_CHUNKS ? F : ZP_PIPE_MAX_CHUNKS);
+  int nch = 1;
   int cut[ZP_PIPE_MAX_CHUNKS + 1];
   cut[0] = 0;
-  for (int c = 1, f = 0; c <= nch; ++c) {
-    const int64_t target = T_tot * c / nch;
-    while (f < F && h_offsets[f] < target) ++f;
-    cut[c] = (c == nch) ? F : f;
+  if (bytes >= ((size_t)8 << 20) && F >= 64) {
+    nch = (int)(sizeof(kCut64) / sizeof(kCut64[0])) - 1;
+    for (int c = 1, f = 0; c <= nch; ++c) {
+      const int64_t target = T_tot / 64 * kCut64[c];
+      while (f < F && h_offsets[f] < target) ++f;
+      cut[c] = (c == nch) ? F : f;
+    }
+  } else {
+    cut[1] = F;
   }
   cudaMemcpyAsync(h.anchors, h_anchors, 8 * (size_t)nv, cudaMemcpyHostToDevice, st);
   cudaMemcpyAsync(h.samples, h_samples, 8 * (size_t)B, cudaMemcpyHostToDevice, st);

@@ -370,6 +370,40 @@ def test_lift_host_entry_matches_device_entry(zp, ref):
     assert (h_out.numpy().view(np.uint64) == want).all() and (h_st.numpy() == wst).all()
 
 
+def test_lift_host_entry_chunked_pipeline(zp, ref):
+    """above 8 MB of values and 64 functions the host entry cuts the batch into 18 chunks of whole functions and
+    pipelines H2D / kernels / D2H: every output equals the device entry's (itself checked against the oracle on
+    sampled functions here); ragged function lengths, status of a planted duplicate node in one chunk"""
+    import torch
+
+    r = np.random.Generator(np.random.Philox(key=[77, 1]))
+    ts = [int(x) for x in r.integers(200, 700, 160)]
+    w = wl.make_box_workload("chunks", wl.SEED_BASE + 55, len(ts), 4, ts, 20, 21, with_planted=False)
+    assert w.vals.nbytes >= (8 << 20)
+    w.exps[int(w.offsets[100]) + 5] = w.exps[int(w.offsets[100]) + 17]  # duplicate node in function 100
+    dev_out, dev_st = zp.zippel_lift_step(zp.to_dev(w.exps), w.offsets, zp.to_dev(w.anchors), zp.to_dev(w.samples),
+                                          zp.to_dev(w.vals), w.p, 0, 1)
+    pin = lambda a: torch.from_numpy(a.view(np.int64) if a.dtype == np.uint64 else a.view(np.int16)).pin_memory()
+    h_out = torch.empty(w.vals.shape, dtype=torch.int64).pin_memory()
+    h_st = torch.empty(w.F, dtype=torch.int32).pin_memory()
+    ws = torch.empty(zp.host_workspace_bytes(w.offsets, w.nv, w.B), dtype=torch.uint8, device="cuda")
+    for _ in range(2):  # twice: the copy streams and events are reused across calls
+        zp.zippel_lift_step_host(pin(w.exps), w.offsets, pin(w.anchors), pin(w.samples), pin(w.vals), w.p, h_out, h_st,
+                                 ws, 0, 1)
+        torch.cuda.synchronize()
+    st = h_st.numpy()
+    assert (st == zp.to_host(dev_st)).all() and st[100] != 0 and np.count_nonzero(st) == 1
+    got = h_out.numpy().view(np.uint64)
+    ok = np.ones(w.T_tot, dtype=bool)
+    ok[int(w.offsets[100]):int(w.offsets[101])] = False  # outputs of the failed function are unspecified
+    assert (got[:, ok] == zp.to_host(dev_out)[:, ok]).all()
+    for f in (0, 63, 159):
+        a, b = int(w.offsets[f]), int(w.offsets[f + 1])
+        want, _, wst = ref.zippel_lift_step(np.ascontiguousarray(w.exps[a:b]), np.array([0, b - a], dtype=np.int64), w.anchors,
+                                            w.samples, np.ascontiguousarray(w.vals[:, a:b]), w.p, 0, 1)
+        assert not wst.any() and (got[:, a:b] == want).all()
+
+
 # ------------------------------------------------------------------------------ balanced step, config 4
 def balanced_inputs(ref, rw):
     """u_{j,s} = true value x per-probe factor h_s; skel = C x coefficients at c_0 (readings G3, G19, G20)."""
