@@ -130,8 +130,8 @@ def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
     t2 = float(sum(int(t) * int(t) for t in ts))
     T = float(sum(int(t) for t in ts))
     node_solve = t2 * (2 * c_mm + B * c_mac)
-    if B == 1 and min(int(t) for t in ts) >= 4096:  # one right-hand side: W = corr(v, M), then two Horner chains
-        node_solve = t2 * (2 * c_mm + c_mac / 2)
+    if B == 1 and min(int(t) for t in ts) >= 4096:  # one right-hand side: W = corr(v, M), then W(m_i) and M'(m_i)
+        node_solve = t2 * (2 * c_mac + c_mac / 2)  # two polynomial evaluations by deferred MACs + the correlation
     total = node_solve + c_mac * t2 / 2 + c_mm * ((nv - 1) * T + (3 + B) * T)
     if newton:
         total += c_mm * T * B * (B - 1) / 2

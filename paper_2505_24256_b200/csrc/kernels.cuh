@@ -332,12 +332,13 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 // (a3) for ONE right-hand side and a long skeleton (C5): with q_{i,l} = sum_{k>l} M_k m_i^(k-l-1),
 //     num_i = sum_l q_{i,l} v_l = sum_j W_j m_i^j = W(m_i),    W_j = sum_l v_l M_{l+j+1}   (M_t = 1),
-// so the per-node work is two Horner chains (W and M') instead of two chains and a MAC: 2 x 16 instead of
-// 2 x 16 + 8 units per (node, stage), for t^2/2 extra MACs once per function (k_corr_w, a tiled correlation like
-// k_tree_level).  Pays only for B = 1 (for B right-hand sides it would trade B MACs for B Horner steps).
+// so the per-node work is the evaluation of two fixed polynomials (W and M') at m_i, which needs no modular product
+// per coefficient: 2 deferred MACs = 16 units per (node, stage) instead of 2 x 16 + 8, for t^2/2 extra MACs once
+// per function (k_corr_w, a tiled correlation like k_tree_level).  Pays only for B = 1 (the quotient q_{i,l} of the
+// general path is needed coefficient by coefficient, one modular multiply-add each).
 //   k_corr_w         W~_j (Montgomery) from the plain values v and the tree's M~
-//   k_solve_table_w  records { W_{l-1}, W_{l-1}', D_l, D_l' } at slot l-1
-//   k_node_eval2     one lane per node: q <- W_{l-1} + m q, d <- D_l + m d for l = t .. 1, then c_i = q / d [/ m]
+//   k_solve_table_w  records { W_j, D_{j+1} } (plain), j = 0 .. t-1
+//   k_node_eval2     one lane per node: W(m_i) and M'(m_i) by blocked deferred evaluation, then c_i = W / M' [/ m]
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(ZP_K2_TC)
 k_corr_w(const uint64_t* __restrict__ vals, const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F,
@@ -375,29 +376,28 @@ k_corr_w(const uint64_t* __restrict__ vals, const uint64_t* __restrict__ Mt, con
 
 __global__ void __launch_bounds__(256)
 k_solve_table_w(const uint64_t* __restrict__ Wt, const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets,
-                int F, ZpMod k, ulonglong4* __restrict__ tab) {
+                int F, ZpMod k, ulonglong2* __restrict__ tab) {
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int64_t t = offsets[f + 1] - off;
-    for (int64_t l = 1 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; l <= t; l += (int64_t)gridDim.x * blockDim.x) {
-      const uint64_t Wm = Wt[off + l - 1];
-      const uint64_t Mm = (l < t) ? Mt[off + l] : k.r1;
-      const uint64_t Dm = mont_mul(Mm, to_mont((uint64_t)zp_canon(l, k.p), k), k);  // (l M_l)~
-      ulonglong4 r;
-      r.x = from_mont(Wm, k);
-      r.y = shoup_companion(Wm, k);
-      r.z = from_mont(Dm, k);
-      r.w = shoup_companion(Dm, k);
-      tab[off + l - 1] = r;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < t; j += (int64_t)gridDim.x * blockDim.x) {
+      const uint64_t Mm = (j + 1 < t) ? Mt[off + j + 1] : k.r1;  // M_{j+1}~, M_t = 1
+      // record j = { W_j, D_{j+1} } plain: the coefficients of z^j in W and in M'  (D_l = l M_l)
+      tab[off + j] = make_ulonglong2(from_mont(Wt[off + j], k), mont_mul(Mm, (uint64_t)zp_canon(j + 1, k.p), k));
     }
   }
 }
 
-#define ZP_K3E_STAGES 64
+// Both polynomials are evaluated at m_i in blocks of 32 coefficients against the lane's own table of powers
+// m^0 .. m^31 (registers): a block is 32 deferred MACs per polynomial, one reduction, and one
+// step V <- V m^32 + S of the outer Horner rule -- 17.8 pipe cycles per coefficient instead of the 35.5 of a
+// modular multiply-add per coefficient.
+#define ZP_K3E_BLK 32
+#define ZP_K3E_TILE 128
 __global__ void __launch_bounds__(ZP_K3_THREADS)
-k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
+k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ tab, const int64_t* __restrict__ offsets,
              int F, int s0, ZpMod k, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
-  __shared__ __align__(16) ulonglong4 sT[2][ZP_K3E_STAGES];
+  __shared__ __align__(16) ulonglong2 sT[2][ZP_K3E_TILE];
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
@@ -407,45 +407,68 @@ k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
     const bool live = i < t;
     const uint64_t m = live ? zp_canon(nodes[off + i], k.p) : 0;
     const uint64_t mm = to_mont(m, k);
-    const uint64_t mp = shoup_companion(mm, k);
-    uint64_t q = 0, d = 0;
-    const ulonglong4* Tf = tab + off;
-    // tile = records l in (l1 - STAGES, l1], slot x holds record l1 - x (descending); records < 1 are zero and are
-    // consumed after the real ones: q <- 0 + m q would spoil the value, so the loop stops at l = 1
-    auto issue_tile = [&](int l1, int buf) {
-      for (int x = threadIdx.x; x < 2 * ZP_K3E_STAGES; x += ZP_K3_THREADS) {
-        const int l = l1 - (x >> 1);
-        const bool ok = l >= 1;
-        cp_async16(reinterpret_cast<ulonglong2*>(&sT[buf][0]) + x,
-                   reinterpret_cast<const ulonglong2*>(Tf + (ok ? l - 1 : 0)) + (x & 1), ok);
+    uint64_t pw[ZP_K3E_BLK];  // plain m^e
+    pw[0] = 1 % k.p;
+#pragma unroll
+    for (int e = 1; e < ZP_K3E_BLK; ++e) pw[e] = mont_mul(pw[e - 1], mm, k);  // plain * Montgomery -> plain
+    const uint64_t m32 = mont_mul(pw[ZP_K3E_BLK - 1], mm, k);
+    const ulonglong2 w32 = make_ulonglong2(m32, shoup_companion(to_mont(m32, k), k));
+    uint64_t VW = 0, VD = 0;
+    Acc pW, pD;  // sums of the previous block: their reduction and the outer Horner step run while the MACs of the
+    acc_zero(pW);  // current block are issued (two independent instruction streams in one loop body)
+    acc_zero(pD);
+    const ulonglong2* Tf = tab + off;
+    auto issue_tile = [&](int tile, int buf) {  // records j in [128 tile, 128 tile + 128), zero beyond t
+      for (int x = threadIdx.x; x < ZP_K3E_TILE; x += ZP_K3_THREADS) {
+        const int j = tile * ZP_K3E_TILE + x;
+        const bool ok = j < t;
+        cp_async16(&sT[buf][x], Tf + (ok ? j : 0), ok);
       }
       cp_async_commit();
     };
+    const int ntile = (t + ZP_K3E_TILE - 1) / ZP_K3E_TILE;
     __syncthreads();
-    issue_tile(t, 0);
+    issue_tile(ntile - 1, 0);
     int buf = 0;
-    for (int l1 = t; l1 >= 1; l1 -= ZP_K3E_STAGES, buf ^= 1) {
-      if (l1 - ZP_K3E_STAGES >= 1) {
-        issue_tile(l1 - ZP_K3E_STAGES, buf ^ 1);
+    for (int tile = ntile - 1; tile >= 0; --tile, buf ^= 1) {
+      if (tile > 0) {
+        issue_tile(tile - 1, buf ^ 1);
         cp_async_wait<1>();
       } else {
         cp_async_wait<0>();
       }
       __syncthreads();
-      const int cnt = l1 < ZP_K3E_STAGES ? l1 : ZP_K3E_STAGES;
-#pragma unroll 4
-      for (int x = 0; x < cnt; ++x) {
-        const ulonglong4 r = sT[buf][x];
-        q = horner_step(q, m, mp, r.x, r.y, k);
-        d = horner_step(d, m, mp, r.z, r.w, k);
+#pragma unroll 1
+      for (int bl = ZP_K3E_TILE / ZP_K3E_BLK - 1; bl >= 0; --bl) {
+        const ulonglong2* rec = &sT[buf][bl * ZP_K3E_BLK];
+        Acc aW, aD;
+        acc_zero(aW);
+        acc_zero(aD);
+#pragma unroll
+        for (int e = 0; e < ZP_K3E_BLK; e += 2) {
+          const ulonglong2 r0 = rec[e], r1 = rec[e + 1];
+          acc_mac2(aW, pw[e], r0.x, pw[e + 1], r1.x);
+          acc_mac2(aD, pw[e], r0.y, pw[e + 1], r1.y);
+        }
+        // previous block: plain * plain sums, 2^-160 (reduction) and 2^-64 (product) cancel against 2^224
+        const uint64_t SW = mont_mul(acc_redc160(pW, k), k.c224, k), SD = mont_mul(acc_redc160(pD, k), k.c224, k);
+        VW = mod_add(shoup_mul(VW, w32, k), SW, k.p);
+        VD = mod_add(shoup_mul(VD, w32, k), SD, k.p);
+        pW = aW;
+        pD = aD;
       }
       __syncthreads();
     }
+    {  // the last block
+      const uint64_t SW = mont_mul(acc_redc160(pW, k), k.c224, k), SD = mont_mul(acc_redc160(pD, k), k.c224, k);
+      VW = mod_add(shoup_mul(VW, w32, k), SW, k.p);
+      VD = mod_add(shoup_mul(VD, w32, k), SD, k.p);
+    }
     if (live) {
-      const uint64_t dm = to_mont(lazy_canon(d, k.p), k);
+      const uint64_t dm = to_mont(VD, k);
       const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
       if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-      coefs[off + i] = mont_mul(lazy_canon(q, k.p), mont_inv(dd, k), k);  // plain * Montgomery -> plain
+      coefs[off + i] = mont_mul(VW, mont_inv(dd, k), k);  // plain * Montgomery -> plain
     }
   }
 }
@@ -474,11 +497,6 @@ __global__ void k_newton_prep(const uint64_t* __restrict__ samples, int B, ZpMod
   }
 }
 
-// x * w mod p for a fixed multiplier w with companion w' (horner_step with a zero addend), canonical result;
-// x may be any 64-bit value
-ZP_DEV uint64_t shoup_mul(uint64_t x, ulonglong2 w, const ZpMod& k) {
-  return lazy_canon(horner_step(x, w.x, w.y, 0, 0, k), k.p);
-}
 
 #define ZP_K5_THREADS 128
 // CANON: the values are known to be canonical (the lifting step feeds the solve's output), skip the reduction

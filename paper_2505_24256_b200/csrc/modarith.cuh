@@ -206,6 +206,11 @@ ZP_DEV uint64_t lazy_canon(uint64_t x, uint64_t p) {  // [0,2p) -> [0,p)
   const uint64_t s = x - p;
   return (x >= p) ? s : x;
 }
+// x * w mod p for a fixed multiplier w = {w, w'} with its companion (horner_step with a zero addend), canonical
+// result; x may be any 64-bit value
+ZP_DEV uint64_t shoup_mul(uint64_t x, ulonglong2 w, const ZpMod& k) {
+  return lazy_canon(horner_step(x, w.x, w.y, 0, 0, k), k.p);
+}
 
 // Deferred accumulator.  value = E + O * 2^32 with
 //   E = e0 + e1*2^64 + e2*2^128  (takes x0*y0 at bit 0 and x1*y1 at bit 64),

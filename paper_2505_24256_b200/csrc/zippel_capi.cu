@@ -173,9 +173,10 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
     dim3 gc((unsigned)((tmax + ZP_K2_TC - 1) / ZP_K2_TC), grid_y(F));
     ++g_launches, k_corr_w<<<gc, ZP_K2_TC, 0, st>>>(vals, Mt, w.d_offsets, F, k, Wt);
     dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
-    ++g_launches, k_solve_table_w<<<gt, 256, 0, st>>>(Wt, Mt, w.d_offsets, F, k, w.tab);
+    ++g_launches, k_solve_table_w<<<gt, 256, 0, st>>>(Wt, Mt, w.d_offsets, F, k, reinterpret_cast<ulonglong2*>(w.tab));
     dim3 ge((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
-    ++g_launches, k_node_eval2<<<ge, ZP_K3_THREADS, 0, st>>>(nodes, w.tab, w.d_offsets, F, s0, k, coefs, w.st_solve);
+    ++g_launches, k_node_eval2<<<ge, ZP_K3_THREADS, 0, st>>>(nodes, reinterpret_cast<const ulonglong2*>(w.tab), w.d_offsets, F, s0, k, coefs,
+                                                               w.st_solve);
     return;
   }
   {
