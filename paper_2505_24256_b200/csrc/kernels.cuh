@@ -411,9 +411,10 @@ k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ 
     pw[0] = 1 % k.p;
 #pragma unroll
     for (int e = 1; e < ZP_K3E_BLK; ++e) pw[e] = mont_mul(pw[e - 1], mm, k);  // plain * Montgomery -> plain
-    const uint64_t m32 = mont_mul(pw[ZP_K3E_BLK - 1], mm, k);
-    const ulonglong2 w32 = make_ulonglong2(m32, shoup_companion(to_mont(m32, k), k));
-    uint64_t VW = 0, VD = 0;
+    // The outer Horner step rides in the same accumulator: with V' = V 2^-160 and g = m^32 2^160,
+    //   V'_new = (S + V' g) 2^-160 = acc_redc160(S + V' g),  no other modular product per block.
+    const uint64_t g = mont_mul(mont_mul(pw[ZP_K3E_BLK - 1], mm, k), k.c224, k);  // m^32 * 2^224 * 2^-64
+    uint64_t VW = 0, VD = 0;  // V' of the two polynomials
     Acc pW, pD;  // sums of the previous block: their reduction and the outer Horner step run while the MACs of the
     acc_zero(pW);  // current block are issued (two independent instruction streams in one loop body)
     acc_zero(pD);
@@ -450,20 +451,19 @@ k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ 
           acc_mac2(aW, pw[e], r0.x, pw[e + 1], r1.x);
           acc_mac2(aD, pw[e], r0.y, pw[e + 1], r1.y);
         }
-        // previous block: plain * plain sums, 2^-160 (reduction) and 2^-64 (product) cancel against 2^224
-        const uint64_t SW = mont_mul(acc_redc160(pW, k), k.c224, k), SD = mont_mul(acc_redc160(pD, k), k.c224, k);
-        VW = mod_add(shoup_mul(VW, w32, k), SW, k.p);
-        VD = mod_add(shoup_mul(VD, w32, k), SD, k.p);
+        acc_mac(pW, VW, g);  // previous block: V' <- (S + V' g) 2^-160
+        acc_mac(pD, VD, g);
+        VW = acc_redc160(pW, k);
+        VD = acc_redc160(pD, k);
         pW = aW;
         pD = aD;
       }
       __syncthreads();
     }
-    {  // the last block
-      const uint64_t SW = mont_mul(acc_redc160(pW, k), k.c224, k), SD = mont_mul(acc_redc160(pD, k), k.c224, k);
-      VW = mod_add(shoup_mul(VW, w32, k), SW, k.p);
-      VD = mod_add(shoup_mul(VD, w32, k), SD, k.p);
-    }
+    acc_mac(pW, VW, g);  // the last block, then back from V' to V = V' 2^160
+    acc_mac(pD, VD, g);
+    VW = mont_mul(acc_redc160(pW, k), k.c224, k);
+    VD = mont_mul(acc_redc160(pD, k), k.c224, k);
     if (live) {
       const uint64_t dm = to_mont(VD, k);
       const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
