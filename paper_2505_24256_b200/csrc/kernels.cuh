@@ -162,7 +162,7 @@ k_tree_level(const uint64_t* __restrict__ src, const int64_t* __restrict__ offse
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F, ZpMod k,
-              ulonglong4* __restrict__ tab) {
+              ulonglong4* __restrict__ tab, uint64_t* __restrict__ Dplain) {
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int64_t t = offsets[f + 1] - off;
@@ -175,6 +175,7 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
       r.z = from_mont(Dm, k);
       r.w = shoup_companion(Dm, k);
       tab[off + l - 1] = r;
+      Dplain[off + l - 1] = r.z;  // coefficient of z^(l-1) in M': the table of k_node_den
     }
   }
 }
@@ -205,7 +206,7 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 #ifdef ZP_K3_FORCE_ORIENT
 #define ZP_K3_ORIENT(NB) (ZP_K3_FORCE_ORIENT)
 #else
-#define ZP_K3_ORIENT_MASK 0x1e18108u
+#define ZP_K3_ORIENT_MASK 0x1810300u
 #define ZP_K3_ORIENT(NB) ((ZP_K3_ORIENT_MASK >> (NB)) & 1u)
 #endif
 
@@ -469,6 +470,78 @@ k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ 
       const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
       if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
       coefs[off + i] = mont_mul(VW, mont_inv(dd, k), k);  // plain * Montgomery -> plain
+    }
+  }
+}
+
+// (a4) denominators for the general path: den_i = M'(m_i) by the same blocked deferred evaluation (17.8 pipe cycles
+// per coefficient), one launch before k_node_solve, which then runs without its second Horner chain (35.5 cycles
+// per stage).  Writes scale_i = den_i^-1 (/ m_i) * 2^224, the factor k_node_solve<., false> applies.
+__global__ void __launch_bounds__(ZP_K3_THREADS)
+k_node_den(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ Dtab, const int64_t* __restrict__ offsets,
+           int F, int s0, ZpMod k, uint64_t* __restrict__ scale, int32_t* __restrict__ status) {
+  __shared__ __align__(16) uint64_t sT[2][ZP_K3E_TILE];
+  for (int f = blockIdx.y; f < F; f += gridDim.y) {
+    const int64_t off = offsets[f];
+    const int t = (int)(offsets[f + 1] - off);
+    const int i0 = blockIdx.x * ZP_K3_THREADS;
+    if (i0 >= t) continue;  // uniform per CTA
+    const int i = i0 + threadIdx.x;
+    const bool live = i < t;
+    const uint64_t m = live ? zp_canon(nodes[off + i], k.p) : 0;
+    const uint64_t mm = to_mont(m, k);
+    uint64_t pw[ZP_K3E_BLK];  // plain m^e
+    pw[0] = 1 % k.p;
+#pragma unroll
+    for (int e = 1; e < ZP_K3E_BLK; ++e) pw[e] = mont_mul(pw[e - 1], mm, k);
+    const uint64_t g = mont_mul(mont_mul(pw[ZP_K3E_BLK - 1], mm, k), k.c224, k);  // m^32 2^160, see k_node_eval2
+    uint64_t VD = 0;
+    Acc pD;
+    acc_zero(pD);
+    const uint64_t* Tf = Dtab + off;
+    auto issue_tile = [&](int tile, int buf) {
+      for (int x = threadIdx.x; x < ZP_K3E_TILE; x += ZP_K3_THREADS) {
+        const int j = tile * ZP_K3E_TILE + x;
+        const bool ok = j < t;
+        cp_async8(&sT[buf][x], Tf + (ok ? j : 0), ok);
+      }
+      cp_async_commit();
+    };
+    const int ntile = (t + ZP_K3E_TILE - 1) / ZP_K3E_TILE;
+    __syncthreads();
+    issue_tile(ntile - 1, 0);
+    int buf = 0;
+    for (int tile = ntile - 1; tile >= 0; --tile, buf ^= 1) {
+      if (tile > 0) {
+        issue_tile(tile - 1, buf ^ 1);
+        cp_async_wait<1>();
+      } else {
+        cp_async_wait<0>();
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int bl = ZP_K3E_TILE / ZP_K3E_BLK - 1; bl >= 0; --bl) {
+        const ulonglong2* rec = reinterpret_cast<const ulonglong2*>(&sT[buf][bl * ZP_K3E_BLK]);
+        Acc aD;
+        acc_zero(aD);
+#pragma unroll
+        for (int e = 0; e < ZP_K3E_BLK; e += 2) {
+          const ulonglong2 r = rec[e >> 1];  // { D_e, D_{e+1} }
+          acc_mac2(aD, pw[e], r.x, pw[e + 1], r.y);
+        }
+        acc_mac(pD, VD, g);  // previous block: V' <- (S + V' g) 2^-160
+        VD = acc_redc160(pD, k);
+        pD = aD;
+      }
+      __syncthreads();
+    }
+    acc_mac(pD, VD, g);
+    VD = mont_mul(acc_redc160(pD, k), k.c224, k);  // plain M'(m_i)
+    if (live) {
+      const uint64_t dm = to_mont(VD, k);
+      const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
+      if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
+      scale[off + i] = mont_mul(mont_inv(dd, k), k.c224, k);
     }
   }
 }

@@ -121,10 +121,8 @@ template <int NB>
 void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
                        const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k,
                        uint64_t* scale, uint64_t* coefs, int32_t* status) {
-  if (first)
-    ++g_launches, k_node_solve<NB, true><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
-  else
-    ++g_launches, k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+  (void)first;  // the denominators come from k_node_den: every pass is a <NB, false> pass
+  ++g_launches, k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
 }
 
 void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
@@ -181,13 +179,14 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
   }
   {
     dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
-    ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(Mt, w.d_offsets, F, k, w.tab);
+    ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(Mt, w.d_offsets, F, k, w.tab, w.R);
   }
   const ulonglong4* M = w.tab;
   const int passes = (B + ZP_NB_MAX - 1) / ZP_NB_MAX;
   const int per = (B + passes - 1) / passes;
   ProfScope prof(ZP_K_NODE_SOLVE, st);
   dim3 g((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
+  ++g_launches, k_node_den<<<g, ZP_K3_THREADS, 0, st>>>(nodes, w.R, w.d_offsets, F, s0, k, w.scale, w.st_solve);
   for (int b0 = 0, pass = 0; b0 < B; b0 += per, ++pass) {
     const int nb = (B - b0 < per) ? (B - b0) : per;
     dispatch_node_solve(nb, pass == 0, g, st, nodes, M, w.d_offsets, F, vals, T_tot, b0, s0, k, w.scale, coefs,
