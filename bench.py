@@ -307,12 +307,12 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {
-            "bound": "alu", "kernel": "k_node_solve" + (" (numerator part)" if idx == 4 else ""),
+            "bound": "alu", "kernel": ("k_corr_w + k_node_eval2" if idx == 5 else "k_node_den + k_node_solve") + (" (numerator part)" if idx == 4 else ""),
             "achieved": achieved, "peak": IMAD_PEAK_TOPS,
             "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
             # dram__bytes_read.sum + dram__bytes_write.sum of this launch from the ncu --set full capture of the same
-            # command (profiles/r01_final.md): 859.5 + 689.0 MB; algorithmic 1507 MB.  Only known for the default config.
-            "traffic": 1548.6e6 if (idx == 2 and not args.F) else None,
+            # command (profiles/r01_final.md): 892.5 + 660.8 MB; algorithmic 1540 MB.  Only known for the default config.
+            "traffic": 1553.3e6 if (idx == 2 and not args.F) else None,
             "peak_source": "derived (DESIGN.md Roofline): 148 SM x 64 lanes/clk of the fma-heavy pipe x 1.965 GHz; "
                            "profiles/r01_baseline.md measures IMAD at 63.5 and IMAD.WIDE at 31.8 lanes/clk/SM",
             "algorithmic_ops_per_launch": ns_ops, "ms_per_launch": ns_ms,
