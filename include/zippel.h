@@ -97,8 +97,9 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
 
 /* Host-buffer form of zippel_lift_step (the end-to-end call): every data pointer is a HOST pointer
  * (pinned memory makes the copies asynchronous).  Staging is carved from `workspace` (device,
- * zippel_host_workspace_bytes() bytes).  Batches above 8 MB of values (and at least 64 functions) are cut into 18 chunks of whole
- * functions, small ones first and last (functions are independent): the H2D copy of chunk c+1 and the D2H copy of
+ * zippel_host_workspace_bytes() bytes).  Batches above 8 MB of values (and at least 64 functions) are cut into 6 chunks of whole
+ * functions (2, 8, 22, 22, 8, 2 sixty-fourths of the terms: small first and last, each chunk's copy hidden behind
+ * its predecessor's kernels; more chunks cost more in partial waves and launches than they hide) (functions are independent): the H2D copy of chunk c+1 and the D2H copy of
  * chunk c-1 run on two copy streams of the library while the kernels of chunk c run on `stream`; the copy
  * streams start after the work already queued on `stream`, and `stream` ends waiting for the last D2H copy.
  * Nothing is synchronised: the caller waits on `stream` before reading h_out / h_status.  The two copy

@@ -371,7 +371,7 @@ def test_lift_host_entry_matches_device_entry(zp, ref):
 
 
 def test_lift_host_entry_chunked_pipeline(zp, ref):
-    """above 8 MB of values and 64 functions the host entry cuts the batch into 18 chunks of whole functions and
+    """above 8 MB of values and 64 functions the host entry cuts the batch into 6 chunks of whole functions and
     pipelines H2D / kernels / D2H: every output equals the device entry's (itself checked against the oracle on
     sampled functions here); ragged function lengths, status of a planted duplicate node in one chunk"""
     import torch
