@@ -195,14 +195,18 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 // pair go into the accumulator together (acc_mac2).
 // All values are plain residues; q and d stay lazy in [0, 2p) (horner_step); nothing of length t is
 // stored per lane (reading G7).
-// Template NB = right-hand sides handled per pass; FIRST = this pass computes d and writes scale.
+// Template NB = right-hand sides handled per pass; FIRST = this pass also runs the d chain and writes scale.
+// Since k_node_den (below) the library launches only the <NB, false> instances: den_i = M'(m_i) is a polynomial
+// evaluation and is cheaper by blocked deferred MACs in its own launch than as a second Horner chain here; the
+// FIRST code path stays as the literal form of PAPER.md L193-196 (and is what the first measured profiles show).
 // ------------------------------------------------------------------------------------------------
 #define ZP_K3_THREADS 128
 #define ZP_K3_PAIRS 32
 // Orientation of the 16-byte value record per template instance.  Both orders put the two limbs of one operand
 // into registers of the same parity; which of the two ptxas's register allocation serves with fewer bank
 // conflicts differs from instance to instance, so it is read off the SASS (share of accumulating IMAD.WIDE whose
-// multiplicands have equal parity; profiles/r01_final.md) and tabulated: bit NB = 1 -> odd stage first.
+// multiplicands have equal parity; profiles/r01_final.md) and tabulated for the <NB, false> instances: bit NB = 1 ->
+// odd stage first.
 #ifdef ZP_K3_FORCE_ORIENT
 #define ZP_K3_ORIENT(NB) (ZP_K3_FORCE_ORIENT)
 #else
