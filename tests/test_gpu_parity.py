@@ -175,7 +175,7 @@ def test_solve_tree_levels_and_tails(zp, ref, ts, B):
     assert (zp.to_host(got) == want).all()
 
 
-@pytest.mark.parametrize("ts", [[4095], [4096], [4097, 5000, 300]])
+@pytest.mark.parametrize("ts", [[4095], [4096], [4097, 5000, 300], [1, 4200, 2, 33]])
 @pytest.mark.parametrize("s0", [0, 1])
 def test_solve_single_rhs_both_paths(zp, ref, ts, s0):
     """B = 1: below t = 4096 the per-node quotient form, from 4096 on W = corr(v, M) and two Horner chains per node
