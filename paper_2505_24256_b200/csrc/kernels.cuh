@@ -641,6 +641,23 @@ __global__ void k_set_identity(uint64_t* __restrict__ I, int B) {
   if (idx < B * B) I[idx] = (idx / B == idx % B) ? 1 : 0;
 }
 
+// R output rows of L x column: R deferred dot products sharing every load of the column
+template <int R>
+ZP_DEV void newton_apply_rows(const uint64_t* r0, int B, int bmax, const uint64_t* col, const ZpMod& k, uint64_t* o,
+                              int64_t ld) {
+  Acc a[R];
+#pragma unroll
+  for (int q = 0; q < R; ++q) acc_zero(a[q]);
+  for (int b = 0; b < bmax; ++b) {
+    const uint64_t x = col[b * ZP_K5_THREADS];
+#pragma unroll
+    for (int q = 0; q < R; ++q) acc_mac(a[q], x, r0[q * B + b]);
+  }
+  // plain * plain sums: 2^-160 from the reduction and 2^-64 from the product cancel against 2^224
+#pragma unroll
+  for (int q = 0; q < R; ++q) o[(int64_t)q * ld] = mont_mul(acc_redc160(a[q], k), k.c224, k);
+}
+
 template <bool CANON>
 __global__ void __launch_bounds__(ZP_K5_THREADS)
 k_newton_apply(const uint64_t* __restrict__ L, int B, const uint64_t* vals, int64_t n, int64_t ld, ZpMod k, int basis,
@@ -654,25 +671,16 @@ k_newton_apply(const uint64_t* __restrict__ L, int B, const uint64_t* vals, int6
   for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
     for (int b = 0; b < B; ++b) col[b * TH] = CANON ? vals[b * ld + i] : zp_canon(vals[b * ld + i], k.p);
     for (int d0 = 0; d0 < B; d0 += 4) {
-      Acc a0, a1, a2, a3;
-      acc_zero(a0);
-      acc_zero(a1);
-      acc_zero(a2);
-      acc_zero(a3);
-      const int bmax = (basis == 0 && d0 + 4 < B) ? d0 + 4 : B;  // Newton basis: L is lower triangular
+      const int rows = B - d0 < 4 ? B - d0 : 4;
+      const int bmax = (basis == 0 && d0 + rows < B) ? d0 + rows : B;  // Newton basis: L is lower triangular
       const uint64_t* r0 = sL + (size_t)d0 * B;
-      for (int b = 0; b < bmax; ++b) {
-        const uint64_t x = col[b * TH];
-        acc_mac(a0, x, r0[b]);
-        acc_mac(a1, x, r0[B + b]);
-        acc_mac(a2, x, r0[2 * B + b]);
-        acc_mac(a3, x, r0[3 * B + b]);
+      uint64_t* o = out + (int64_t)d0 * ld + i;
+      switch (rows) {  // the last group has B mod 4 rows: no products against padding
+        case 4: newton_apply_rows<4>(r0, B, bmax, col, k, o, ld); break;
+        case 3: newton_apply_rows<3>(r0, B, bmax, col, k, o, ld); break;
+        case 2: newton_apply_rows<2>(r0, B, bmax, col, k, o, ld); break;
+        default: newton_apply_rows<1>(r0, B, bmax, col, k, o, ld); break;
       }
-      // plain * plain sums: 2^-160 from the reduction and 2^-64 from the product cancel against 2^224
-      out[(int64_t)d0 * ld + i] = mont_mul(acc_redc160(a0, k), k.c224, k);
-      if (d0 + 1 < B) out[(int64_t)(d0 + 1) * ld + i] = mont_mul(acc_redc160(a1, k), k.c224, k);
-      if (d0 + 2 < B) out[(int64_t)(d0 + 2) * ld + i] = mont_mul(acc_redc160(a2, k), k.c224, k);
-      if (d0 + 3 < B) out[(int64_t)(d0 + 3) * ld + i] = mont_mul(acc_redc160(a3, k), k.c224, k);
     }
   }
 }
