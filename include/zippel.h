@@ -5,14 +5,21 @@
  *
  * Conventions for every entry point
  *   - Pointers are DEVICE pointers unless the name starts with h_ (host).  The caller owns every
- *     buffer; the library allocates nothing and keeps no state between calls.  Scratch comes from
- *     the caller's `workspace` (device, 256-byte aligned, zippel_workspace_bytes() bytes).
+ *     buffer; the library allocates no device memory and keeps no per-call state.  Scratch comes from
+ *     the caller's `workspace` (device, 256-byte aligned, zippel_workspace_bytes() bytes).  Process-wide
+ *     state, all of it listed here: the tuning knobs (zippel_set_tuning), the measurement hook and launch
+ *     counter (zippel_profile_events, zippel_launch_count), and the two copy streams + events that
+ *     zippel_lift_step_host creates per device on first use (zippel_shutdown destroys them).  None of it
+ *     is thread-safe: one host thread per process calls the library.
  *   - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default stream).
  *   - Residues are canonical, in [0, p); p is an odd prime, 3 <= p < 2^63 (primality is the caller's
- *     contract; reading G14, G22).
+ *     contract; reading G14, G22).  There is no ZP_FLAG_CHECK_RANGE / ZP_ST_RANGE (SURVEY.md 8(b) proposed
+ *     them): every kernel canonicalises each input word as it loads it (x < p ? x : x % p), so a residue
+ *     >= p gives the result of its canonical representative instead of a status.
  *   - Batch layout: F functions, function f owns the terms [h_offsets[f], h_offsets[f+1]);
- *     T_tot = h_offsets[F].  A "[B x T_tot]" array holds row b at x + b*T_tot; inside a row the
- *     entries of function f start at h_offsets[f].
+ *     T_tot = h_offsets[F] < 2^31.  A "[B x T_tot]" array holds row b at x + b*T_tot; inside a row the
+ *     entries of function f start at h_offsets[f].  One function has at most 2^23 - 1 terms (the status
+ *     word keeps 23 bits for the index; the NTT engine's longest transform is 2^24).
  *   - Return value: ZP_OK, or an error found on the host before anything was enqueued.
  *     Data-dependent failures are written to status[f] (device int32): 0 = ok, else
  *     (index << 8) | code with the smallest offending index.  Outputs of a failed function are
@@ -195,19 +202,16 @@ int zippel_profile_events(int kernel, void* ev_start, void* ev_stop);
 /* Number of kernels this library has enqueued in this process so far (bench.py's gpu_launches). */
 unsigned long long zippel_launch_count(void);
 
-/* Self-test hook for the arithmetic substrate (a0), section 2.1: out[i] = op(a[i], b[i]) mod p,
- * op: 0 mul, 1 add, 2 sub, 3 pow (b = exponent), 4 inverse of a (0 -> 0),
- *     5 deferred dot: out[0] = sum_i a[i]*b[i] mod p through the 160-bit accumulator,
- *     6 Horner step: out[i] = (b[i] * a[i] + a[(i+1) % n]) mod p, where the multiplicand a[i] is taken as a
- *       LAZY value (any 64-bit number, not reduced first) -- the hot recurrence of (a3). */
-int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
-                             void* stream);
+/* Tuning knobs (process-wide; set them before sizing a workspace, not concurrently with other calls).
+ *   ZP_TUNE_SUBQ_MIN_T: functions with at least this many terms (and more than 1024) take the sub-quadratic route
+ *   (three-prime NTT product tree, tails, leaf solves: csrc/subq.cuh) instead of the quadratic
+ *   kernels of PAPER.md section 2.2.  Same results bit for bit; default = the measured crossover. */
+#define ZP_TUNE_SUBQ_MIN_T 1
+int zippel_set_tuning(int key, int64_t value);
 
-/* Roofline micro-benchmarks of the integer multiplier pipe:
- * launches `blocks` CTAs of 256 lanes, each running `iters` x 64 statements of `kind` per chain group
- * (kinds: csrc/ubench.cuh).  out: device scratch [blocks * 256].  *h_chain_steps (host, optional)
- * receives the number of lane-statements executed, for the caller to divide by its event time. */
-int zippel_ubench(int kind, int iters, int blocks, uint64_t p, uint64_t* out, double* h_chain_steps, void* stream);
+/* Destroys the copy streams and events that zippel_lift_step_host created (on every device that used it).  The
+ * caller makes sure no call of the library is in flight.  A later zippel_lift_step_host creates them again. */
+int zippel_shutdown(void);
 
 #ifdef __cplusplus
 }

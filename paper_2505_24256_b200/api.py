@@ -9,6 +9,7 @@ compute call raises if the library or a CUDA device is missing.
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 from typing import Optional, Sequence
@@ -27,9 +28,12 @@ MAX_NV, MAX_B = 32, 64
 EXPORTS = (
     "zippel_strerror", "zippel_workspace_bytes", "zippel_eval_nodes", "vandermonde_solve_batch",
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
-    "zippel_modarith_selftest", "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
-    "zippel_launch_count", "zippel_ubench", "thiele_reconstruct_batch", "zippel_extend_skeleton", "crt_rational_reconstruct_batch",
+    "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
+    "zippel_launch_count", "thiele_reconstruct_batch", "zippel_extend_skeleton", "crt_rational_reconstruct_batch",
+    "zippel_set_tuning", "zippel_shutdown",
 )
+TUNE_SUBQ_MIN_T = 1
+SUBQ_MIN_T_DEFAULT = 8192  # g_subq_min_t in csrc/zippel_capi.cu
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
 
@@ -45,6 +49,34 @@ class _Part(C.Structure):
 _lib = None
 
 
+def declare(L: C.CDLL) -> C.CDLL:
+    """Argument types of the entry points of include/zippel.h on a loaded library."""
+    vp, i32, i64, u64, sz = C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.c_size_t
+    L.zippel_strerror.restype = C.c_char_p
+    L.zippel_strerror.argtypes = [i32]
+    L.zippel_workspace_bytes.restype = sz
+    L.zippel_workspace_bytes.argtypes = [vp, i32, i32, i32]
+    L.zippel_host_workspace_bytes.restype = sz
+    L.zippel_host_workspace_bytes.argtypes = [vp, i32, i32, i32]
+    L.zippel_eval_nodes.argtypes = [vp, i64, i32, vp, u64, vp, vp]
+    L.vandermonde_solve_batch.argtypes = [vp, vp, i32, vp, i32, i32, u64, vp, vp, vp, sz, vp]
+    L.newton_interp_batch.argtypes = [vp, i32, vp, i64, i64, u64, i32, vp, vp, vp, sz, vp]
+    L.zippel_lift_step.argtypes = [vp, vp, i32, i32, vp, vp, i32, i32, vp, u64, i32, vp, vp, vp, vp, sz, vp]
+    L.zippel_lift_step_host.argtypes = [vp, vp, i32, i32, vp, vp, i32, i32, vp, u64, i32, vp, vp, vp, sz, vp]
+    L.zippel_power_sums.argtypes = [vp, vp, i32, vp, i32, i32, u64, vp, vp, sz, vp]
+    L.balanced_zippel_lift_step.argtypes = [C.POINTER(_Part), C.POINTER(_Part), i32, i32, vp, vp, i32, i32,
+                                            u64, i32, vp, vp, sz, vp]
+    L.zippel_profile_events.argtypes = [i32, vp, vp]
+    L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    L.zippel_extend_skeleton.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp, C.c_size_t, vp]
+    L.crt_rational_reconstruct_batch.argtypes = [vp, vp, C.c_int64, u64, u64, vp, vp, vp, vp]
+    L.zippel_launch_count.restype = C.c_ulonglong
+    L.zippel_launch_count.argtypes = []
+    L.zippel_set_tuning.argtypes = [i32, i64]
+    L.zippel_shutdown.argtypes = []
+    return L
+
+
 def lib() -> C.CDLL:
     """Load libzippel.so (building it with nvcc if it is missing or stale).  Fails loudly."""
     global _lib
@@ -52,32 +84,15 @@ def lib() -> C.CDLL:
         path = _build.SO_PATH
         if not os.path.exists(path) or _build.is_stale():
             path = _build.build()
-        L = C.CDLL(path)
-        vp, i32, i64, u64, sz = C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.c_size_t
-        L.zippel_strerror.restype = C.c_char_p
-        L.zippel_strerror.argtypes = [i32]
-        L.zippel_workspace_bytes.restype = sz
-        L.zippel_workspace_bytes.argtypes = [vp, i32, i32, i32]
-        L.zippel_host_workspace_bytes.restype = sz
-        L.zippel_host_workspace_bytes.argtypes = [vp, i32, i32, i32]
-        L.zippel_eval_nodes.argtypes = [vp, i64, i32, vp, u64, vp, vp]
-        L.vandermonde_solve_batch.argtypes = [vp, vp, i32, vp, i32, i32, u64, vp, vp, vp, sz, vp]
-        L.newton_interp_batch.argtypes = [vp, i32, vp, i64, i64, u64, i32, vp, vp, vp, sz, vp]
-        L.zippel_lift_step.argtypes = [vp, vp, i32, i32, vp, vp, i32, i32, vp, u64, i32, vp, vp, vp, vp, sz, vp]
-        L.zippel_lift_step_host.argtypes = [vp, vp, i32, i32, vp, vp, i32, i32, vp, u64, i32, vp, vp, vp, sz, vp]
-        L.zippel_power_sums.argtypes = [vp, vp, i32, vp, i32, i32, u64, vp, vp, sz, vp]
-        L.balanced_zippel_lift_step.argtypes = [C.POINTER(_Part), C.POINTER(_Part), i32, i32, vp, vp, i32, i32,
-                                                u64, i32, vp, vp, sz, vp]
-        L.zippel_modarith_selftest.argtypes = [i32, vp, vp, i64, u64, vp, vp]
-        L.zippel_profile_events.argtypes = [i32, vp, vp]
-        L.zippel_ubench.argtypes = [i32, i32, i32, u64, vp, C.POINTER(C.c_double), vp]
-        L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
-        L.zippel_extend_skeleton.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp, C.c_size_t, vp]
-        L.crt_rational_reconstruct_batch.argtypes = [vp, vp, C.c_int64, u64, u64, vp, vp, vp, vp]
-        L.zippel_launch_count.restype = C.c_ulonglong
-        L.zippel_launch_count.argtypes = []
-        _lib = L
+        _lib = declare(C.CDLL(path))
     return _lib
+
+
+def use_library(L: C.CDLL):
+    """Route every binding of this module through an already loaded library (testhooks.routed(): the test build
+    holds the same entry points plus the hooks, with its own process-wide state)."""
+    global _lib
+    _lib = L
 
 
 def _need_cuda():
@@ -93,6 +108,13 @@ def _check(rc: int, what: str):
 def _stream(stream) -> int:
     s = torch.cuda.current_stream() if stream is None else stream
     return int(s.cuda_stream)
+
+
+def _on(stream):
+    """Context in which the bindings allocate their temporaries and outputs: the stream the kernels are enqueued
+    on, so that the caching allocator orders every reuse of those blocks after the kernels (a tensor allocated
+    on another stream could be handed out again while they are still in flight)."""
+    return contextlib.nullcontext() if stream is None else torch.cuda.stream(stream)
 
 
 def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
@@ -143,12 +165,13 @@ def zippel_eval_nodes(exps: torch.Tensor, anchors: torch.Tensor, p: int, out: Op
                       stream=None) -> torch.Tensor:
     """(a1) nodes m_i = prod_j y_j^{e_ij}; exps int16-view [T_tot, nv], anchors [nv]."""
     _need_cuda()
-    T_tot, nv = exps.shape
-    if out is None:
-        out = torch.empty(T_tot, dtype=torch.int64, device=exps.device)
-    _check(lib().zippel_eval_nodes(_ptr(exps), T_tot, nv, _ptr(anchors), p, _ptr(out), _stream(stream)),
-           "zippel_eval_nodes")
-    return out
+    with _on(stream):
+        T_tot, nv = exps.shape
+        if out is None:
+            out = torch.empty(T_tot, dtype=torch.int64, device=exps.device)
+        _check(lib().zippel_eval_nodes(_ptr(exps), T_tot, nv, _ptr(anchors), p, _ptr(out), _stream(stream)),
+               "zippel_eval_nodes")
+        return out
 
 
 def vandermonde_solve_batch(nodes: torch.Tensor, offsets, vals: torch.Tensor, p: int, s0: int = 0,
@@ -156,18 +179,19 @@ def vandermonde_solve_batch(nodes: torch.Tensor, offsets, vals: torch.Tensor, p:
                             workspace: Optional[torch.Tensor] = None, stream=None):
     """(a2)-(a4); vals [B, T_tot] -> (coefs [B, T_tot], status [F])."""
     _need_cuda()
-    o = _offs(offsets)
-    F, B = len(o) - 1, vals.shape[0]
-    if out is None:
-        out = torch.empty_like(vals)
-    if status is None:
-        status = torch.empty(F, dtype=torch.int32, device=vals.device)
-    if workspace is None:
-        workspace = alloc_workspace(o, B)
-    _check(lib().vandermonde_solve_batch(_ptr(nodes), o.ctypes.data, F, _ptr(vals), B, s0, p, _ptr(out),
-                                         _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)),
-           "vandermonde_solve_batch")
-    return out, status
+    with _on(stream):
+        o = _offs(offsets)
+        F, B = len(o) - 1, vals.shape[0]
+        if out is None:
+            out = torch.empty_like(vals)
+        if status is None:
+            status = torch.empty(F, dtype=torch.int32, device=vals.device)
+        if workspace is None:
+            workspace = alloc_workspace(o, B)
+        _check(lib().vandermonde_solve_batch(_ptr(nodes), o.ctypes.data, F, _ptr(vals), B, s0, p, _ptr(out),
+                                             _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)),
+               "vandermonde_solve_batch")
+        return out, status
 
 
 def newton_interp_batch(samples: torch.Tensor, vals: torch.Tensor, p: int, basis: int = 0,
@@ -175,19 +199,20 @@ def newton_interp_batch(samples: torch.Tensor, vals: torch.Tensor, p: int, basis
                         workspace: Optional[torch.Tensor] = None, stream=None):
     """(a5); vals [B, n] (row j = values at c_j) -> (out [B, n], status [1]).  out may alias vals."""
     _need_cuda()
-    B, n = vals.shape
-    ld = vals.stride(0) if B > 1 else n
-    assert vals.stride(1) == 1
-    if out is None:
-        out = torch.empty_like(vals)
-    if status is None:
-        status = torch.empty(1, dtype=torch.int32, device=vals.device)
-    if workspace is None:
-        workspace = alloc_workspace([0, 1], B)
-    _check(lib().newton_interp_batch(samples.data_ptr(), B, vals.data_ptr(), n, ld, p, basis, out.data_ptr(),
-                                     _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)),
-           "newton_interp_batch")
-    return out, status
+    with _on(stream):
+        B, n = vals.shape
+        ld = vals.stride(0) if B > 1 else n
+        assert vals.stride(1) == 1
+        if out is None:
+            out = torch.empty_like(vals)
+        if status is None:
+            status = torch.empty(1, dtype=torch.int32, device=vals.device)
+        if workspace is None:
+            workspace = alloc_workspace([0, 1], B)
+        _check(lib().newton_interp_batch(samples.data_ptr(), B, vals.data_ptr(), n, ld, p, basis, out.data_ptr(),
+                                         _ptr(status), _ptr(workspace), workspace.numel(), _stream(stream)),
+               "newton_interp_batch")
+        return out, status
 
 
 def zippel_lift_step(exps: torch.Tensor, offsets, anchors: torch.Tensor, samples: torch.Tensor,
@@ -197,37 +222,39 @@ def zippel_lift_step(exps: torch.Tensor, offsets, anchors: torch.Tensor, samples
                      stream=None):
     """(a1)-(a5): one lifting step; returns (out [B, T_tot], status [F])."""
     _need_cuda()
-    o = _offs(offsets)
-    F, B = len(o) - 1, vals.shape[0]
-    nv = exps.shape[1]
-    if out is None:
-        out = torch.empty_like(vals)
-    if status is None:
-        status = torch.empty(F, dtype=torch.int32, device=vals.device)
-    if workspace is None:
-        workspace = alloc_workspace(o, B)
-    _check(lib().zippel_lift_step(_ptr(exps), o.ctypes.data, F, nv, _ptr(anchors), _ptr(samples), B, s0,
-                                  _ptr(vals), p, basis, _ptr(out), _ptr(nodes_out), _ptr(status),
-                                  _ptr(workspace), workspace.numel(), _stream(stream)),
-           "zippel_lift_step")
-    return out, status
+    with _on(stream):
+        o = _offs(offsets)
+        F, B = len(o) - 1, vals.shape[0]
+        nv = exps.shape[1]
+        if out is None:
+            out = torch.empty_like(vals)
+        if status is None:
+            status = torch.empty(F, dtype=torch.int32, device=vals.device)
+        if workspace is None:
+            workspace = alloc_workspace(o, B)
+        _check(lib().zippel_lift_step(_ptr(exps), o.ctypes.data, F, nv, _ptr(anchors), _ptr(samples), B, s0,
+                                      _ptr(vals), p, basis, _ptr(out), _ptr(nodes_out), _ptr(status),
+                                      _ptr(workspace), workspace.numel(), _stream(stream)),
+               "zippel_lift_step")
+        return out, status
 
 
 def zippel_power_sums(nodes: torch.Tensor, offsets, coef: torch.Tensor, p: int, s0: int = 0,
                       out: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None, stream=None):
     """(a6) forward evaluation R_{b,s} = sum_i a_{b,i} m_i^(s+s0); coef [B, T_tot] -> out [B, T_tot]."""
     _need_cuda()
-    o = _offs(offsets)
-    if coef.dim() == 1:
-        coef = coef[None, :]
-    B = coef.shape[0]
-    if out is None:
-        out = torch.empty_like(coef)
-    if workspace is None:
-        workspace = alloc_workspace(o, B)
-    _check(lib().zippel_power_sums(_ptr(nodes), o.ctypes.data, len(o) - 1, _ptr(coef), B, s0, p, _ptr(out),
-                                   _ptr(workspace), workspace.numel(), _stream(stream)), "zippel_power_sums")
-    return out
+    with _on(stream):
+        o = _offs(offsets)
+        if coef.dim() == 1:
+            coef = coef[None, :]
+        B = coef.shape[0]
+        if out is None:
+            out = torch.empty_like(coef)
+        if workspace is None:
+            workspace = alloc_workspace(o, B)
+        _check(lib().zippel_power_sums(_ptr(nodes), o.ctypes.data, len(o) - 1, _ptr(coef), B, s0, p, _ptr(out),
+                                       _ptr(workspace), workspace.numel(), _stream(stream)), "zippel_power_sums")
+        return out
 
 
 def balanced_zippel_lift_step(num: dict, den: dict, anchors: torch.Tensor, samples: torch.Tensor, p: int,
@@ -236,36 +263,27 @@ def balanced_zippel_lift_step(num: dict, den: dict, anchors: torch.Tensor, sampl
     """(a6) balanced step; num / den: dicts with device tensors exps, skel, uvals, host offsets and an
     optional out.  Returns (out_num, out_den, status [2F])."""
     _need_cuda()
-    keep, parts = [], []
-    F = len(num["offsets"]) - 1
-    nv = num["exps"].shape[1]
-    B = num["uvals"].shape[0]
-    for d in (num, den):
-        o = _offs(d["offsets"])
-        out = d.get("out")
-        if out is None:
-            out = torch.empty_like(d["uvals"])
-        keep.append((o, out))
-        parts.append(_Part(_ptr(d["exps"]), o.ctypes.data, _ptr(d["skel"]), _ptr(d["uvals"]), _ptr(out)))
-    if status is None:
-        status = torch.empty(2 * F, dtype=torch.int32, device=anchors.device)
-    if workspace is None:
-        big = max((num, den), key=lambda d: int(_offs(d["offsets"])[-1]))
-        workspace = alloc_workspace(big["offsets"], B, WS_BALANCED)
-    _check(lib().balanced_zippel_lift_step(C.byref(parts[0]), C.byref(parts[1]), F, nv, _ptr(anchors),
-                                           _ptr(samples), B, s0, p, basis, _ptr(status), _ptr(workspace),
-                                           workspace.numel(), _stream(stream)), "balanced_zippel_lift_step")
-    return keep[0][1], keep[1][1], status
-
-
-def zippel_modarith_selftest(op: int, a: torch.Tensor, b: Optional[torch.Tensor], p: int, stream=None):
-    """(a0) out[i] = op(a[i], b[i]) mod p on the device (see include/zippel.h)."""
-    _need_cuda()
-    n = a.numel()
-    out = torch.empty(1 if op == 5 else n, dtype=torch.int64, device=a.device)
-    _check(lib().zippel_modarith_selftest(op, _ptr(a), _ptr(b), n, p, _ptr(out), _stream(stream)),
-           "zippel_modarith_selftest")
-    return out
+    with _on(stream):
+        keep, parts = [], []
+        F = len(num["offsets"]) - 1
+        nv = num["exps"].shape[1]
+        B = num["uvals"].shape[0]
+        for d in (num, den):
+            o = _offs(d["offsets"])
+            out = d.get("out")
+            if out is None:
+                out = torch.empty_like(d["uvals"])
+            keep.append((o, out))
+            parts.append(_Part(_ptr(d["exps"]), o.ctypes.data, _ptr(d["skel"]), _ptr(d["uvals"]), _ptr(out)))
+        if status is None:
+            status = torch.empty(2 * F, dtype=torch.int32, device=anchors.device)
+        if workspace is None:
+            big = max((num, den), key=lambda d: int(_offs(d["offsets"])[-1]))
+            workspace = alloc_workspace(big["offsets"], B, WS_BALANCED)
+        _check(lib().balanced_zippel_lift_step(C.byref(parts[0]), C.byref(parts[1]), F, nv, _ptr(anchors),
+                                               _ptr(samples), B, s0, p, basis, _ptr(status), _ptr(workspace),
+                                               workspace.numel(), _stream(stream)), "balanced_zippel_lift_step")
+        return keep[0][1], keep[1][1], status
 
 
 # ---- host-buffer entry (the e2e path: copies inside the call) -----------------------------------------
@@ -314,12 +332,13 @@ def zippel_launch_count() -> int:
     return int(lib().zippel_launch_count())
 
 
-def zippel_ubench(kind: int, iters: int, blocks: int, p: int, out: torch.Tensor, stream=None) -> float:
-    """Enqueue one micro-benchmark launch (csrc/ubench.cuh); returns the lane-statements it executes."""
-    _need_cuda()
-    n = C.c_double(0.0)
-    _check(lib().zippel_ubench(kind, iters, blocks, p, _ptr(out), C.byref(n), _stream(stream)), "zippel_ubench")
-    return n.value
+def zippel_set_tuning(key: int, value: int):
+    """Process-wide tuning knob (TUNE_SUBQ_MIN_T: shortest skeleton that takes the sub-quadratic route)."""
+    _check(lib().zippel_set_tuning(key, value), "zippel_set_tuning")
+
+
+def zippel_shutdown():
+    _check(lib().zippel_shutdown(), "zippel_shutdown")
 
 
 ST_THIELE_DEGENERATE = 20
@@ -329,20 +348,21 @@ def thiele_reconstruct_batch(points: torch.Tensor, vals: torch.Tensor, p: int, w
                              workspace: Optional[torch.Tensor] = None, stream=None):
     """(f2) eq. (2): vals [T, n] -> (num [T, n], den [T, n], degs [2, n] int32, cf [T, n] or None, status [n])."""
     _need_cuda()
-    T, n = vals.shape
-    assert vals.stride(1) == 1
-    ld = vals.stride(0) if T > 1 else n
-    mk = lambda: torch.empty((T, ld), dtype=vals.dtype, device=vals.device)  # outputs share the input's leading dimension
-    num, den = mk(), mk()
-    cf = mk() if want_cf else None
-    degs = torch.empty((2, ld), dtype=torch.int32, device=vals.device)
-    status = torch.empty(n, dtype=torch.int32, device=vals.device)
-    if workspace is None:
-        workspace = alloc_workspace([0, 1], T)
-    _check(lib().thiele_reconstruct_batch(points.data_ptr(), T, vals.data_ptr(), n, ld, p, num.data_ptr(), den.data_ptr(),
-                                          degs.data_ptr(), _ptr(cf), status.data_ptr(), _ptr(workspace),
-                                          workspace.numel(), _stream(stream)), "thiele_reconstruct_batch")
-    return num[:, :n], den[:, :n], degs[:, :n], None if cf is None else cf[:, :n], status
+    with _on(stream):
+        T, n = vals.shape
+        assert vals.stride(1) == 1
+        ld = vals.stride(0) if T > 1 else n
+        mk = lambda: torch.empty((T, ld), dtype=vals.dtype, device=vals.device)  # outputs share the input's leading dimension
+        num, den = mk(), mk()
+        cf = mk() if want_cf else None
+        degs = torch.empty((2, ld), dtype=torch.int32, device=vals.device)
+        status = torch.empty(n, dtype=torch.int32, device=vals.device)
+        if workspace is None:
+            workspace = alloc_workspace([0, 1], T)
+        _check(lib().thiele_reconstruct_batch(points.data_ptr(), T, vals.data_ptr(), n, ld, p, num.data_ptr(), den.data_ptr(),
+                                              degs.data_ptr(), _ptr(cf), status.data_ptr(), _ptr(workspace),
+                                              workspace.numel(), _stream(stream)), "thiele_reconstruct_batch")
+        return num[:, :n], den[:, :n], degs[:, :n], None if cf is None else cf[:, :n], status
 
 
 def zippel_extend_skeleton(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: int, cap: Optional[int] = None,
@@ -350,19 +370,20 @@ def zippel_extend_skeleton(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: 
     """(f1): coefs [B, T_tot] monomial in x_k -> (new_exps [cap, nv+1] int16, new_coefs [cap], new_offsets [F+1]
     int64 on the device, degs [F] int32).  The caller trims to new_offsets[-1] after a synchronisation."""
     _need_cuda()
-    o = _offs(offsets)
-    F, (B, T_tot), nv = len(o) - 1, coefs.shape, exps.shape[1]
-    cap = B * T_tot if cap is None else cap
-    ne = torch.empty((max(cap, 1), nv + 1), dtype=torch.int16, device=coefs.device)
-    nc = torch.empty(max(cap, 1), dtype=torch.int64, device=coefs.device)
-    no = torch.empty(F + 1, dtype=torch.int64, device=coefs.device)
-    degs = torch.empty(F, dtype=torch.int32, device=coefs.device)
-    if workspace is None:
-        workspace = alloc_workspace(o, B)
-    _check(lib().zippel_extend_skeleton(_ptr(exps), o.ctypes.data, F, nv, _ptr(coefs), B, p, _ptr(ne), _ptr(nc), cap,
-                                        _ptr(no), _ptr(degs), _ptr(workspace), workspace.numel(), _stream(stream)),
-           "zippel_extend_skeleton")
-    return ne, nc, no, degs
+    with _on(stream):
+        o = _offs(offsets)
+        F, (B, T_tot), nv = len(o) - 1, coefs.shape, exps.shape[1]
+        cap = B * T_tot if cap is None else cap
+        ne = torch.empty((max(cap, 1), nv + 1), dtype=torch.int16, device=coefs.device)
+        nc = torch.empty(max(cap, 1), dtype=torch.int64, device=coefs.device)
+        no = torch.empty(F + 1, dtype=torch.int64, device=coefs.device)
+        degs = torch.empty(F, dtype=torch.int32, device=coefs.device)
+        if workspace is None:
+            workspace = alloc_workspace(o, B)
+        _check(lib().zippel_extend_skeleton(_ptr(exps), o.ctypes.data, F, nv, _ptr(coefs), B, p, _ptr(ne), _ptr(nc), cap,
+                                            _ptr(no), _ptr(degs), _ptr(workspace), workspace.numel(), _stream(stream)),
+               "zippel_extend_skeleton")
+        return ne, nc, no, degs
 
 
 ST_NO_RATIONAL = 21
@@ -371,9 +392,10 @@ ST_NO_RATIONAL = 21
 def crt_rational_reconstruct_batch(r1: torch.Tensor, r2: torch.Tensor, p1: int, p2: int, stream=None):
     """(f4): images mod p1 and mod p2 [n] -> (num int64 [n] signed, den int64 [n] > 0, status int32 [n])."""
     _need_cuda()
-    n = r1.numel()
-    num, den = torch.empty(n, dtype=torch.int64, device=r1.device), torch.empty(n, dtype=torch.int64, device=r1.device)
-    status = torch.empty(n, dtype=torch.int32, device=r1.device)
-    _check(lib().crt_rational_reconstruct_batch(r1.data_ptr(), r2.data_ptr(), n, p1, p2, num.data_ptr(), den.data_ptr(),
-                                                status.data_ptr(), _stream(stream)), "crt_rational_reconstruct_batch")
-    return num, den, status
+    with _on(stream):
+        n = r1.numel()
+        num, den = torch.empty(n, dtype=torch.int64, device=r1.device), torch.empty(n, dtype=torch.int64, device=r1.device)
+        status = torch.empty(n, dtype=torch.int32, device=r1.device)
+        _check(lib().crt_rational_reconstruct_batch(r1.data_ptr(), r2.data_ptr(), n, p1, p2, num.data_ptr(), den.data_ptr(),
+                                                    status.data_ptr(), _stream(stream)), "crt_rational_reconstruct_batch")
+        return num, den, status

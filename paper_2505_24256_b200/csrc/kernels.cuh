@@ -184,29 +184,25 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 // (a3)+(a4) K3 node_solve: the hot loop (PAPER.md L189-197 ZippelMultiplePrime(), L203-213).
 // One lane per node i of one function; the CTA streams tiles of the table above and of the NB right-hand
 // sides through shared memory (every lane needs the same M_l, v_{b,l}: warp-uniform broadcast reads).
-// Per lane, stages l = t-1 .. 0 with q = q_l (q_{t-1} = 1) and d:
-//     acc_b += q_l * v_{b,l}                       NB deferred MACs (L194-195 "vector of powers" x "values", L205-209)
-//     q_{l-1} = M_l + m q_l ;  d <- D_l + m d   (l >= 1)   2 Horner steps (L193: synthetic division; Horner of M')
-// then  c_{b,i} = acc_b / d  [ / m if s0 = 1 ]   (L196).  d = M'(m_i) = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15):
-// the paper's "polynomial value computed via Horner's method"; running Horner on M' instead of on the
-// quotient gives the same number and keeps the two chains independent.
-// Stages are taken in pairs (2j+1, 2j), j = J-1 .. 0, J = t/2 + 1, starting from q = d = 0 at a stage >= t
+// Per lane, stages l = t-1 .. 0 with q = q_l (q_{t-1} = 1):
+//     acc_b += q_l * v_{b,l}              NB deferred MACs (L194-195 "vector of powers" x "values", L205-209)
+//     q_{l-1} = M_l + m q_l   (l >= 1)    one Horner step (L193: synthetic division)
+// then  c_{b,i} = acc_b * scale_i,  scale_i = 1 / (M'(m_i) [m_i if s0 = 1])  (L196) from k_node_den below:
+// M'(m_i) = Q_i(m_i) = prod_{j != i}(m_i - m_j) (G15) is the paper's "polynomial value computed via Horner's
+// method"; it is a polynomial evaluation and is cheaper by blocked deferred MACs in its own launch than as a
+// second Horner chain in this loop (which is what the first measured profiles of round 1 show).
+// Stages are taken in pairs (2j+1, 2j), j = J-1 .. 0, J = t/2 + 1, starting from q = 0 at a stage >= t
 // (records beyond t and values v_{b,l}, l >= t, are zero; record t carries M_t = 1): the two MACs of a
 // pair go into the accumulator together (acc_mac2).
-// All values are plain residues; q and d stay lazy in [0, 2p) (horner_step); nothing of length t is
-// stored per lane (reading G7).
-// Template NB = right-hand sides handled per pass; FIRST = this pass also runs the d chain and writes scale.
-// Since k_node_den (below) the library launches only the <NB, false> instances: den_i = M'(m_i) is a polynomial
-// evaluation and is cheaper by blocked deferred MACs in its own launch than as a second Horner chain here; the
-// FIRST code path stays as the literal form of PAPER.md L193-196 (and is what the first measured profiles show).
+// All values are plain residues; q stays lazy in [0, 2p) (horner_step); nothing of length t is stored per
+// lane (reading G7).  Template NB = right-hand sides handled per pass.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K3_THREADS 128
 #define ZP_K3_PAIRS 32
 // Orientation of the 16-byte value record per template instance.  Both orders put the two limbs of one operand
 // into registers of the same parity; which of the two ptxas's register allocation serves with fewer bank
 // conflicts differs from instance to instance, so it is read off the SASS (share of accumulating IMAD.WIDE whose
-// multiplicands have equal parity; profiles/r01_final.md) and tabulated for the <NB, false> instances: bit NB = 1 ->
-// odd stage first.
+// multiplicands have equal parity; profiles/r02_k3_orient.md) and tabulated per instance: bit NB = 1 -> odd stage first.
 #ifdef ZP_K3_FORCE_ORIENT
 #define ZP_K3_ORIENT(NB) (ZP_K3_FORCE_ORIENT)
 #else
@@ -231,11 +227,11 @@ ZP_DEV void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memor
 template <int N>
 ZP_DEV void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int NB, bool FIRST>
+template <int NB>
 __global__ void __launch_bounds__(ZP_K3_THREADS)
 k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ tab, const int64_t* __restrict__ offsets,
              int F, const uint64_t* __restrict__ vals, int64_t T_tot, int b0, int s0, ZpMod k,
-             uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
+             const uint64_t* __restrict__ scale, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
   // two buffers: the tile after the current one is in flight (cp.async) while the current one is consumed
   __shared__ __align__(16) ulonglong4 sT[2][2 * ZP_K3_PAIRS];      // record of stage l = 2 j0 + x
   __shared__ __align__(16) ulonglong2 sV[2][ZP_K3_PAIRS * NB];     // [pair][b]: 16-byte record of limbs, see issue_tile
@@ -248,9 +244,8 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
     const int i = i0 + threadIdx.x;
     const bool live = i < t;
     const uint64_t m = live ? zp_canon(nodes[off + i], k.p) : 0;
-    const uint64_t mm = to_mont(m, k);
-    const uint64_t mp = shoup_companion(mm, k);
-    uint64_t q = 0, d = 0;
+    const uint64_t mp = shoup_companion(to_mont(m, k), k);
+    uint64_t q = 0;
     Acc acc[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) acc_zero(acc[b]);
@@ -299,7 +294,6 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         const ulonglong4 r1 = cT[2 * jj + 1];
         const uint64_t qa = q;
         const uint64_t qb = horner_step(qa, m, mp, r1.x, r1.y, k);
-        if (FIRST) d = horner_step(d, m, mp, r1.z, r1.w, k);
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
           const uint4 w = reinterpret_cast<const uint4*>(cV)[jj * NB + b];
@@ -311,22 +305,12 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
         if (j0 + jj > 0) {
           const ulonglong4 r0 = cT[2 * jj];
           q = horner_step(qb, m, mp, r0.x, r0.y, k);
-          if (FIRST) d = horner_step(d, m, mp, r0.z, r0.w, k);
         }
       }
       __syncthreads();  // this buffer is refilled by the next iteration's prefetch
     }
     if (live) {
-      uint64_t sc;
-      if (FIRST) {
-        const uint64_t dm = to_mont(lazy_canon(d, k.p), k);
-        const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
-        if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-        sc = mont_mul(mont_inv(dd, k), k.c224, k);  // plain d^-1 * 2^224: acc_redc160 (x 2^-160) and mont_mul (x 2^-64) undo it
-        if (scale) scale[off + i] = sc;
-      } else {
-        sc = scale[off + i];
-      }
+      const uint64_t sc = scale[off + i];  // plain d^-1 * 2^224: acc_redc160 (x 2^-160) and mont_mul (x 2^-64) undo it
 #pragma unroll
       for (int b = 0; b < NB; ++b)
         coefs[(int64_t)(b0 + b) * T_tot + off + i] = mont_mul(acc_redc160(acc[b], k), sc, k);
@@ -1114,37 +1098,5 @@ k_crt_rational(const uint64_t* __restrict__ r1, const uint64_t* __restrict__ r2,
     num[i] = ok ? (int64_t)a : 0;
     den[i] = ok ? (int64_t)b : 0;
     status[i] = ok ? 0 : ZP_ST_NO_RATIONAL;
-  }
-}
-
-// (a0) self-test kernel for the substrate
-__global__ void k_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, ZpMod k, uint64_t* out) {
-  if (op == 5) {  // deferred dot through the wide accumulator, one CTA
-    __shared__ uint64_t part[256];
-    Acc acc;
-    acc_zero(acc);
-    for (int64_t i = threadIdx.x; i < n; i += blockDim.x) acc_mac(acc, to_mont(zp_canon(a[i], k.p), k), b[i]);
-    part[threadIdx.x] = mont_mul(acc_redc160(acc, k), k.c160, k);  // mont * plain -> plain
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      uint64_t r = 0;
-      for (int x = 0; x < (int)blockDim.x; ++x) r = mod_add(r, part[x], k.p);
-      out[0] = r;
-    }
-    return;
-  }
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    const uint64_t x = zp_canon(a[i], k.p), y = b ? b[i] : 0;
-    uint64_t r = 0;
-    if (op == 0) r = from_mont(mont_mul(to_mont(x, k), to_mont(zp_canon(y, k.p), k), k), k);
-    if (op == 1) r = mod_add(x, zp_canon(y, k.p), k.p);
-    if (op == 2) r = mod_sub(x, zp_canon(y, k.p), k.p);
-    if (op == 3) r = from_mont(mont_pow(to_mont(x, k), y, k), k);
-    if (op == 4) r = from_mont(mont_inv(to_mont(x, k), k), k);
-    if (op == 6) {  // Horner step on a LAZY x (any 64-bit value): (y x + a[(i+1) % n]) mod p
-      const uint64_t m = zp_canon(y, k.p), ad = zp_canon(a[(i + 1) % n], k.p);
-      r = lazy_canon(horner_step(a[i], m, shoup_companion(to_mont(m, k), k), ad, shoup_companion(to_mont(ad, k), k), k), k.p);
-    }
-    out[i] = r;
   }
 }

@@ -1,0 +1,295 @@
+// subq.cuh -- sub-quadratic transposed Vandermonde solve for long skeletons (PAPER.md L37, L250-254,
+// Table 3: 125k .. 4.8m monomials).  Same answer as the quadratic route of section 2.2 (the solution is unique,
+// reading G21); the operations are reorganised around products of polynomials (ntt.cuh):
+//
+//   sum_s v_s z^-(s+1) = sum_i c_i / (z - m_i) = N(z) / M(z),  N(m_i) = c_i M'(m_i)   (G15),
+//
+// so the right-hand side v IS the tail of N / M at infinity.  For a block S of nodes with master polynomial M_S write
+// tail_S(P) = the first |S| coefficients of z^-1, z^-2, .. in P / M_S.  Then
+//   (up)    M_{L u R} = M_L M_R                                        -- product tree above the 1024-node leaves
+//   (down)  tail_L(P)_k = sum_j (M_R)_j tail_{L u R}(P)_{k+j}          -- a correlation with the SIBLING's polynomial
+//           (because P / M_L = M_R * P / M_{L u R}, and the polynomial part contributes nothing to the tail)
+//   (leaf)  sum_l q_{i,l} tail_S(P)_l = (P mod M_S)(m_i)               -- the synthetic-division dot of (a3), unscaled
+// For P = N the root tail is v itself; for P = M' it is the power sums of the nodes, rev(M') / rev(M) mod x^t, which
+// needs one power-series inverse of rev(M) (Newton iteration).  Finally c_i = N(m_i) / M'(m_i) [/ m_i if s0 = 1].
+// Every product is a cyclic convolution of length 2a at block size a (ntt.cuh); the leaf step runs the existing
+// k_node_solve on the leaves as if they were functions, with B + 1 right-hand sides (the values and the M' tail).
+//
+// Storage: a monic polynomial of degree n is kept WITHOUT its leading 1, as n Montgomery coefficients in the slots of
+// the nodes it covers (as in k_tree_leaf); level l holds the polynomials of the blocks of LEAF 2^l nodes.  Tails are
+// plain residues in the same slots.  All indices below are local to a "run" of consecutive long functions.
+#pragma once
+#include "ntt.cuh"
+
+struct SqTask {
+  int64_t base;  // first slot of the left block
+  int32_t a;     // left block length (pairs: the level's block size; copies: the length to copy)
+  int32_t b;     // right block length (>= 1); 0 marks a copy task
+};
+
+// ---- (up) ---------------------------------------------------------------------------------------------------------------
+// X[j][2t][i] = A'_i (i < a), X[j][2t+1][i] = B'_i (i < b), zero-padded to n = 2a.  The residues mod p are < 2^63 < 4q:
+// valid lazy inputs for all three primes as they are.
+__global__ void __launch_bounds__(256)
+k_sq_up_prep(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn, uint64_t* __restrict__ X,
+             int64_t EX) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t seg = e >> logn, i = e & (n - 1);
+    const SqTask t = tasks[seg >> 1];
+    uint64_t v = 0;
+    if (seg & 1) {
+      if (i < t.b) v = lev[t.base + t.a + i];
+    } else {
+      if (i < t.a) v = lev[t.base + i];
+    }
+    X[e] = v;
+    X[EX + e] = v;
+    X[2 * EX + e] = v;
+  }
+}
+// C' = A' B' + z^a B' + z^b A'  (Montgomery in, Montgomery out: co carries K = 2^-64)
+__global__ void __launch_bounds__(256)
+k_sq_up_fin(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn,
+            const uint64_t* __restrict__ O, int64_t EO, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ nxt) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t c = e & (n - 1);
+    const SqTask t = tasks[e >> logn];
+    if (c >= t.a + t.b) continue;
+    uint64_t r = ntt_crt(O[e], O[EO + e], O[2 * EO + e], cx, co, kp);
+    if (c >= t.a) r = mod_add(r, lev[t.base + t.a + (c - t.a)], kp.p);
+    if (c >= t.b) r = mod_add(r, lev[t.base + (c - t.b)], kp.p);
+    nxt[t.base + c] = r;
+  }
+}
+// blocks without a sibling pass through: dst[v ld + slot] = src[v ld + slot]
+__global__ void __launch_bounds__(256)
+k_sq_copy(const SqTask* __restrict__ tasks, int ntasks, const uint64_t* __restrict__ src, uint64_t* __restrict__ dst, int V,
+          int64_t ld) {
+  for (int x = blockIdx.y; x < ntasks * V; x += gridDim.y) {
+    const SqTask t = tasks[x % ntasks];
+    const int64_t o = (int64_t)(x / ntasks) * ld + t.base;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < t.a; i += gridDim.x * blockDim.x) dst[o + i] = src[o + i];
+  }
+}
+
+// ---- (down) -------------------------------------------------------------------------------------------------------------
+// X[j][2t][i] = A'_{a-1-i}, X[j][2t+1][i] = B'_{b-1-i}  (the reversed children), n = 2a
+__global__ void __launch_bounds__(256)
+k_sq_down_prepx(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn,
+                uint64_t* __restrict__ X, int64_t EX) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t seg = e >> logn, i = e & (n - 1);
+    const SqTask t = tasks[seg >> 1];
+    uint64_t v = 0;
+    if (seg & 1) {
+      if (i < t.b) v = lev[t.base + t.a + t.b - 1 - i];
+    } else {
+      if (i < t.a) v = lev[t.base + t.a - 1 - i];
+    }
+    X[e] = v;
+    X[EX + e] = v;
+    X[2 * EX + e] = v;
+  }
+}
+// Y[j][v P + t][i] = tail_{L u R}(P_v)_i, i < a + b
+__global__ void __launch_bounds__(256)
+k_sq_down_prepy(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
+                uint64_t* __restrict__ Y, int64_t EY) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EY; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t seg = e >> logn, i = e & (n - 1);
+    const int64_t v = seg / P;
+    const SqTask t = tasks[seg - v * P];
+    const uint64_t x = (i < t.a + t.b) ? cur[v * ld + t.base + i] : 0;
+    Y[e] = x;
+    Y[EY + e] = x;
+    Y[2 * EY + e] = x;
+  }
+}
+// O segment o = (v P + t) 2 + side.  side 0: tail_L_k = c_{k+b} + (rev(B') * c)_{k+b-1}, k < a;
+//                                    side 1: tail_R_k = c_{k+a} + (rev(A') * c)_{k+a-1}, k < b.
+__global__ void __launch_bounds__(256)
+k_sq_down_fin(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
+              const uint64_t* __restrict__ O, int64_t EO, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ nxt) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t o = e >> logn, k = e & (n - 1);
+    const int side = (int)(o & 1);
+    const int64_t vt = o >> 1, v = vt / P;
+    const SqTask t = tasks[vt - v * P];
+    const int64_t len = side ? t.b : t.a, sh = side ? t.a : t.b;  // own length, sibling's length
+    if (k >= len) continue;
+    const int64_t src = e - k + (k + sh - 1);
+    const uint64_t r = ntt_crt(O[src], O[EO + src], O[2 * EO + src], cx, co, kp);
+    const uint64_t* c = cur + v * ld + t.base;
+    nxt[v * ld + t.base + (side ? t.a : 0) + k] = mod_add(r, c[k + sh], kp.p);
+  }
+}
+
+// ---- power-series inverse of f = rev(M):  f_0 = 1, f_i = M_{t-i} (i <= t), 0 beyond -------------------------------------
+ZP_DEV uint64_t sq_f(const uint64_t* __restrict__ Mtop, int64_t t, int64_t i, const ZpMod& kp) {  // Montgomery
+  return i == 0 ? kp.r1 : (i <= t ? Mtop[t - i] : 0);
+}
+// base case: alpha = 1 / f mod x^KB by Newton steps with schoolbook products in shared memory, one CTA per function
+#define ZP_SQ_KB 1024
+__global__ void __launch_bounds__(512)
+k_sq_inv_base(const uint64_t* __restrict__ Mtop, int64_t t, ZpMod kp, uint64_t* __restrict__ alpha) {
+  __shared__ uint64_t f[ZP_SQ_KB], g[ZP_SQ_KB], ev[ZP_SQ_KB / 2];
+  for (int i = threadIdx.x; i < ZP_SQ_KB; i += blockDim.x) {
+    f[i] = sq_f(Mtop, t, i, kp);
+    g[i] = 0;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) g[0] = kp.r1;
+  __syncthreads();
+  for (int k = 1; k < ZP_SQ_KB; k <<= 1) {
+    // e_i = (f g)_{k+i} = sum_{j<k} f_{k+i-j} g_j,  i < k
+    for (int i = threadIdx.x; i < k; i += blockDim.x) {
+      Acc acc;
+      acc_zero(acc);
+      for (int j = 0; j < k; ++j) acc_mac(acc, f[k + i - j], g[j]);
+      ev[i] = mont_mul(acc_redc160(acc, kp), kp.c160, kp);
+    }
+    __syncthreads();
+    // g_{k+i} = -(g e)_i = -sum_{j<=i} g_j e_{i-j}
+    for (int i = threadIdx.x; i < k; i += blockDim.x) {
+      Acc acc;
+      acc_zero(acc);
+      for (int j = 0; j <= i; ++j) acc_mac(acc, g[j], ev[i - j]);
+      g[k + i] = mod_neg(mont_mul(acc_redc160(acc, kp), kp.c160, kp), kp.p);
+    }
+    __syncthreads();
+  }
+  for (int i = threadIdx.x; i < ZP_SQ_KB; i += blockDim.x) alpha[i] = g[i];
+}
+// Newton step k -> 2k, first product: X[0] = f mod x^2k, X[1] = alpha mod x^k (n = 2k)
+__global__ void __launch_bounds__(256)
+k_sq_newton_prep1(const uint64_t* __restrict__ Mtop, int64_t t, const uint64_t* __restrict__ alpha, int logn, ZpMod kp,
+                  uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, EX = 2 * n, k = n >> 1;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = e & (n - 1);
+    const uint64_t v = (e < n) ? sq_f(Mtop, t, i, kp) : (i < k ? alpha[i] : 0);
+    X[e] = v;
+    X[EX + e] = v;
+    X[2 * EX + e] = v;
+  }
+}
+// Y[0][i] = e_i = (f alpha)_{k+i}, i < k, zero-padded to n (O = inverse transform of the first product)
+__global__ void __launch_bounds__(256)
+k_sq_newton_mid(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ Y) {
+  const int64_t n = (int64_t)1 << logn, k = n >> 1;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t v = 0;
+    if (i < k) v = ntt_crt(O[k + i], O[n + k + i], O[2 * n + k + i], cx, co, kp);
+    Y[i] = v;
+    Y[n + i] = v;
+    Y[2 * n + i] = v;
+  }
+}
+// alpha_{k+i} = -(alpha e)_i, i < k
+__global__ void __launch_bounds__(256)
+k_sq_newton_fin(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ alpha) {
+  const int64_t n = (int64_t)1 << logn, k = n >> 1;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < k; i += (int64_t)gridDim.x * blockDim.x)
+    alpha[k + i] = mod_neg(ntt_crt(O[i], O[n + i], O[2 * n + i], cx, co, kp), kp.p);
+}
+// root tail of M': X[0][i] = rev(M')_i = (t - i) f_i, X[1][i] = alpha_i, i < t, zero-padded to n >= 2t
+__global__ void __launch_bounds__(256)
+k_sq_root_prep(const uint64_t* __restrict__ Mtop, int64_t t, const uint64_t* __restrict__ alpha, int logn, ZpMod kp,
+               uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, EX = 2 * n;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = e & (n - 1);
+    uint64_t v = 0;
+    if (i < t) v = (e < n) ? mont_mul(sq_f(Mtop, t, i, kp), to_mont(zp_canon((uint64_t)(t - i), kp.p), kp), kp) : alpha[i];
+    X[e] = v;
+    X[EX + e] = v;
+    X[2 * EX + e] = v;
+  }
+}
+// tail_k = (rev(M') alpha)_k, k < t: the power sums of the nodes, plain (co carries K = 2^-128)
+__global__ void __launch_bounds__(256)
+k_sq_root_fin(const uint64_t* __restrict__ O, int logn, int64_t t, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ tail) {
+  const int64_t n = (int64_t)1 << logn;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < t; i += (int64_t)gridDim.x * blockDim.x)
+    tail[i] = ntt_crt(O[i], O[n + i], O[2 * n + i], cx, co, kp);
+}
+// root tails of the right-hand sides: the values themselves (canonicalised, reading G22)
+__global__ void __launch_bounds__(256)
+k_sq_load_vals(const uint64_t* __restrict__ vals, int64_t ldv, int B, int64_t T, ZpMod kp, uint64_t* __restrict__ tails,
+               int64_t ld) {
+  for (int b = blockIdx.y; b < B; b += gridDim.y)
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < T; i += (int64_t)gridDim.x * blockDim.x)
+      tails[b * ld + i] = zp_canon(vals[b * ldv + i], kp.p);
+}
+__global__ void k_fill_u64(uint64_t* x, int64_t n, uint64_t v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) x[i] = v;
+}
+
+// ---- batched inversion (Montgomery's trick): N values per lane, one Fermat power per lane ------------
+// x[] Montgomery, in place -> inverses; zeros are skipped (left 0) and reported through the return mask.
+template <int N>
+ZP_DEV uint32_t batch_inv(uint64_t (&x)[N], const ZpMod& k) {
+  uint64_t pre[N];
+  uint64_t run = k.r1;
+  uint32_t zero = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    pre[i] = run;
+    if (x[i] == 0) zero |= 1u << i;
+    else run = mont_mul(run, x[i], k);
+  }
+  uint64_t inv = mont_inv(run, k);
+#pragma unroll
+  for (int i = N - 1; i >= 0; --i) {
+    if (zero >> i & 1) continue;
+    const uint64_t xi = x[i];
+    x[i] = mont_mul(inv, pre[i], k);
+    inv = mont_mul(inv, xi, k);
+  }
+  return zero;
+}
+
+// ---- final division: c_{b,i} = num_{b,i} / (num_{B,i} [m_i]) ------------------------------------------------------------
+// num: [(B+1) x ld] plain (row B = the M' row); coefs: [B x ldc] at the run's first slot; offs: the run's function offsets
+// (device, relative to the run's first slot is offs[f] - offs[0]).
+#define ZP_SQ_INVB 8
+__global__ void __launch_bounds__(128)
+k_sq_final(const uint64_t* __restrict__ num, int64_t ld, int B, const uint64_t* __restrict__ nodes, int s0, int64_t T,
+           const int64_t* __restrict__ offs, int F, ZpMod kp, uint64_t* __restrict__ coefs, int64_t ldc,
+           int32_t* __restrict__ status) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i0 >= T) return;
+  uint64_t d[ZP_SQ_INVB];
+#pragma unroll
+  for (int x = 0; x < ZP_SQ_INVB; ++x) {
+    const int64_t i = i0 + x * stride;
+    uint64_t v = kp.r1;
+    if (i < T) {
+      v = mont_mul(num[(int64_t)B * ld + i], kp.r2, kp);  // to Montgomery
+      if (s0) v = mont_mul(v, to_mont(zp_canon(nodes[i], kp.p), kp), kp);
+    }
+    d[x] = v;
+  }
+  const uint32_t zero = batch_inv<ZP_SQ_INVB>(d, kp);
+#pragma unroll
+  for (int x = 0; x < ZP_SQ_INVB; ++x) {
+    const int64_t i = i0 + x * stride;
+    if (i >= T) continue;
+    if (zero >> x & 1) {
+      int lo = 0, hi = F;  // function of slot i
+      const int64_t gi = i + offs[0];
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (offs[mid] <= gi) lo = mid; else hi = mid;
+      }
+      atomicMin(&status[lo], (int32_t)(((uint32_t)(gi - offs[lo]) << 8) | ZP_ST_DUPLICATE_NODE));
+    }
+    for (int b = 0; b < B; ++b) coefs[(int64_t)b * ldc + i] = mont_mul(num[(int64_t)b * ld + i], d[x], kp);  // plain x Montgomery
+  }
+}

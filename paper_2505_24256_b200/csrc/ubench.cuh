@@ -24,6 +24,118 @@
 #pragma once
 #include "modarith.cuh"
 
+// ---- forms of the Montgomery product and of the deferred MAC that lost against the ones in modarith.cuh; kept for the
+// ---- micro-benchmarks only (kinds 8, 21, 14, 15) --------------------------------------------------------------------
+// Montgomery product, column form (mont_mul_v1: the first version, kept for the micro-benchmark).  Requires a*b < p*2^64 (true for a < 2^64, b < p); a_hi, b_hi < 2^31
+// is NOT required.  With T = a*b and two 32-bit REDC rounds:
+//   T + m0*p + m1*p*2^32 = (P00 + Q0) + (P01 + P10 + Q1 + S0)*2^32 + (P11 + S1)*2^64,  divisible by 2^64.
+// Column 0: the low words of P00 and Q0 cancel, its carry is c0 = hi(P00) + hi(Q0) + (lo(P00) != 0) < 2^33.
+// Column 1: P01 + P10 + Q1 + S0 + c0 may exceed 64 bits; `carry` counts the overflows (weight 2^64).
+// Result (T + ...)/2^64 < p + p = 2p < 2^64, then one conditional subtraction.
+ZP_DEV uint64_t mont_mul_v1(uint64_t a, uint64_t b, const ZpMod& k) {
+  const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32), b0 = (uint32_t)b, b1 = (uint32_t)(b >> 32);
+  const uint64_t P00 = zp_mulw(a0, b0);
+  const uint64_t P01 = zp_mulw(a0, b1);
+  const uint64_t P10 = zp_mulw(a1, b0);
+  const uint64_t P11 = zp_mulw(a1, b1);
+  const uint32_t m0 = (uint32_t)P00 * k.pinv;
+  const uint64_t Q0 = zp_mulw(m0, k.p0), Q1 = zp_mulw(m0, k.p1);
+  const uint64_t c0 = (P00 >> 32) + (Q0 >> 32) + ((uint32_t)P00 != 0);
+  uint64_t col1;
+  uint32_t carry;
+  asm("{\n\t"
+      ".reg .u64 t;\n\t"
+      "add.cc.u64 t, %2, %3;\n\t"
+      "addc.u32 %1, 0, 0;\n\t"
+      "add.cc.u64 t, t, %4;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "add.cc.u64 %0, t, %5;\n\t"
+      "addc.u32 %1, %1, 0;\n\t"
+      "}"
+      : "=l"(col1), "=r"(carry)
+      : "l"(P01), "l"(P10), "l"(Q1), "l"(c0));
+  const uint32_t m1 = (uint32_t)col1 * k.pinv;
+  const uint64_t S0 = zp_mulw(m1, k.p0);
+  const uint64_t c1 = (col1 >> 32) + (S0 >> 32) + ((uint32_t)col1 != 0) + ((uint64_t)carry << 32);
+  // P11 + S1 + c1 = exact quotient < 2p + 1 <= 2^64 - ... : no overflow
+  const uint64_t r = zp_madw(m1, k.p1, P11 + c1);
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+
+// v3: two 32-bit REDC rounds, every product a bare mul.wide, every addition a 32-bit carry chain (alu pipe).
+ZP_DEV uint64_t mont_mul_v3(uint64_t a, uint64_t b, const ZpMod& k) {
+  const uint32_t a0 = (uint32_t)a, a1 = (uint32_t)(a >> 32), b0 = (uint32_t)b, b1 = (uint32_t)(b >> 32);
+  const uint64_t P00 = zp_mulw(a0, b0), P01 = zp_mulw(a0, b1), P10 = zp_mulw(a1, b0), P11 = zp_mulw(a1, b1);
+  uint32_t t0, t1, t2, t3;
+  asm("{\n\t.reg .u32 x1, y0, y1, z0, z1, w0, w1;\n\t"
+      "mov.b64 {%0, x1}, %4;\n\tmov.b64 {y0, y1}, %5;\n\tmov.b64 {z0, z1}, %6;\n\tmov.b64 {w0, w1}, %7;\n\t"
+      "add.cc.u32 %1, x1, y0;\n\taddc.cc.u32 %2, y1, w0;\n\taddc.u32 %3, w1, 0;\n\t"
+      "add.cc.u32 %1, %1, z0;\n\taddc.cc.u32 %2, %2, z1;\n\taddc.u32 %3, %3, 0;\n\t}"
+      : "=r"(t0), "=r"(t1), "=r"(t2), "=r"(t3)
+      : "l"(P00), "l"(P01), "l"(P10), "l"(P11));
+  const uint32_t m0 = t0 * k.pinv;
+  const uint64_t Q0 = zp_mulw(m0, k.p0), Q1 = zp_mulw(m0, k.p1);
+  asm("{\n\t.reg .u32 q0, q1, r0, r1, dummy;\n\t"
+      "mov.b64 {q0, q1}, %4;\n\tmov.b64 {r0, r1}, %5;\n\t"
+      "add.cc.u32 dummy, %3, q0;\n\taddc.cc.u32 %0, %0, q1;\n\taddc.cc.u32 %1, %1, r1;\n\taddc.u32 %2, %2, 0;\n\t"
+      "add.cc.u32 %0, %0, r0;\n\taddc.cc.u32 %1, %1, 0;\n\taddc.u32 %2, %2, 0;\n\t}"
+      : "+r"(t1), "+r"(t2), "+r"(t3)
+      : "r"(t0), "l"(Q0), "l"(Q1));
+  const uint32_t m1 = t1 * k.pinv;
+  const uint64_t S0 = zp_mulw(m1, k.p0), S1 = zp_mulw(m1, k.p1);
+  asm("{\n\t.reg .u32 q0, q1, r0, r1, dummy;\n\t"
+      "mov.b64 {q0, q1}, %3;\n\tmov.b64 {r0, r1}, %4;\n\t"
+      "add.cc.u32 dummy, %2, q0;\n\taddc.cc.u32 %0, %0, q1;\n\taddc.u32 %1, %1, r1;\n\t"
+      "add.cc.u32 %0, %0, r0;\n\taddc.u32 %1, %1, 0;\n\t}"
+      : "+r"(t2), "+r"(t3)
+      : "r"(t1), "l"(S0), "l"(S1));
+  const uint64_t r = ((uint64_t)t3 << 32) | t2;
+  const uint64_t s = r - k.p;
+  return (r >= k.p) ? s : r;
+}
+
+// Alternative forms of the same MAC, for the pipe-balance micro-benchmarks (zippel_ubench kinds 12-16).
+// acc_mac_split: every product is a bare IMAD.WIDE (zero addend, 4 pipe cycles instead of the > 5 of the
+// accumulating form, profiles/r01_baseline.md); the 160-bit additions run on the alu pipe as 32-bit carry chains.
+ZP_DEV void acc_mac_split(Acc& a, uint64_t x, uint64_t y) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0);
+  asm("{\n\t.reg .u32 a0, a1, a2, a3, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {a2, a3}, %1;\n\tmov.b64 {l0, l1}, %3;\n\tmov.b64 {h0, h1}, %4;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.cc.u32 a2, a2, h0;\n\taddc.cc.u32 a3, a3, h1;\n\t"
+      "addc.u32 %2, %2, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\tmov.b64 %1, {a2, a3};\n\t}"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi));
+  asm("{\n\t.reg .u32 a0, a1, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {l0, l1}, %2;\n\tmov.b64 {h0, h1}, %3;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "add.cc.u32 a0, a0, h0;\n\taddc.cc.u32 a1, a1, h1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\t}"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1));
+}
+// acc_mac_hyb: the two 64-bit aligned products of the even lattice accumulate inside IMAD.WIDE (as acc_mac),
+// the two middle products are bare and are added on the alu pipe.
+ZP_DEV void acc_mac_hyb(Acc& a, uint64_t x, uint64_t y) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), y0 = (uint32_t)y, y1 = (uint32_t)(y >> 32);
+  const uint64_t lo = zp_mulw(x0, y0), hi = zp_mulw(x1, y1), m0 = zp_mulw(x0, y1), m1 = zp_mulw(x1, y0);
+  asm("add.cc.u64 %0, %0, %3;\n\t"
+      "addc.cc.u64 %1, %1, %4;\n\t"
+      "addc.u32 %2, %2, 0;"
+      : "+l"(a.e0), "+l"(a.e1), "+r"(a.e2)
+      : "l"(lo), "l"(hi));
+  asm("{\n\t.reg .u32 a0, a1, l0, l1, h0, h1;\n\t"
+      "mov.b64 {a0, a1}, %0;\n\tmov.b64 {l0, l1}, %2;\n\tmov.b64 {h0, h1}, %3;\n\t"
+      "add.cc.u32 a0, a0, l0;\n\taddc.cc.u32 a1, a1, l1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "add.cc.u32 a0, a0, h0;\n\taddc.cc.u32 a1, a1, h1;\n\taddc.u32 %1, %1, 0;\n\t"
+      "mov.b64 %0, {a0, a1};\n\t}"
+      : "+l"(a.o0), "+r"(a.o1)
+      : "l"(m0), "l"(m1));
+}
+
+
 #define ZP_UB_THREADS 256
 #define ZP_UB_CH 8
 

@@ -4,10 +4,11 @@
 
 #include <cstdint>
 #include <cstring>
+#include <vector>
 
 #include "../../include/zippel.h"
 #include "kernels.cuh"
-#include "ubench.cuh"
+#include "subq.cuh"
 
 namespace {
 
@@ -39,6 +40,168 @@ bool make_mod(uint64_t p, ZpMod* k) {
   return true;
 }
 
+// ---- sub-quadratic route (subq.cuh): host constants, plan, workspace sizes -----------------------------------------
+// The three NTT primes q = c 2^26 + 1 just below 2^62 and a generator of their 2-power subgroups (x^((q-1)/2^24) has
+// order 2^24); tests/test_ntt_constants.py re-derives both facts with Python integers through zippel_ntt_constants().
+const uint64_t kNttQ[3] = {4611686017554972673ull, 4611686015004835841ull, 4611686009971671041ull};
+const uint64_t kNttGen[3] = {5, 3, 3};
+int64_t g_subq_min_t = 8192;  // functions with at least this many terms take the sub-quadratic route (zippel_set_tuning)
+
+uint64_t h_mulmod(uint64_t a, uint64_t b, uint64_t m) { return (uint64_t)((u128)a * b % m); }
+uint64_t h_powmod(uint64_t a, uint64_t e, uint64_t m) {
+  uint64_t r = 1 % m;
+  a %= m;
+  while (e) {
+    if (e & 1) r = h_mulmod(r, a, m);
+    a = h_mulmod(a, a, m);
+    e >>= 1;
+  }
+  return r;
+}
+uint64_t h_invmod(uint64_t a, uint64_t m) { return h_powmod(a, m - 2, m); }  // m prime
+
+struct SqHost {
+  NttCtx cx;               // table pointers are filled per call
+  uint64_t wroot_mont[3];  // the root of order 2^24 of each prime, Montgomery form
+};
+const SqHost& sq_host() {
+  static const SqHost H = [] {
+    SqHost h;
+    memset(&h, 0, sizeof(h));
+    for (int j = 0; j < 3; ++j) {
+      const uint64_t q = kNttQ[j];
+      make_mod(q, &h.cx.q[j]);
+      const uint64_t w = h_powmod(kNttGen[j], (q - 1) >> ZP_NTT_LOGMAX, q);
+      h.wroot_mont[j] = h_mulmod(w, h.cx.q[j].r1, q);
+    }
+    const uint64_t q1 = kNttQ[0], q2 = kNttQ[1], q3 = kNttQ[2];
+    h.cx.g2 = h_mulmod(h_invmod(q1 % q2, q2), h.cx.q[1].r1, q2);
+    h.cx.g3a = h_mulmod(q1 % q3, h.cx.q[2].r1, q3);
+    h.cx.g3b = h_mulmod(h_invmod(h_mulmod(q1 % q3, q2 % q3, q3), q3), h.cx.q[2].r1, q3);
+    return h;
+  }();
+  return H;
+}
+// c K mod p with K = 2^(-64 kexp)
+CrtOut make_crt_out(const ZpMod& k, int kexp) {
+  const uint64_t p = k.p;
+  const uint64_t K = h_powmod((p + 1) / 2, 64 * (uint64_t)kexp, p);  // (1/2)^(64 kexp): p odd
+  CrtOut co;
+  co.C1 = h_mulmod(K, k.r1, p);
+  co.C2 = h_mulmod(co.C1, kNttQ[0] % p, p);
+  co.C3 = h_mulmod(co.C2, kNttQ[1] % p, p);
+  return co;
+}
+// 2^128 / n mod q_j
+void make_kq(int logn, uint64_t Kq[3]) {
+  for (int j = 0; j < 3; ++j) {
+    const uint64_t q = kNttQ[j];
+    const ZpMod& m = sq_host().cx.q[j];
+    Kq[j] = h_mulmod(m.r2, h_powmod((q + 1) / 2, (uint64_t)logn, q), q);
+  }
+}
+
+inline int ceil_log2(int64_t x) {
+  int l = 0;
+  while (((int64_t)1 << l) < x) ++l;
+  return l;
+}
+
+// one run of consecutive long functions [f0, f1): slots [a0, a0 + T)
+struct SqRun {
+  int f0, f1;
+  int64_t a0, T, tmax;
+  int nlev;  // levels 0 .. nlev; block size at level l = ZP_LEAF << l
+};
+struct SqSizes {
+  bool any = false;
+  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0;
+  int maxLev = 0, Vc = 1;
+};
+inline bool sq_is_long(int64_t t) { return t >= g_subq_min_t && t > ZP_LEAF; }
+
+// pair and copy tasks of level l (children of size a = LEAF << l) for a run; slots relative to the run
+void sq_level_tasks(const int64_t* h_offs, const SqRun& r, int l, std::vector<SqTask>* pairs, std::vector<SqTask>* copies) {
+  const int64_t a = (int64_t)ZP_LEAF << l;
+  for (int f = r.f0; f < r.f1; ++f) {
+    const int64_t off = h_offs[f] - r.a0, t = h_offs[f + 1] - h_offs[f];
+    int64_t base = 0;
+    for (; base + a < t; base += 2 * a) {
+      const int64_t b = (t - base - a < a) ? t - base - a : a;
+      if (pairs) pairs->push_back(SqTask{off + base, (int32_t)a, (int32_t)b});
+    }
+    if (base < t && copies) {  // a last block without a sibling (or a function already complete): copy through, in
+      for (int64_t c = base; c < t; c += ((int64_t)1 << 30))  // pieces that fit the 32-bit length field
+        copies->push_back(SqTask{off + c, (int32_t)((t - c < ((int64_t)1 << 30)) ? t - c : ((int64_t)1 << 30)), 0});
+    }
+  }
+}
+
+void sq_find_runs(const int64_t* h_offs, int F, std::vector<SqRun>* runs) {
+  for (int f = 0; f < F;) {
+    if (!sq_is_long(h_offs[f + 1] - h_offs[f])) {
+      ++f;
+      continue;
+    }
+    SqRun r;
+    r.f0 = f;
+    r.tmax = 0;
+    while (f < F && sq_is_long(h_offs[f + 1] - h_offs[f])) {
+      const int64_t t = h_offs[f + 1] - h_offs[f];
+      r.tmax = t > r.tmax ? t : r.tmax;
+      ++f;
+    }
+    r.f1 = f;
+    r.a0 = h_offs[r.f0];
+    r.T = h_offs[r.f1] - r.a0;
+    r.nlev = ceil_log2((r.tmax + ZP_LEAF - 1) / ZP_LEAF);
+    runs->push_back(r);
+  }
+}
+
+SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
+  SqSizes z;
+  std::vector<SqRun> runs;
+  sq_find_runs(h_offs, F, &runs);
+  if (runs.empty()) return z;
+  z.any = true;
+  auto mx = [](int64_t& a, int64_t b) { a = b > a ? b : a; };
+  for (const SqRun& r : runs) mx(z.maxT, r.T);
+  // vectors per down-tree chunk: the product buffer holds 2 Vc T words per prime; cap it at 2^27 words in all
+  int64_t vc = ((int64_t)1 << 27) / (6 * z.maxT);
+  z.Vc = (int)(vc < 1 ? 1 : (vc > B + 1 ? B + 1 : vc));
+  for (const SqRun& r : runs) {
+    z.maxLev = r.nlev > z.maxLev ? r.nlev : z.maxLev;
+    int64_t ntasks = 0, leaves = 0;
+    for (int l = 0; l < r.nlev; ++l) {
+      std::vector<SqTask> pairs, copies;
+      sq_level_tasks(h_offs, r, l, &pairs, &copies);
+      const int64_t n = (int64_t)2 * ZP_LEAF << l, P = (int64_t)pairs.size();
+      mx(z.maxX, 2 * P * n);
+      mx(z.maxO, P * n);
+      mx(z.maxY, z.Vc * P * n);
+      mx(z.maxO, 2 * z.Vc * P * n);
+      ntasks += (int64_t)pairs.size() + (int64_t)copies.size();
+    }
+    mx(z.maxTasks, ntasks);
+    for (int f = r.f0; f < r.f1; ++f) {
+      const int64_t t = h_offs[f + 1] - h_offs[f];
+      leaves += (t + ZP_LEAF - 1) / ZP_LEAF;
+      int64_t kf = ZP_SQ_KB;
+      while (kf < t) kf <<= 1;
+      mx(z.alphaN, kf);
+      mx(z.maxX, 2 * kf);  // Newton's last step: n = kf
+      mx(z.maxY, kf);
+      mx(z.maxO, kf);
+      const int64_t nr = (int64_t)1 << ceil_log2(2 * t);  // root product
+      mx(z.maxX, 2 * nr);
+      mx(z.maxO, nr);
+    }
+    mx(z.maxLeaves, leaves);
+  }
+  return z;
+}
+
 // ---- workspace ----------------------------------------------------------------------------------
 struct Ws {
   int64_t* d_offsets;
@@ -46,12 +209,18 @@ struct Ws {
   uint64_t *nodes, *M0, *M1, *scale, *R, *V, *newtI, *newtL;
   ulonglong2 *invd, *smont;  // Newton: {w, w'} tables
   ulonglong4* tab;
+  // sub-quadratic route (null unless some function is long)
+  SqSizes sq;
+  ulonglong2* ntt_tab;  // [3][4][4096]: U, Ui, Tlo, Thi per prime
+  SqTask* sq_tasks;
+  int64_t* sq_leafoffs;
+  uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Y, *sq_O;
   size_t bytes;
 };
 
 inline size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
 
-Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
+Ws carve(void* base, int64_t T_tot, int F, int B, int flags, const SqSizes& sq = SqSizes()) {
   Ws w;
   size_t o = 0;
   auto take = [&](size_t n) {
@@ -74,6 +243,20 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags) {
   w.newtL = (uint64_t*)take(8 * (size_t)B * B);
   w.R = (uint64_t*)take(8 * (size_t)T_tot);
   w.V = (flags & ZP_WS_BALANCED) ? (uint64_t*)take(8 * (size_t)T_tot * B) : nullptr;
+  w.sq = sq;
+  w.ntt_tab = nullptr;
+  if (sq.any) {
+    w.ntt_tab = (ulonglong2*)take(16 * (size_t)12 * ZP_NTT_TAB);
+    w.sq_tasks = (SqTask*)take(sizeof(SqTask) * (size_t)(sq.maxTasks + 1));
+    w.sq_leafoffs = (int64_t*)take(8 * (size_t)(sq.maxLeaves + 1));
+    w.sq_lev = (uint64_t*)take(8 * (size_t)(sq.maxLev + 1) * sq.maxT);
+    w.sq_tailA = (uint64_t*)take(8 * (size_t)(B + 1) * sq.maxT);
+    w.sq_tailB = (uint64_t*)take(8 * (size_t)(B + 1) * sq.maxT);
+    w.sq_alpha = (uint64_t*)take(8 * (size_t)sq.alphaN);
+    w.sq_X = (uint64_t*)take(8 * 3 * (size_t)sq.maxX);
+    w.sq_Y = (uint64_t*)take(8 * 3 * (size_t)sq.maxY);
+    w.sq_O = (uint64_t*)take(8 * 3 * (size_t)sq.maxO);
+  }
   w.bytes = o;
   return w;
 }
@@ -83,7 +266,7 @@ bool check_offsets(const int64_t* h, int F, int64_t* T_tot, int64_t* tmax) {
   int64_t mx = 0;
   for (int f = 0; f < F; ++f) {
     const int64_t t = h[f + 1] - h[f];
-    if (t <= 0 || t >= ((int64_t)1 << 31)) return false;
+    if (t <= 0 || t >= ((int64_t)1 << 23)) return false;  // status index field; NTT length (zippel.h)
     if (t > mx) mx = t;
   }
   if (h[F] >= ((int64_t)1 << 31)) return false;
@@ -112,24 +295,35 @@ struct ProfScope {  // records start at construction and stop at destruction whe
 };
 
 inline int cuda_ok() { return cudaGetLastError() == cudaSuccess ? ZP_OK : ZP_ERR_CUDA; }
+// SMs of the current device (grid caps of the grid-stride kernels are multiples of it)
+int sm_count() {
+  static int n_cached[16] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 16) return 148;
+  if (!n_cached[dev]) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    n_cached[dev] = n;
+  }
+  return n_cached[dev];
+}
 inline unsigned grid_y(int F) { return (unsigned)(F < 65535 ? F : 65535); }
 
 // ---- K3 dispatch ----------------------------------------------------------------------------------
 #define ZP_NB_MAX 25
 
 template <int NB>
-void launch_node_solve(bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
-                       const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k,
-                       uint64_t* scale, uint64_t* coefs, int32_t* status) {
-  (void)first;  // the denominators come from k_node_den: every pass is a <NB, false> pass
-  ++g_launches, k_node_solve<NB, false><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
+void launch_node_solve(dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M, const int64_t* offs, int F,
+                       const uint64_t* vals, int64_t T_tot, int b0, int s0, const ZpMod& k, uint64_t* scale,
+                       uint64_t* coefs, int32_t* status) {
+  ++g_launches, k_node_solve<NB><<<grid, ZP_K3_THREADS, 0, st>>>(nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status);
 }
 
-void dispatch_node_solve(int nb, bool first, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
+void dispatch_node_solve(int nb, dim3 grid, cudaStream_t st, const uint64_t* nodes, const ulonglong4* M,
                          const int64_t* offs, int F, const uint64_t* vals, int64_t T_tot, int b0, int s0,
                          const ZpMod& k, uint64_t* scale, uint64_t* coefs, int32_t* status) {
 #define ZP_CASE(N) \
-  case N: launch_node_solve<N>(first, grid, st, nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status); break;
+  case N: launch_node_solve<N>(grid, st, nodes, M, offs, F, vals, T_tot, b0, s0, k, scale, coefs, status); break;
   switch (nb) {
     ZP_CASE(1) ZP_CASE(2) ZP_CASE(3) ZP_CASE(4) ZP_CASE(5) ZP_CASE(6) ZP_CASE(7) ZP_CASE(8) ZP_CASE(9)
     ZP_CASE(10) ZP_CASE(11) ZP_CASE(12) ZP_CASE(13) ZP_CASE(14) ZP_CASE(15) ZP_CASE(16) ZP_CASE(17)
@@ -159,10 +353,200 @@ const uint64_t* run_master_poly(const Ws& w, const uint64_t* nodes, int F, int64
   return src;
 }
 
-// (a2)-(a4): solve into coefs; per-function codes into w.st_solve (NONE = ok)
-void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
-               int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
-  ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
+// ---- sub-quadratic route: launches ---------------------------------------------------------------------------------
+inline unsigned sq_blocks(int64_t n, int per = 256) {
+  int64_t b = (n + per - 1) / per;
+  const int64_t cap = (int64_t)sm_count() * 64;
+  return (unsigned)(b < 1 ? 1 : (b > cap ? cap : b));
+}
+// transform every segment of `buf` ([3][E] words, segments of 2^logn) in place (ntt.cuh: one to three passes)
+void ntt_run(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
+  const dim3 g((unsigned)((E + ZP_NTT_C - 1) / ZP_NTT_C), 3);
+  int lr1 = 0, lr2 = 0;  // rows of the strided passes
+  if (logn > ZP_NTT_LOGC) {
+    const int e = logn - ZP_NTT_LOGC;
+    if (e <= 9) lr1 = e;
+    else lr1 = (e + 1) / 2, lr2 = e - lr1;
+  }
+  if (!inverse) {
+    if (lr1) ++g_launches, k_ntt_strided<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, lr1, 0, cx);
+    if (lr2) ++g_launches, k_ntt_strided<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1, lr2, lr1, cx);
+    ++g_launches, k_ntt_chunk<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1 - lr2, lr2 ? lr2 : lr1, cx);
+  } else {
+    ++g_launches, k_ntt_chunk<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1 - lr2, lr2 ? lr2 : lr1, cx);
+    if (lr2) ++g_launches, k_ntt_strided<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1, lr2, lr1, cx);
+    if (lr1) ++g_launches, k_ntt_strided<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, lr1, 0, cx);
+  }
+}
+void ntt_pointwise(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* O, int64_t EO, int logn, int mode,
+                   int64_t P, const NttCtx& cx, cudaStream_t st) {
+  uint64_t Kq[3];
+  make_kq(logn, Kq);
+  const dim3 g(sq_blocks(EO), 3);
+  ++g_launches, k_ntt_pointwise<<<g, 256, 0, st>>>(A, EA, B, EB, O, EO, logn, mode, P, cx, Kq[0], Kq[1], Kq[2]);
+}
+// the per-call context: host constants + this workspace's tables (built by the first launch of the call)
+NttCtx ntt_begin(const Ws& w, cudaStream_t st) {
+  NttCtx cx = sq_host().cx;
+  for (int j = 0; j < 3; ++j) {
+    ulonglong2* t = w.ntt_tab + (size_t)j * 4 * ZP_NTT_TAB;
+    cx.U[j] = t;
+    cx.Ui[j] = t + ZP_NTT_TAB;
+    cx.Tlo[j] = t + 2 * ZP_NTT_TAB;
+    cx.Thi[j] = t + 3 * ZP_NTT_TAB;
+    ++g_launches, k_ntt_tables<<<4 * ZP_NTT_TAB / 256, 256, 0, st>>>(cx.q[j], sq_host().wroot_mont[j], t, t + ZP_NTT_TAB,
+                                                                   t + 2 * ZP_NTT_TAB, t + 3 * ZP_NTT_TAB);
+  }
+  return cx;
+}
+
+#ifdef ZP_TEST_HOOKS
+int g_sq_dump_stage = 0;  // zippel_test_subq_dump
+uint64_t* g_sq_dump_out = nullptr;
+#define SQ_DUMP(stage, ptr, words) \
+  if (g_sq_dump_stage == (stage) && g_sq_dump_out) cudaMemcpyAsync(g_sq_dump_out, (ptr), 8 * (size_t)(words), cudaMemcpyDeviceToDevice, st)
+#else
+#define SQ_DUMP(stage, ptr, words)
+#endif
+
+// (a2)-(a4) for one run of long functions; nodes / vals / coefs point at the run's first slot (row strides ldv, ldc)
+void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun& r, const uint64_t* nodes,
+              const uint64_t* vals, int64_t ldv, int B, int s0, const ZpMod& k, uint64_t* coefs, int64_t ldc,
+              cudaStream_t st) {
+  const int64_t T = r.T;
+  const int Fr = r.f1 - r.f0;
+  const CrtOut co0 = make_crt_out(k, 0), co1 = make_crt_out(k, 1), co2 = make_crt_out(k, 2);
+  (void)co0;
+  // task lists of every level, and the leaf offsets: one upload per array
+  std::vector<SqTask> tasks;
+  std::vector<size_t> pair0(r.nlev + 1), copy0(r.nlev + 1), copy1(r.nlev + 1);
+  for (int l = 0; l < r.nlev; ++l) {
+    pair0[l] = tasks.size();
+    sq_level_tasks(h_offs, r, l, &tasks, nullptr);
+    copy0[l] = tasks.size();
+    sq_level_tasks(h_offs, r, l, nullptr, &tasks);
+    copy1[l] = tasks.size();
+  }
+  std::vector<int64_t> leafoffs;
+  for (int f = r.f0; f < r.f1; ++f)
+    for (int64_t x = h_offs[f]; x < h_offs[f + 1]; x += ZP_LEAF) leafoffs.push_back(x - r.a0);
+  leafoffs.push_back(T);
+  const int nleaves = (int)leafoffs.size() - 1;
+  if (!tasks.empty()) cudaMemcpyAsync(w.sq_tasks, tasks.data(), sizeof(SqTask) * tasks.size(), cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(w.sq_leafoffs, leafoffs.data(), 8 * leafoffs.size(), cudaMemcpyHostToDevice, st);
+  const int64_t* d_offs = w.d_offsets + r.f0;  // absolute slots: kernels that use them get pointers at slot 0 of the batch
+
+  // (up) leaves, then one product per pair and level
+  auto lev = [&](int l) { return w.sq_lev + (size_t)l * T; };
+  {
+    ProfScope prof(ZP_K_MASTER_POLY, st);
+    dim3 g((unsigned)((r.tmax + ZP_LEAF - 1) / ZP_LEAF), grid_y(Fr));
+    // k_tree_leaf indexes nodes and out by absolute slots: shift both so that the run starts at its own slot 0
+    ++g_launches, k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes - r.a0, d_offs, Fr, k, lev(0) - r.a0);
+    for (int l = 0; l < r.nlev; ++l) {
+      const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
+      const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
+      const SqTask* tp = w.sq_tasks + pair0[l];
+      if (P) {
+        const int64_t EX = 2 * P * n, EO = P * n;
+        ++g_launches, k_sq_up_prep<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_X, EX);
+        ntt_run(false, w.sq_X, EX, logn, cx, st);
+        ntt_pointwise(w.sq_X, EX, w.sq_X, EX, w.sq_O, EO, logn, 0, P, cx, st);
+        ntt_run(true, w.sq_O, EO, logn, cx, st);
+        ++g_launches, k_sq_up_fin<<<sq_blocks(EO), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_O, EO, cx, co1, k, lev(l + 1));
+      }
+      const int nc = (int)(copy1[l] - copy0[l]);
+      if (nc) ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(nc < 1024 ? nc : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, lev(l), lev(l + 1), 1, 0);
+    }
+  }
+  SQ_DUMP(1, lev(r.nlev), T);
+  ProfScope prof(ZP_K_NODE_SOLVE, st);
+  // root tails: rows 0 .. B-1 = the values; row B = rev(M') / rev(M) mod x^t per function
+  const int V = B + 1;
+  uint64_t *cur = w.sq_tailA, *nxt = w.sq_tailB;
+  ++g_launches, k_sq_load_vals<<<dim3(sq_blocks(T), (unsigned)(B < 64 ? B : 64)), 256, 0, st>>>(vals, ldv, B, T, k, cur, T);
+  for (int f = r.f0; f < r.f1; ++f) {
+    const int64_t off = h_offs[f] - r.a0, t = h_offs[f + 1] - h_offs[f];
+    const uint64_t* Mtop = lev(r.nlev) + off;
+    ++g_launches, k_sq_inv_base<<<1, 512, 0, st>>>(Mtop, t, k, w.sq_alpha);
+    for (int64_t kk = ZP_SQ_KB; kk < t; kk <<= 1) {  // precision kk -> 2 kk, products of length n = 2 kk
+      const int logn = ceil_log2(2 * kk);
+      const int64_t n = 2 * kk;
+      ++g_launches, k_sq_newton_prep1<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
+      ntt_run(false, w.sq_X, 2 * n, logn, cx, st);
+      ntt_pointwise(w.sq_X, 2 * n, w.sq_X, 2 * n, w.sq_O, n, logn, 0, 1, cx, st);
+      ntt_run(true, w.sq_O, n, logn, cx, st);
+      ++g_launches, k_sq_newton_mid<<<sq_blocks(n), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_Y);
+      ntt_run(false, w.sq_Y, n, logn, cx, st);
+      ntt_pointwise(w.sq_Y, n, w.sq_X, 2 * n, w.sq_O, n, logn, 2, 1, cx, st);
+      ntt_run(true, w.sq_O, n, logn, cx, st);
+      ++g_launches, k_sq_newton_fin<<<sq_blocks(kk), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_alpha);
+    }
+    SQ_DUMP(2, w.sq_alpha, t);
+    const int logn = ceil_log2(2 * t);
+    const int64_t n = (int64_t)1 << logn;
+    ++g_launches, k_sq_root_prep<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
+    ntt_run(false, w.sq_X, 2 * n, logn, cx, st);
+    ntt_pointwise(w.sq_X, 2 * n, w.sq_X, 2 * n, w.sq_O, n, logn, 0, 1, cx, st);
+    ntt_run(true, w.sq_O, n, logn, cx, st);
+    ++g_launches, k_sq_root_fin<<<sq_blocks(t), 256, 0, st>>>(w.sq_O, logn, t, cx, co2, k, cur + (size_t)B * T + off);
+  }
+  SQ_DUMP(3, cur, (size_t)V * T);
+  // (down) level by level, vectors in chunks of Vc
+  for (int l = r.nlev - 1; l >= 0; --l) {
+    const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
+    const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
+    const SqTask* tp = w.sq_tasks + pair0[l];
+    if (P) {
+      const int64_t EX = 2 * P * n;
+      ++g_launches, k_sq_down_prepx<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_X, EX);
+      ntt_run(false, w.sq_X, EX, logn, cx, st);
+      for (int v0 = 0; v0 < V; v0 += w.sq.Vc) {
+        const int nv = (V - v0 < w.sq.Vc) ? V - v0 : w.sq.Vc;
+        const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
+        ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
+        ntt_run(false, w.sq_Y, EY, logn, cx, st);
+        ntt_pointwise(w.sq_Y, EY, w.sq_X, EX, w.sq_O, EO, logn, 1, P, cx, st);
+        ntt_run(true, w.sq_O, EO, logn, cx, st);
+        ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
+                                                                    nxt + (size_t)v0 * T);
+      }
+    }
+    const int nc = (int)(copy1[l] - copy0[l]);
+    if (nc) {
+      const int ny = nc * V;
+      ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(ny < 1024 ? ny : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, cur, nxt, V, T);
+    }
+    uint64_t* tmp = cur;
+    cur = nxt;
+    nxt = tmp;
+  }
+  SQ_DUMP(4, cur, (size_t)V * T);
+  // (leaf) the synthetic-division dots of (a3) on the leaves as functions, B + 1 right-hand sides, unscaled
+  {
+    dim3 gt((unsigned)((ZP_LEAF + 255) / 256), grid_y(nleaves));
+    ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(lev(0), w.sq_leafoffs, nleaves, k, w.tab, w.R);
+    ++g_launches, k_fill_u64<<<sq_blocks(T), 256, 0, st>>>(w.scale, T, k.c224);  // scale = 1: plain numerators out
+    const int passes = (V + ZP_NB_MAX - 1) / ZP_NB_MAX;
+    const int per = (V + passes - 1) / passes;
+    dim3 g((unsigned)((ZP_LEAF + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(nleaves));
+    for (int b0 = 0; b0 < V; b0 += per) {
+      const int nb = (V - b0 < per) ? (V - b0) : per;
+      dispatch_node_solve(nb, g, st, nodes, w.tab, w.sq_leafoffs, nleaves, cur, T, b0, 0, k, w.scale, nxt, nullptr);
+    }
+  }
+  SQ_DUMP(5, nxt, (size_t)V * T);
+  // c = N(m_i) / M'(m_i) [/ m_i]: one batched inversion
+  {
+    const int64_t lanes = (T + ZP_SQ_INVB - 1) / ZP_SQ_INVB;
+    ++g_launches, k_sq_final<<<(unsigned)((lanes + 127) / 128), 128, 0, st>>>(nxt, T, B, nodes, s0, T, d_offs, Fr, k, coefs, ldc,
+                                                                           w.st_solve + r.f0);
+  }
+}
+
+// (a2)-(a4) by the quadratic route of PAPER.md section 2.2 for the functions [0, F) behind w.d_offsets
+void run_solve_quadratic(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
+                         int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
   const uint64_t* Mt = run_master_poly(w, nodes, F, tmax, k, st);
   if (B == 1 && tmax >= ZP_EVAL2_MIN_T) {
     // one right-hand side, long skeleton: num_i = W(m_i) with W = correlation of v and M (kernels.cuh, k_corr_w)
@@ -187,11 +571,41 @@ void run_solve(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t
   ProfScope prof(ZP_K_NODE_SOLVE, st);
   dim3 g((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
   ++g_launches, k_node_den<<<g, ZP_K3_THREADS, 0, st>>>(nodes, w.R, w.d_offsets, F, s0, k, w.scale, w.st_solve);
-  for (int b0 = 0, pass = 0; b0 < B; b0 += per, ++pass) {
+  for (int b0 = 0; b0 < B; b0 += per) {
     const int nb = (B - b0 < per) ? (B - b0) : per;
-    dispatch_node_solve(nb, pass == 0, g, st, nodes, M, w.d_offsets, F, vals, T_tot, b0, s0, k, w.scale, coefs,
-                        w.st_solve);
+    dispatch_node_solve(nb, g, st, nodes, M, w.d_offsets, F, vals, T_tot, b0, s0, k, w.scale, coefs, w.st_solve);
   }
+}
+
+// (a2)-(a4): solve into coefs; per-function codes into w.st_solve (NONE = ok).  h_offs: the host offsets of the functions
+// behind w.d_offsets (absolute slots).  Runs of consecutive long functions take the sub-quadratic route (subq.cuh), the
+// others the quadratic one.
+void run_solve(const Ws& w, const int64_t* h_offs, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax,
+               const uint64_t* vals, int B, int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
+  ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
+  std::vector<SqRun> runs;
+  if (w.sq.any) sq_find_runs(h_offs, F, &runs);
+  if (runs.empty()) {
+    run_solve_quadratic(w, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
+    return;
+  }
+  const NttCtx cx = ntt_begin(w, st);
+  auto quad = [&](int f0, int f1) {  // the functions [f0, f1) by the quadratic route: same launches on shifted offsets
+    if (f1 <= f0) return;
+    int64_t tm = 0;
+    for (int f = f0; f < f1; ++f) tm = (h_offs[f + 1] - h_offs[f] > tm) ? h_offs[f + 1] - h_offs[f] : tm;
+    Ws wc = w;
+    wc.d_offsets += f0;
+    wc.st_solve += f0;
+    run_solve_quadratic(wc, nodes, f1 - f0, T_tot, tm, vals, B, s0, k, coefs, st);
+  };
+  int f = 0;
+  for (const SqRun& r : runs) {
+    quad(f, r.f0);
+    sq_solve(w, cx, h_offs, r, nodes + r.a0, vals + r.a0, T_tot, B, s0, k, coefs + r.a0, T_tot, st);
+    f = r.f1;
+  }
+  quad(f, F);
 }
 
 // (a5): Newton on [B x n] with leading dimension ld; code into w.st_newton[0]
@@ -202,7 +616,7 @@ void run_newton(const Ws& w, const uint64_t* samples, int B, const uint64_t* val
   ProfScope prof(ZP_K_NEWTON, st);
   const size_t smem = 16 * ((size_t)B * B + B) + 8 * (size_t)B * ZP_K5_THREADS;
   int64_t blocks = (n + ZP_K5_THREADS - 1) / ZP_K5_THREADS;
-  if (blocks > 148 * 64) blocks = 148 * 64;
+  if (blocks > sm_count() * 64) blocks = sm_count() * 64;
   if (n >= 4 * (int64_t)B) {
     // many coefficients: L = Newton(identity) once, then the batch is the product L x vals (k_newton_apply)
     ++g_launches, k_set_identity<<<(B * B + 255) / 256, 256, 0, st>>>(w.newtI, B);
@@ -235,7 +649,7 @@ void run_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t*
                     uint64_t* nodes, cudaStream_t st) {
   ProfScope prof(ZP_K_EVAL_NODES, st);
   int64_t blocks = (T_tot + ZP_K1_THREADS - 1) / ZP_K1_THREADS;
-  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks > sm_count() * 16) blocks = sm_count() * 16;
   ++g_launches, k_eval_nodes<<<(unsigned)blocks, ZP_K1_THREADS, 0, st>>>(exps, T_tot, nv, anchors, k, nodes);
 }
 
@@ -258,7 +672,7 @@ struct HostWs {
   void* inner;
   size_t inner_bytes, bytes;
 };
-HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B) {
+HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B, const SqSizes& sq) {
   HostWs h;
   size_t o = 0;
   auto take = [&](size_t n) {
@@ -272,7 +686,7 @@ HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B) {
   h.vals = (uint64_t*)take(8 * (size_t)T_tot * B);
   h.out = (uint64_t*)take(8 * (size_t)T_tot * B);
   h.status = (int32_t*)take(4 * (size_t)F);
-  h.inner_bytes = carve(nullptr, T_tot, F, B, 0).bytes;
+  h.inner_bytes = carve(nullptr, T_tot, F, B, 0, sq).bytes;
   h.inner = take(h.inner_bytes);
   h.bytes = o;
   return h;
@@ -293,7 +707,7 @@ void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T
   wc.st_pre += f0;
   const int Fc = f1 - f0;
   run_eval_nodes(exps + a * nv, n, nv, anchors, k, nodes + a, st);
-  run_solve(wc, nodes, Fc, T_tot, tmax, vals, B, s0, k, out, st);
+  run_solve(wc, h_offsets + f0, nodes, Fc, T_tot, tmax, vals, B, s0, k, out, st);
   run_newton(wc, samples, B, out + a, n, T_tot, k, basis, out + a, st, true);
   ++g_launches, k_status_finish<<<(Fc + 255) / 256, 256, 0, st>>>(nullptr, wc.st_solve, wc.st_newton, Fc, status + f0);
 }
@@ -346,7 +760,7 @@ const char* zippel_strerror(int code) {
 size_t zippel_workspace_bytes(const int64_t* h_offsets, int F, int B, int flags) {
   int64_t T_tot, tmax;
   if (!check_offsets(h_offsets, F, &T_tot, &tmax) || B <= 0 || B > ZP_MAX_B) return 0;
-  return carve(nullptr, T_tot, F, B, flags).bytes;
+  return carve(nullptr, T_tot, F, B, flags, sq_sizes(h_offsets, F, B)).bytes;
 }
 
 int zippel_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t* anchors, uint64_t p,
@@ -367,11 +781,12 @@ int vandermonde_solve_batch(const uint64_t* nodes, const int64_t* h_offsets, int
   if (!nodes || !vals || !coefs || !status || B <= 0 || B > ZP_MAX_B || (s0 != 0 && s0 != 1) || !make_mod(p, &k) ||
       !check_offsets(h_offsets, F, &T_tot, &tmax))
     return ZP_ERR_ARG;
-  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
-  const Ws w = carve(workspace, T_tot, F, B, 0);
+  const SqSizes sq = sq_sizes(h_offsets, F, B);
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0, sq).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0, sq);
   cudaStream_t st = (cudaStream_t)stream;
   upload_offsets(w, h_offsets, F, st);
-  run_solve(w, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
+  run_solve(w, h_offsets, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
   ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(nullptr, w.st_solve, nullptr, F, status);
   return cuda_ok();
 }
@@ -383,10 +798,8 @@ int newton_interp_batch(const uint64_t* samples, int B, const uint64_t* vals, in
   if (!samples || !vals || !out || !status || B <= 0 || B > ZP_MAX_B || n <= 0 || ld < n || (basis != 0 && basis != 1) ||
       !make_mod(p, &k))
     return ZP_ERR_ARG;
-  const int64_t one[2] = {0, 1};
   if (!ws_ok(workspace, workspace_bytes, carve(nullptr, 1, 1, B, 0).bytes)) return ZP_ERR_WORKSPACE;
   const Ws w = carve(workspace, 1, 1, B, 0);
-  (void)one;
   cudaStream_t st = (cudaStream_t)stream;
   run_newton(w, samples, B, vals, n, ld, k, basis, out, st, false);
   ++g_launches, k_status_finish<<<1, 32, 0, st>>>(nullptr, nullptr, w.st_newton, 1, status);
@@ -403,8 +816,9 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
       B > ZP_MAX_B || (s0 != 0 && s0 != 1) || (basis != 0 && basis != 1) || !make_mod(p, &k) ||
       !check_offsets(h_offsets, F, &T_tot, &tmax))
     return ZP_ERR_ARG;
-  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0).bytes)) return ZP_ERR_WORKSPACE;
-  const Ws w = carve(workspace, T_tot, F, B, 0);
+  const SqSizes sq = sq_sizes(h_offsets, F, B);
+  if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0, sq).bytes)) return ZP_ERR_WORKSPACE;
+  const Ws w = carve(workspace, T_tot, F, B, 0, sq);
   cudaStream_t st = (cudaStream_t)stream;
   upload_offsets(w, h_offsets, F, st);
   lift_chunk(w, h_offsets, 0, F, T_tot, nv, exps, anchors, samples, B, s0, vals, k, basis, out,
@@ -415,7 +829,7 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
 size_t zippel_host_workspace_bytes(const int64_t* h_offsets, int F, int nv, int B) {
   int64_t T_tot, tmax;
   if (!check_offsets(h_offsets, F, &T_tot, &tmax) || B <= 0 || B > ZP_MAX_B || nv <= 0 || nv > ZP_MAX_NV) return 0;
-  return carve_host(nullptr, T_tot, F, nv, B).bytes;
+  return carve_host(nullptr, T_tot, F, nv, B, sq_sizes(h_offsets, F, B)).bytes;
 }
 
 int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int F, int nv,
@@ -428,9 +842,10 @@ int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int 
       B <= 0 || B > ZP_MAX_B || (s0 != 0 && s0 != 1) || (basis != 0 && basis != 1) || !make_mod(p, &k) ||
       !check_offsets(h_offsets, F, &T_tot, &tmax))
     return ZP_ERR_ARG;
-  if (!ws_ok(workspace, workspace_bytes, carve_host(nullptr, T_tot, F, nv, B).bytes)) return ZP_ERR_WORKSPACE;
-  const HostWs h = carve_host(workspace, T_tot, F, nv, B);
-  const Ws w = carve(h.inner, T_tot, F, B, 0);
+  const SqSizes sq = sq_sizes(h_offsets, F, B);
+  if (!ws_ok(workspace, workspace_bytes, carve_host(nullptr, T_tot, F, nv, B, sq).bytes)) return ZP_ERR_WORKSPACE;
+  const HostWs h = carve_host(workspace, T_tot, F, nv, B, sq);
+  const Ws w = carve(h.inner, T_tot, F, B, 0, sq);
   cudaStream_t st = (cudaStream_t)stream;
   Pipe* P = get_pipe();
   if (!P) return ZP_ERR_CUDA;
@@ -508,23 +923,24 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
     const zp_part* q = parts[x];
     if (!q->exps || !q->skel || !q->uvals || !q->out || !check_offsets(q->h_offsets, F, &T_tot[x], &tmax[x]))
       return ZP_ERR_ARG;
-    if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot[x], F, B, ZP_WS_BALANCED).bytes)) return ZP_ERR_WORKSPACE;
+    if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot[x], F, B, ZP_WS_BALANCED, sq_sizes(q->h_offsets, F, B)).bytes))
+      return ZP_ERR_WORKSPACE;
   }
   cudaStream_t st = (cudaStream_t)stream;
   for (int x = 0; x < 2; ++x) {  // the two parts run back to back on the stream and reuse the workspace
     const zp_part* q = parts[x];
-    const Ws w = carve(workspace, T_tot[x], F, B, ZP_WS_BALANCED);
+    const Ws w = carve(workspace, T_tot[x], F, B, ZP_WS_BALANCED, sq_sizes(q->h_offsets, F, B));
     upload_offsets(w, q->h_offsets, F, st);
     ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
     run_eval_nodes(q->exps, T_tot[x], nv, anchors, k, w.nodes, st);
     run_power_sums(w, w.nodes, F, T_tot[x], tmax[x], q->skel, 1, s0, k, w.R, st);
     int64_t blocks = (T_tot[x] + 255) / 256;
-    if (blocks > 148 * 32) blocks = 148 * 32;
+    if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     {
       ProfScope prof(ZP_K_BALANCE, st);
       ++g_launches, k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
     }
-    run_solve(w, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
+    run_solve(w, q->h_offsets, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
     run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st, true);
     ++g_launches, k_status_finish<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, w.st_solve, w.st_newton, F, status + (size_t)x * F);
   }
@@ -548,7 +964,7 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
   const size_t smem = 8 * 2 * (size_t)(T + 2) * ZP_K8_THREADS;  // two columns per lane
   cudaFuncSetAttribute(k_thiele, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   int64_t blocks = (n + ZP_K8_THREADS - 1) / ZP_K8_THREADS;
-  if (blocks > 148 * 64) blocks = 148 * 64;
+  if (blocks > sm_count() * 64) blocks = sm_count() * 64;
   ++g_launches, k_thiele<<<(unsigned)blocks, ZP_K8_THREADS, smem, st>>>(xd, xm, w.st_newton, T, vals, n, ld, k, num, den,
                                                                          degs, cf, status);
   return cuda_ok();
@@ -597,7 +1013,7 @@ int crt_rational_reconstruct_batch(const uint64_t* r1, const uint64_t* r2, int64
     e >>= 1;
   }
   int64_t blocks = (n + 255) / 256;
-  if (blocks > 148 * 32) blocks = 148 * 32;
+  if (blocks > sm_count() * 32) blocks = sm_count() * 32;
   ++g_launches, k_crt_rational<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
       r1, r2, n, p1, k2, inv, (uint64_t)(m >> 64), (uint64_t)m, (uint64_t)N, num, den, status);
   return cuda_ok();
@@ -616,30 +1032,34 @@ int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
   return ZP_OK;
 }
 
-int zippel_modarith_selftest(int op, const uint64_t* a, const uint64_t* b, int64_t n, uint64_t p, uint64_t* out,
-                             void* stream) {
-  ZpMod k;
-  if (!a || !out || n <= 0 || op < 0 || op > 6 || !make_mod(p, &k) || ((op <= 3 || op >= 5) && !b)) return ZP_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (op == 5) {
-    ++g_launches, k_modarith_selftest<<<1, 256, 0, st>>>(op, a, b, n, k, out);
-  } else {
-    int64_t blocks = (n + 255) / 256;
-    if (blocks > 148 * 8) blocks = 148 * 8;
-    ++g_launches, k_modarith_selftest<<<(unsigned)blocks, 256, 0, st>>>(op, a, b, n, k, out);
+int zippel_shutdown(void) {
+  for (int dev = 0; dev < 16; ++dev) {
+    Pipe& P = g_pipe[dev];
+    if (!P.ready) continue;
+    cudaSetDevice(dev);
+    cudaStreamDestroy(P.s_in);
+    cudaStreamDestroy(P.s_out);
+    cudaEventDestroy(P.ev_start);
+    cudaEventDestroy(P.ev_end);
+    for (int c = 0; c < ZP_PIPE_MAX_CHUNKS; ++c) {
+      cudaEventDestroy(P.ev_in[c]);
+      cudaEventDestroy(P.ev_done[c]);
+    }
+    P = Pipe();
   }
   return cuda_ok();
 }
 
-int zippel_ubench(int kind, int iters, int blocks, uint64_t p, uint64_t* out, double* h_chain_steps, void* stream) {
-  ZpMod k;
-  if (kind < 0 || kind > 21 || iters <= 0 || blocks <= 0 || !out || !make_mod(p, &k)) return ZP_ERR_ARG;
-  cudaStream_t st = (cudaStream_t)stream;
-#define ZP_UB(K) case K: ++g_launches, k_ubench<K><<<blocks, ZP_UB_THREADS, 0, st>>>(iters, k, out); break;
-  switch (kind) { ZP_UB(0) ZP_UB(1) ZP_UB(2) ZP_UB(3) ZP_UB(4) ZP_UB(5) ZP_UB(6) ZP_UB(7) ZP_UB(8) ZP_UB(9) ZP_UB(10) ZP_UB(11) ZP_UB(12) ZP_UB(13) ZP_UB(14) ZP_UB(15) ZP_UB(16) ZP_UB(17) ZP_UB(18) ZP_UB(19) ZP_UB(20) ZP_UB(21) }
-#undef ZP_UB
-  if (h_chain_steps) *h_chain_steps = (double)blocks * ZP_UB_THREADS * (double)iters * 8.0 * ZP_UB_CH;
-  return cuda_ok();
+int zippel_set_tuning(int key, int64_t value) {
+  if (key == ZP_TUNE_SUBQ_MIN_T && value > 0) {
+    g_subq_min_t = value;
+    return ZP_OK;
+  }
+  return ZP_ERR_ARG;
 }
+
+#ifdef ZP_TEST_HOOKS
+#include "test_hooks.cuh"
+#endif
 
 }  // extern "C"

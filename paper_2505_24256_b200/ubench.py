@@ -13,7 +13,7 @@ import subprocess
 
 import torch
 
-from . import api
+from . import api, testhooks
 
 P = (1 << 63) - 25
 KINDS = [
@@ -56,7 +56,7 @@ def main():
         for r in range(a.reps + 1):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(st)
-            n = api.zippel_ubench(kind, a.iters, blocks, P, out, stream=st)
+            n = testhooks.zippel_ubench(kind, a.iters, blocks, P, out, stream=st)
             e1.record(st)
             if r == a.reps // 2:
                 clk = sm_clock()

@@ -170,20 +170,26 @@ class RationalWorkload:
     meta: dict = field(default_factory=dict)
 
 
-def make_rational_workload(name: str, seed: int, F: int, nvars: int, t_num: int, t_den: int,
+def make_rational_workload(name: str, seed: int, F: int, nvars: int, t_num, t_den,
                            total: int, B: int, p: int = P63, s0: int = 0,
                            with_vals: bool = True) -> RationalWorkload:
+    """t_num, t_den: terms of every numerator / denominator, an int or a per-function list (ragged batches)."""
     nv = nvars - 1
     anchors = uniform_residues(_rng(seed, 3), 2, p, nv)
     samples = distinct_residues(_rng(seed, 4), 2, p, B)
     parts = []
+    tmax = 0
     for part, t, stream in (("num", t_num, 10), ("den", t_den, 20)):
-        offsets = np.arange(F + 1, dtype=np.int64) * t
-        T_tot = F * t
+        ts = [int(t)] * F if np.isscalar(t) else [int(x) for x in t]
+        assert len(ts) == F
+        tmax = max(tmax, max(ts))
+        offsets = np.zeros(F + 1, dtype=np.int64)
+        offsets[1:] = np.cumsum(ts)
+        T_tot = int(offsets[-1])
         r_exp = _rng(seed, stream + 1)
         full = np.empty((T_tot, nvars), dtype=np.uint16)
         for f in range(F):
-            full[f * t:(f + 1) * t] = simplex_rows(r_exp, t, nvars, total)
+            full[offsets[f]:offsets[f + 1]] = simplex_rows(r_exp, ts[f], nvars, total)
         exps = np.ascontiguousarray(full[:, :nv])
         xk_exp = full[:, nv].astype(np.int64)
         if xk_exp.max() >= B:
@@ -195,8 +201,8 @@ def make_rational_workload(name: str, seed: int, F: int, nvars: int, t_num: int,
         w.meta["skel_standin"] = uniform_residues(_rng(seed, stream + 7), 1, p, T_tot) if with_vals else None
         parts.append(w)
     num, den = parts
-    low = np.array([lowest_monomial(den.exps[f * t_den:(f + 1) * t_den]) for f in range(F)], dtype=np.int64)
-    h = uniform_residues(_rng(seed, 30), 1, p, max(t_num, t_den))
+    low = np.array([lowest_monomial(den.exps[den.offsets[f]:den.offsets[f + 1]]) for f in range(F)], dtype=np.int64)
+    h = uniform_residues(_rng(seed, 30), 1, p, tmax)
     return RationalWorkload(name, num, den, low, h, None, {"seed": seed})
 
 

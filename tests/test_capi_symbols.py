@@ -9,11 +9,11 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "zippel.h")).read()
+def declared_symbols(header="zippel.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"^\s*(?:const\s+char\s*\*|size_t|int|unsigned long long)\s+([a-z_0-9]+)\s*\(", src, flags=re.M)
-    assert len(names) >= 9
+    names = re.findall(r"^\s*(?:const\s+char\s*\*|size_t|int|void|unsigned long long)\s+([a-z_0-9]+)\s*\(", src, flags=re.M)
+    assert len(names) >= 6
     return names
 
 
@@ -28,6 +28,40 @@ def test_library_exports_every_declared_symbol():
     for must in ("zippel_eval_nodes", "vandermonde_solve_batch", "newton_interp_batch", "zippel_lift_step",
                  "balanced_zippel_lift_step"):  # BASELINE.json north_star
         assert must in names
+
+
+def test_test_library_exports_every_declared_symbol():
+    """include/zippel_test.h: the test build has the hooks AND the product's entry points; the product has no hook."""
+    from paper_2505_24256_b200 import api, testhooks
+
+    T = testhooks.lib()
+    hooks = declared_symbols("zippel_test.h")
+    assert set(hooks) == set(testhooks.EXPORTS)
+    for n in hooks + declared_symbols():
+        assert hasattr(T, n), n
+    L = api.lib()
+    for n in hooks:
+        assert not hasattr(L, n), f"the product library exports the test hook {n}"
+
+
+def test_long_skeleton_workspace_and_limits():
+    """Host logic of the sub-quadratic route (no device): the workspace grows when a function crosses the
+    threshold, shrinks back when the threshold is raised, and a function of 2^23 terms is refused."""
+    from paper_2505_24256_b200 import api
+
+    L = api.lib()
+    offs = np.array([0, 1000, 21000, 22000], dtype=np.int64)  # short, long, short
+    base = L.zippel_workspace_bytes(offs.ctypes.data, 3, 3, 0)
+    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 1 << 22) == api.ZP_OK
+    quad = L.zippel_workspace_bytes(offs.ctypes.data, 3, 3, 0)
+    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 8192) == api.ZP_OK
+    assert quad < base and quad % 256 == 0
+    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 0) == api.ZP_ERR_ARG
+    assert L.zippel_set_tuning(99, 1) == api.ZP_ERR_ARG
+    big = np.array([0, 1 << 23], dtype=np.int64)
+    assert L.zippel_workspace_bytes(big.ctypes.data, 1, 1, 0) == 0
+    ok = np.array([0, (1 << 23) - 1], dtype=np.int64)
+    assert L.zippel_workspace_bytes(ok.ctypes.data, 1, 1, 0) > 0
 
 
 def test_host_side_checks_without_device():

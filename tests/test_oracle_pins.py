@@ -368,8 +368,19 @@ def test_batched_planted_recovery_ragged():
 
 
 # ---------------------------------------------------------------------------- balanced (eq. 4)
-def test_balanced_recovers_C_times_planted_and_cross_multiplied_probes():
-    rw = wl.config(4, F=3, t=30)  # t_num = 30, t_den = 12
+def ragged_rational(s0):
+    """Three rational functions of different sizes (numerators 30 / 7 / 19 terms, denominators 12 / 1 / 9)."""
+    return wl.make_rational_workload("rag4", wl.SEED_BASE + 44, 3, 6, [30, 7, 19], [12, 1, 9], 24, 25, s0=s0)
+
+
+@pytest.mark.parametrize("s0", [0, 1])
+@pytest.mark.parametrize("ragged", [False, True])
+def test_balanced_recovers_C_times_planted_and_cross_multiplied_probes(s0, ragged):
+    """eq. (4) (readings G3, G20) with probes at the powers s0 .. s0 + t - 1 (reading G1: s0 = 1
+    divides by m_i at the end) and with functions of different lengths in one batch (the per-probe factor h_s is
+    shared by numerator and denominator: the numerator uses s < t_N, the denominator s < t_D)."""
+    rw = ragged_rational(s0) if ragged else wl.config(4, F=3, t=30)  # t_num = 30, t_den = 12
+    rw.num.s0 = rw.den.s0 = s0
     p = rw.num.p
     c0 = int(rw.num.samples[0])
     parts, Cs = {}, None
@@ -391,7 +402,7 @@ def test_balanced_recovers_C_times_planted_and_cross_multiplied_probes():
                     u[j, o + s] = int(true_vals[j, o + s]) * int(rw.h[s]) % p
         parts[name] = dict(exps=w.exps, offsets=w.offsets, skel=skel, uvals=u)
     on, od, status = ref.balanced_zippel_lift_step(parts["num"], parts["den"], rw.num.anchors, rw.num.samples, p,
-                                                   0, basis=1)
+                                                   s0, basis=1)
     assert not status.any()
     for name, w, out in (("num", rw.num, on), ("den", rw.den, od)):
         a0 = ref.poly_rows_eval(w.samples, out, p)[0]
@@ -410,6 +421,25 @@ def test_balanced_recovers_C_times_planted_and_cross_multiplied_probes():
         lhs = eval_planted(rw.num, on, f, z) * eval_planted(rw.den, rw.den.planted, f, z) % p
         rhs = eval_planted(rw.num, rw.num.planted, f, z) * eval_planted(rw.den, od, f, z) % p
         assert lhs == rhs
+
+
+def test_eval_sparse_vs_python():
+    """ref_eval_sparse (the fresh-probe evaluator) against Python integers: random rows, a zero
+    exponent row, the largest exponent 65535, a zero coordinate, one term, and a small prime."""
+    r = random.Random(31)
+    for p in (101, 65537, P63):
+        for t, nv in ((1, 1), (7, 3), (40, 6)):
+            exps = np.array([[r.choice([0, 1, 2, 5, 40, 65535]) for _ in range(nv)] for _ in range(t)], dtype=np.uint16)
+            exps[0, :] = 0  # the constant term
+            coef = np.array([r.randrange(p) for _ in range(t)], dtype=np.uint64)
+            for point in ([r.randrange(p) for _ in range(nv)], [0] * nv, [p - 1] * nv, [1] + [r.randrange(p) for _ in range(nv - 1)]):
+                want = 0
+                for row, c in zip(exps, coef):
+                    term = int(c)
+                    for e, z in zip(row, point):
+                        term = term * pow(int(z), int(e), p) % p  # Python: 0 ** 0 == 1, as in the polynomial ring
+                    want += term
+                assert ref.eval_sparse(exps, coef, np.array(point, dtype=np.uint64), p) == want % p
 
 
 def test_balanced_zero_pivot_status():
