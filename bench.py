@@ -38,7 +38,7 @@ UNIT = "terms/s"
 # 64 lanes/clk/SM of the 32-bit low multiply-add (IMAD) and 32 lanes/clk/SM of anything that needs the
 # 64-bit product (IMAD.WIDE, IMAD.HI).  Unit = one lane-cycle of that pipe's 64-lane issue rate:
 # IMAD = 1 unit, a 32x32->64 product = 2 units.  peak = 148 SMs x 64 units/clk x 1.965 GHz.
-IMAD_PEAK_TOPS = 148 * 64 * 1.965e9 / 1e12
+IMAD_PEAK_TOPS = 148 * 64 * 1.965e9 / 1e12  # planning figure; run_ours() re-derives it from the device (imad_peak)
 # algorithmic cost of the method's two primitives in those units (cheapest known generic-p forms):
 #   modular multiply-add x <- m x + a : 6 wide + 4 low = 16 ; deferred 64x64 MAC : 4 wide = 8
 C_MM, C_MAC = 16, 8
@@ -46,18 +46,35 @@ C_MM, C_MAC = 16, 8
 C_MM_INSTR, C_MAC_INSTR = 10, 4
 
 
+def imad_peak(device_index=0, sm_max_mhz=None):
+    """T units/s = SMs (cudaDeviceProp) x 64 lanes/clk x max SM clock (nvidia-smi clocks.max.sm as sampled during the
+    run, else cudaDeviceProp's clock rate)."""
+    import torch
+
+    pr = torch.cuda.get_device_properties(device_index)
+    mhz = sm_max_mhz
+    src = "nvidia-smi clocks.max.sm"
+    if not mhz:
+        khz = getattr(pr, "clock_rate", 0)
+        mhz, src = (khz / 1e3, "cudaDeviceProp.clockRate") if khz else (1965.0, "B200_PROFILING.md clocks.max.sm")
+    return pr.multi_processor_count * 64 * mhz * 1e6 / 1e12, f"{pr.multi_processor_count} SMs x 64 lanes/clk x {mhz:.0f} MHz ({src})"
+
+
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6, 7, 8],
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6, 7, 8, 9],
                     help="1-5: BASELINE.json configs; 6: batched Thiele reconstruction (row f2), C4's input side; "
-                         "7: skeleton extension (row f1) on C2's output; 8: two-prime CRT + rational reconstruction (row f4)")
+                         "7: skeleton extension (row f1) on C2's output; 8: two-prime CRT + rational reconstruction (row f4); "
+                         "9: one solve at the paper's largest skeleton, t = 4.8e6, B = 1 (PAPER.md L250; row f3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra-legs", action="store_true",
+                    help="default config only: skip the C5 and C1 legs attached to the line as \"c5\" and \"c1\"")
     return ap.parse_args()
 
 
@@ -125,8 +142,64 @@ def load_workload(idx: int, seed_shift: int, F_override):
                                 sh["emax"], sh["B"], with_planted=False)
 
 
+# the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_LEAF, g_subq_min_t)
+SQ_LEAF, SQ_MIN_T, SQ_KB = 1024, 8192, 1024
+C_MONT = 18  # Montgomery product: 8 wide + 2 low
+
+
+def subq_units(t, B):
+    """Algorithmic multiplier-pipe units of the sub-quadratic solve of ONE function of t terms with B right-hand sides,
+    counted on the plan csrc/zippel_capi.cu:sq_solve executes: a length-n transform modulo one prime = (n/2) log2 n
+    butterflies of one Shoup product (16 units); a pointwise product = 2 Montgomery products per prime; Garner CRT +
+    reduction modulo p = 5 Montgomery products per coefficient; the leaves are the quadratic node solve with B + 1
+    right-hand sides.  Returns (total, parts)."""
+    from math import ceil, log2
+
+    ntt = lambda n: 3 * (n / 2) * log2(n) * C_MM  # three primes
+    pw = lambda n: 3 * n * 2 * C_MONT
+    crt = lambda n: n * 5 * C_MONT
+    V = B + 1
+    nlev = max(0, ceil(log2(ceil(t / SQ_LEAF))))
+    up = down = 0.0
+    for l in range(nlev):
+        a = SQ_LEAF << l
+        n = 2 * a
+        pairs, base = [], 0
+        while base + a < t:
+            pairs.append(min(a, t - base - a))
+            base += 2 * a
+        P = len(pairs)
+        outs = sum(a + b for b in pairs)
+        up += P * (3 * ntt(n) + pw(n)) + crt(outs)
+        down += P * 2 * ntt(n) + V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(outs))
+    newton = sum(1.5 * k * k * C_MAC for k in (1 << i for i in range(10)))  # schoolbook base case to x^1024
+    kk = SQ_KB
+    while kk < t:
+        n = 2 * kk
+        newton += 5 * ntt(n) + 2 * pw(n) + crt(2 * kk)
+        kk <<= 1
+    nr = 1 << ceil(log2(2 * t))
+    root = 3 * ntt(nr) + pw(nr) + crt(t)
+    leaf_t2 = sum(min(SQ_LEAF, t - x) ** 2 for x in range(0, t, SQ_LEAF))
+    leaves = leaf_t2 * (C_MAC / 2 + C_MM + V * C_MAC)  # in-leaf product tree + node solve with B + 1 right-hand sides
+    fin = t * (3 + B + 2) * C_MONT
+    parts = {"up_tree": up, "power_sums_of_nodes (Newton inverse + root product)": newton + root, "down_tree": down,
+             "leaves": leaves, "final_division": fin}
+    return sum(parts.values()), parts
+
+
 def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
     """Algorithmic multiplier-pipe units (SURVEY.md 8(d).4 formula), total and for the node-solve kernel."""
+    long_ts = [int(t) for t in ts if int(t) >= SQ_MIN_T]
+    if long_ts:  # sub-quadratic route for the long functions, the quadratic formula for the rest
+        short = [int(t) for t in ts if int(t) < SQ_MIN_T]
+        tot_s, ns_s = work_model(short, B, nv, newton, balanced, c_mm, c_mac) if short else (0.0, 0.0)
+        T = float(sum(long_ts))
+        sq = sum(subq_units(t, B)[0] for t in long_ts)
+        total = sq + c_mm * (nv - 1) * T + (c_mm * T * B * (B - 1) / 2 if newton else 0.0)
+        if balanced:
+            total += c_mac * float(sum(t * t for t in long_ts))
+        return tot_s + total, ns_s + sq
     t2 = float(sum(int(t) * int(t) for t in ts))
     T = float(sum(int(t) for t in ts))
     # per (node, stage): one modular multiply-add (the quotient), B deferred MACs, one more MAC for the denominator
@@ -143,25 +216,15 @@ def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
 
 
 # ---------------------------------------------------------------------------------------- ours
-def run_ours(args):
+def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=True):
+    """One configuration: W warm-up steps, K timed steps on resident inputs, then (optionally) the same through the
+    host-buffer entry.  Returns the fields of the JSON line (every rank returns; ms is the max over ranks)."""
     import torch
 
     from paper_2505_24256_b200 import api, sharding
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        import torch.distributed as dist
-
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    torch.cuda.set_device(local)
-    api.lib()
-    idx = args.config
-    w = load_workload(idx, sharding.rank_seed_shift(rank), args.F)
+    w = load_workload(idx, sharding.rank_seed_shift(rank), F_override)
     stream = torch.cuda.Stream()
-    K, W = args.steps, args.warmup
 
     # ---- resident inputs and the step closure --------------------------------------------------
     if idx == 4:
@@ -183,6 +246,7 @@ def run_ours(args):
                                           stream=stream)
         total_ops, _ = work_model(ts, B, nv, True, True)
         _, ns_ops = work_model([500] * F, B, nv, True, True)  # the hook times the numerator part's node solve
+        ns_ts = [500] * F
         workload = f"C4 balanced lift 5->6 vars: F={F} rational functions, t_N=500, t_D=200, B=25"
         in_bytes = sum(q.exps.nbytes + q.vals.nbytes + q.meta["skel_standin"].nbytes for q in parts)
         out_bytes = sum(q.vals.nbytes for q in parts)
@@ -193,7 +257,7 @@ def run_ours(args):
         out = torch.empty_like(vals)
         status = torch.empty(F, dtype=torch.int32, device="cuda")
         ws = api.alloc_workspace(w.offsets, B)
-        newton = idx != 5
+        newton = idx not in (5, 9)
         if newton:
             def step():
                 api.zippel_lift_step(exps, w.offsets, anchors, samples, vals, p, 0, 1, out=out, status=status,
@@ -206,10 +270,13 @@ def run_ours(args):
                 api.vandermonde_solve_batch(nodes, w.offsets, vals, p, 0, out=out, status=status, workspace=ws,
                                             stream=stream)
         total_ops, ns_ops = work_model(ts, B, nv, newton, False)
+        ns_ts = ts
         workload = (f"C{idx} {'lift' if newton else 'solve'}: F={F}, t={int(ts.max())}, nv={nv}, B={B}"
-                    + (" (BASELINE.json configs[1])" if idx == 2 and not args.F else ""))
+                    + (" (BASELINE.json configs[1])" if idx == 2 and not F_override else "")
+                    + (" (PAPER.md L250: the largest skeleton, 4.8m monomials)" if idx == 9 else ""))
         in_bytes = w.exps.nbytes + w.vals.nbytes + w.anchors.nbytes + w.samples.nbytes
         out_bytes = w.vals.nbytes + 4 * F
+    subq = int(max(ts)) >= SQ_MIN_T
 
     def barrier():
         if world > 1:
@@ -228,7 +295,7 @@ def run_ours(args):
         for a, b in ev_k:
             a.record(stream); b.record(stream)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        sampler = ClockSampler(local) if rank == 0 else None
+        sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None
         time.sleep(0.3 if sampler else 0.0)
         barrier()
         torch.cuda.synchronize()
@@ -254,7 +321,7 @@ def run_ours(args):
 
     # ---- e2e: host (pinned) buffers through the host-buffer C-ABI call ---------------------------
     e2e = None
-    if not args.no_e2e and idx != 4 and idx != 5:
+    if want_e2e and idx not in (4, 5, 9):
         pin = lambda a: torch.from_numpy(a.view(np.int64) if a.dtype == np.uint64 else a.view(np.int16)).pin_memory()
         h_exps, h_anch, h_samp, h_vals = pin(w.exps), pin(w.anchors), pin(w.samples), pin(w.vals)
         h_out = torch.empty(w.vals.shape, dtype=torch.int64).pin_memory()
@@ -281,53 +348,96 @@ def run_ours(args):
                "h2d_bytes_per_step": int(in_bytes), "d2h_bytes_per_step": int(out_bytes),
                "call": "zippel_lift_step_host (pinned host buffers; chunked H2D / step / D2H pipeline on 3 streams + stream sync per step)"}
 
-    if rank != 0:
-        if world > 1:
-            import torch.distributed as dist
-
-            dist.destroy_process_group()
-        return
-
-    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) -------------------------
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        cpu = oracle_sample(idx, steps=1)
-
+    peak, peak_how = imad_peak(local, clocks.get("sm_max_mhz") if clocks else None)
     achieved = ns_ops / (ns_ms * 1e-3) / 1e12
-    ns_ops_instr = float(sum(int(t) ** 2 for t in (ts if idx != 4 else [500] * F))) * (2 * C_MM_INSTR + B * C_MAC_INSTR)  # SURVEY.md 8(d).4 accounting
+    ns_ops_instr = float(sum(int(t) ** 2 for t in ns_ts)) * (2 * C_MM_INSTR + B * C_MAC_INSTR)  # SURVEY.md 8(d).4 accounting
+    if subq:
+        kernel = "sub-quadratic solve after the product tree: tails down the tree (k_ntt_* passes, pointwise, CRT), leaf k_node_solve, k_inv_finish"
+        cost = ("W_alg of the sub-quadratic route (bench.py subq_units, DESIGN.md section 12): butterfly = one Shoup product = 16 units, "
+                "pointwise = 2 Montgomery products (36), CRT + reduction = 5 (90), leaves = quadratic node solve with B + 1 right-hand sides")
+    elif idx == 5 or (B == 1 and int(min(ts)) >= 4096):
+        kernel, cost = "k_corr_w + k_node_eval2", "per (node, stage) 8 (2 + 1/2) units: two evaluations by deferred MACs + the correlation"
+    else:
+        kernel = "k_node_den + k_node_solve" + (" (numerator part)" if idx == 4 else "")
+        cost = "modular multiply-add = 16 units (6 wide + 4 low), deferred 64x64 MAC = 8 units (4 wide); per (node, stage) 16 + 8 (B + 1)"
+    quad_equiv = float(sum(int(t) ** 2 for t in ts)) * (C_MM + (B + 1) * C_MAC + C_MAC / 2)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": workload, "p": "2^63-25", "basis": "monomial", "functions_per_gpu": int(F),
                    "terms_per_gpu": int(T_tot), "l2": "inputs larger than L2 (688 MB of values per step)" if idx == 2
-                   else "inputs smaller than L2; compute-bound kernels (see DESIGN.md)", "parallelism": f"dp{world}"},
+                   else "inputs smaller than L2; compute-bound kernels (see DESIGN.md)", "parallelism": f"dp{world}",
+                   "route": "sub-quadratic (three-prime NTT product tree)" if subq else "quadratic (PAPER.md section 2.2)"},
         "lift_steps_per_s": F * world / (ms_per_step * 1e-3),
         "credited_modmuls_per_s": B * float(sum(int(t) ** 2 for t in ts)) * world / (ms_per_step * 1e-3),
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {
-            "bound": "alu", "kernel": ("k_corr_w + k_node_eval2" if idx == 5 else "k_node_den + k_node_solve") + (" (numerator part)" if idx == 4 else ""),
-            "achieved": achieved, "peak": IMAD_PEAK_TOPS,
-            "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
-            # dram__bytes_read.sum + dram__bytes_write.sum of this launch from the ncu --set full capture of the same
-            # command (profiles/r01_final.md): 892.5 + 660.8 MB; algorithmic 1540 MB.  Only known for the default config.
-            "traffic": 1553.3e6 if (idx == 2 and not args.F) else None,
-            "peak_source": "derived (DESIGN.md Roofline): 148 SM x 64 lanes/clk of the fma-heavy pipe x 1.965 GHz; "
-                           "profiles/r01_baseline.md measures IMAD at 63.5 and IMAD.WIDE at 31.8 lanes/clk/SM",
+            "bound": "alu", "kernel": kernel, "achieved": achieved, "peak": peak,
+            "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / peak,
+            # dram__bytes_read.sum + dram__bytes_write.sum of the k_node_solve<21> launch from an ncu --set full capture of
+            # the same command; algorithmic 1540 MB.  Only known for the default config; not measured in this run.
+            "traffic": 1553.3e6 if (idx == 2 and not F_override) else None,
+            "traffic_source": "ncu --set full capture of the same command (profiles/r01_final.md: 892.5 MB read + 660.8 MB written), not this run"
+                              if (idx == 2 and not F_override) else None,
+            "peak_source": "derived (DESIGN.md 5.1): " + peak_how + "; profiles/r01_baseline.md measures IMAD at 63.5 and "
+                           "IMAD.WIDE at 31.8 lanes/clk/SM",
+            "frac_is": "multiplier-pipe utilisation of the formulation built (the algorithmic operation count in pipe units)",
             "algorithmic_ops_per_launch": ns_ops, "ms_per_launch": ns_ms,
-            "algorithmic_cost": "modular multiply-add = 16 units (6 wide + 4 low), deferred 64x64 MAC = 8 units (4 wide); per (node, stage) 16 + 8 (B + 1), for B = 1: 8 (2 + 1/2)",
-            "whole_step_frac": total_ops / (ms_per_step * 1e-3) / 1e12 / IMAD_PEAK_TOPS,
-            "frac_instr_count_10_4": ns_ops_instr / (ns_ms * 1e-3) / 1e12 / IMAD_PEAK_TOPS,
+            "algorithmic_cost": cost,
+            "whole_step_frac": total_ops / (ms_per_step * 1e-3) / 1e12 / peak,
         },
         "e2e": e2e,
-        "cpu_baseline": cpu,
     }
+    if subq:
+        line["roofline"]["speedup_vs_quadratic_work"] = quad_equiv / total_ops
+        line["roofline"]["quadratic_equivalent_frac"] = quad_equiv / (ms_per_step * 1e-3) / 1e12 / peak
+    else:
+        line["roofline"]["frac_instr_count_10_4"] = ns_ops_instr / (ns_ms * 1e-3) / 1e12 / peak
+    return line
+
+
+def run_ours(args):
+    import torch
+
+    from paper_2505_24256_b200 import api
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    api.lib()
+    idx = args.config
+    line = run_leg(idx, args.steps, args.warmup, args.F, not args.no_e2e, rank, world, local)
+    # the default line carries the other half of north_star's target (the t = 2^19 solve, configs[4]) and the latency
+    # of the small case (configs[0]) as sub-objects; every rank runs them (the barriers inside match), rank 0 prints
+    if idx == 2 and not args.F and not args.no_extra_legs:
+        c5 = run_leg(5, 10, 3, None, False, rank, world, local)
+        line["c5"] = {k: c5[k] for k in ("value", "unit", "ms_per_step", "steps", "warmup", "gpu_launches", "clocks", "roofline")}
+        line["c5"]["workload"] = c5["config"]["workload"] + "; " + c5["config"]["route"]
+        c1 = run_leg(1, 200, 10, None, True, rank, world, local)
+        line["c1"] = {"workload": c1["config"]["workload"], "us_per_step": c1["ms_per_step"] * 1e3, "steps": 200, "warmup": 10,
+                      "launches_per_step": c1["gpu_launches"] / 200, "e2e_us_per_step": c1["e2e"]["ms_per_step"] * 1e3,
+                      "lift_steps_per_s": c1["lift_steps_per_s"], "clocks": c1["clocks"]}
+    if rank != 0:
+        if world > 1:
+            import torch.distributed as dist
+
+            dist.destroy_process_group()
+        return
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only) -------------------------
+    line["cpu_baseline"] = oracle_sample(idx, steps=1, all_cores=True) if (world == 1 and not args.no_cpu_baseline) else None
     print(json.dumps(line))
 
 
 # ---------------------------------------------------------------------------------------- oracle legs
-SAMPLE = {1: dict(), 2: dict(F=32), 3: dict(t=6000), 4: dict(F=24), 5: dict(t=1 << 14)}
+SAMPLE = {1: dict(), 2: dict(F=32), 3: dict(t=6000), 4: dict(F=24), 5: dict(t=1 << 14), 9: dict(t=1 << 14)}
 
 
 def oracle_step(idx, w):
@@ -338,7 +448,7 @@ def oracle_step(idx, w):
                  for n, q in (("num", w.num), ("den", w.den))}
         ref.balanced_zippel_lift_step(parts["num"], parts["den"], w.num.anchors, w.num.samples, w.num.p, 0, 1)
         return w.num.B * (w.num.T_tot + w.den.T_tot), w.num.F
-    if idx == 5:
+    if idx in (5, 9):
         nodes = ref.eval_nodes(w.exps, w.anchors, w.p)
         ref.vandermonde_solve_batch(nodes, w.offsets, w.vals, w.p, 0)
     else:
@@ -346,7 +456,63 @@ def oracle_step(idx, w):
     return w.B * w.T_tot, w.F
 
 
-def oracle_sample(idx, steps=1, warmup=0):
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def oracle_all_cores(idx):
+    """The oracle on all the host cores this process may use: the unmodified single-threaded
+    routines on independent units from one thread each (ctypes releases the GIL during a call) -- functions for C2 / C4,
+    node ranges after one shared master-polynomial build for the single skeletons.  Returns (terms/s at the sample's t,
+    cores, seconds, description)."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    from oracle import ref
+    from paper_2505_24256_b200 import workloads as wl
+
+    cores = host_cores()
+    if idx in (2, 4):
+        per = 8 if idx == 2 else 6
+        F = cores * per
+        w = wl.config(idx, F=F)
+
+        def unit(c):
+            f0, f1 = c * per, (c + 1) * per
+            if idx == 4:
+                parts = {}
+                for n, q in (("num", w.num), ("den", w.den)):
+                    a, b = int(q.offsets[f0]), int(q.offsets[f1])
+                    parts[n] = dict(exps=np.ascontiguousarray(q.exps[a:b]), offsets=(q.offsets[f0:f1 + 1] - a).copy(),
+                                    skel=np.ascontiguousarray(q.meta["skel_standin"][a:b]), uvals=np.ascontiguousarray(q.vals[:, a:b]))
+                ref.balanced_zippel_lift_step(parts["num"], parts["den"], w.num.anchors, w.num.samples, w.num.p, 0, 1)
+            else:
+                a, b = int(w.offsets[f0]), int(w.offsets[f1])
+                ref.zippel_lift_step(np.ascontiguousarray(w.exps[a:b]), (w.offsets[f0:f1 + 1] - a).copy(), w.anchors, w.samples,
+                                     np.ascontiguousarray(w.vals[:, a:b]), w.p, 0, 1)
+
+        terms = (w.num.B * (w.num.T_tot + w.den.T_tot)) if idx == 4 else w.B * w.T_tot
+        with ThreadPoolExecutor(cores) as ex:
+            ta = time.perf_counter()
+            list(ex.map(unit, range(cores)))
+            dt = time.perf_counter() - ta
+        return terms / dt, cores, dt, f"{F} functions, {per} per thread, {cores} threads"
+    w = wl.config(idx, **SAMPLE[idx])
+    t = w.T_tot
+    with ThreadPoolExecutor(cores) as ex:
+        ta = time.perf_counter()
+        nodes = ref.eval_nodes(w.exps, w.anchors, w.p)
+        M = ref.master_poly(nodes, w.p)  # shared, single thread (t^2 / 2 of the (2 + B) t^2 products)
+        cuts = [t * c // cores for c in range(cores + 1)]
+        list(ex.map(lambda c: ref.node_solve_at(nodes[cuts[c]:cuts[c + 1]], M, w.vals, w.p), range(cores)))
+        dt = time.perf_counter() - ta
+    return w.B * t / dt, cores, dt, (f"{t}-term prefix: nodes and master polynomial on one thread, then the per-node routine "
+                                     f"(PAPER.md L193-195) on {cores} node ranges; the O(t) division and Newton are left out")
+
+
+def oracle_sample(idx, steps=1, warmup=0, all_cores=False):
     """Time the oracle, as it stands (single thread, unsigned __int128 mulmod), on a bounded sample of the
     bench workload.  The metric is terms/s AT THE SAMPLE'S t; for configs 3 and 5 the sample has a shorter
     skeleton, so the value is also given scaled by (t_sample / t_full) (cost per term is linear in t)."""
@@ -367,9 +533,15 @@ def oracle_sample(idx, steps=1, warmup=0):
     desc = {2: "first 32 of the 4096 functions (same t = 1000, B = 21)", 4: "first 24 of the 1024 functions",
             3: "6000-term prefix as a complete problem, value scaled by 6000/100000",
             5: "2^14-term prefix as a complete problem (BASELINE.json), value scaled by 2^14/2^19",
+            9: "2^14-term prefix as a complete problem, value scaled by 2^14/4.8e6",
             1: "the whole config"}[idx]
-    return {"value": terms / dt * scale, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
-            "seconds_per_sample_step": dt, "lift_steps_per_s": F / dt * (scale * scale if scale != 1.0 else 1.0)}
+    out = {"value": terms / dt * scale, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc,
+           "seconds_per_sample_step": dt, "lift_steps_per_s": F / dt * (scale * scale if scale != 1.0 else 1.0)}
+    if all_cores and idx != 1:
+        v, cores, secs, how = oracle_all_cores(idx)
+        out["all_cores"] = {"value": v * scale, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": how,
+                            "seconds": secs, "speedup_over_one_core": v * scale / out["value"]}
+    return out
 
 
 def run_reference(args):

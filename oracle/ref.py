@@ -63,6 +63,8 @@ def lib():
         L.ref_node_quotient.argtypes = [u64p, C.c_int64, u64, u64, u64p]
         L.ref_node_solve.restype = None
         L.ref_node_solve.argtypes = [u64p, u64p, C.c_int64, u64p, C.c_int64, C.c_int, u64, u64p, u64p]
+        L.ref_node_solve_at.restype = None
+        L.ref_node_solve_at.argtypes = [u64p, C.c_int64, u64p, C.c_int64, u64p, C.c_int64, C.c_int, u64, u64p, u64p]
         L.ref_vandermonde_solve_batch.argtypes = [u64p, i64p, C.c_int, u64p, C.c_int, C.c_int, u64, u64p, i32p]
         L.ref_gauss_solve.argtypes = [u64p, C.c_int64, u64p, C.c_int, u64, u64p]
         L.ref_newton_interp_batch.argtypes = [u64p, C.c_int, u64p, C.c_int64, C.c_int64, u64, C.c_int, u64p, i32p]
@@ -136,6 +138,18 @@ def node_solve(m, M, vals, p):
     den = np.empty(t, dtype=np.uint64)
     num = np.empty((B, t), dtype=np.uint64)
     lib().ref_node_solve(_p(m, u64p), _p(M, u64p), t, _p(vals, u64p), t, B, p, _p(den, u64p), _p(num, u64p))
+    return den, num
+
+
+def node_solve_at(x, M, vals, p):
+    """The per-node routine at the node values x [n]: vals [B, t] -> (den [n], num [B, n])."""
+    x, M, vals = _a(x, np.uint64), _a(M, np.uint64), _a(vals, np.uint64)
+    B, t = vals.shape
+    assert len(M) == t + 1
+    n = len(x)
+    den = np.empty(n, dtype=np.uint64)
+    num = np.empty((B, n), dtype=np.uint64)
+    lib().ref_node_solve_at(_p(x, u64p), n, _p(M, u64p), t, _p(vals, u64p), t, B, p, _p(den, u64p), _p(num, u64p))
     return den, num
 
 

@@ -138,6 +138,26 @@ void ref_node_solve(const uint64_t* m, const uint64_t* M, int64_t t, const uint6
   }
 }
 
+/* The same per-node routine for n node values picked by the caller (the full-size parity check of SURVEY.md 8(c).3:
+ * "the oracle's per-node routine on 256 random node indices"): M has degree t, x[] are n of its roots (or any
+ * residues: then d = Q_x(x) with Q_x = the quotient of M by (z - x), remainder dropped).  den [n], num [B x n].
+ */
+void ref_node_solve_at(const uint64_t* x, int64_t n, const uint64_t* M, int64_t t, const uint64_t* vals, int64_t ld,
+                       int B, uint64_t p, uint64_t* den, uint64_t* num) {
+  for (int64_t i = 0; i < n; ++i) {
+    uint64_t q = 1 % p, d = 1 % p;
+    for (int b = 0; b < B; ++b) num[(int64_t)b * n + i] = vals[(int64_t)b * ld + (t - 1)] % p;
+    for (int64_t l = t - 1; l >= 1; --l) {
+      q = ref_addmod(M[l], ref_mulmod(x[i], q, p), p);
+      d = ref_addmod(ref_mulmod(d, x[i], p), q, p);
+      for (int b = 0; b < B; ++b)
+        num[(int64_t)b * n + i] =
+            ref_addmod(num[(int64_t)b * n + i], ref_mulmod(q, vals[(int64_t)b * ld + (l - 1)], p), p);
+    }
+    den[i] = d;
+  }
+}
+
 /* ------------------------------------------------------------------------------------------
  * (a2)-(a4) Transposed Vandermonde solve, all functions, all right-hand sides.
  * System (reading G1):  sum_i c_i m_i^(s+s0) = v_s,  s = 0..t-1.

@@ -75,6 +75,10 @@ void ref_node_quotient(const uint64_t* M, int64_t t, uint64_t m_i, uint64_t p, u
 void ref_node_solve(const uint64_t* m, const uint64_t* M, int64_t t, const uint64_t* vals, int64_t ld,
                     int B, uint64_t p, uint64_t* den /* [t] */, uint64_t* num /* [B x t], ld = t */);
 
+/* the same per-node routine for n node values x[] chosen by the caller; den [n], num [B x n] */
+void ref_node_solve_at(const uint64_t* x, int64_t n, const uint64_t* M, int64_t t, const uint64_t* vals, int64_t ld,
+                       int B, uint64_t p, uint64_t* den, uint64_t* num);
+
 int ref_vandermonde_solve_batch(const uint64_t* nodes, const int64_t* offsets, int F,
                                 const uint64_t* vals, int B, int s0, uint64_t p, uint64_t* coefs,
                                 int32_t* status);

@@ -319,6 +319,105 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------------
+// (a4) batched inversion (Montgomery's trick: "scalar-multiplied by the modular inverse
+// of the polynomial value").  A warp inverts 32 N values with ONE Fermat power: every lane multiplies its N values up
+// (prefix products in registers), the 32 lane products are scanned from both ends with shuffles (10 products per lane),
+// all lanes raise the warp's total to p - 2 together (the same instructions once per warp), and each lane unwinds its
+// own prefix products: 3 N + 12 + 125 / 1 products per lane for N inverses, i.e. about 3 + 137 / N per value against 125
+// for a Fermat power per value.  x[] Montgomery, in place -> inverses; zeros are skipped (left 0) and reported through
+// the returned mask.  Every lane of the warp must call it (full-mask shuffles).
+// ------------------------------------------------------------------------------------------------
+ZP_DEV uint64_t shfl_up64(uint64_t v, int o) {
+  return ((uint64_t)__shfl_up_sync(0xffffffffu, (uint32_t)(v >> 32), o) << 32) | __shfl_up_sync(0xffffffffu, (uint32_t)v, o);
+}
+ZP_DEV uint64_t shfl_down64(uint64_t v, int o) {
+  return ((uint64_t)__shfl_down_sync(0xffffffffu, (uint32_t)(v >> 32), o) << 32) | __shfl_down_sync(0xffffffffu, (uint32_t)v, o);
+}
+ZP_DEV uint64_t shfl_idx64(uint64_t v, int l) {
+  return ((uint64_t)__shfl_sync(0xffffffffu, (uint32_t)(v >> 32), l) << 32) | __shfl_sync(0xffffffffu, (uint32_t)v, l);
+}
+template <int N>
+ZP_DEV uint32_t warp_batch_inv(uint64_t (&x)[N], const ZpMod& k) {
+  uint64_t pre[N];
+  uint64_t run = k.r1;
+  uint32_t zero = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    pre[i] = run;
+    if (x[i] == 0) zero |= 1u << i;
+    else run = mont_mul(run, x[i], k);
+  }
+  const int lane = threadIdx.x & 31;
+  uint64_t below = run, above = run;  // products over the lanes <= this one / >= this one
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint64_t a = mont_mul(below, shfl_up64(below, o), k), b = mont_mul(above, shfl_down64(above, o), k);
+    below = (lane >= o) ? a : below;
+    above = (lane + o < 32) ? b : above;
+  }
+  const uint64_t tinv = mont_inv(shfl_idx64(below, 31), k);  // 1 / (product of the whole warp)
+  const uint64_t lo = shfl_up64(below, 1), hi = shfl_down64(above, 1);
+  uint64_t inv = tinv;  // 1 / run = tinv * (lanes below) * (lanes above)
+  if (lane > 0) inv = mont_mul(inv, lo, k);
+  if (lane < 31) inv = mont_mul(inv, hi, k);
+#pragma unroll
+  for (int i = N - 1; i >= 0; --i) {
+    if (zero >> i & 1) continue;
+    const uint64_t xi = x[i];
+    x[i] = mont_mul(inv, pre[i], k);
+    inv = mont_mul(inv, xi, k);
+  }
+  return zero;
+}
+
+// The division that ends every solve: for the slots i of the functions behind `offs` (all pointers at the batch's slot
+// 0, the functions cover the slots [a0, a0 + T)),  d_i = den_i [m_i if s0 = 1]  (den plain) and
+//   APPLY = false:  scale_i = 2^224 / d_i  (plain; the factor k_node_solve multiplies its reduced sums by), in place or not
+//   APPLY = true :  out_{b,i} = num_{b,i} / d_i,  b < B  (num plain, rows of ldn; out rows of ldo)
+// d_i = 0 (duplicate node, or a zero node with s0 = 1: readings G24/G25) -> ZP_ST_DUPLICATE_NODE with the term index.
+// A warp owns 32 N consecutive slots (lane + 32 j: unit-stride rows).
+#define ZP_INV_N 8
+template <bool APPLY>
+__global__ void __launch_bounds__(128)
+k_inv_finish(const uint64_t* den, const uint64_t* __restrict__ nodes, int s0, int64_t a0, int64_t T,
+             const int64_t* __restrict__ offs, int F, ZpMod kp, const uint64_t* num, int64_t ldn, int B, uint64_t* out,
+             int64_t ldo, int32_t* __restrict__ status) {
+  const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int64_t i0 = a0 + warp * (32 * ZP_INV_N) + (threadIdx.x & 31), iend = a0 + T;
+  if (i0 - (threadIdx.x & 31) >= iend) return;  // uniform per warp
+  uint64_t d[ZP_INV_N];
+#pragma unroll
+  for (int x = 0; x < ZP_INV_N; ++x) {
+    const int64_t i = i0 + 32 * x;
+    uint64_t v = kp.r1;
+    if (i < iend) {
+      v = to_mont(den[i], kp);
+      if (s0) v = mont_mul(v, to_mont(zp_canon(nodes[i], kp.p), kp), kp);
+    }
+    d[x] = v;
+  }
+  const uint32_t zero = warp_batch_inv<ZP_INV_N>(d, kp);
+#pragma unroll
+  for (int x = 0; x < ZP_INV_N; ++x) {
+    const int64_t i = i0 + 32 * x;
+    if (i >= iend) continue;
+    if (zero >> x & 1) {
+      int lo = 0, hi = F;  // function of slot i: offs[lo] <= i < offs[lo + 1]
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (offs[mid] <= i) lo = mid; else hi = mid;
+      }
+      atomicMin(&status[lo], (int32_t)(((uint32_t)(i - offs[lo]) << 8) | ZP_ST_DUPLICATE_NODE));
+    }
+    if (APPLY) {
+      for (int b = 0; b < B; ++b) out[(int64_t)b * ldo + i] = mont_mul(num[(int64_t)b * ldn + i], d[x], kp);  // plain x Montgomery
+    } else {
+      out[i] = mont_mul(d[x], kp.c224, kp);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // (a3) for ONE right-hand side and a long skeleton (C5): with q_{i,l} = sum_{k>l} M_k m_i^(k-l-1),
 //     num_i = sum_l q_{i,l} v_l = sum_j W_j m_i^j = W(m_i),    W_j = sum_l v_l M_{l+j+1}   (M_t = 1),
 // so the per-node work is the evaluation of two fixed polynomials (W and M') at m_i, which needs no modular product
@@ -327,7 +426,7 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 // general path is needed coefficient by coefficient, one modular multiply-add each).
 //   k_corr_w         W~_j (Montgomery) from the plain values v and the tree's M~
 //   k_solve_table_w  records { W_j, D_{j+1} } (plain), j = 0 .. t-1
-//   k_node_eval2     one lane per node: W(m_i) and M'(m_i) by blocked deferred evaluation, then c_i = W / M' [/ m]
+//   k_node_eval2     one lane per node: W(m_i) and M'(m_i) by blocked deferred evaluation; k_inv_finish<true> divides
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(ZP_K2_TC)
 k_corr_w(const uint64_t* __restrict__ vals, const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offsets, int F,
@@ -385,7 +484,7 @@ k_solve_table_w(const uint64_t* __restrict__ Wt, const uint64_t* __restrict__ Mt
 #define ZP_K3E_TILE 128
 __global__ void __launch_bounds__(ZP_K3_THREADS)
 k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ tab, const int64_t* __restrict__ offsets,
-             int F, int s0, ZpMod k, uint64_t* __restrict__ coefs, int32_t* __restrict__ status) {
+             int F, ZpMod k, uint64_t* __restrict__ num, uint64_t* __restrict__ den) {
   __shared__ __align__(16) ulonglong2 sT[2][ZP_K3E_TILE];
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
@@ -453,21 +552,20 @@ k_node_eval2(const uint64_t* __restrict__ nodes, const ulonglong2* __restrict__ 
     acc_mac(pD, VD, g);
     VW = mont_mul(acc_redc160(pW, k), k.c224, k);
     VD = mont_mul(acc_redc160(pD, k), k.c224, k);
-    if (live) {
-      const uint64_t dm = to_mont(VD, k);
-      const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
-      if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-      coefs[off + i] = mont_mul(VW, mont_inv(dd, k), k);  // plain * Montgomery -> plain
+    if (live) {  // plain W(m_i) and M'(m_i): k_inv_finish divides
+      num[off + i] = VW;
+      den[off + i] = VD;
     }
   }
 }
 
 // (a4) denominators for the general path: den_i = M'(m_i) by the same blocked deferred evaluation (17.8 pipe cycles
 // per coefficient), one launch before k_node_solve, which then runs without its second Horner chain (35.5 cycles
-// per stage).  Writes scale_i = den_i^-1 (/ m_i) * 2^224, the factor k_node_solve<., false> applies.
+// per stage).  Writes the plain den_i; k_inv_finish<false> turns them into scale_i = den_i^-1 (/ m_i) * 2^224, the factor
+// k_node_solve applies.
 __global__ void __launch_bounds__(ZP_K3_THREADS)
 k_node_den(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ Dtab, const int64_t* __restrict__ offsets,
-           int F, int s0, ZpMod k, uint64_t* __restrict__ scale, int32_t* __restrict__ status) {
+           int F, ZpMod k, uint64_t* __restrict__ den) {
   __shared__ __align__(16) uint64_t sT[2][ZP_K3E_TILE];
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
@@ -525,12 +623,7 @@ k_node_den(const uint64_t* __restrict__ nodes, const uint64_t* __restrict__ Dtab
     }
     acc_mac(pD, VD, g);
     VD = mont_mul(acc_redc160(pD, k), k.c224, k);  // plain M'(m_i)
-    if (live) {
-      const uint64_t dm = to_mont(VD, k);
-      const uint64_t dd = s0 ? mont_mul(dm, mm, k) : dm;
-      if (dd == 0) atomicMin(&status[f], (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-      scale[off + i] = mont_mul(mont_inv(dd, k), k.c224, k);
-    }
+    if (live) den[off + i] = VD;
   }
 }
 
@@ -749,24 +842,46 @@ k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ off
   }
 }
 
-// (a6) K7 balance: V_{j,s} = u_{j,s} * R_s / u_{0,s}   (eq. (4), readings G3, G20).
-__global__ void k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R,
-                          const int64_t* __restrict__ offsets, int F, int64_t T_tot, int B, ZpMod k,
-                          uint64_t* __restrict__ V, int32_t* __restrict__ pre) {
-  for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < T_tot; x += (int64_t)gridDim.x * blockDim.x) {
-    const uint64_t u0 = zp_canon(u[x], k.p);
-    uint64_t sc = 0;
-    if (u0 == 0) {
-      int lo = 0, hi = F;  // function of slot x: offsets[lo] <= x < offsets[lo+1]
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (offsets[mid] <= x) lo = mid; else hi = mid;
-      }
-      atomicMin(&pre[lo], (int32_t)(((uint32_t)(x - offsets[lo]) << 8) | ZP_ST_ZERO_PIVOT));
-    } else {
-      sc = mont_mul(to_mont(R[x], k), mont_inv(to_mont(u0, k), k), k);  // (R_s / u_{0,s})~
+// (a6) K7 balance: V_{j,s} = u_{j,s} * R_s / u_{0,s}   (eq. (4), readings G3, G20).  HBM stream
+// (16 B bytes per probe); the pivots u_{0,s} are inverted 32 x ZP_BAL_N at a time per warp (warp_batch_inv above).
+#define ZP_BAL_N 4
+__global__ void __launch_bounds__(256)
+k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const int64_t* __restrict__ offsets, int F,
+          int64_t T_tot, int B, ZpMod k, uint64_t* __restrict__ V, int32_t* __restrict__ pre) {
+  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  for (int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w * (32 * ZP_BAL_N) < T_tot; w += nwarp) {
+    const int64_t x0 = w * (32 * ZP_BAL_N) + lane;
+    uint64_t sc[ZP_BAL_N];
+#pragma unroll
+    for (int y = 0; y < ZP_BAL_N; ++y) {
+      const int64_t x = x0 + 32 * y;
+      sc[y] = (x < T_tot) ? to_mont(zp_canon(u[x], k.p), k) : k.r1;
     }
-    for (int j = 0; j < B; ++j) V[(int64_t)j * T_tot + x] = mont_mul(zp_canon(u[(int64_t)j * T_tot + x], k.p), sc, k);
+    const uint32_t zero = warp_batch_inv<ZP_BAL_N>(sc, k);
+#pragma unroll
+    for (int y = 0; y < ZP_BAL_N; ++y) {
+      const int64_t x = x0 + 32 * y;
+      if (x >= T_tot) continue;
+      if (zero >> y & 1) {
+        int lo = 0, hi = F;  // function of slot x: offsets[lo] <= x < offsets[lo+1]
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (offsets[mid] <= x) lo = mid; else hi = mid;
+        }
+        atomicMin(&pre[lo], (int32_t)(((uint32_t)(x - offsets[lo]) << 8) | ZP_ST_ZERO_PIVOT));
+      } else {
+        sc[y] = mont_mul(to_mont(R[x], k), sc[y], k);  // (R_s / u_{0,s})~
+      }
+    }
+    for (int j = 0; j < B; ++j) {
+      uint64_t v[ZP_BAL_N];
+#pragma unroll
+      for (int y = 0; y < ZP_BAL_N; ++y) v[y] = (x0 + 32 * y < T_tot) ? u[(int64_t)j * T_tot + x0 + 32 * y] : 0;
+#pragma unroll
+      for (int y = 0; y < ZP_BAL_N; ++y)
+        if (x0 + 32 * y < T_tot) V[(int64_t)j * T_tot + x0 + 32 * y] = mont_mul(zp_canon(v[y], k.p), sc[y], k);
+    }
   }
 }
 

@@ -229,67 +229,3 @@ k_sq_load_vals(const uint64_t* __restrict__ vals, int64_t ldv, int B, int64_t T,
 __global__ void k_fill_u64(uint64_t* x, int64_t n, uint64_t v) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) x[i] = v;
 }
-
-// ---- batched inversion (Montgomery's trick): N values per lane, one Fermat power per lane ------------
-// x[] Montgomery, in place -> inverses; zeros are skipped (left 0) and reported through the return mask.
-template <int N>
-ZP_DEV uint32_t batch_inv(uint64_t (&x)[N], const ZpMod& k) {
-  uint64_t pre[N];
-  uint64_t run = k.r1;
-  uint32_t zero = 0;
-#pragma unroll
-  for (int i = 0; i < N; ++i) {
-    pre[i] = run;
-    if (x[i] == 0) zero |= 1u << i;
-    else run = mont_mul(run, x[i], k);
-  }
-  uint64_t inv = mont_inv(run, k);
-#pragma unroll
-  for (int i = N - 1; i >= 0; --i) {
-    if (zero >> i & 1) continue;
-    const uint64_t xi = x[i];
-    x[i] = mont_mul(inv, pre[i], k);
-    inv = mont_mul(inv, xi, k);
-  }
-  return zero;
-}
-
-// ---- final division: c_{b,i} = num_{b,i} / (num_{B,i} [m_i]) ------------------------------------------------------------
-// num: [(B+1) x ld] plain (row B = the M' row); coefs: [B x ldc] at the run's first slot; offs: the run's function offsets
-// (device, relative to the run's first slot is offs[f] - offs[0]).
-#define ZP_SQ_INVB 8
-__global__ void __launch_bounds__(128)
-k_sq_final(const uint64_t* __restrict__ num, int64_t ld, int B, const uint64_t* __restrict__ nodes, int s0, int64_t T,
-           const int64_t* __restrict__ offs, int F, ZpMod kp, uint64_t* __restrict__ coefs, int64_t ldc,
-           int32_t* __restrict__ status) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i0 >= T) return;
-  uint64_t d[ZP_SQ_INVB];
-#pragma unroll
-  for (int x = 0; x < ZP_SQ_INVB; ++x) {
-    const int64_t i = i0 + x * stride;
-    uint64_t v = kp.r1;
-    if (i < T) {
-      v = mont_mul(num[(int64_t)B * ld + i], kp.r2, kp);  // to Montgomery
-      if (s0) v = mont_mul(v, to_mont(zp_canon(nodes[i], kp.p), kp), kp);
-    }
-    d[x] = v;
-  }
-  const uint32_t zero = batch_inv<ZP_SQ_INVB>(d, kp);
-#pragma unroll
-  for (int x = 0; x < ZP_SQ_INVB; ++x) {
-    const int64_t i = i0 + x * stride;
-    if (i >= T) continue;
-    if (zero >> x & 1) {
-      int lo = 0, hi = F;  // function of slot i
-      const int64_t gi = i + offs[0];
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (offs[mid] <= gi) lo = mid; else hi = mid;
-      }
-      atomicMin(&status[lo], (int32_t)(((uint32_t)(gi - offs[lo]) << 8) | ZP_ST_DUPLICATE_NODE));
-    }
-    for (int b = 0; b < B; ++b) coefs[(int64_t)b * ldc + i] = mont_mul(num[(int64_t)b * ld + i], d[x], kp);  // plain x Montgomery
-  }
-}

@@ -308,6 +308,8 @@ int sm_count() {
   return n_cached[dev];
 }
 inline unsigned grid_y(int F) { return (unsigned)(F < 65535 ? F : 65535); }
+// CTAs of k_inv_finish (128 lanes, ZP_INV_N slots per lane) for n slots
+inline unsigned inv_blocks(int64_t n) { return (unsigned)((n + 4 * 32 * ZP_INV_N - 1) / (4 * 32 * ZP_INV_N)); }
 
 // ---- K3 dispatch ----------------------------------------------------------------------------------
 #define ZP_NB_MAX 25
@@ -537,16 +539,15 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   }
   SQ_DUMP(5, nxt, (size_t)V * T);
   // c = N(m_i) / M'(m_i) [/ m_i]: one batched inversion
-  {
-    const int64_t lanes = (T + ZP_SQ_INVB - 1) / ZP_SQ_INVB;
-    ++g_launches, k_sq_final<<<(unsigned)((lanes + 127) / 128), 128, 0, st>>>(nxt, T, B, nodes, s0, T, d_offs, Fr, k, coefs, ldc,
-                                                                           w.st_solve + r.f0);
-  }
+  // (all pointers shifted to the batch's slot 0: d_offs holds absolute slots)
+  ++g_launches, k_inv_finish<true><<<inv_blocks(T), 128, 0, st>>>(nxt + (size_t)B * T - r.a0, nodes - r.a0, s0, r.a0, T, d_offs, Fr, k,
+                                                                   nxt - r.a0, T, B, coefs - r.a0, ldc, w.st_solve + r.f0);
 }
 
 // (a2)-(a4) by the quadratic route of PAPER.md section 2.2 for the functions [0, F) behind w.d_offsets
-void run_solve_quadratic(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* vals, int B,
-                         int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
+// (the functions cover the slots [a0, a0 + n) of the batch)
+void run_solve_quadratic(const Ws& w, const uint64_t* nodes, int F, int64_t a0, int64_t n, int64_t T_tot, int64_t tmax,
+                         const uint64_t* vals, int B, int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
   const uint64_t* Mt = run_master_poly(w, nodes, F, tmax, k, st);
   if (B == 1 && tmax >= ZP_EVAL2_MIN_T) {
     // one right-hand side, long skeleton: num_i = W(m_i) with W = correlation of v and M (kernels.cuh, k_corr_w)
@@ -557,8 +558,10 @@ void run_solve_quadratic(const Ws& w, const uint64_t* nodes, int F, int64_t T_to
     dim3 gt((unsigned)((tmax + 255) / 256), grid_y(F));
     ++g_launches, k_solve_table_w<<<gt, 256, 0, st>>>(Wt, Mt, w.d_offsets, F, k, reinterpret_cast<ulonglong2*>(w.tab));
     dim3 ge((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
-    ++g_launches, k_node_eval2<<<ge, ZP_K3_THREADS, 0, st>>>(nodes, reinterpret_cast<const ulonglong2*>(w.tab), w.d_offsets, F, s0, k, coefs,
-                                                               w.st_solve);
+    ++g_launches, k_node_eval2<<<ge, ZP_K3_THREADS, 0, st>>>(nodes, reinterpret_cast<const ulonglong2*>(w.tab), w.d_offsets, F, k, w.R,
+                                                               w.scale);
+    ++g_launches, k_inv_finish<true><<<inv_blocks(n), 128, 0, st>>>(w.scale, nodes, s0, a0, n, w.d_offsets, F, k, w.R, 0, 1, coefs, 0,
+                                                                     w.st_solve);
     return;
   }
   {
@@ -570,7 +573,9 @@ void run_solve_quadratic(const Ws& w, const uint64_t* nodes, int F, int64_t T_to
   const int per = (B + passes - 1) / passes;
   ProfScope prof(ZP_K_NODE_SOLVE, st);
   dim3 g((unsigned)((tmax + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(F));
-  ++g_launches, k_node_den<<<g, ZP_K3_THREADS, 0, st>>>(nodes, w.R, w.d_offsets, F, s0, k, w.scale, w.st_solve);
+  ++g_launches, k_node_den<<<g, ZP_K3_THREADS, 0, st>>>(nodes, w.R, w.d_offsets, F, k, w.scale);
+  ++g_launches, k_inv_finish<false><<<inv_blocks(n), 128, 0, st>>>(w.scale, nodes, s0, a0, n, w.d_offsets, F, k, nullptr, 0, 0, w.scale, 0,
+                                                                    w.st_solve);
   for (int b0 = 0; b0 < B; b0 += per) {
     const int nb = (B - b0 < per) ? (B - b0) : per;
     dispatch_node_solve(nb, g, st, nodes, M, w.d_offsets, F, vals, T_tot, b0, s0, k, w.scale, coefs, w.st_solve);
@@ -586,7 +591,7 @@ void run_solve(const Ws& w, const int64_t* h_offs, const uint64_t* nodes, int F,
   std::vector<SqRun> runs;
   if (w.sq.any) sq_find_runs(h_offs, F, &runs);
   if (runs.empty()) {
-    run_solve_quadratic(w, nodes, F, T_tot, tmax, vals, B, s0, k, coefs, st);
+    run_solve_quadratic(w, nodes, F, h_offs[0], h_offs[F] - h_offs[0], T_tot, tmax, vals, B, s0, k, coefs, st);
     return;
   }
   const NttCtx cx = ntt_begin(w, st);
@@ -597,7 +602,7 @@ void run_solve(const Ws& w, const int64_t* h_offs, const uint64_t* nodes, int F,
     Ws wc = w;
     wc.d_offsets += f0;
     wc.st_solve += f0;
-    run_solve_quadratic(wc, nodes, f1 - f0, T_tot, tm, vals, B, s0, k, coefs, st);
+    run_solve_quadratic(wc, nodes, f1 - f0, h_offs[f0], h_offs[f1] - h_offs[f0], T_tot, tm, vals, B, s0, k, coefs, st);
   };
   int f = 0;
   for (const SqRun& r : runs) {
@@ -934,7 +939,7 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
     ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
     run_eval_nodes(q->exps, T_tot[x], nv, anchors, k, w.nodes, st);
     run_power_sums(w, w.nodes, F, T_tot[x], tmax[x], q->skel, 1, s0, k, w.R, st);
-    int64_t blocks = (T_tot[x] + 255) / 256;
+    int64_t blocks = (T_tot[x] + 256 * ZP_BAL_N - 1) / (256 * ZP_BAL_N);
     if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     {
       ProfScope prof(ZP_K_BALANCE, st);

@@ -214,6 +214,9 @@ CONFIG_SHAPES = {
     3: dict(F=1, nv=7, t=100000, emax=30, B=9),
     4: dict(F=1024, nvars=6, t_num=500, t_den=200, total=24, B=25),
     5: dict(F=1, nv=10, t=524288, emax=40, B=1),
+    # not a BASELINE.json config: the paper's largest skeleton (4.8m monomials, reconstructing the 6th
+    # variable), one right-hand side -- bench.py --config 9 (row f3)
+    9: dict(F=1, nv=5, t=4_800_000, emax=40, B=1),
 }
 
 

@@ -22,14 +22,39 @@ def test_work_model_matches_design_md():
     total, ns = b.work_model(ts, 21, 4, True, False)
     assert ns == 4096 * 1000 * 1000 * (16 + 8 * 22)  # one multiply-add + (B + 1) MACs per (node, stage)
     assert total > ns and (total - ns) / ns < 0.05  # tree, Newton, nodes: a few per cent
-    _, ns5 = b.work_model([1 << 19], 1, 10, False, False)
-    assert ns5 == (1 << 38) * 20  # B = 1 route: two evaluations by MACs + the correlation
+    _, ns5 = b.work_model([4096], 1, 10, False, False)
+    assert ns5 == (1 << 24) * 20  # B = 1 route below the sub-quadratic threshold: two evaluations by MACs + the correlation
     _, ns_small = b.work_model([1000], 1, 10, False, False)
     assert ns_small == 1000 * 1000 * (16 + 8 * 2)  # below t = 4096 the general path
     tb, _ = b.work_model([500] * 4, 25, 5, True, True)
     tn, _ = b.work_model([500] * 4, 25, 5, True, False)
     assert tb - tn == 8 * 4 * 500 * 500  # balanced: one MAC per (probe, node) of the forward evaluation
     assert abs(b.IMAD_PEAK_TOPS - 148 * 64 * 1.965e-3) < 1e-9
+
+
+def test_work_model_of_the_subquadratic_route():
+    """bench.py subq_units counts the plan of csrc/zippel_capi.cu:sq_solve; checked here against the counts written
+    out by hand for t = 4096 (two levels above the 1024-node leaves), B = 1, and for its growth (t log^2 t)."""
+    from math import log2
+
+    b = load_bench()
+    ntt = lambda n: 3 * (n / 2) * log2(n) * 16
+    pw = lambda n: 3 * n * 36
+    crt = lambda n: n * 90
+    tot, parts = b.subq_units(4096, 1)
+    up = 2 * (3 * ntt(2048) + pw(2048)) + crt(4096) + 1 * (3 * ntt(4096) + pw(4096)) + crt(4096)
+    assert parts["up_tree"] == up
+    V = 2
+    down = sum(P * 2 * ntt(n) + V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in ((2, 2048), (1, 4096)))
+    assert parts["down_tree"] == down
+    assert parts["leaves"] == 4 * 1024 * 1024 * (4 + 16 + 2 * 8)
+    t19, _ = b.subq_units(1 << 19, 1)
+    t20, _ = b.subq_units(1 << 20, 1)
+    assert 2.0 < t20 / t19 < 2.3  # quasi-linear
+    total, ns = b.work_model([1 << 19], 1, 10, False, False)
+    assert ns == t19 and total == t19 + 16 * 9 * (1 << 19)  # + the node evaluation
+    quad = (1 << 38) * 20
+    assert quad / t19 > 100  # the quadratic B = 1 route does over 100 x the multiplier work at t = 2^19
 
 
 def test_clock_sampler_without_nvidia_smi(monkeypatch):

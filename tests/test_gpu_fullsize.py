@@ -158,3 +158,56 @@ def test_config3_full_size_lift_properties_and_round_trip(zp, ref):
     torch.cuda.synchronize()
     assert not zp.to_host(st).any()
     assert (zp.to_host(out) == w.planted).all(), "lift(forward(planted)) != planted"
+
+
+# ------------------------------------------------------------------------------------------- C3, C5: intermediates
+@pytest.mark.parametrize("idx,n_nodes", [(5, 256), (3, 256)])
+def test_full_size_intermediates_on_sampled_nodes(zp, ref, idx, n_nodes):
+    """SURVEY.md 8(c).3 at full size (t = 2^19 and t = 10^5): (1) the master polynomial of the CUDA path, read through
+    the dump hook of the test build, passes M(r) = prod_i (r - m_i) at random r in Python integers (O(t), with the
+    ORACLE's nodes); (2) with that M, the oracle's per-node routine (ref_node_solve_at: synthetic division, Horner
+    denominator, B dot products) on 256 random node indices gives exactly the numerators and
+    denominators the CUDA path holds before its final division, and the quotients are the solved coefficients."""
+    import torch
+
+    from paper_2505_24256_b200 import testhooks
+
+    w = wl.config(idx, with_planted=False)
+    t, B, p = w.T_tot, w.B, w.p
+    nodes = ref.eval_nodes(w.exps, w.anchors, p)
+    dn, dv = zp.to_dev(nodes), zp.to_dev(w.vals)
+    inv64 = pow(1 << 64, -1, p)
+    dumps = {}
+    with testhooks.routed():
+        for stage, words in ((1, t), (5, (B + 1) * t)):
+            out = torch.zeros(words, dtype=torch.int64, device="cuda")
+            testhooks.subq_dump(stage, out)
+            got, st = zp.vandermonde_solve_batch(dn, w.offsets, dv, p, 0)
+            torch.cuda.synchronize()
+            testhooks.subq_dump(0, None)
+            assert not zp.to_host(st).any()
+            dumps[stage] = zp.to_host(out)
+    coefs = zp.to_host(got)
+    # (1) M: Montgomery coefficients 0 .. t-1 (monic, leading 1 not stored)
+    M = np.empty(t + 1, dtype=np.uint64)
+    M[:t] = [int(x) * inv64 % p for x in dumps[1]]
+    M[t] = 1
+    rng = random.Random(500 + idx)
+    for r in [rng.randrange(2, p) for _ in range(2)] + [int(nodes[rng.randrange(t)])]:
+        horner = 0
+        for c in M[::-1]:
+            horner = (horner * r + int(c)) % p
+        prod = 1
+        for m in nodes:
+            prod = prod * (r - int(m)) % p
+        assert horner == prod
+    # (2) per-node routine of the oracle on sampled nodes
+    pick = sample_indices(rng, t, n_nodes, always=(0, 1023, 1024, t - 1))
+    den, num = ref.node_solve_at(nodes[pick], M, w.vals, p)
+    g = dumps[5].reshape(B + 1, t)
+    assert (g[B, pick] == den).all(), "denominators M'(m_i) differ from the oracle's Horner values"
+    assert (g[:B, pick] == num).all(), "numerators differ from the oracle's synthetic-division dot products"
+    for k, i in enumerate(pick):
+        dinv = pow(int(den[k]), -1, p)
+        for b in range(B):
+            assert int(coefs[b, i]) == int(num[b, k]) * dinv % p

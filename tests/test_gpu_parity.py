@@ -476,6 +476,134 @@ def test_balanced_zero_pivot_status(zp, ref):
         assert (gn[:, sl] == wn[:, sl]).all()
 
 
+def run_balanced_both(zp, ref, rw, parts, s0, basis):
+    p = rw.num.p
+    wn, wd, wst = ref.balanced_zippel_lift_step(parts["num"], parts["den"], rw.num.anchors, rw.num.samples, p, s0, basis)
+    dev = {k: dict(exps=zp.to_dev(v["exps"]), offsets=v["offsets"], skel=zp.to_dev(v["skel"]),
+                   uvals=zp.to_dev(v["uvals"])) for k, v in parts.items()}
+    gn, gd, st = zp.balanced_zippel_lift_step(dev["num"], dev["den"], zp.to_dev(rw.num.anchors),
+                                              zp.to_dev(rw.num.samples), p, s0, basis)
+    return (wn, wd, wst), (zp.to_host(gn), zp.to_host(gd), zp.to_host(st))
+
+
+@pytest.mark.parametrize("s0", [0, 1])
+@pytest.mark.parametrize("ragged", [False, True])
+def test_balanced_probe_offset_and_ragged_lengths(zp, ref, s0, ragged):
+    """eq. (4) (readings G1, G3, G20) with probes at the powers s0 .. s0 + t - 1 and with functions
+    of different lengths in one batch (k_balance's search over ragged offsets, the division by m_i of s0 = 1)."""
+    if ragged:  # lengths around the CTA, warp and batched-inversion group sizes
+        rw = wl.make_rational_workload("rag4g", wl.SEED_BASE + 45, 7, 6, [300, 7, 129, 1, 513, 64, 31], [12, 1, 90, 1, 257, 33, 128],
+                                       24, 25, s0=s0)
+    else:
+        rw = wl.config(4, F=3, t=140)
+    rw.num.s0 = rw.den.s0 = s0
+    parts, f_scale = balanced_inputs(ref, rw)
+    (wn, wd, wst), (gn, gd, st) = run_balanced_both(zp, ref, rw, parts, s0, 1)
+    assert not wst.any() and (st == wst).all()
+    assert (gn == wn).all() and (gd == wd).all()
+    p = rw.num.p
+    for w, g in ((rw.num, gn), (rw.den, gd)):  # = C x planted, per function
+        for f in range(w.F):
+            sl = slice(int(w.offsets[f]), int(w.offsets[f + 1]))
+            assert (g[:, sl].astype(object) == w.planted[:, sl].astype(object) * f_scale[f] % p).all()
+
+
+def test_balanced_zero_pivots_in_a_ragged_batch(zp, ref):
+    """Zero pivots u_{0,s} in several functions of a ragged batch, inside and at the ends of a warp's group of the
+    batched inversion: status word (smallest probe index) and every other function's output as the oracle's."""
+    rw = wl.make_rational_workload("rag4z", wl.SEED_BASE + 46, 5, 6, [140, 3, 129, 40, 260], [50, 2, 9, 33, 100], 24, 25)
+    parts, _ = balanced_inputs(ref, rw)
+    o = rw.num.offsets
+    for f, ss in ((1, [2]), (2, [128, 5, 77]), (4, [0, 259])):
+        for s in ss:
+            parts["num"]["uvals"][0, int(o[f]) + s] = 0
+    parts["den"]["uvals"][0, int(rw.den.offsets[3]) + 32] = 0
+    (wn, wd, wst), (gn, gd, st) = run_balanced_both(zp, ref, rw, parts, 0, 0)
+    assert (st == wst).all()
+    F = rw.num.F
+    assert st[1] == ((2 << 8) | zp.ST_ZERO_PIVOT) and st[2] == ((5 << 8) | zp.ST_ZERO_PIVOT) and st[4] == zp.ST_ZERO_PIVOT
+    assert st[F + 3] == ((32 << 8) | zp.ST_ZERO_PIVOT) and st[0] == 0 and st[3] == 0
+    for w, want, got, base in ((rw.num, wn, gn, 0), (rw.den, wd, gd, F)):
+        for f in range(F):
+            if st[base + f] == 0:
+                sl = slice(int(w.offsets[f]), int(w.offsets[f + 1]))
+                assert (got[:, sl] == want[:, sl]).all()
+
+
+# ------------------------------------------------------------------------------ many tiny functions (F > 65535)
+def test_more_functions_than_grid_rows(zp, ref):
+    """F = 70 001 functions of 1 .. 3 terms: every kernel walks the functions with blockIdx.y strides of at most 65 535
+    (grid_y in csrc/zippel_capi.cu); the polynomial and the balanced step, == the oracle."""
+    F = 70_001
+    r = np.random.Generator(np.random.Philox(key=[10, 4242]))
+    ts = r.integers(1, 4, F)
+    w = wl.make_box_workload("tiny", wl.SEED_BASE + 77, F, 3, ts, 6, 3, dense=True)
+    vals, _ = probe_values(ref, w)
+    got = lift_both(zp, ref, w, vals, 1)  # == the oracle inside
+    assert (got == w.planted).all()
+    # balanced: arbitrary residues as u and skel (parity with the oracle does not need a planted function)
+    td = r.integers(1, 3, F)
+    rw = wl.make_rational_workload("tinyr", wl.SEED_BASE + 78, F, 4, ts, td, 6, 7)
+    parts = {n: dict(exps=q.exps, offsets=q.offsets, skel=q.meta["skel_standin"], uvals=q.vals)
+             for n, q in (("num", rw.num), ("den", rw.den))}
+    (wn, wd, wst), (gn, gd, st) = run_balanced_both(zp, ref, rw, parts, 1, 1)
+    assert (st == wst).all() and (gn == wn).all() and (gd == wd).all()
+
+
+# ------------------------------------------------------------------------------ non-canonical inputs (reading G22)
+def test_inputs_offset_by_p_give_the_canonical_answer(zp, ref):
+    """Anchors, samples and values passed as x + p (still below 2^64): same outputs as for the canonical residues, on
+    the quadratic route, the B = 1 evaluation route and the sub-quadratic route, and for the balanced step."""
+    import torch
+
+    for ts, B in (([300, 41], 3), ([4200], 1), ([9000, 100], 2)):
+        w = wl.make_box_workload("nc", wl.SEED_BASE + 90 + B, len(ts), 3, ts, 30, B)
+        want, wnodes, wst = ref.zippel_lift_step(w.exps, w.offsets, w.anchors, w.samples, w.vals, w.p, 1, 1)
+        up = lambda a: (a.astype(np.uint64) + np.uint64(w.p))
+        got, st = zp.zippel_lift_step(zp.to_dev(w.exps), w.offsets, zp.to_dev(up(w.anchors)), zp.to_dev(up(w.samples)),
+                                      zp.to_dev(up(w.vals)), w.p, 1, 1)
+        assert not wst.any() and not zp.to_host(st).any() and (zp.to_host(got) == want).all()
+        nodes = zp.to_dev(up(wnodes))
+        c, st = zp.vandermonde_solve_batch(nodes, w.offsets, zp.to_dev(up(w.vals)), w.p, 0)
+        wc, wst = ref.vandermonde_solve_batch(wnodes, w.offsets, w.vals, w.p, 0)
+        assert (zp.to_host(c) == wc).all()
+    rw = wl.config(4, F=2, t=70)
+    parts = {n: dict(exps=q.exps, offsets=q.offsets, skel=q.meta["skel_standin"], uvals=q.vals)
+             for n, q in (("num", rw.num), ("den", rw.den))}
+    p = rw.num.p
+    wn, wd, wst = ref.balanced_zippel_lift_step(parts["num"], parts["den"], rw.num.anchors, rw.num.samples, p, 0, 1)
+    dev = {k: dict(exps=zp.to_dev(v["exps"]), offsets=v["offsets"], skel=zp.to_dev(v["skel"] + np.uint64(p)),
+                   uvals=zp.to_dev(v["uvals"] + np.uint64(p))) for k, v in parts.items()}
+    gn, gd, st = zp.balanced_zippel_lift_step(dev["num"], dev["den"], zp.to_dev(rw.num.anchors + np.uint64(p)),
+                                              zp.to_dev(rw.num.samples + np.uint64(p)), p, 0, 1)
+    assert (zp.to_host(st) == wst).all() and (zp.to_host(gn) == wn).all() and (zp.to_host(gd) == wd).all()
+
+
+# ------------------------------------------------------------------------------ bindings on a non-current stream
+def test_bindings_on_a_side_stream_without_a_workspace(zp, ref):
+    """Every binding that allocates its own workspace and outputs does so on the stream the kernels are enqueued on
+    (api._on): calls on a side stream, while the current stream keeps allocating and overwriting blocks, still give
+    the oracle's numbers."""
+    import torch
+
+    w = wl.config(2, F=40)
+    want, _, _ = ref.zippel_lift_step(w.exps, w.offsets, w.anchors, w.samples, w.vals, w.p, 0, 1)
+    side = torch.cuda.Stream()
+    de, da, ds, dv = (zp.to_dev(x) for x in (w.exps, w.anchors, w.samples, w.vals))
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(4):
+        got, st = zp.zippel_lift_step(de, w.offsets, da, ds, dv, w.p, 0, 1, stream=side)
+        outs.append((got, st))
+        for _ in range(8):  # churn on the current stream: blocks freed by the binding must not be handed out early
+            junk = torch.full((1 << 20,), -1, dtype=torch.int64, device="cuda")
+            del junk
+    side.synchronize()
+    torch.cuda.synchronize()
+    for got, st in outs:
+        assert not zp.to_host(st).any() and (zp.to_host(got) == want).all()
+
+
 # ------------------------------------------------------------------------------ host-side argument checks
 def test_argument_errors_are_reported_not_launched(zp):
     import torch

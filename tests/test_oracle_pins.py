@@ -148,6 +148,39 @@ def test_quotient_times_linear_factor_is_master_and_den_is_product(p, t):
             assert int(num[b, i]) == sum(q[s] * int(vals[b, s]) for s in range(t)) % p
 
 
+@pytest.mark.parametrize("p,t", [(101, 7), (P63, 1), (P63, 23)])
+def test_node_solve_at_sampled_nodes_and_arbitrary_points(p, t):
+    """ref_node_solve_at (the per-node routine on caller-chosen node values) against Python
+    integers: at a root m_i of M, den = prod_{j != i}(m_i - m_j) and num_b = sum_s q_{i,s} v_{b,s} with the quotient
+    defined by Q_i(z)(z - m_i) = M(z); at a non-root x the quotient of the division with remainder."""
+    rr = random.Random(70 + t)
+    m = rr.sample(range(1, p), t) if p < 200 else rr.sample(range(2, 1 << 62), t)
+    M = ref.master_poly(m, p)
+    Mi = [int(x) for x in M]
+    vals = np.array([rnd(p, t, 18), rnd(p, t, 19), rnd(p, t, 20)], dtype=np.uint64)
+    pick = [t - 1, 0, t // 2][: min(t, 3)]
+    extra = [x for x in rnd(p, 3, 71) if x not in m]
+    xs = [m[i] for i in pick] + extra
+    den, num = ref.node_solve_at(xs, M, vals, p)
+    assert den.shape == (len(xs),) and num.shape == (3, len(xs))
+    for k, x in enumerate(xs):
+        q = [0] * t  # synthetic division of M by (z - x) in big integers: q_{t-1} = 1, q_{l-1} = M_l + x q_l
+        q[t - 1] = 1
+        for l in range(t - 1, 0, -1):
+            q[l - 1] = Mi[l] + x * q[l]
+        rem = Mi[0] + x * q[0]
+        assert (rem % p == 0) == (x in m)
+        if x in m:
+            assert int(den[k]) == math.prod((x - mj) for mj in m if mj != x) % p
+        assert int(den[k]) == sum(c * pow(x, l, p) for l, c in enumerate(q)) % p  # Q_x(x)
+        for b in range(3):
+            assert int(num[b, k]) == sum(q[s] * int(vals[b, s]) for s in range(t)) % p
+    if t > 1:  # on all the nodes it is ref_node_solve's answer
+        d_all, n_all = ref.node_solve(m, M, vals, p)
+        d_at, n_at = ref.node_solve_at(m, M, vals, p)
+        assert (d_all == d_at).all() and (n_all == n_at).all()
+
+
 # ---------------------------------------------------------------------------- solve (L60, L191-197)
 def py_gauss(A, b, p):
     n = len(A)
