@@ -45,8 +45,42 @@ struct CrtOut {
 };
 
 #if defined(__CUDACC__)
-// x * w mod q, lazily: any 64-bit x in, [0, 2q) out (w = {w, w'} with its Shoup companion)
-ZP_DEV uint64_t ntt_mul(uint64_t x, ulonglong2 w, const ZpMod& q) { return horner_step(x, w.x, w.y, 0, 0, q); }
+// x * w mod q, lazily: any 64-bit x in, [0, 2q) out (w = {w, w'} with its Shoup companion w' = floor(w 2^64 / q)).
+// modarith.cuh's horner_step without its addends (whose carry plumbing ptxas keeps even when they are zero):
+// qq = floor(w' x / 2^64) exactly (4 wide products, the carries through predicates), then w x - qq q modulo 2^64
+// (2 wide + 4 low products): 16 units of the multiplier pipe and 4 instructions on the alu pipe.
+ZP_DEV uint64_t ntt_mul(uint64_t x, ulonglong2 w, const ZpMod& q) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), p0 = (uint32_t)w.y, p1 = (uint32_t)(w.y >> 32);
+  const uint32_t w0 = (uint32_t)w.x, w1 = (uint32_t)(w.x >> 32);
+  const uint32_t np0 = (uint32_t)q.np, np1 = (uint32_t)(q.np >> 32);
+  uint64_t qq;
+  asm("{\n\t"
+      ".reg .u64 a, s, s2, t;\n\t"
+      ".reg .u32 alo, ahi, slo, shi, c1, tlo, thi, dummy;\n\t"
+      "mul.wide.u32 a, %1, %3;\n\t"   // p0 x0 (its high word carries into the middle)
+      "mul.wide.u32 s, %1, %4;\n\t"   // p0 x1
+      "mul.wide.u32 s2, %2, %3;\n\t"  // p1 x0
+      "add.cc.u64 s, s2, s;\n\t"      // middle sum, carry c1 (weight 2^96)
+      "addc.u32 c1, 0, 0;\n\t"
+      "mov.b64 {alo, ahi}, a;\n\t"
+      "mov.b64 {slo, shi}, s;\n\t"
+      "add.cc.u32 dummy, slo, ahi;\n\t"
+      "addc.cc.u32 tlo, shi, 0;\n\t"
+      "addc.u32 thi, c1, 0;\n\t"
+      "mov.b64 t, {tlo, thi};\n\t"
+      "mad.wide.u32 %0, %2, %4, t;\n\t"  // p1 x1 + (middle >> 32)
+      "}"
+      : "=l"(qq)
+      : "r"(p0), "r"(p1), "r"(x0), "r"(x1));
+  const uint32_t q0 = (uint32_t)qq, q1 = (uint32_t)(qq >> 32);
+  uint32_t uh = zp_madlo(w0, x1, 0);
+  uh = zp_madlo(w1, x0, uh);
+  uh = zp_madlo(q0, np1, uh);
+  uh = zp_madlo(q1, np0, uh);
+  uint64_t u = (uint64_t)uh << 32;
+  u = zp_madw(w0, x0, u);
+  return zp_madw(q0, np0, u);
+}
 ZP_DEV uint32_t brev_bits(uint32_t x, int bits) { return bits ? (__brev(x) >> (32 - bits)) : 0u; }
 
 // x * w^E (forward) or x * w^-E (inverse), E < 2^24, from the two-level tables
@@ -82,188 +116,269 @@ __global__ void k_ntt_tables(ZpMod q, uint64_t wroot_mont, ulonglong2* U, ulongl
   (which == 0 ? U : which == 1 ? Ui : which == 2 ? Tlo : Thi)[i] = r;
 }
 
-// ---- chunk pass: every CTA transforms 4096 consecutive words of one prime in shared memory -----------------------
-// The chunk holds 4096 / ln complete transforms of length ln = 2^logn <= 4096 (the whole transform, or the rows of the
-// last pass of a longer one).  logRp > 0: the transforms are the rows of parents of length ln 2^logRp; row c's
-// element j is twisted by w_parent^(brev(c) j) on load (forward) / by its inverse on store (inverse).
-// buf: [3][E] words (prime-major), E = words per prime (a multiple of ln).
-template <bool INV>
-__global__ void __launch_bounds__(ZP_NTT_THREADS)
-k_ntt_chunk(uint64_t* __restrict__ buf, int64_t E, int logn, int logRp, NttCtx cx) {
-  __shared__ uint64_t x[ZP_NTT_C];
-  const int j = blockIdx.y;
-  const ZpMod q = cx.q[j];
+// ---- the CTA-level transform: a tile of 4096 words in shared memory, radix-8 rounds in registers ---------------------
+// A CTA works on a tile of 4096 words e (12 bits).  A pass runs the stages that act on the bits hi .. lo of e (hi >= lo;
+// forward from hi down, inverse from lo up); the stage on bit b pairs e with e + 2^b and uses the twiddle U[2^ls + i],
+// ls = hi - b, i = the bits hi .. b+1 of e (the block the pair lies in).  The stages are taken three at a time: in the
+// round of field f (bits 3f+2 .. 3f) a lane loads the 8 words of a group that differ in that field only, runs up to three
+// stages on them in registers and writes them back -- one load and one store of shared memory per word and round
+// instead of one per word and stage, in a loop over the rounds (the code stays small: the butterfly is ~30
+// instructions that fill the multiplier pipe and the issue slots alike, so instruction fetch and every extra instruction
+// count).  512 groups per round, two per lane.  Shared memory holds word e at e ^ ((e >> 3) & 15): conflict-free for
+// 64-bit accesses in all four rounds and for unit-stride staging.
+#define ZP_NTT_SMEM ZP_NTT_C
+ZP_DEV int ntt_pad(int e) { return e ^ ((e >> 3) & 15); }
+// first word of group gidx (9 bits) in the round whose field starts at bit sh: the field bits are zero
+ZP_DEV int ntt_gbase(int gidx, int sh) { return ((gidx >> sh) << (sh + 3)) | (gidx & ((1 << sh) - 1)); }
+
+// the twiddles of the (up to three) stages of the field at bit sh for the group whose first word is eb: slot 4 >> bb ..
+// of stage bb holds its 4 >> bb entries (w[1]: stage 2; w[2..3]: stage 1; w[4..7]: stage 0); stages outside [lo, hi] load
+// nothing.  Issued before the words of the group are read, so that the two latencies overlap.
+ZP_DEV void ntt_group_twiddles(ulonglong2 (&w)[8], int eb, int sh, int hi, int lo, const ulonglong2* __restrict__ tab) {
+#pragma unroll
+  for (int bb = 2; bb >= 0; --bb) {
+    const int b = sh + bb;
+    if (b > hi || b < lo) continue;  // uniform
+    const int ls = hi - b, mask = (1 << ls) - 1;
+    const int ihi = (eb >> (sh + 3)) << (2 - bb);  // the block bits above the field; j's bits above bb fill the rest
+#pragma unroll
+    for (int k = 0; k < (4 >> bb); ++k) w[(4 >> bb) + k] = __ldg(tab + (1 << ls) + ((ihi | k) & mask));
+  }
+}
+// the forward stages of one field on one group (values in [0, 4q), Harvey butterflies)
+ZP_DEV void ntt_group_fwd(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int hi, int lo, const ZpMod& q) {
   const uint64_t q2 = 2 * q.p;
-  uint64_t* g = buf + (int64_t)j * E;
-  const int64_t c0 = (int64_t)blockIdx.x * ZP_NTT_C;
-  const int ln = 1 << logn;
-  const ulonglong2* __restrict__ U = INV ? cx.Ui[j] : cx.U[j];
-  const int lpar = logn + logRp;  // log2 of the parent length
-  for (int e = threadIdx.x; e < ZP_NTT_C; e += ZP_NTT_THREADS) {
-    uint64_t v = 0;
-    if (c0 + e < E) {
-      v = g[c0 + e];
-      if (!INV && logRp) {
-        const int64_t tr = (c0 + e) >> logn;  // transform index; row c = tr mod R
-        const uint32_t c = (uint32_t)(tr & ((1 << logRp) - 1)), jj = (uint32_t)((c0 + e) & (ln - 1));
-        const uint32_t Ex = (brev_bits(c, logRp) * jj) << (ZP_NTT_LOGMAX - lpar);
-        v = ntt_twist<false>(v, Ex, cx.Tlo[j], cx.Thi[j], q);
-      }
-    }
-    x[e] = v;
-  }
-  __syncthreads();
-  if (!INV) {
-    for (int lm = 0; lm < logn; ++lm) {  // stage M = 2^lm, half = ln / 2M
-      const int lh = logn - 1 - lm, half = 1 << lh;
-      for (int bf = threadIdx.x; bf < ZP_NTT_C / 2; bf += ZP_NTT_THREADS) {
-        const int s = bf >> (logn - 1), r = bf & ((ln >> 1) - 1);
-        const int i = r >> lh, jj = r & (half - 1);
-        const int pos = (s << logn) + (i << (lh + 1)) + jj;
-        const ulonglong2 w = __ldg(U + (1 << lm) + i);
-        uint64_t u = x[pos];
-        u = (u >= q2) ? u - q2 : u;
-        const uint64_t v = ntt_mul(x[pos + half], w, q);
-        x[pos] = u + v;
-        x[pos + half] = u - v + q2;
-      }
-      __syncthreads();
-    }
-  } else {
-    for (int lm = logn - 1; lm >= 0; --lm) {
-      const int lh = logn - 1 - lm, half = 1 << lh;
-      for (int bf = threadIdx.x; bf < ZP_NTT_C / 2; bf += ZP_NTT_THREADS) {
-        const int s = bf >> (logn - 1), r = bf & ((ln >> 1) - 1);
-        const int i = r >> lh, jj = r & (half - 1);
-        const int pos = (s << logn) + (i << (lh + 1)) + jj;
-        const ulonglong2 w = __ldg(U + (1 << lm) + i);
-        const uint64_t u = x[pos], v = x[pos + half];  // [0, 2q)
-        const uint64_t sum = u + v;
-        x[pos] = (sum >= q2) ? sum - q2 : sum;
-        x[pos + half] = ntt_mul(u - v + q2, w, q);
-      }
-      __syncthreads();
-    }
-  }
-  for (int e = threadIdx.x; e < ZP_NTT_C; e += ZP_NTT_THREADS) {
-    if (c0 + e < E) {
-      uint64_t v = x[e];
-      if (INV && logRp) {
-        const int64_t tr = (c0 + e) >> logn;
-        const uint32_t c = (uint32_t)(tr & ((1 << logRp) - 1)), jj = (uint32_t)((c0 + e) & (ln - 1));
-        const uint32_t Ex = (brev_bits(c, logRp) * jj) << (ZP_NTT_LOGMAX - lpar);
-        v = ntt_twist<true>(v, Ex, cx.Tlo[j], cx.Thi[j], q);
-      }
-      g[c0 + e] = v;
+#pragma unroll
+  for (int bb = 2; bb >= 0; --bb) {
+    const int b = sh + bb;
+    if (b > hi || b < lo) continue;  // uniform
+#pragma unroll
+    for (int j0 = 0; j0 < 8; ++j0) {
+      if (j0 >> bb & 1) continue;
+      const int j1 = j0 | (1 << bb);
+      uint64_t u = x[j0];
+      u = (u >= q2) ? u - q2 : u;
+      const uint64_t v = ntt_mul(x[j1], w[(4 >> bb) + (j0 >> (bb + 1))], q);
+      x[j0] = u + v;
+      x[j1] = u - v + q2;
     }
   }
 }
-
-// ---- strided pass: the first logR stages of transforms of length n = 2^logn on the [R x L] view (L = n / R) ------
-// CTA = (transform, tile of G = 4096 / R consecutive columns); R <= 512.  logRp as above (these transforms are rows of
-// a longer parent: the middle pass of a three-pass plan).
-template <bool INV>
-__global__ void __launch_bounds__(ZP_NTT_THREADS)
-k_ntt_strided(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp, NttCtx cx) {
-  __shared__ uint64_t x[ZP_NTT_C];
-  const int j = blockIdx.y;
-  const ZpMod q = cx.q[j];
+// inverse: values in [0, 2q), Gentleman-Sande butterflies with the inverse twiddles
+ZP_DEV void ntt_group_inv(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int hi, int lo, const ZpMod& q) {
   const uint64_t q2 = 2 * q.p;
-  const int logG = ZP_NTT_LOGC - logR, G = 1 << logG, R = 1 << logR;
-  const int logL = logn - logR;
-  const int tiles_log = logL - logG;  // column tiles per transform
-  const int64_t tr = (int64_t)blockIdx.x >> tiles_log;
-  const int col0 = (int)(blockIdx.x & ((1 << tiles_log) - 1)) << logG;
-  uint64_t* g = buf + (int64_t)j * E + (tr << logn) + col0;
-  if ((tr << logn) >= E) return;
-  const ulonglong2* __restrict__ U = INV ? cx.Ui[j] : cx.U[j];
+#pragma unroll
+  for (int bb = 0; bb < 3; ++bb) {
+    const int b = sh + bb;
+    if (b > hi || b < lo) continue;  // uniform
+#pragma unroll
+    for (int j0 = 0; j0 < 8; ++j0) {
+      if (j0 >> bb & 1) continue;
+      const int j1 = j0 | (1 << bb);
+      const uint64_t u = x[j0], v = x[j1];
+      const uint64_t sum = u + v;
+      x[j0] = (sum >= q2) ? sum - q2 : sum;
+      x[j1] = ntt_mul(u - v + q2, w[(4 >> bb) + (j0 >> (bb + 1))], q);
+    }
+  }
+}
+// all the stages of [lo, hi] on the tile in shared memory (the tile is complete and visible on entry and on exit)
+template <bool INV>
+ZP_DEV void ntt_tile(uint64_t* sm, int hi, int lo, const ulonglong2* __restrict__ tab, const ZpMod& q) {
+#pragma unroll 1
+  for (int r = 0; r < 4; ++r) {
+    const int f = INV ? r : 3 - r, sh = 3 * f;
+    if (sh > hi || sh + 2 < lo) continue;  // no stage in this field
+#pragma unroll 1
+    for (int g = 0; g < ZP_NTT_C / 8 / ZP_NTT_THREADS; ++g) {
+      const int eb = ntt_gbase(threadIdx.x + ZP_NTT_THREADS * g, sh);
+      ulonglong2 w[8];
+      ntt_group_twiddles(w, eb, sh, hi, lo, tab);
+      uint64_t x[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) x[j] = sm[ntt_pad(eb + (j << sh))];
+      if (INV) ntt_group_inv(x, w, sh, hi, lo, q);
+      else ntt_group_fwd(x, w, sh, hi, lo, q);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) sm[ntt_pad(eb + (j << sh))] = x[j];
+    }
+    __syncthreads();
+  }
+}
+
+// ---- one pass over a buffer: every CTA transforms one tile of 4096 words of one prime ---------------------------
+// buf: [3][E] words (prime-major), E = words per prime.  Two kinds of tile:
+//   chunk (logR = 0):  4096 consecutive words = 4096 / ln complete transforms of length ln = 2^logn <= 4096 (a whole
+//                      transform, or the rows of the last pass of a longer one): the stages on the bits logn-1 .. 0;
+//   strided (logR > 0): the first logR stages of a transform of length n = 2^logn on its [R x L] view (L = n / R): the
+//                      tile is R rows x G = 4096 / R consecutive columns, word e = r G + c: the stages on the bits
+//                      11 .. 12 - logR.  R <= 512 (rows of G >= 8 words).
+// logRp > 0: the transforms are the rows of parents of length 2^(logn + logRp); row c's element j is twisted by
+// w_parent^(brev(c) j) on load (forward) / by its inverse on store (inverse).
+template <bool INV>
+__global__ void __launch_bounds__(ZP_NTT_THREADS, 4)
+k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp, NttCtx cx) {
+  __shared__ uint64_t sm[ZP_NTT_SMEM];
+  const int jp = blockIdx.y;
+  const ZpMod q = cx.q[jp];
+  const int T = threadIdx.x;
+  uint64_t* g = buf + (int64_t)jp * E;
   const int lpar = logn + logRp;
-  const uint32_t crow = (uint32_t)(tr & ((1 << logRp) - 1));  // this transform's row in its parent
-  const uint32_t cb = brev_bits(crow, logRp);
-  for (int e = threadIdx.x; e < ZP_NTT_C; e += ZP_NTT_THREADS) {
-    const int r = e >> logG, c = e & (G - 1);
-    uint64_t v = g[((int64_t)r << logL) + c];
-    if (!INV && logRp) {
-      const uint32_t jj = ((uint32_t)r << logL) + col0 + c;  // position inside this transform
-      v = ntt_twist<false>(v, (cb * jj) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[j], cx.Thi[j], q);
+  // word e of the tile <-> offset into g: base + ((e >> logG) << rowshift) + (e & (G - 1))
+  int64_t base;
+  int logG, rowshift;
+  if (logR == 0) {
+    base = (int64_t)blockIdx.x * ZP_NTT_C;
+    logG = ZP_NTT_LOGC;
+    rowshift = 0;
+  } else {
+    const int logL = logn - logR;
+    logG = ZP_NTT_LOGC - logR;
+    const int tiles_log = logL - logG;  // column tiles per transform
+    const int64_t tr = (int64_t)blockIdx.x >> tiles_log;
+    const int col0 = (int)(blockIdx.x & ((1 << tiles_log) - 1)) << logG;
+    base = (tr << logn) + col0;
+    rowshift = logL;
+    if ((tr << logn) >= E) return;
+  }
+  const int G1 = (1 << logG) - 1;
+  const int ln1 = (1 << logn) - 1;
+#pragma unroll 4
+  for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+    const int e = T + ZP_NTT_THREADS * m;
+    const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+    uint64_t v = 0;
+    if (off < E) {
+      v = g[off];
+      if (!INV && logRp) {
+        const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
+        v = ntt_twist<false>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
+      }
     }
-    x[e] = v;
+    sm[ntt_pad(e)] = v;
   }
   __syncthreads();
-  if (!INV) {
-    for (int lm = 0; lm < logR; ++lm) {
-      const int lh = logR - 1 - lm, half = 1 << lh;
-      for (int bf = threadIdx.x; bf < ZP_NTT_C / 2; bf += ZP_NTT_THREADS) {
-        const int c = bf & (G - 1), rb = bf >> logG;
-        const int i = rb >> lh, jj = rb & (half - 1);
-        const int pos = (((i << (lh + 1)) + jj) << logG) + c;
-        const ulonglong2 w = __ldg(U + (1 << lm) + i);
-        uint64_t u = x[pos];
-        u = (u >= q2) ? u - q2 : u;
-        const uint64_t v = ntt_mul(x[pos + (half << logG)], w, q);
-        x[pos] = u + v;
-        x[pos + (half << logG)] = u - v + q2;
+  const int hi = logR ? 11 : logn - 1, lo = logR ? 12 - logR : 0;
+  ntt_tile<INV>(sm, hi, lo, INV ? cx.Ui[jp] : cx.U[jp], q);
+#pragma unroll 4
+  for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+    const int e = T + ZP_NTT_THREADS * m;
+    const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+    if (off < E) {
+      uint64_t v = sm[ntt_pad(e)];
+      if (INV && logRp) {
+        const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
+        v = ntt_twist<true>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
       }
-      __syncthreads();
+      g[off] = v;
     }
-  } else {
-    for (int lm = logR - 1; lm >= 0; --lm) {
-      const int lh = logR - 1 - lm, half = 1 << lh;
-      for (int bf = threadIdx.x; bf < ZP_NTT_C / 2; bf += ZP_NTT_THREADS) {
-        const int c = bf & (G - 1), rb = bf >> logG;
-        const int i = rb >> lh, jj = rb & (half - 1);
-        const int pos = (((i << (lh + 1)) + jj) << logG) + c;
-        const ulonglong2 w = __ldg(U + (1 << lm) + i);
-        const uint64_t u = x[pos], v = x[pos + (half << logG)];
-        const uint64_t sum = u + v;
-        x[pos] = (sum >= q2) ? sum - q2 : sum;
-        x[pos + (half << logG)] = ntt_mul(u - v + q2, w, q);
-      }
-      __syncthreads();
-    }
-  }
-  for (int e = threadIdx.x; e < ZP_NTT_C; e += ZP_NTT_THREADS) {
-    const int r = e >> logG, c = e & (G - 1);
-    uint64_t v = x[e];
-    if (INV && logRp) {
-      const uint32_t jj = ((uint32_t)r << logL) + col0 + c;
-      v = ntt_twist<true>(v, (cb * jj) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[j], cx.Thi[j], q);
-    }
-    g[((int64_t)r << logL) + c] = v;
   }
 }
 
-// ---- pointwise products in the transformed domain -------------------------------------------------------------------
-// out segment o = A segment ia(o) * B segment ib(o) * (1/n), per prime; segments are n = 2^logn words.
-//   mode 0 (pairs)  : A = B = X,  ia = 2o, ib = 2o + 1                          (up-tree; Newton; root)
-//   mode 1 (down)   : A = Y, ia = o / 2;  B = X, ib = 2 ((o / 2) mod P) + 1 - (o & 1)   (tails x reversed siblings)
-//   mode 2 (against): A = Y, ia = o;  B = X, ib = 1                             (Newton's second product)
-// Kq[j] = 2^128 / n mod q_j: mont_mul(mont_mul(a, b), Kq) = a b / n.  EA, EB, EO: words per prime of the three buffers.
-__global__ void __launch_bounds__(256)
-k_ntt_pointwise(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict__ B, int64_t EB,
-                uint64_t* __restrict__ O, int64_t EO, int logn, int mode, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1,
-                uint64_t Kq2) {
-  const int j = blockIdx.y;
-  const ZpMod q = cx.q[j];
-  const uint64_t Kq = j == 0 ? Kq0 : j == 1 ? Kq1 : Kq2;
-  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t o = e >> logn, i = e & (((int64_t)1 << logn) - 1);
-    int64_t ia, ib;
-    if (mode == 0) {
-      ia = 2 * o;
-      ib = 2 * o + 1;
-    } else if (mode == 1) {
-      ia = o >> 1;
-      ib = 2 * ((o >> 1) % P) + 1 - (o & 1);
-    } else {
-      ia = o;
-      ib = 1;
+// ---- products: forward chunk stages, pointwise product, inverse chunk stages in ONE kernel ----------------------------
+// Segments are n = 2^logseg words; the last logn <= 12 stages of their transforms (all of them when logseg <= 12; else
+// the strided passes have run on A and B before, and run on O after, this kernel; logRp as in k_ntt_pass) act inside
+// chunks of 4096 consecutive words, and the pointwise product is position-wise, so a CTA can take the chunk of the two
+// operands through the forward stages, multiply, and take the product back through the inverse stages without the
+// transformed operands ever leaving the SM.  The factor 1/n rides on the product (Kq[j] = 2^128 / n mod q_j:
+// mont_mul(mont_mul(a, b), Kq) = a b / n).  A CTA = one chunk of one prime.
+//   MODE 0 (pairs): O segment o = A segment 2o * A segment 2o + 1               (up-tree; Newton; root; B unused)
+//   MODE 1 (down) : O segments 2 vt + side = A segment vt * B segment 2 (vt mod P) + 1 - side, side = 0, 1, where B holds
+//                   COMPLETE forward transforms (k_ntt_pass): tails x reversed siblings, the siblings' transforms are
+//                   shared by all the vectors of a level.  EA, EB, EO: words per prime of the three buffers.
+ZP_DEV uint64_t ntt_canon4(uint64_t b, const ZpMod& q) {  // [0, 4q) -> [0, q)
+  b = (b >= 2 * q.p) ? b - 2 * q.p : b;
+  return (b >= q.p) ? b - q.p : b;
+}
+template <int MODE>
+__global__ void __launch_bounds__(ZP_NTT_THREADS, 3)
+k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict__ B, int64_t EB, uint64_t* __restrict__ O,
+          int64_t EO, int logn, int logRp, int logseg, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1, uint64_t Kq2) {
+  extern __shared__ __align__(16) uint64_t ntt_mul_smem[];  // 2 x 32 KB (dynamic: above the 48 KB static limit)
+  uint64_t *sm = ntt_mul_smem, *smA = ntt_mul_smem + ZP_NTT_SMEM;  // the working tile; the first operand's transform
+  const int jp = blockIdx.y;
+  const ZpMod q = cx.q[jp];
+  const uint64_t Kq = jp == 0 ? Kq0 : jp == 1 ? Kq1 : Kq2;
+  const int T = threadIdx.x;
+  const int64_t c0 = (int64_t)blockIdx.x * ZP_NTT_C;  // first word of the chunk in the driving buffer (O / A)
+  const int64_t Edrv = MODE == 0 ? EO : EA;
+  const uint32_t segmask = (1u << logseg) - 1;
+  const ulonglong2 *Tlo = cx.Tlo[jp], *Thi = cx.Thi[jp];
+  A += (int64_t)jp * EA;
+  B += (int64_t)jp * EB;
+  O += (int64_t)jp * EO;
+  // Segments of at least a chunk (logseg >= 12): the chunk lies in ONE segment, seg0, at the positions pos0 + e, and
+  // (transforms longer than a chunk, logRp > 0, have logn = 12) in one row of its parent: word e is twisted by
+  // w^((bc e) << tsh).  Shorter segments: several per chunk, no twist; the segment of word e is seg0 + ((pos0 + e) >> logseg).
+  const uint32_t seg0 = (uint32_t)(c0 >> logseg), pos0 = (uint32_t)c0 & segmask;
+  const uint32_t bc = logRp ? brev_bits((pos0 >> logn) & ((1u << logRp) - 1), logRp) : 0;
+  const int tsh = ZP_NTT_LOGMAX - logn - logRp;
+  const uint32_t Pu = (uint32_t)P, t0 = seg0 % Pu;
+  // the first (and in MODE 0 the second) operand's chunk -> forward stages; the first one's transform is parked in smA
+#pragma unroll 1
+  for (int which = 0; which < (MODE == 0 ? 2 : 1); ++which) {
+#pragma unroll 4
+    for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+      const int e = T + ZP_NTT_THREADS * m;
+      uint64_t v = 0;
+      if (c0 + e < Edrv) {
+        if (MODE == 0) {
+          const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+          v = A[((int64_t)(2 * seg + which) << logseg) | pos];
+        } else {
+          v = A[c0 + e];
+        }
+        if (logRp) v = ntt_twist<false>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
+      }
+      sm[ntt_pad(e)] = v;
     }
-    const uint64_t a = A[(int64_t)j * EA + (ia << logn) + i];
-    uint64_t b = B[(int64_t)j * EB + (ib << logn) + i];  // lazy, < 4q
-    b = (b >= 2 * q.p) ? b - 2 * q.p : b;
-    b = (b >= q.p) ? b - q.p : b;
-    O[(int64_t)j * EO + e] = mont_mul(mont_mul(a, b, q), Kq, q);
+    __syncthreads();
+    ntt_tile<false>(sm, logn - 1, 0, cx.U[jp], q);
+    if (which == 0) {
+#pragma unroll 4
+      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) smA[T + ZP_NTT_THREADS * m] = sm[T + ZP_NTT_THREADS * m];  // same swizzle
+      __syncthreads();  // the working tile is reused
+    }
+  }
+#pragma unroll 1
+  for (int side = 0; side < (MODE == 0 ? 1 : 2); ++side) {
+    if (MODE == 0) {  // the second operand's transform is in the working tile
+#pragma unroll 4
+      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+        const int se = T + ZP_NTT_THREADS * m;  // any order: the product is position-wise
+        sm[se] = mont_mul(mont_mul(smA[se], ntt_canon4(sm[se], q), q), Kq, q);
+      }
+    } else {  // the sibling's transform at the same positions of its segment: all 16 loads of a lane in flight together
+      uint64_t b[ZP_NTT_C / ZP_NTT_THREADS];
+#pragma unroll
+      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+        const int e = T + ZP_NTT_THREADS * m;
+        const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+        const uint32_t tsk = (logseg >= ZP_NTT_LOGC) ? t0 : seg % Pu;  // uniform branch: the division only for short segments
+        b[m] = (c0 + e < Edrv) ? __ldg(B + (((int64_t)(2 * tsk + 1 - side) << logseg) | pos)) : 0;
+      }
+#pragma unroll
+      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+        const int se = ntt_pad(T + ZP_NTT_THREADS * m);
+        sm[se] = mont_mul(mont_mul(smA[se], ntt_canon4(b[m], q), q), Kq, q);
+      }
+    }
+    __syncthreads();
+    ntt_tile<true>(sm, logn - 1, 0, cx.Ui[jp], q);
+#pragma unroll 4
+    for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
+      const int e = T + ZP_NTT_THREADS * m;
+      if (c0 + e >= Edrv) continue;
+      uint64_t v = sm[ntt_pad(e)];
+      if (logRp) v = ntt_twist<true>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
+      if (MODE == 0) {
+        O[c0 + e] = v;
+      } else {
+        const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+        O[((int64_t)(2 * seg + side) << logseg) | pos] = v;
+      }
+    }
+    __syncthreads();  // MODE 1: the tile is reused by the other side
   }
 }
 

@@ -178,16 +178,19 @@ k_sq_newton_prep1(const uint64_t* __restrict__ Mtop, int64_t t, const uint64_t* 
     X[2 * EX + e] = v;
   }
 }
-// Y[0][i] = e_i = (f alpha)_{k+i}, i < k, zero-padded to n (O = inverse transform of the first product)
+// second product of the step: X[0][i] = e_i = (f alpha)_{k+i}, i < k (O = inverse transform of the first product),
+// X[1][i] = alpha_i, i < k, both zero-padded to n
 __global__ void __launch_bounds__(256)
-k_sq_newton_mid(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ Y) {
-  const int64_t n = (int64_t)1 << logn, k = n >> 1;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+k_sq_newton_mid(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, const uint64_t* __restrict__ alpha,
+                uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, k = n >> 1, EX = 2 * n;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t i = e & (n - 1);
     uint64_t v = 0;
-    if (i < k) v = ntt_crt(O[k + i], O[n + k + i], O[2 * n + k + i], cx, co, kp);
-    Y[i] = v;
-    Y[n + i] = v;
-    Y[2 * n + i] = v;
+    if (i < k) v = (e < n) ? ntt_crt(O[k + i], O[n + k + i], O[2 * n + k + i], cx, co, kp) : alpha[i];
+    X[e] = v;
+    X[EX + e] = v;
+    X[2 * EX + e] = v;
   }
 }
 // alpha_{k+i} = -(alpha e)_i, i < k

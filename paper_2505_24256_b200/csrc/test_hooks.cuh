@@ -135,8 +135,8 @@ int zippel_test_polymul(const uint64_t* a, int64_t na, const uint64_t* b, int64_
   uint64_t* O = (uint64_t*)((char*)X + al(8 * 3 * 2 * (size_t)n));
   const NttCtx cx = ntt_begin(w, st);
   ++g_launches, k_test_pm_prep<<<sq_blocks(2 * n), 256, 0, st>>>(a, na, b, nb, logn, k, X);
-  ntt_run(false, X, 2 * n, logn, cx, st);
   if (roundtrip) {
+    ntt_run(false, X, 2 * n, logn, cx, st);
     uint64_t Kq[3];
     make_kq(logn, Kq);
     ++g_launches, k_test_canon<<<dim3(sq_blocks(2 * n), 3), 256, 0, st>>>(X, 2 * n, 1, cx, Kq[0], Kq[1], Kq[2]);
@@ -145,8 +145,7 @@ int zippel_test_polymul(const uint64_t* a, int64_t na, const uint64_t* b, int64_
     cudaMemcpyAsync(out, X, 8 * 6 * (size_t)n, cudaMemcpyDeviceToDevice, st);
     return cuda_ok();
   }
-  ntt_pointwise(X, 2 * n, X, 2 * n, O, n, logn, 0, 1, cx, st);
-  ntt_run(true, O, n, logn, cx, st);
+  ntt_mul_pairs(X, 2 * n, O, logn, cx, st);
   ++g_launches, k_test_pm_fin<<<sq_blocks(na + nb - 1), 256, 0, st>>>(O, logn, na + nb - 1, cx, make_crt_out(k, 0), k, out);
   return cuda_ok();
 }

@@ -361,31 +361,71 @@ inline unsigned sq_blocks(int64_t n, int per = 256) {
   const int64_t cap = (int64_t)sm_count() * 64;
   return (unsigned)(b < 1 ? 1 : (b > cap ? cap : b));
 }
-// transform every segment of `buf` ([3][E] words, segments of 2^logn) in place (ntt.cuh: one to three passes)
-void ntt_run(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
-  const dim3 g((unsigned)((E + ZP_NTT_C - 1) / ZP_NTT_C), 3);
-  int lr1 = 0, lr2 = 0;  // rows of the strided passes
+// Pass plan of a transform of length 2^logn (ntt.cuh): up to two strided passes of lr1 and lr2 stages, then the chunk
+// stages (lc <= 12 of them) on rows that are twisted by their parent's row index (lrp stages above them).
+struct NttPlan {
+  int lr1 = 0, lr2 = 0, lc, lrp;
+};
+NttPlan ntt_plan(int logn) {
+  NttPlan pl;
   if (logn > ZP_NTT_LOGC) {
     const int e = logn - ZP_NTT_LOGC;
-    if (e <= 9) lr1 = e;
-    else lr1 = (e + 1) / 2, lr2 = e - lr1;
+    if (e <= 9) pl.lr1 = e;
+    else pl.lr1 = (e + 1) / 2, pl.lr2 = e - pl.lr1;
   }
+  pl.lc = logn - pl.lr1 - pl.lr2;
+  pl.lrp = pl.lr2 ? pl.lr2 : pl.lr1;
+  return pl;
+}
+inline dim3 ntt_grid(int64_t E) { return dim3((unsigned)((E + ZP_NTT_C - 1) / ZP_NTT_C), 3); }
+// the strided passes alone, on every segment of `buf` ([3][E] words, segments of 2^logn), in place
+void ntt_strided(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
+  const NttPlan pl = ntt_plan(logn);
+  const dim3 g = ntt_grid(E);
   if (!inverse) {
-    if (lr1) ++g_launches, k_ntt_strided<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, lr1, 0, cx);
-    if (lr2) ++g_launches, k_ntt_strided<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1, lr2, lr1, cx);
-    ++g_launches, k_ntt_chunk<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1 - lr2, lr2 ? lr2 : lr1, cx);
+    if (pl.lr1) ++g_launches, k_ntt_pass<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, pl.lr1, 0, cx);
+    if (pl.lr2) ++g_launches, k_ntt_pass<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx);
   } else {
-    ++g_launches, k_ntt_chunk<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1 - lr2, lr2 ? lr2 : lr1, cx);
-    if (lr2) ++g_launches, k_ntt_strided<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - lr1, lr2, lr1, cx);
-    if (lr1) ++g_launches, k_ntt_strided<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, lr1, 0, cx);
+    if (pl.lr2) ++g_launches, k_ntt_pass<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx);
+    if (pl.lr1) ++g_launches, k_ntt_pass<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, pl.lr1, 0, cx);
   }
 }
-void ntt_pointwise(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* O, int64_t EO, int logn, int mode,
-                   int64_t P, const NttCtx& cx, cudaStream_t st) {
+// complete transforms of every segment, in place (one to three passes)
+void ntt_run(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
+  const NttPlan pl = ntt_plan(logn);
+  if (!inverse) {
+    ntt_strided(false, buf, E, logn, cx, st);
+    ++g_launches, k_ntt_pass<false><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, pl.lc, 0, pl.lrp, cx);
+  } else {
+    ++g_launches, k_ntt_pass<true><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, pl.lc, 0, pl.lrp, cx);
+    ntt_strided(true, buf, E, logn, cx, st);
+  }
+}
+// products of segments of 2^logn words (k_ntt_mul): the strided passes on the operands, the fused chunk kernel, the
+// strided passes on the product.
+//   pairs: O segment o = X segment 2o * X segment 2o + 1 (EO = EX / 2); X is overwritten by its strided passes
+void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx& cx, cudaStream_t st) {
+  const NttPlan pl = ntt_plan(logn);
+  const int64_t EO = EX / 2;
   uint64_t Kq[3];
   make_kq(logn, Kq);
-  const dim3 g(sq_blocks(EO), 3);
-  ++g_launches, k_ntt_pointwise<<<g, 256, 0, st>>>(A, EA, B, EB, O, EO, logn, mode, P, cx, Kq[0], Kq[1], Kq[2]);
+  ntt_strided(false, X, EX, logn, cx, st);
+  cudaFuncSetAttribute(k_ntt_mul<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * ZP_NTT_SMEM);
+  ++g_launches, k_ntt_mul<0><<<ntt_grid(EO), ZP_NTT_THREADS, 16 * ZP_NTT_SMEM, st>>>(X, EX, nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq[0], Kq[1], Kq[2]);
+  ntt_strided(true, O, EO, logn, cx, st);
+}
+//   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds complete
+//   transforms (ntt_run); Y is overwritten by its strided passes
+void ntt_mul_down(uint64_t* Y, int64_t EY, const uint64_t* Xhat, int64_t EX, uint64_t* O, int logn, int64_t P, const NttCtx& cx,
+                  cudaStream_t st) {
+  const NttPlan pl = ntt_plan(logn);
+  const int64_t EO = 2 * EY;
+  uint64_t Kq[3];
+  make_kq(logn, Kq);
+  ntt_strided(false, Y, EY, logn, cx, st);
+  cudaFuncSetAttribute(k_ntt_mul<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * ZP_NTT_SMEM);
+  ++g_launches, k_ntt_mul<1><<<ntt_grid(EY), ZP_NTT_THREADS, 16 * ZP_NTT_SMEM, st>>>(Y, EY, Xhat, EX, O, EO, pl.lc, pl.lrp, logn, P, cx, Kq[0], Kq[1], Kq[2]);
+  ntt_strided(true, O, EO, logn, cx, st);
 }
 // the per-call context: host constants + this workspace's tables (built by the first launch of the call)
 NttCtx ntt_begin(const Ws& w, cudaStream_t st) {
@@ -452,9 +492,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       if (P) {
         const int64_t EX = 2 * P * n, EO = P * n;
         ++g_launches, k_sq_up_prep<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_X, EX);
-        ntt_run(false, w.sq_X, EX, logn, cx, st);
-        ntt_pointwise(w.sq_X, EX, w.sq_X, EX, w.sq_O, EO, logn, 0, P, cx, st);
-        ntt_run(true, w.sq_O, EO, logn, cx, st);
+        ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
         ++g_launches, k_sq_up_fin<<<sq_blocks(EO), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_O, EO, cx, co1, k, lev(l + 1));
       }
       const int nc = (int)(copy1[l] - copy0[l]);
@@ -475,22 +513,16 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       const int logn = ceil_log2(2 * kk);
       const int64_t n = 2 * kk;
       ++g_launches, k_sq_newton_prep1<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
-      ntt_run(false, w.sq_X, 2 * n, logn, cx, st);
-      ntt_pointwise(w.sq_X, 2 * n, w.sq_X, 2 * n, w.sq_O, n, logn, 0, 1, cx, st);
-      ntt_run(true, w.sq_O, n, logn, cx, st);
-      ++g_launches, k_sq_newton_mid<<<sq_blocks(n), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_Y);
-      ntt_run(false, w.sq_Y, n, logn, cx, st);
-      ntt_pointwise(w.sq_Y, n, w.sq_X, 2 * n, w.sq_O, n, logn, 2, 1, cx, st);
-      ntt_run(true, w.sq_O, n, logn, cx, st);
+      ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
+      ++g_launches, k_sq_newton_mid<<<sq_blocks(2 * n), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_alpha, w.sq_X);
+      ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
       ++g_launches, k_sq_newton_fin<<<sq_blocks(kk), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_alpha);
     }
     SQ_DUMP(2, w.sq_alpha, t);
     const int logn = ceil_log2(2 * t);
     const int64_t n = (int64_t)1 << logn;
     ++g_launches, k_sq_root_prep<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
-    ntt_run(false, w.sq_X, 2 * n, logn, cx, st);
-    ntt_pointwise(w.sq_X, 2 * n, w.sq_X, 2 * n, w.sq_O, n, logn, 0, 1, cx, st);
-    ntt_run(true, w.sq_O, n, logn, cx, st);
+    ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
     ++g_launches, k_sq_root_fin<<<sq_blocks(t), 256, 0, st>>>(w.sq_O, logn, t, cx, co2, k, cur + (size_t)B * T + off);
   }
   SQ_DUMP(3, cur, (size_t)V * T);
@@ -507,9 +539,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
         const int nv = (V - v0 < w.sq.Vc) ? V - v0 : w.sq.Vc;
         const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
         ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
-        ntt_run(false, w.sq_Y, EY, logn, cx, st);
-        ntt_pointwise(w.sq_Y, EY, w.sq_X, EX, w.sq_O, EO, logn, 1, P, cx, st);
-        ntt_run(true, w.sq_O, EO, logn, cx, st);
+        ntt_mul_down(w.sq_Y, EY, w.sq_X, EX, w.sq_O, logn, P, cx, st);
         ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
                                                                     nxt + (size_t)v0 * T);
       }
