@@ -143,7 +143,14 @@ def load_workload(idx: int, seed_shift: int, F_override):
 
 
 # the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_LEAF, g_subq_min_t)
-SQ_LEAF, SQ_MIN_T, SQ_KB = 1024, 8192, 1024
+SQ_LEAF, SQ_KB = 1024, 1024
+
+
+def sq_threshold(ts, B):
+    """csrc/zippel_capi.cu sq_threshold: functions with at least this many terms take the sub-quadratic route."""
+    if sum(int(t) for t in ts if int(t) >= 3072) >= 65536:
+        return 3072
+    return 3072 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 16384
 C_MONT = 18  # Montgomery product: 8 wide + 2 low
 
 
@@ -190,9 +197,10 @@ def subq_units(t, B):
 
 def work_model(ts, B, nv, newton=True, balanced=False, c_mm=C_MM, c_mac=C_MAC):
     """Algorithmic multiplier-pipe units (SURVEY.md 8(d).4 formula), total and for the node-solve kernel."""
-    long_ts = [int(t) for t in ts if int(t) >= SQ_MIN_T]
+    thr = sq_threshold(ts, B) if len(ts) else 0
+    long_ts = [int(t) for t in ts if int(t) >= thr]
     if long_ts:  # sub-quadratic route for the long functions, the quadratic formula for the rest
-        short = [int(t) for t in ts if int(t) < SQ_MIN_T]
+        short = [int(t) for t in ts if int(t) < thr]
         tot_s, ns_s = work_model(short, B, nv, newton, balanced, c_mm, c_mac) if short else (0.0, 0.0)
         T = float(sum(long_ts))
         sq = sum(subq_units(t, B)[0] for t in long_ts)
@@ -276,7 +284,7 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
                     + (" (PAPER.md L250: the largest skeleton, 4.8m monomials)" if idx == 9 else ""))
         in_bytes = w.exps.nbytes + w.vals.nbytes + w.anchors.nbytes + w.samples.nbytes
         out_bytes = w.vals.nbytes + 4 * F
-    subq = int(max(ts)) >= SQ_MIN_T
+    subq = int(max(ts)) >= sq_threshold(ts, B)
 
     def barrier():
         if world > 1:

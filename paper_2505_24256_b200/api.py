@@ -33,7 +33,7 @@ EXPORTS = (
     "zippel_set_tuning", "zippel_shutdown",
 )
 TUNE_SUBQ_MIN_T = 1
-SUBQ_MIN_T_DEFAULT = 8192  # g_subq_min_t in csrc/zippel_capi.cu
+SUBQ_MIN_T_DEFAULT = 0  # g_subq_min_t in csrc/zippel_capi.cu: 0 = the built-in rule (sq_threshold)
 K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
 
 

@@ -1033,115 +1033,229 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
 // ------------------------------------------------------------------------------------------------
 // (f1) skeleton extension between two lifting steps: the pairs (term i,
 // degree d) with a non-zero monomial coefficient become the terms of the next skeleton, in the order i
-// ascending, d ascending.  HBM-bound stream compaction in three launches:
-//   k_ext_count   one lane per term: 64-bit mask of its non-zero degrees (B <= 64), block-exclusive scan of the
-//                 popcounts, block totals; per-function maximum degree (early-termination test)
-//   k_ext_scan    exclusive scan of the block totals (one CTA)
-//   k_ext_emit    one lane per term: writes its rows (exps row, d) and coefficients, and the new offsets
-// The coefficient matrix is read once (the emit pass re-reads only the non-zero entries).
+// ascending, d ascending.  An HBM-bound stream compaction in ONE pass over the coefficient matrix:
+//   a CTA takes the next block of 256 consecutive terms (a ticket, so that blocks start in index order), reads their
+//   B coefficients (unit-stride rows), keeps a 64-bit mask of the non-zero degrees per term (B <= 64), scans the
+//   popcounts inside the block, obtains the number of rows emitted by all earlier blocks by a decoupled look-back
+//   over the per-block descriptors {flag, count} (flag 1: the block's own count, 2: the inclusive prefix; one 64-bit
+//   word each, so a plain load sees a consistent pair), and writes its rows (exps row, d), coefficients (re-read: the
+//   lines are still in L1 / L2), the new offsets of the functions that start inside the block and the per-function
+//   maximum degree (the early-termination test).
+// desc: [nb + 1] words, zeroed before the launch; desc[nb] is the ticket counter.  stage_rows: rows of the staging buffer in
+// dynamic shared memory (stage_rows x (8 + 2 (nv + 1)) bytes, then the block's exponent rows, 2 nv BLOCK bytes + 16); blocks
+// that emit more rows than that write them directly.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K9_THREADS 256
-__global__ void __launch_bounds__(ZP_K9_THREADS)
-k_ext_count(const uint64_t* __restrict__ coefs, int64_t T_tot, int B, const int64_t* __restrict__ offsets, int F,
-            ZpMod k, uint64_t* __restrict__ mask, int32_t* __restrict__ lpos, int64_t* __restrict__ bsum,
-            int32_t* __restrict__ degs) {
+#define ZP_K9_ITEMS 8  // consecutive terms per lane: 64 contiguous bytes of every coefficient row
+#define ZP_K9_BLOCK (ZP_K9_THREADS * ZP_K9_ITEMS)
+__global__ void __launch_bounds__(ZP_K9_THREADS, 3)
+k_ext_fused(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restrict__ coefs, int64_t T_tot, int B,
+            const int64_t* __restrict__ offsets, int F, ZpMod k, unsigned long long* __restrict__ desc, int64_t nb,
+            uint16_t* __restrict__ new_exps, uint64_t* __restrict__ new_coefs, int64_t cap, int64_t* __restrict__ new_offsets,
+            int32_t* __restrict__ degs, int stage_rows) {
   __shared__ int32_t wsum[ZP_K9_THREADS / 32];
-  const int64_t i = (int64_t)blockIdx.x * ZP_K9_THREADS + threadIdx.x;
-  uint64_t m = 0;
-  if (i < T_tot) {
-    int d = 0;
-    for (; d + 8 <= B; d += 8) {  // eight independent loads in flight per lane (the pass is a pure HBM stream)
-      uint64_t v[8];
+  __shared__ long long s_base;
+  __shared__ int s_bid, s_flo, s_fhi;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_bid = (int)atomicAdd(desc + nb, 1ull);
+  __syncthreads();
+  const int64_t bid = s_bid;
+  const int64_t i0 = bid * ZP_K9_BLOCK, i1 = i0 + (int64_t)threadIdx.x * ZP_K9_ITEMS;  // this lane: terms i1 .. i1 + 7
+  // ---- the one pass over the coefficients: masks of the non-zero degrees of the lane's terms
+  uint64_t m[ZP_K9_ITEMS], c1[ZP_K9_ITEMS];  // c1: the term's first non-zero coefficient (no second read for it)
 #pragma unroll
-      for (int x = 0; x < 8; ++x) v[x] = __ldcs(coefs + (int64_t)(d + x) * T_tot + i);
+  for (int x = 0; x < ZP_K9_ITEMS; ++x) m[x] = c1[x] = 0;
+  if (i1 + ZP_K9_ITEMS <= T_tot && (T_tot & 1) == 0) {  // whole group, rows 16-byte aligned: four 16-byte loads per row
+#pragma unroll 3
+    for (int d = 0; d < B; ++d) {
+      const ulonglong2* src = reinterpret_cast<const ulonglong2*>(coefs + (int64_t)d * T_tot + i1);
+      ulonglong2 v[ZP_K9_ITEMS / 2];
 #pragma unroll
-      for (int x = 0; x < 8; ++x) m |= (uint64_t)(zp_canon(v[x], k.p) != 0) << (d + x);
-    }
-    for (; d < B; ++d) m |= (uint64_t)(zp_canon(__ldcs(coefs + (int64_t)d * T_tot + i), k.p) != 0) << d;
-    mask[i] = m;
-  }
-  {  // per-function maximum degree: one atomic per warp when the warp lies inside one function (the usual case)
-    int lo = 0;
-    if (i < T_tot) {  // function of term i: offsets[f] <= i < offsets[f+1]
-      int hi = F;
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (offsets[mid] <= i) lo = mid; else hi = mid;
+      for (int x = 0; x < ZP_K9_ITEMS / 2; ++x) v[x] = __ldcs(src + x);
+#pragma unroll
+      for (int x = 0; x < ZP_K9_ITEMS; ++x) {
+        const uint64_t cv = zp_canon((x & 1) ? v[x >> 1].y : v[x >> 1].x, k.p);
+        c1[x] = m[x] ? c1[x] : cv;
+        m[x] |= (uint64_t)(cv != 0) << d;
       }
     }
-    const int deg = m ? 63 - __clzll((long long)m) : -1;
-    const unsigned full = 0xffffffffu;
-    const int f0 = __shfl_sync(full, lo, 0);
-    if (__all_sync(full, lo == f0 || i >= T_tot)) {
-      const int wmax = __reduce_max_sync(full, deg);
-      if ((threadIdx.x & 31) == 0 && wmax >= 0) atomicMax(&degs[f0], wmax);
-    } else if (deg >= 0) {
-      atomicMax(&degs[lo], deg);
-    }
+  } else {
+    for (int d = 0; d < B; ++d)
+#pragma unroll
+      for (int x = 0; x < ZP_K9_ITEMS; ++x)
+        if (i1 + x < T_tot) {
+          const uint64_t cv = zp_canon(coefs[(int64_t)d * T_tot + i1 + x], k.p);
+          c1[x] = m[x] ? c1[x] : cv;
+          m[x] |= (uint64_t)(cv != 0) << d;
+        }
   }
-  const int c = __popcll(m);
-  int incl = c;  // inclusive scan inside the warp
+  // ---- the block's exponent rows -> shared memory (unit-stride 16-byte loads; in flight during the scan and the look-back)
+  extern __shared__ __align__(16) unsigned char ext_smem[];
+  uint64_t* sc = reinterpret_cast<uint64_t*>(ext_smem);                               // [stage_rows] coefficients
+  uint16_t* sr = reinterpret_cast<uint16_t*>(ext_smem + 8 * (size_t)stage_rows);      // [stage_rows x (nv + 1)] rows
+  uint16_t* se = sr + (size_t)stage_rows * (nv + 1) + ((stage_rows * (nv + 1)) & 1 ? 1 : 0) + 0;  // [BLOCK x nv] exponents
+  se = reinterpret_cast<uint16_t*>((reinterpret_cast<uintptr_t>(se) + 15) & ~(uintptr_t)15);
+  if (stage_rows) {
+    const int64_t nterm = (T_tot - i0 < ZP_K9_BLOCK) ? T_tot - i0 : ZP_K9_BLOCK;
+    const int n16 = (int)((nterm * nv * 2) / 16), rem0 = n16 * 8;  // 16-byte pieces, then the u16 tail
+    const uint4* src = reinterpret_cast<const uint4*>(exps + i0 * nv);  // i0 nv 2 bytes: a multiple of 16
+    for (int x = threadIdx.x; x < n16; x += ZP_K9_THREADS) reinterpret_cast<uint4*>(se)[x] = src[x];
+    for (int x = rem0 + threadIdx.x; x < nterm * nv; x += ZP_K9_THREADS) se[x] = exps[i0 * nv + x];
+  }
+  // ---- block scan of the lanes' row counts
+  int c = 0;
+#pragma unroll
+  for (int x = 0; x < ZP_K9_ITEMS; ++x) c += __popcll(m[x]);
+  int incl = c;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
     const int v = __shfl_up_sync(0xffffffffu, incl, o);
-    if ((threadIdx.x & 31) >= o) incl += v;
+    if (lane >= o) incl += v;
   }
-  if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = incl;
-  __syncthreads();
-  int base = 0;
-  for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) base += wsum[w];
-  if (i < T_tot) lpos[i] = base + incl - c;
-  if (threadIdx.x == ZP_K9_THREADS - 1) bsum[blockIdx.x] = base + incl;
-}
-
-__global__ void __launch_bounds__(1024)
-k_ext_scan(int64_t* __restrict__ bsum, int64_t nb) {  // in place: exclusive prefix; bsum[nb] = total
-  __shared__ int64_t part[1024];
-  const int64_t chunk = (nb + 1023) / 1024;
-  const int64_t lo = (int64_t)threadIdx.x * chunk, hi = (lo + chunk < nb) ? lo + chunk : nb;
-  int64_t s = 0;
-  for (int64_t x = lo; x < hi; ++x) s += bsum[x];
-  part[threadIdx.x] = s;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    int64_t run = 0;
-    for (int x = 0; x < 1024; ++x) {
-      const int64_t v = part[x];
-      part[x] = run;
-      run += v;
+  if (lane == 31) wsum[warp] = incl;
+  if (threadIdx.x == 0) {  // functions that start inside the block: flo = first f with offsets[f] >= i0, fhi = first beyond
+    int lo = 0, hi = F + 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (offsets[mid] < i0) lo = mid + 1; else hi = mid;
     }
-    bsum[nb] = run;
+    s_flo = lo;
+    hi = F + 1;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (offsets[mid] < i0 + ZP_K9_BLOCK) lo = mid + 1; else hi = mid;
+    }
+    s_fhi = lo;
   }
   __syncthreads();
-  int64_t run = part[threadIdx.x];
-  for (int64_t x = lo; x < hi; ++x) {
-    const int64_t v = bsum[x];
-    bsum[x] = run;
-    run += v;
+  int base_w = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < ZP_K9_THREADS / 32; ++w) {
+    if (w < warp) base_w += wsum[w];
+    total += wsum[w];
   }
-}
-
-__global__ void __launch_bounds__(ZP_K9_THREADS)
-k_ext_emit(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restrict__ coefs, int64_t T_tot, ZpMod k,
-           const uint64_t* __restrict__ mask, const int32_t* __restrict__ lpos, const int64_t* __restrict__ bsum,
-           const int64_t* __restrict__ offsets, int F, uint16_t* __restrict__ new_exps, uint64_t* __restrict__ new_coefs,
-           int64_t cap, int64_t* __restrict__ new_offsets) {
-  const int64_t i = (int64_t)blockIdx.x * ZP_K9_THREADS + threadIdx.x;
-  if (i <= F) {  // the first F+1 lanes also translate the offsets
-    const int64_t o = offsets[i];
-    new_offsets[i] = (o < T_tot) ? bsum[o / ZP_K9_THREADS] + lpos[o] : bsum[(T_tot + ZP_K9_THREADS - 1) / ZP_K9_THREADS];
+  const int lpos = base_w + incl - c;
+  // ---- rows emitted by the earlier blocks: decoupled look-back by the first warp
+  if (warp == 0) {
+    volatile unsigned long long* vd = desc;
+    if (lane == 0) vd[bid] = ((bid == 0 ? 2ull : 1ull) << 62) | (unsigned long long)total;
+    long long excl = 0;
+    int64_t j = bid - 1;
+    while (j >= 0) {
+      const int64_t jj = j - lane;
+      unsigned long long w = 2ull << 62;  // before the first block: an inclusive prefix of 0
+      if (jj >= 0) {
+        do {
+          w = vd[jj];
+        } while ((w >> 62) == 0);
+      }
+      const unsigned fl = (unsigned)(w >> 62);
+      const unsigned done = __ballot_sync(0xffffffffu, fl == 2);
+      const int first = done ? __ffs(done) - 1 : 32;  // the nearest block that knows its inclusive prefix
+      long long v = (lane <= first) ? (long long)(w & ((1ull << 62) - 1)) : 0;
+#pragma unroll
+      for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      excl += v;
+      if (done) break;
+      j -= 32;
+    }
+    if (lane == 0) {
+      if (bid > 0) vd[bid] = (2ull << 62) | (unsigned long long)(excl + total);
+      s_base = excl;
+    }
   }
-  if (i >= T_tot) return;
-  uint64_t m = mask[i];
-  int64_t pos = bsum[blockIdx.x] + lpos[i];
-  while (m && pos < cap) {
-    const int d = __ffsll((long long)m) - 1;
-    m &= m - 1;
-    uint16_t* row = new_exps + pos * (nv + 1);
-    for (int j = 0; j < nv; ++j) row[j] = exps[i * nv + j];
-    row[nv] = (uint16_t)d;
-    new_coefs[pos] = zp_canon(coefs[(int64_t)d * T_tot + i], k.p);
-    ++pos;
+  __syncthreads();
+  const int64_t base = s_base;
+  const int flo = s_flo, fhi = s_fhi;
+  // ---- new offsets of the functions that start in this block (the lane that owns the first term writes); the total
+  for (int f = flo; f < fhi; ++f) {
+    const int64_t o = offsets[f] - i1;
+    if (o >= 0 && o < ZP_K9_ITEMS && offsets[f] < T_tot) {
+      int before = 0;
+#pragma unroll
+      for (int x = 0; x < ZP_K9_ITEMS; ++x) before += (x < o) ? __popcll(m[x]) : 0;
+      new_offsets[f] = base + lpos + before;
+    }
+  }
+  if (i0 + ZP_K9_BLOCK >= T_tot && threadIdx.x == 0) new_offsets[F] = base + total;
+  // ---- per-function maximum degree (the early-termination test): function of a term = the last start at or before
+  // it; one atomic per warp when the warp lies inside one function (the usual case), else one per term
+  auto fn_of = [&](int64_t i) {
+    int lo = flo > 0 ? flo - 1 : 0, hi = fhi;  // offsets[lo] <= i; find the last g < hi with offsets[g] <= i
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (offsets[mid] <= i) lo = mid; else hi = mid;
+    }
+    return lo;
+  };
+  if (i1 < T_tot) {
+    const int64_t ilast = (i1 + ZP_K9_ITEMS <= T_tot ? i1 + ZP_K9_ITEMS : T_tot) - 1;
+    const int fa = fn_of(i1), fb = (flo == fhi) ? fa : fn_of(ilast);
+    uint64_t all = 0;
+#pragma unroll
+    for (int x = 0; x < ZP_K9_ITEMS; ++x) all |= m[x];
+    const int deg = all ? 63 - __clzll((long long)all) : -1;
+    const unsigned act = __activemask();
+    const int f0 = __shfl_sync(act, fa, __ffs(act) - 1);
+    if (__all_sync(act, fa == f0 && fb == f0)) {
+      const int wmax = __reduce_max_sync(act, deg);
+      if (lane == __ffs(act) - 1 && wmax >= 0) atomicMax(&degs[f0], wmax);
+    } else if (fa == fb) {
+      if (deg >= 0) atomicMax(&degs[fa], deg);
+    } else {
+#pragma unroll
+      for (int x = 0; x < ZP_K9_ITEMS; ++x)
+        if (m[x]) atomicMax(&degs[fn_of(i1 + x)], 63 - __clzll((long long)m[x]));
+    }
+  }
+  // ---- emit.  Usual case (the block's rows fit the staging buffer): rows and coefficients go to shared memory at
+  // their local positions and the block writes its contiguous output range with unit-stride stores
+  if (total <= stage_rows && base + total <= cap) {  // uniform
+    const int rw = nv + 1;
+    if (i1 < T_tot) {
+      int lp = lpos;
+#pragma unroll
+      for (int x = 0; x < ZP_K9_ITEMS; ++x) {
+        uint64_t mm = m[x];
+        const int64_t i = i1 + x;
+        bool first = true;
+        while (mm) {
+          const int d = __ffsll((long long)mm) - 1;
+          mm &= mm - 1;
+          uint16_t* row = sr + lp * rw;
+          const uint16_t* er = se + (i - i0) * nv;
+          for (int j = 0; j < nv; ++j) row[j] = er[j];
+          row[nv] = (uint16_t)d;
+          sc[lp] = first ? c1[x] : zp_canon(coefs[(int64_t)d * T_tot + i], k.p);
+          first = false;
+          ++lp;
+        }
+      }
+    }
+    __syncthreads();
+    for (int x = threadIdx.x; x < total; x += ZP_K9_THREADS) new_coefs[base + x] = sc[x];
+    uint16_t* dst = new_exps + base * rw;
+    for (int x = threadIdx.x; x < total * rw; x += ZP_K9_THREADS) dst[x] = sr[x];
+    return;
+  }
+  if (i1 >= T_tot) return;
+  int64_t pos = base + lpos;
+#pragma unroll
+  for (int x = 0; x < ZP_K9_ITEMS; ++x) {
+    uint64_t mm = m[x];
+    const int64_t i = i1 + x;
+    bool first = true;
+    while (mm && pos < cap) {
+      const int d = __ffsll((long long)mm) - 1;
+      mm &= mm - 1;
+      uint16_t* row = new_exps + pos * (nv + 1);
+      for (int j = 0; j < nv; ++j) row[j] = exps[i * nv + j];
+      row[nv] = (uint16_t)d;
+      new_coefs[pos] = first ? c1[x] : zp_canon(coefs[(int64_t)d * T_tot + i], k.p);
+      first = false;
+      ++pos;
+    }
+    pos += __popcll(mm);  // rows beyond cap are counted, not written
   }
 }
 

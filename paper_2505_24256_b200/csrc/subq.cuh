@@ -130,16 +130,27 @@ k_sq_down_fin(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __rest
 }
 
 // ---- power-series inverse of f = rev(M):  f_0 = 1, f_i = M_{t-i} (i <= t), 0 beyond -------------------------------------
+// All the functions of a run go through the iteration together (one segment, or pair of segments, per function and
+// step).  SqFn describes a function; the host sorts the array by t, longest first, so that the functions still
+// iterating at precision k (t > k) are a prefix of it.
+struct SqFn {
+  int64_t moff;  // slot of the function's first node in the run: its top-level polynomial and its tails start there
+  int64_t aoff;  // first word of its inverse series alpha in the alpha buffer (room for its final precision)
+  int64_t t;
+};
 ZP_DEV uint64_t sq_f(const uint64_t* __restrict__ Mtop, int64_t t, int64_t i, const ZpMod& kp) {  // Montgomery
   return i == 0 ? kp.r1 : (i <= t ? Mtop[t - i] : 0);
 }
 // base case: alpha = 1 / f mod x^KB by Newton steps with schoolbook products in shared memory, one CTA per function
 #define ZP_SQ_KB 1024
 __global__ void __launch_bounds__(512)
-k_sq_inv_base(const uint64_t* __restrict__ Mtop, int64_t t, ZpMod kp, uint64_t* __restrict__ alpha) {
+k_sq_inv_base(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, ZpMod kp, uint64_t* __restrict__ alphas) {
   __shared__ uint64_t f[ZP_SQ_KB], g[ZP_SQ_KB], ev[ZP_SQ_KB / 2];
+  const SqFn fn = fns[blockIdx.x];
+  const uint64_t* Mtop = top + fn.moff;
+  uint64_t* alpha = alphas + fn.aoff;
   for (int i = threadIdx.x; i < ZP_SQ_KB; i += blockDim.x) {
-    f[i] = sq_f(Mtop, t, i, kp);
+    f[i] = sq_f(Mtop, fn.t, i, kp);
     g[i] = 0;
   }
   __syncthreads();
@@ -165,29 +176,33 @@ k_sq_inv_base(const uint64_t* __restrict__ Mtop, int64_t t, ZpMod kp, uint64_t* 
   }
   for (int i = threadIdx.x; i < ZP_SQ_KB; i += blockDim.x) alpha[i] = g[i];
 }
-// Newton step k -> 2k, first product: X[0] = f mod x^2k, X[1] = alpha mod x^k (n = 2k)
+// Newton step k -> 2k (n = 2k) for the first nact functions, first product: X[2s] = f_s mod x^2k, X[2s+1] = alpha_s mod x^k
 __global__ void __launch_bounds__(256)
-k_sq_newton_prep1(const uint64_t* __restrict__ Mtop, int64_t t, const uint64_t* __restrict__ alpha, int logn, ZpMod kp,
-                  uint64_t* __restrict__ X) {
-  const int64_t n = (int64_t)1 << logn, EX = 2 * n, k = n >> 1;
+k_sq_newton_prep1(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, int64_t nact, const uint64_t* __restrict__ alphas,
+                  int logn, ZpMod kp, uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, EX = 2 * nact * n, k = n >> 1;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t i = e & (n - 1);
-    const uint64_t v = (e < n) ? sq_f(Mtop, t, i, kp) : (i < k ? alpha[i] : 0);
+    const int64_t seg = e >> logn, i = e & (n - 1);
+    const SqFn fn = fns[seg >> 1];
+    const uint64_t v = (seg & 1) ? (i < k ? alphas[fn.aoff + i] : 0) : sq_f(top + fn.moff, fn.t, i, kp);
     X[e] = v;
     X[EX + e] = v;
     X[2 * EX + e] = v;
   }
 }
-// second product of the step: X[0][i] = e_i = (f alpha)_{k+i}, i < k (O = inverse transform of the first product),
-// X[1][i] = alpha_i, i < k, both zero-padded to n
+// second product of the step: X[2s][i] = e_i = (f alpha)_{k+i}, i < k (O = inverse transforms of the first products),
+// X[2s+1][i] = alpha_i, i < k, both zero-padded to n
 __global__ void __launch_bounds__(256)
-k_sq_newton_mid(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, const uint64_t* __restrict__ alpha,
-                uint64_t* __restrict__ X) {
-  const int64_t n = (int64_t)1 << logn, k = n >> 1, EX = 2 * n;
+k_sq_newton_mid(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t nact, int logn, NttCtx cx, CrtOut co,
+                ZpMod kp, const uint64_t* __restrict__ alphas, uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, k = n >> 1, EX = 2 * nact * n, EO = nact * n;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t i = e & (n - 1);
+    const int64_t seg = e >> logn, i = e & (n - 1), s = seg >> 1;
     uint64_t v = 0;
-    if (i < k) v = (e < n) ? ntt_crt(O[k + i], O[n + k + i], O[2 * n + k + i], cx, co, kp) : alpha[i];
+    if (i < k) {
+      const int64_t o = s * n + k + i;
+      v = (seg & 1) ? alphas[fns[s].aoff + i] : ntt_crt(O[o], O[EO + o], O[2 * EO + o], cx, co, kp);
+    }
     X[e] = v;
     X[EX + e] = v;
     X[2 * EX + e] = v;
@@ -195,31 +210,42 @@ k_sq_newton_mid(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, 
 }
 // alpha_{k+i} = -(alpha e)_i, i < k
 __global__ void __launch_bounds__(256)
-k_sq_newton_fin(const uint64_t* __restrict__ O, int logn, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ alpha) {
-  const int64_t n = (int64_t)1 << logn, k = n >> 1;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < k; i += (int64_t)gridDim.x * blockDim.x)
-    alpha[k + i] = mod_neg(ntt_crt(O[i], O[n + i], O[2 * n + i], cx, co, kp), kp.p);
+k_sq_newton_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t nact, int logn, NttCtx cx, CrtOut co,
+                ZpMod kp, uint64_t* __restrict__ alphas) {
+  const int64_t n = (int64_t)1 << logn, k = n >> 1, EO = nact * n;
+  for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < nact * k; x += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t s = x / k, i = x - s * k, o = s * n + i;
+    alphas[fns[s].aoff + k + i] = mod_neg(ntt_crt(O[o], O[EO + o], O[2 * EO + o], cx, co, kp), kp.p);
+  }
 }
-// root tail of M': X[0][i] = rev(M')_i = (t - i) f_i, X[1][i] = alpha_i, i < t, zero-padded to n >= 2t
+// root tails of M' for the functions fns[g0 .. g0 + ng), which share the product length n >= 2t:
+// X[2s][i] = rev(M')_i = (t - i) f_i, X[2s+1][i] = alpha_i, i < t, zero-padded to n
 __global__ void __launch_bounds__(256)
-k_sq_root_prep(const uint64_t* __restrict__ Mtop, int64_t t, const uint64_t* __restrict__ alpha, int logn, ZpMod kp,
-               uint64_t* __restrict__ X) {
-  const int64_t n = (int64_t)1 << logn, EX = 2 * n;
+k_sq_root_prep(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, int64_t ng, const uint64_t* __restrict__ alphas,
+               int logn, ZpMod kp, uint64_t* __restrict__ X) {
+  const int64_t n = (int64_t)1 << logn, EX = 2 * ng * n;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t i = e & (n - 1);
+    const int64_t seg = e >> logn, i = e & (n - 1);
+    const SqFn fn = fns[seg >> 1];
     uint64_t v = 0;
-    if (i < t) v = (e < n) ? mont_mul(sq_f(Mtop, t, i, kp), to_mont(zp_canon((uint64_t)(t - i), kp.p), kp), kp) : alpha[i];
+    if (i < fn.t)
+      v = (seg & 1) ? alphas[fn.aoff + i]
+                    : mont_mul(sq_f(top + fn.moff, fn.t, i, kp), to_mont(zp_canon((uint64_t)(fn.t - i), kp.p), kp), kp);
     X[e] = v;
     X[EX + e] = v;
     X[2 * EX + e] = v;
   }
 }
-// tail_k = (rev(M') alpha)_k, k < t: the power sums of the nodes, plain (co carries K = 2^-128)
+// tail_k = (rev(M') alpha)_k, k < t: the power sums of the nodes, plain (co carries K = 2^-128); tails: the M' row of the run
 __global__ void __launch_bounds__(256)
-k_sq_root_fin(const uint64_t* __restrict__ O, int logn, int64_t t, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ tail) {
-  const int64_t n = (int64_t)1 << logn;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < t; i += (int64_t)gridDim.x * blockDim.x)
-    tail[i] = ntt_crt(O[i], O[n + i], O[2 * n + i], cx, co, kp);
+k_sq_root_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t ng, int logn, NttCtx cx, CrtOut co, ZpMod kp,
+              uint64_t* __restrict__ tails) {
+  const int64_t n = (int64_t)1 << logn, EO = ng * n;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t s = e >> logn, i = e & (n - 1);
+    const SqFn fn = fns[s];
+    if (i < fn.t) tails[fn.moff + i] = ntt_crt(O[e], O[EO + e], O[2 * EO + e], cx, co, kp);
+  }
 }
 // root tails of the right-hand sides: the values themselves (canonicalised, reading G22)
 __global__ void __launch_bounds__(256)

@@ -2,6 +2,7 @@
 // workspace carving and kernel launches.  No torch types, no allocation, no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -45,7 +46,8 @@ bool make_mod(uint64_t p, ZpMod* k) {
 // order 2^24); tests/test_ntt_constants.py re-derives both facts with Python integers through zippel_ntt_constants().
 const uint64_t kNttQ[3] = {4611686017554972673ull, 4611686015004835841ull, 4611686009971671041ull};
 const uint64_t kNttGen[3] = {5, 3, 3};
-int64_t g_subq_min_t = 8192;  // functions with at least this many terms take the sub-quadratic route (zippel_set_tuning)
+int64_t g_subq_min_t = 0;  // > 0: functions with at least this many terms take the sub-quadratic route (zippel_set_tuning);
+                           // 0: the measured rule of sq_threshold below
 
 uint64_t h_mulmod(uint64_t a, uint64_t b, uint64_t m) { return (uint64_t)((u128)a * b % m); }
 uint64_t h_powmod(uint64_t a, uint64_t e, uint64_t m) {
@@ -115,10 +117,25 @@ struct SqRun {
 };
 struct SqSizes {
   bool any = false;
-  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0;
+  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0, maxFns = 0;
   int maxLev = 0, Vc = 1;
+  int64_t thr = 0;  // the threshold the runs were found with (sq_threshold on the whole batch)
 };
-inline bool sq_is_long(int64_t t) { return t >= g_subq_min_t && t > ZP_LEAF; }
+// Which functions take the sub-quadratic route: those with at least sq_threshold terms.  Measured on B200 (profiles/
+// r02_crossover.md): a batch with enough long functions to fill the GPU crosses over at t = 3072 for every B; a single
+// function (or a few) is bound by the latency of the route's ~170 dependent launches and crosses over later, the later
+// the fewer right-hand sides there are to amortise them (B = 1: 16384, B = 3: 8192, B = 9: 4096, B = 21: 3072).
+int64_t sq_threshold(const int64_t* h_offs, int F, int B) {
+  if (g_subq_min_t > 0) return g_subq_min_t;
+  int64_t sum = 0;
+  for (int f = 0; f < F; ++f) {
+    const int64_t t = h_offs[f + 1] - h_offs[f];
+    if (t >= 3072) sum += t;
+  }
+  if (sum >= 65536) return 3072;
+  return B >= 16 ? 3072 : B >= 6 ? 4096 : B >= 2 ? 8192 : 16384;
+}
+inline bool sq_is_long(int64_t t, int64_t thr) { return t >= thr && t > ZP_LEAF; }
 
 // pair and copy tasks of level l (children of size a = LEAF << l) for a run; slots relative to the run
 void sq_level_tasks(const int64_t* h_offs, const SqRun& r, int l, std::vector<SqTask>* pairs, std::vector<SqTask>* copies) {
@@ -137,16 +154,16 @@ void sq_level_tasks(const int64_t* h_offs, const SqRun& r, int l, std::vector<Sq
   }
 }
 
-void sq_find_runs(const int64_t* h_offs, int F, std::vector<SqRun>* runs) {
+void sq_find_runs(const int64_t* h_offs, int F, int64_t thr, std::vector<SqRun>* runs) {
   for (int f = 0; f < F;) {
-    if (!sq_is_long(h_offs[f + 1] - h_offs[f])) {
+    if (!sq_is_long(h_offs[f + 1] - h_offs[f], thr)) {
       ++f;
       continue;
     }
     SqRun r;
     r.f0 = f;
     r.tmax = 0;
-    while (f < F && sq_is_long(h_offs[f + 1] - h_offs[f])) {
+    while (f < F && sq_is_long(h_offs[f + 1] - h_offs[f], thr)) {
       const int64_t t = h_offs[f + 1] - h_offs[f];
       r.tmax = t > r.tmax ? t : r.tmax;
       ++f;
@@ -161,8 +178,9 @@ void sq_find_runs(const int64_t* h_offs, int F, std::vector<SqRun>* runs) {
 
 SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
   SqSizes z;
+  z.thr = sq_threshold(h_offs, F, B);
   std::vector<SqRun> runs;
-  sq_find_runs(h_offs, F, &runs);
+  sq_find_runs(h_offs, F, z.thr, &runs);
   if (runs.empty()) return z;
   z.any = true;
   auto mx = [](int64_t& a, int64_t b) { a = b > a ? b : a; };
@@ -184,19 +202,19 @@ SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
       ntasks += (int64_t)pairs.size() + (int64_t)copies.size();
     }
     mx(z.maxTasks, ntasks);
+    int64_t sumK = 0, sumR = 0;  // the functions of a run take the Newton steps and the root products together
     for (int f = r.f0; f < r.f1; ++f) {
       const int64_t t = h_offs[f + 1] - h_offs[f];
       leaves += (t + ZP_LEAF - 1) / ZP_LEAF;
       int64_t kf = ZP_SQ_KB;
       while (kf < t) kf <<= 1;
-      mx(z.alphaN, kf);
-      mx(z.maxX, 2 * kf);  // Newton's last step: n = kf
-      mx(z.maxY, kf);
-      mx(z.maxO, kf);
-      const int64_t nr = (int64_t)1 << ceil_log2(2 * t);  // root product
-      mx(z.maxX, 2 * nr);
-      mx(z.maxO, nr);
+      sumK += kf;                                 // final precision of alpha; Newton's last step: n = kf
+      sumR += (int64_t)1 << ceil_log2(2 * t);     // root product
     }
+    mx(z.alphaN, sumK);
+    mx(z.maxX, 2 * (sumK > sumR ? sumK : sumR));
+    mx(z.maxO, sumK > sumR ? sumK : sumR);
+    mx(z.maxFns, r.f1 - r.f0);
     mx(z.maxLeaves, leaves);
   }
   return z;
@@ -213,6 +231,7 @@ struct Ws {
   SqSizes sq;
   ulonglong2* ntt_tab;  // [3][4][4096]: U, Ui, Tlo, Thi per prime
   SqTask* sq_tasks;
+  SqFn* sq_fns;
   int64_t* sq_leafoffs;
   uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Y, *sq_O;
   size_t bytes;
@@ -248,6 +267,7 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags, const SqSizes& sq =
   if (sq.any) {
     w.ntt_tab = (ulonglong2*)take(16 * (size_t)12 * ZP_NTT_TAB);
     w.sq_tasks = (SqTask*)take(sizeof(SqTask) * (size_t)(sq.maxTasks + 1));
+    w.sq_fns = (SqFn*)take(sizeof(SqFn) * (size_t)(sq.maxFns + 1));
     w.sq_leafoffs = (int64_t*)take(8 * (size_t)(sq.maxLeaves + 1));
     w.sq_lev = (uint64_t*)take(8 * (size_t)(sq.maxLev + 1) * sq.maxT);
     w.sq_tailA = (uint64_t*)take(8 * (size_t)(B + 1) * sq.maxT);
@@ -505,25 +525,43 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   const int V = B + 1;
   uint64_t *cur = w.sq_tailA, *nxt = w.sq_tailB;
   ++g_launches, k_sq_load_vals<<<dim3(sq_blocks(T), (unsigned)(B < 64 ? B : 64)), 256, 0, st>>>(vals, ldv, B, T, k, cur, T);
-  for (int f = r.f0; f < r.f1; ++f) {
-    const int64_t off = h_offs[f] - r.a0, t = h_offs[f + 1] - h_offs[f];
-    const uint64_t* Mtop = lev(r.nlev) + off;
-    ++g_launches, k_sq_inv_base<<<1, 512, 0, st>>>(Mtop, t, k, w.sq_alpha);
-    for (int64_t kk = ZP_SQ_KB; kk < t; kk <<= 1) {  // precision kk -> 2 kk, products of length n = 2 kk
-      const int logn = ceil_log2(2 * kk);
-      const int64_t n = 2 * kk;
-      ++g_launches, k_sq_newton_prep1<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
-      ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
-      ++g_launches, k_sq_newton_mid<<<sq_blocks(2 * n), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_alpha, w.sq_X);
-      ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
-      ++g_launches, k_sq_newton_fin<<<sq_blocks(kk), 256, 0, st>>>(w.sq_O, logn, cx, co1, k, w.sq_alpha);
+  {
+    // the functions of the run, longest first: those still iterating at precision kk (t > kk) are a prefix
+    std::vector<SqFn> fns;
+    for (int f = r.f0; f < r.f1; ++f) fns.push_back(SqFn{h_offs[f] - r.a0, 0, h_offs[f + 1] - h_offs[f]});
+    std::stable_sort(fns.begin(), fns.end(), [](const SqFn& a, const SqFn& b) { return a.t > b.t; });
+    int64_t ao = 0;
+    for (SqFn& fn : fns) {
+      fn.aoff = ao;
+      int64_t kf = ZP_SQ_KB;
+      while (kf < fn.t) kf <<= 1;
+      ao += kf;
     }
-    SQ_DUMP(2, w.sq_alpha, t);
-    const int logn = ceil_log2(2 * t);
-    const int64_t n = (int64_t)1 << logn;
-    ++g_launches, k_sq_root_prep<<<sq_blocks(2 * n), 256, 0, st>>>(Mtop, t, w.sq_alpha, logn, k, w.sq_X);
-    ntt_mul_pairs(w.sq_X, 2 * n, w.sq_O, logn, cx, st);
-    ++g_launches, k_sq_root_fin<<<sq_blocks(t), 256, 0, st>>>(w.sq_O, logn, t, cx, co2, k, cur + (size_t)B * T + off);
+    cudaMemcpyAsync(w.sq_fns, fns.data(), sizeof(SqFn) * fns.size(), cudaMemcpyHostToDevice, st);
+    const uint64_t* top = lev(r.nlev);
+    ++g_launches, k_sq_inv_base<<<(unsigned)Fr, 512, 0, st>>>(top, w.sq_fns, k, w.sq_alpha);
+    for (int64_t kk = ZP_SQ_KB; kk < r.tmax; kk <<= 1) {  // precision kk -> 2 kk, products of length n = 2 kk
+      int64_t nact = 0;
+      while (nact < Fr && fns[nact].t > kk) ++nact;
+      const int logn = ceil_log2(2 * kk);
+      const int64_t n = 2 * kk, EX = 2 * nact * n;
+      ++g_launches, k_sq_newton_prep1<<<sq_blocks(EX), 256, 0, st>>>(top, w.sq_fns, nact, w.sq_alpha, logn, k, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
+      ++g_launches, k_sq_newton_mid<<<sq_blocks(EX), 256, 0, st>>>(w.sq_O, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
+      ++g_launches, k_sq_newton_fin<<<sq_blocks(nact * kk), 256, 0, st>>>(w.sq_O, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha);
+    }
+    SQ_DUMP(2, w.sq_alpha + fns[0].aoff, fns[0].t);
+    for (int g0 = 0; g0 < Fr;) {  // root products: the functions with the same product length n >= 2 t together
+      const int logn = ceil_log2(2 * fns[g0].t);
+      int g1 = g0;
+      while (g1 < Fr && ceil_log2(2 * fns[g1].t) == logn) ++g1;
+      const int64_t n = (int64_t)1 << logn, ng = g1 - g0, EX = 2 * ng * n;
+      ++g_launches, k_sq_root_prep<<<sq_blocks(EX), 256, 0, st>>>(top, w.sq_fns + g0, ng, w.sq_alpha, logn, k, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
+      ++g_launches, k_sq_root_fin<<<sq_blocks(ng * n), 256, 0, st>>>(w.sq_O, w.sq_fns + g0, ng, logn, cx, co2, k, cur + (size_t)B * T);
+      g0 = g1;
+    }
   }
   SQ_DUMP(3, cur, (size_t)V * T);
   // (down) level by level, vectors in chunks of Vc
@@ -619,7 +657,7 @@ void run_solve(const Ws& w, const int64_t* h_offs, const uint64_t* nodes, int F,
                const uint64_t* vals, int B, int s0, const ZpMod& k, uint64_t* coefs, cudaStream_t st) {
   ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_solve, F, ZP_ST_NONE);
   std::vector<SqRun> runs;
-  if (w.sq.any) sq_find_runs(h_offs, F, &runs);
+  if (w.sq.any) sq_find_runs(h_offs, F, w.sq.thr, &runs);
   if (runs.empty()) {
     run_solve_quadratic(w, nodes, F, h_offs[0], h_offs[F] - h_offs[0], T_tot, tmax, vals, B, s0, k, coefs, st);
     return;
@@ -1017,16 +1055,17 @@ int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F
   const Ws w = carve(workspace, T_tot, F, B, 0);
   cudaStream_t st = (cudaStream_t)stream;
   upload_offsets(w, h_offsets, F, st);
-  const int64_t nb = (T_tot + ZP_K9_THREADS - 1) / ZP_K9_THREADS;
-  uint64_t* mask = w.nodes;                                   // [T_tot]
-  int32_t* lpos = reinterpret_cast<int32_t*>(w.scale);        // [T_tot]
-  int64_t* bsum = reinterpret_cast<int64_t*>(w.tab);          // [nb + 1] (the slice holds 32 T_tot bytes)
+  const int64_t nb = (T_tot + ZP_K9_BLOCK - 1) / ZP_K9_BLOCK;
+  unsigned long long* desc = reinterpret_cast<unsigned long long*>(w.tab);  // [nb + 1] (the slice holds 32 T_tot bytes)
   ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(degs, F, -1);
-  ++g_launches, k_ext_count<<<(unsigned)nb, ZP_K9_THREADS, 0, st>>>(coefs, T_tot, B, w.d_offsets, F, k, mask, lpos, bsum, degs);
-  ++g_launches, k_ext_scan<<<1, 1024, 0, st>>>(bsum, nb);
-  const int64_t ne = (T_tot > F + 1 ? T_tot : F + 1);
-  ++g_launches, k_ext_emit<<<(unsigned)((ne + ZP_K9_THREADS - 1) / ZP_K9_THREADS), ZP_K9_THREADS, 0, st>>>(
-      exps, nv, coefs, T_tot, k, mask, lpos, bsum, w.d_offsets, F, new_exps, new_coefs, cap, new_offsets);
+  cudaMemsetAsync(desc, 0, 8 * (size_t)(nb + 1), st);
+  // staging buffer: room for one row per term and a quarter more, within 64 KB (else the blocks write directly)
+  int stage_rows = ZP_K9_BLOCK + ZP_K9_BLOCK / 4;
+  size_t smem = (size_t)stage_rows * (8 + 2 * (size_t)(nv + 1)) + 2 * (size_t)nv * ZP_K9_BLOCK + 32;
+  if (smem > 98304) stage_rows = 0, smem = 0;
+  cudaFuncSetAttribute(k_ext_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, 98304);
+  ++g_launches, k_ext_fused<<<(unsigned)nb, ZP_K9_THREADS, smem, st>>>(exps, nv, coefs, T_tot, B, w.d_offsets, F, k, desc, nb, new_exps,
+                                                                        new_coefs, cap, new_offsets, degs, stage_rows);
   return cuda_ok();
 }
 
@@ -1086,7 +1125,7 @@ int zippel_shutdown(void) {
 }
 
 int zippel_set_tuning(int key, int64_t value) {
-  if (key == ZP_TUNE_SUBQ_MIN_T && value > 0) {
+  if (key == ZP_TUNE_SUBQ_MIN_T && value >= 0) {  // 0: back to the built-in rule
     g_subq_min_t = value;
     return ZP_OK;
   }

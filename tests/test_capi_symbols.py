@@ -54,10 +54,22 @@ def test_long_skeleton_workspace_and_limits():
     base = L.zippel_workspace_bytes(offs.ctypes.data, 3, 3, 0)
     assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 1 << 22) == api.ZP_OK
     quad = L.zippel_workspace_bytes(offs.ctypes.data, 3, 3, 0)
-    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 8192) == api.ZP_OK
+    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 0) == api.ZP_OK  # back to the built-in rule
     assert quad < base and quad % 256 == 0
-    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 0) == api.ZP_ERR_ARG
+    assert L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, -1) == api.ZP_ERR_ARG
     assert L.zippel_set_tuning(99, 1) == api.ZP_ERR_ARG
+    # the built-in rule (include/zippel.h): one function of 5000 terms is long for 21 right-hand sides, not for one;
+    # a batch of 32 such functions is long for any B
+    def grows(o, B):
+        L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 1 << 22)
+        q = L.zippel_workspace_bytes(o.ctypes.data, len(o) - 1, B, 0)
+        L.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 0)
+        return L.zippel_workspace_bytes(o.ctypes.data, len(o) - 1, B, 0) > q
+    one = np.array([0, 5000], dtype=np.int64)
+    many = np.arange(33, dtype=np.int64) * 5000
+    assert not grows(one, 1) and not grows(one, 5) and grows(one, 9) and grows(one, 21)
+    assert grows(many, 1) and grows(many, 21)
+    assert not grows(np.arange(4097, dtype=np.int64) * 1000, 21)  # configs[1]: t = 1000 stays on the quadratic kernels
     big = np.array([0, 1 << 23], dtype=np.int64)
     assert L.zippel_workspace_bytes(big.ctypes.data, 1, 1, 0) == 0
     ok = np.array([0, (1 << 23) - 1], dtype=np.int64)
