@@ -626,10 +626,11 @@ def run_thiele(args):
         t1 = time.perf_counter()
         ms = e0.elapsed_time(e1) / K
     clocks = sampler.stop(t0, t1)
-    # algorithmic Montgomery products per column, fraction form: 4 per point and level
-    # (2T^2 - 2T), one batched inversion of the b_k (3T + 93), expansion (T^2/2 + 2T), monic scaling (T + 94);
-    # 18 units each
-    units = n * 18.0 * (2.5 * T * T + 4 * T + 187)
+    # algorithmic products per column, fraction form.  Shoup products (fixed multiplier, 16 units):
+    # 4 per point and level (2T^2 - 2T) and the expansion (T^2/2 + 2T).  Montgomery products (18 units): the companions of
+    # the two pivots per level and of b_k per expansion step (3T), one batched inversion of the b_k (4T + 93), the monic
+    # scaling (T + 94).
+    units = n * (16.0 * (2.5 * T * T) + 18.0 * (8 * T + 187))
     achieved = units / (ms * 1e-3) / 1e12
     cpu = None
     if not args.no_cpu_baseline:
@@ -650,7 +651,7 @@ def run_thiele(args):
         "roofline": {"bound": "alu", "kernel": "k_thiele", "achieved": achieved, "peak": IMAD_PEAK_TOPS,
                      "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / IMAD_PEAK_TOPS,
                      "traffic": None, "algorithmic_ops_per_launch": units, "ms_per_launch": ms,
-                     "algorithmic_cost": "Montgomery product = 18 units; (2.5 T^2 + 4 T + 187) products per column"},
+                     "algorithmic_cost": "2.5 T^2 Shoup products of 16 units + (8 T + 187) Montgomery products of 18 units per column"},
         "e2e": None, "cpu_baseline": cpu}))
 
 

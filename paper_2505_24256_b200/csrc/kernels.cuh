@@ -874,10 +874,11 @@ k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const 
         sc[y] = mont_mul(to_mont(R[x], k), sc[y], k);  // (R_s / u_{0,s})~
       }
     }
-    for (int j = 0; j < B; ++j) {
+#pragma unroll 4
+    for (int j = 0; j < B; ++j) {  // (unrolled: the loads of four rows are in flight together)
       uint64_t v[ZP_BAL_N];
 #pragma unroll
-      for (int y = 0; y < ZP_BAL_N; ++y) v[y] = (x0 + 32 * y < T_tot) ? u[(int64_t)j * T_tot + x0 + 32 * y] : 0;
+      for (int y = 0; y < ZP_BAL_N; ++y) v[y] = (x0 + 32 * y < T_tot) ? __ldcs(u + (int64_t)j * T_tot + x0 + 32 * y) : 0;
 #pragma unroll
       for (int y = 0; y < ZP_BAL_N; ++y)
         if (x0 + 32 * y < T_tot) V[(int64_t)j * T_tot + x0 + 32 * y] = mont_mul(zp_canon(v[y], k.p), sc[y], k);
@@ -894,28 +895,37 @@ k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const 
 // some but not all vanishing -> ZP_ST_THIELE_DEGENERATE.  Expansion from the tail, in place in two columns:
 //   (N, D) <- (b_k N + (x - x_k) D, N),  then trim to the true degrees and scale D monic.
 // Columns live in shared memory (column stride = lanes per CTA); everything is in Montgomery form.
-// k_thiele_prep: xd[j*T + k] = (x_j - x_k)~, xm[j] = x_j~, duplicate check.
+// k_thiele_prep: xd[j*T + k] = {x_j - x_k, companion}, xm[j] = {x_j, companion} (plain residues with their Shoup
+// companions, modarith.cuh), duplicate check.
 // ------------------------------------------------------------------------------------------------
 #define ZP_ST_THIELE_DEGENERATE 20
-__global__ void k_thiele_prep(const uint64_t* __restrict__ points, int T, ZpMod k, uint64_t* __restrict__ xd,
-                              uint64_t* __restrict__ xm, int32_t* __restrict__ dup) {
+__global__ void k_thiele_prep(const uint64_t* __restrict__ points, int T, ZpMod k, ulonglong2* __restrict__ xd,
+                              ulonglong2* __restrict__ xm, int32_t* __restrict__ dup) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= T * T) return;
   const int j = idx / T, kk = idx % T;
-  const uint64_t diff = mod_sub(zp_canon(points[j], k.p), zp_canon(points[kk], k.p), k.p);
+  const uint64_t xj = zp_canon(points[j], k.p);
+  const uint64_t diff = mod_sub(xj, zp_canon(points[kk], k.p), k.p);
   if (kk < j && diff == 0) atomicMin(dup, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
-  xd[idx] = to_mont(diff, k);
-  if (kk == 0) xm[j] = to_mont(zp_canon(points[j], k.p), k);
+  xd[idx] = make_ulonglong2(diff, shoup_companion(to_mont(diff, k), k));
+  if (kk == 0) xm[j] = make_ulonglong2(xj, shoup_companion(to_mont(xj, k), k));
 }
 
 #define ZP_K8_THREADS 64
-// The inverse differences are carried as fractions phi_k(x_j) = A_j / B_j, so that a level is four independent
-// Montgomery products per point and no inversion:
+// x * w mod p, lazily ([0, 2p) out, any 64-bit x in), for a multiplier w in [0, p) with its companion
+ZP_DEV uint64_t shoup_lazy(uint64_t x, uint64_t w, uint64_t wc, const ZpMod& k) { return shoup_mul_lazy(x, w, wc, k); }
+// The inverse differences are carried as fractions phi_k(x_j) = A_j / B_j, so that a level is four independent products
+// per point and no inversion:
 //   A_j <- (x_j - x_{k-1}) B_j B_p ,   B_j <- A_j B_p - A_p B_j      (p = k-1, the pivot; j = k .. T-1),
-// B_j = 0 <=> the oracle's zero denominator.  The b_k = A_k / B_k come from ONE batched inversion at the end
-// (prefix products, Montgomery's trick), the monic scaling from a second one: 2 inversions per column in all.
+// B_j = 0 <=> the oracle's zero denominator.  Every product of a level has a FIXED multiplier -- the pivot's A_p or B_p
+// (per lane: their Shoup companions cost one Montgomery product and one low product per level) or the table entry
+// x_j - x_{k-1} -- so all four are Shoup products (16 multiplier-pipe units and no carry plumbing, against 18 and more
+// for a Montgomery product); the values are plain residues, lazy where they only feed another product, and a common
+// factor picked up along the way cancels in A_j / B_j.  The b_k = A_k / B_k come from ONE batched inversion at the end
+// (prefix products, Montgomery's trick), the monic scaling from a second one: 2 inversions per column in all.  The
+// expansion (N, D) <- (b_k N + (x - x_k) D, N) multiplies by b_k (per lane and step) and x_k (table): Shoup again.
 __global__ void __launch_bounds__(ZP_K8_THREADS)
-k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const int32_t* __restrict__ dup, int T,
+k_thiele(const ulonglong2* __restrict__ xd, const ulonglong2* __restrict__ xm, const int32_t* __restrict__ dup, int T,
          const uint64_t* __restrict__ vals, int64_t n, int64_t ld, ZpMod k, uint64_t* __restrict__ num,
          uint64_t* __restrict__ den, int32_t* __restrict__ degs, uint64_t* __restrict__ cf, int32_t* __restrict__ status) {
   extern __shared__ __align__(16) uint64_t sh[];
@@ -923,6 +933,7 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
   uint64_t* Ac = sh + threadIdx.x;                 // column A_j (ends as b_0 .. b_{K-1}), stride TH
   uint64_t* Bc = Ac + (size_t)(T + 2) * TH;        // column B_j; later N (slots 0 ..) and D (slots T/2+1 ..)
   const int32_t dupst = dup[0];
+  const uint64_t p = k.p;
   for (int64_t i = (int64_t)blockIdx.x * TH + threadIdx.x; i < n; i += (int64_t)gridDim.x * TH) {
     for (int d = 0; d < T; ++d) {
       num[d * ld + i] = 0;
@@ -936,21 +947,24 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
       continue;
     }
     for (int j = 0; j < T; ++j) {
-      Ac[j * TH] = to_mont(zp_canon(vals[j * ld + i], k.p), k);
-      Bc[j * TH] = k.r1;
+      Ac[j * TH] = zp_canon(vals[j * ld + i], p);
+      Bc[j * TH] = 1 % p;
     }
     int K = T, bad = 0;
     for (int kk = 1; kk < T; ++kk) {
-      const uint64_t Ap = Ac[(kk - 1) * TH], Bp = Bc[(kk - 1) * TH];
-      const uint64_t* xrow = xd + (kk - 1);  // xd[j*T + kk-1] = (x_j - x_{kk-1})~
+      const uint64_t Ap = lazy_canon(Ac[(kk - 1) * TH], p), Bp = Bc[(kk - 1) * TH];  // A lazy in [0, 2p), B canonical
+      const uint64_t Apc = shoup_companion(to_mont(Ap, k), k), Bpc = shoup_companion(to_mont(Bp, k), k);
+      const ulonglong2* xrow = xd + (kk - 1);  // xd[j*T + kk-1] = x_j - x_{kk-1}
       int zeros = 0;
       int j = kk;
       for (; j + 1 < T; j += 2) {  // two points at a time: eight independent products in flight
         const uint64_t a0 = Ac[j * TH], b0 = Bc[j * TH], a1 = Ac[(j + 1) * TH], b1 = Bc[(j + 1) * TH];
-        const uint64_t nb0 = mod_sub(mont_mul(a0, Bp, k), mont_mul(Ap, b0, k), k.p);
-        const uint64_t nb1 = mod_sub(mont_mul(a1, Bp, k), mont_mul(Ap, b1, k), k.p);
-        const uint64_t na0 = mont_mul(mont_mul(b0, Bp, k), __ldg(xrow + (size_t)j * T), k);
-        const uint64_t na1 = mont_mul(mont_mul(b1, Bp, k), __ldg(xrow + (size_t)(j + 1) * T), k);
+        const ulonglong2 x0 = __ldg(xrow + (size_t)j * T), x1 = __ldg(xrow + (size_t)(j + 1) * T);
+        // (2p can exceed 2^63: each lazy product is brought to [0, p) before the difference)
+        const uint64_t nb0 = mod_sub(lazy_canon(shoup_lazy(a0, Bp, Bpc, k), p), lazy_canon(shoup_lazy(b0, Ap, Apc, k), p), p);
+        const uint64_t nb1 = mod_sub(lazy_canon(shoup_lazy(a1, Bp, Bpc, k), p), lazy_canon(shoup_lazy(b1, Ap, Apc, k), p), p);
+        const uint64_t na0 = shoup_lazy(shoup_lazy(b0, Bp, Bpc, k), x0.x, x0.y, k);
+        const uint64_t na1 = shoup_lazy(shoup_lazy(b1, Bp, Bpc, k), x1.x, x1.y, k);
         zeros += (nb0 == 0) + (nb1 == 0);
         Ac[j * TH] = na0;
         Bc[j * TH] = nb0;
@@ -959,8 +973,9 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
       }
       if (j < T) {
         const uint64_t a0 = Ac[j * TH], b0 = Bc[j * TH];
-        const uint64_t nb0 = mod_sub(mont_mul(a0, Bp, k), mont_mul(Ap, b0, k), k.p);
-        Ac[j * TH] = mont_mul(mont_mul(b0, Bp, k), __ldg(xrow + (size_t)j * T), k);
+        const ulonglong2 x0 = __ldg(xrow + (size_t)j * T);
+        const uint64_t nb0 = mod_sub(lazy_canon(shoup_lazy(a0, Bp, Bpc, k), p), lazy_canon(shoup_lazy(b0, Ap, Apc, k), p), p);
+        Ac[j * TH] = shoup_lazy(shoup_lazy(b0, Bp, Bpc, k), x0.x, x0.y, k);
         Bc[j * TH] = nb0;
         zeros += (nb0 == 0);
       }
@@ -978,38 +993,42 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
       continue;
     }
     // b_k = A_k / B_k, k < K, by one batched inversion; the prefix products are parked in this lane's own
-    // output column num[., i] (global, unit stride across lanes, overwritten with the result below)
+    // output column num[., i] (global, unit stride across lanes, overwritten with the result below).  The values are
+    // plain, so the running product picks up 2^-64 per step: run_k = B_0 .. B_k 2^(-64 k), and with
+    // I_k = mont_inv(run_k) = 2^128 / run_k:  mont_mul(I_k, run_{k-1}) = 2^128 / B_k,  I_{k-1} = mont_mul(I_k, B_k).
     {
-      uint64_t run = k.r1;
-      for (int kk = 0; kk < K; ++kk) {
+      uint64_t run = Bc[0];
+      num[i] = run;
+      for (int kk = 1; kk < K; ++kk) {
         run = mont_mul(run, Bc[kk * TH], k);
         num[kk * ld + i] = run;  // scratch: prefix products (overwritten with zeros / results below)
       }
       uint64_t inv = mont_inv(run, k);
       for (int kk = K - 1; kk >= 0; --kk) {
-        const uint64_t invk = (kk > 0) ? mont_mul(inv, num[(kk - 1) * ld + i], k) : inv;  // 1 / B_k
+        const uint64_t invk = (kk > 0) ? mont_mul(inv, num[(kk - 1) * ld + i], k) : inv;  // 2^128 / B_k
         inv = mont_mul(inv, Bc[kk * TH], k);
-        Ac[kk * TH] = mont_mul(Ac[kk * TH], invk, k);  // b_k
+        Ac[kk * TH] = mont_mul(mont_mul(Ac[kk * TH], invk, k), 1, k);  // b_k, plain and canonical
         num[kk * ld + i] = 0;
       }
     }
     if (cf)
-      for (int kk = 0; kk < K; ++kk) cf[kk * ld + i] = from_mont(Ac[kk * TH], k);
+      for (int kk = 0; kk < K; ++kk) cf[kk * ld + i] = Ac[kk * TH];
     // expansion from the tail, in place: after s steps deg N <= (s+1)/2, deg D <= s/2
     uint64_t* Nc = Bc;
     uint64_t* Dc = Bc + (size_t)(T / 2 + 1) * TH;
     const int half = T / 2;
     for (int d = 0; d <= half; ++d) Nc[d * TH] = Dc[d * TH] = 0;
     Nc[0] = Ac[(K - 1) * TH];
-    Dc[0] = k.r1;
+    Dc[0] = 1 % p;
     for (int kk = K - 2, s2 = 1; kk >= 0; --kk, ++s2) {
       const uint64_t bk = Ac[kk * TH];
-      const uint64_t xk = __ldg(xm + kk);
+      const uint64_t bkc = shoup_companion(to_mont(bk, k), k);
+      const ulonglong2 xk = __ldg(xm + kk);
       for (int d = (s2 + 1) / 2; d >= 0; --d) {  // descending: D[d-1] is still the old one
         const uint64_t Nd = Nc[d * TH], Dd = Dc[d * TH];
-        uint64_t v = mont_mul(bk, Nd, k);
-        if (d >= 1) v = mod_add(v, Dc[(d - 1) * TH], k.p);
-        v = mod_sub(v, mont_mul(xk, Dd, k), k.p);
+        uint64_t v = lazy_canon(shoup_lazy(Nd, bk, bkc, k), p);
+        if (d >= 1) v = mod_add(v, Dc[(d - 1) * TH], p);
+        v = mod_sub(v, lazy_canon(shoup_lazy(Dd, xk.x, xk.y, k), p), p);
         Dc[d * TH] = Nd;
         Nc[d * TH] = v;
       }
@@ -1021,9 +1040,9 @@ k_thiele(const uint64_t* __restrict__ xd, const uint64_t* __restrict__ xm, const
       status[i] = (int32_t)ZP_ST_THIELE_DEGENERATE;
       continue;
     }
-    const uint64_t sc = mont_inv(Dc[dd * TH], k);
-    for (int d = 0; d <= dn; ++d) num[d * ld + i] = from_mont(mont_mul(Nc[d * TH], sc, k), k);
-    for (int d = 0; d <= dd; ++d) den[d * ld + i] = from_mont(mont_mul(Dc[d * TH], sc, k), k);
+    const uint64_t sc = mont_inv(to_mont(Dc[dd * TH], k), k);  // (1 / lc D)~: plain x Montgomery -> plain
+    for (int d = 0; d <= dn; ++d) num[d * ld + i] = mont_mul(Nc[d * TH], sc, k);
+    for (int d = 0; d <= dd; ++d) den[d * ld + i] = mont_mul(Dc[d * TH], sc, k);
     degs[i] = dn;
     degs[ld + i] = dd;
     status[i] = 0;

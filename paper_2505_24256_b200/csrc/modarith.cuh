@@ -140,10 +140,45 @@ ZP_DEV uint64_t lazy_canon(uint64_t x, uint64_t p) {  // [0,2p) -> [0,p)
   const uint64_t s = x - p;
   return (x >= p) ? s : x;
 }
-// x * w mod p for a fixed multiplier w = {w, w'} with its companion (horner_step with a zero addend), canonical
-// result; x may be any 64-bit value
+// x * w mod p, lazily, for a fixed multiplier w in [0, p) with its companion w' = floor(w 2^64 / p): ANY 64-bit x in,
+// [0, 2p) out.  horner_step without its addends (whose carry plumbing ptxas keeps even when they are zero):
+// qq = floor(w' x / 2^64) exactly (4 wide products, the carries through predicates), then w x - qq p modulo 2^64
+// (2 wide + 4 low products): 16 units of the multiplier pipe and 4 instructions on the alu pipe.
+ZP_DEV uint64_t shoup_mul_lazy(uint64_t x, uint64_t w, uint64_t wc, const ZpMod& k) {
+  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), p0 = (uint32_t)wc, p1 = (uint32_t)(wc >> 32);
+  const uint32_t w0 = (uint32_t)w, w1 = (uint32_t)(w >> 32);
+  const uint32_t np0 = (uint32_t)k.np, np1 = (uint32_t)(k.np >> 32);
+  uint64_t qq;
+  asm("{\n\t"
+      ".reg .u64 a, s, s2, t;\n\t"
+      ".reg .u32 alo, ahi, slo, shi, c1, tlo, thi, dummy;\n\t"
+      "mul.wide.u32 a, %1, %3;\n\t"   // w'0 x0 (its high word carries into the middle)
+      "mul.wide.u32 s, %1, %4;\n\t"   // w'0 x1
+      "mul.wide.u32 s2, %2, %3;\n\t"  // w'1 x0
+      "add.cc.u64 s, s2, s;\n\t"      // middle sum, carry c1 (weight 2^96)
+      "addc.u32 c1, 0, 0;\n\t"
+      "mov.b64 {alo, ahi}, a;\n\t"
+      "mov.b64 {slo, shi}, s;\n\t"
+      "add.cc.u32 dummy, slo, ahi;\n\t"
+      "addc.cc.u32 tlo, shi, 0;\n\t"
+      "addc.u32 thi, c1, 0;\n\t"
+      "mov.b64 t, {tlo, thi};\n\t"
+      "mad.wide.u32 %0, %2, %4, t;\n\t"  // w'1 x1 + (middle >> 32)
+      "}"
+      : "=l"(qq)
+      : "r"(p0), "r"(p1), "r"(x0), "r"(x1));
+  const uint32_t q0 = (uint32_t)qq, q1 = (uint32_t)(qq >> 32);
+  uint32_t uh = zp_madlo(w0, x1, 0);
+  uh = zp_madlo(w1, x0, uh);
+  uh = zp_madlo(q0, np1, uh);
+  uh = zp_madlo(q1, np0, uh);
+  uint64_t u = (uint64_t)uh << 32;
+  u = zp_madw(w0, x0, u);
+  return zp_madw(q0, np0, u);
+}
+// the same with a canonical result
 ZP_DEV uint64_t shoup_mul(uint64_t x, ulonglong2 w, const ZpMod& k) {
-  return lazy_canon(horner_step(x, w.x, w.y, 0, 0, k), k.p);
+  return lazy_canon(shoup_mul_lazy(x, w.x, w.y, k), k.p);
 }
 
 // Deferred accumulator.  value = E + O * 2^32 with

@@ -45,42 +45,8 @@ struct CrtOut {
 };
 
 #if defined(__CUDACC__)
-// x * w mod q, lazily: any 64-bit x in, [0, 2q) out (w = {w, w'} with its Shoup companion w' = floor(w 2^64 / q)).
-// modarith.cuh's horner_step without its addends (whose carry plumbing ptxas keeps even when they are zero):
-// qq = floor(w' x / 2^64) exactly (4 wide products, the carries through predicates), then w x - qq q modulo 2^64
-// (2 wide + 4 low products): 16 units of the multiplier pipe and 4 instructions on the alu pipe.
-ZP_DEV uint64_t ntt_mul(uint64_t x, ulonglong2 w, const ZpMod& q) {
-  const uint32_t x0 = (uint32_t)x, x1 = (uint32_t)(x >> 32), p0 = (uint32_t)w.y, p1 = (uint32_t)(w.y >> 32);
-  const uint32_t w0 = (uint32_t)w.x, w1 = (uint32_t)(w.x >> 32);
-  const uint32_t np0 = (uint32_t)q.np, np1 = (uint32_t)(q.np >> 32);
-  uint64_t qq;
-  asm("{\n\t"
-      ".reg .u64 a, s, s2, t;\n\t"
-      ".reg .u32 alo, ahi, slo, shi, c1, tlo, thi, dummy;\n\t"
-      "mul.wide.u32 a, %1, %3;\n\t"   // p0 x0 (its high word carries into the middle)
-      "mul.wide.u32 s, %1, %4;\n\t"   // p0 x1
-      "mul.wide.u32 s2, %2, %3;\n\t"  // p1 x0
-      "add.cc.u64 s, s2, s;\n\t"      // middle sum, carry c1 (weight 2^96)
-      "addc.u32 c1, 0, 0;\n\t"
-      "mov.b64 {alo, ahi}, a;\n\t"
-      "mov.b64 {slo, shi}, s;\n\t"
-      "add.cc.u32 dummy, slo, ahi;\n\t"
-      "addc.cc.u32 tlo, shi, 0;\n\t"
-      "addc.u32 thi, c1, 0;\n\t"
-      "mov.b64 t, {tlo, thi};\n\t"
-      "mad.wide.u32 %0, %2, %4, t;\n\t"  // p1 x1 + (middle >> 32)
-      "}"
-      : "=l"(qq)
-      : "r"(p0), "r"(p1), "r"(x0), "r"(x1));
-  const uint32_t q0 = (uint32_t)qq, q1 = (uint32_t)(qq >> 32);
-  uint32_t uh = zp_madlo(w0, x1, 0);
-  uh = zp_madlo(w1, x0, uh);
-  uh = zp_madlo(q0, np1, uh);
-  uh = zp_madlo(q1, np0, uh);
-  uint64_t u = (uint64_t)uh << 32;
-  u = zp_madw(w0, x0, u);
-  return zp_madw(q0, np0, u);
-}
+// x * w mod q, lazily: any 64-bit x in, [0, 2q) out (w = {w, w'} with its Shoup companion; modarith.cuh)
+ZP_DEV uint64_t ntt_mul(uint64_t x, ulonglong2 w, const ZpMod& q) { return shoup_mul_lazy(x, w.x, w.y, q); }
 ZP_DEV uint32_t brev_bits(uint32_t x, int bits) { return bits ? (__brev(x) >> (32 - bits)) : 0u; }
 
 // x * w^E (forward) or x * w^-E (inverse), E < 2^24, from the two-level tables

@@ -1030,8 +1030,8 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
   if (!ws_ok(workspace, workspace_bytes, carve(nullptr, 1, 1, T, 0).bytes)) return ZP_ERR_WORKSPACE;
   const Ws w = carve(workspace, 1, 1, T, 0);
   cudaStream_t st = (cudaStream_t)stream;
-  uint64_t* xd = reinterpret_cast<uint64_t*>(w.invd);   // [T*T] (the slice holds 16 T^2 bytes)
-  uint64_t* xm = reinterpret_cast<uint64_t*>(w.smont);  // [T]
+  ulonglong2* xd = w.invd;   // [T*T] {x_j - x_k, companion}
+  ulonglong2* xm = w.smont;  // [T]   {x_j, companion}
   ++g_launches, k_fill_i32<<<1, 32, 0, st>>>(w.st_newton, 1, ZP_ST_NONE);
   ++g_launches, k_thiele_prep<<<(T * T + 127) / 128, 128, 0, st>>>(points, T, k, xd, xm, w.st_newton);
   const size_t smem = 8 * 2 * (size_t)(T + 2) * ZP_K8_THREADS;  // two columns per lane
