@@ -23,7 +23,7 @@ _INC = os.path.join(os.path.dirname(_HERE), "include")
 SO_PATH = os.path.join(_HERE, "libzippel.so")
 TEST_SO_PATH = os.path.join(_HERE, "libzippel_test.so")
 SOURCES = [os.path.join(_CSRC, "zippel_capi.cu")]
-HEADERS = [os.path.join(_CSRC, h) for h in ("modarith.cuh", "kernels.cuh", "ntt.cuh", "subq.cuh")] + [
+HEADERS = [os.path.join(_CSRC, h) for h in ("modarith.cuh", "kernels.cuh", "ntt.cuh", "subq.cuh", "small.cuh")] + [
     os.path.join(_INC, "zippel.h")]
 TEST_HEADERS = HEADERS + [os.path.join(_CSRC, h) for h in ("ubench.cuh", "test_hooks.cuh")] + [
     os.path.join(_INC, "zippel_test.h")]

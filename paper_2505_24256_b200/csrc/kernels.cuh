@@ -1282,8 +1282,9 @@ k_ext_fused(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restric
 // (f4) two-prime CRT + rational reconstruction, one lane per coefficient:
 //   x = r1 + p1 ((r2 - r1) p1^-1 mod p2) in [0, m = p1 p2);  extended Euclid on (m, x) down to the first
 //   remainder <= N = floor(sqrt((m-1)/2)) (Wang's bounds);  a/b = remainder / cofactor, b > 0, b <= N, gcd 1.
-// 128-bit integers; Euclid's quotients are mostly 1, 2, 3 (tried by subtraction before the 128-bit division),
-// and the tail of the sequence runs in 64 bits.  Data-dependent and divergent by nature; HBM traffic 32 B/lane.
+// 128-bit remainders, 64-bit cofactor magnitudes; Euclid's quotients come from a double-precision estimate and one
+// correction (no subtraction ladder, no 128-bit division on the usual path).  The number of steps is data-dependent
+// (about 37 on average for two 63-bit primes); HBM traffic 32 B/lane.
 // ------------------------------------------------------------------------------------------------
 #define ZP_ST_NO_RATIONAL 21
 typedef unsigned __int128 zp_u128;
@@ -1298,42 +1299,46 @@ k_crt_rational(const uint64_t* __restrict__ r1, const uint64_t* __restrict__ r2,
     const uint64_t diff = mod_sub(a2, zp_canon(a1, k2.p), k2.p);
     const uint64_t h = mont_mul(to_mont(diff, k2), p1inv, k2);  // Montgomery x plain -> plain: diff / p1 mod p2
     const zp_u128 x = (zp_u128)a1 + (zp_u128)p1 * h;
+    // cofactors: t_i alternates in sign and |t_i| <= m / r_{i-1} < 2^64 while r_{i-1} > N, so the magnitudes fit 64 bits
+    // and |t_{i+1}| = |t_{i-1}| + q |t_i| needs no 128-bit product; sign(t_i) = (-1)^(i+1) (t_0 = 0, t_1 = 1)
     zp_u128 ra = m, rb = x;
-    zp_i128 ta = 0, tb = 1;
+    uint64_t ta = 0, tb = 1;
+    bool tb_neg = false;
     while (rb > N) {
-      zp_u128 q, rn;
-      if ((uint64_t)(ra >> 64) == 0) {
-        const uint64_t a = (uint64_t)ra, b = (uint64_t)rb, qq = a / b;
-        q = qq;
-        rn = a - qq * b;
-      } else {
-        rn = ra - rb;
-        q = 1;
+      // quotient: estimate in double precision (relative error about 2^-52, so off by at most one for q < 2^50), then
+      // one multiply-subtract and the corrections; the exact 128-bit division only for the quotients beyond that
+      // (probability about 2^-50 per step).  Every lane takes the same path: no subtraction ladder, no divergence.
+      uint64_t q;
+      zp_u128 rn;
+      const double da = __ull2double_rn((uint64_t)(ra >> 64)) * 18446744073709551616.0 + __ull2double_rn((uint64_t)ra);
+      const double db = __ull2double_rn((uint64_t)(rb >> 64)) * 18446744073709551616.0 + __ull2double_rn((uint64_t)rb);
+      const double qd = da / db;
+      if (qd < 1125899906842624.0) {  // 2^50
+        q = (uint64_t)qd;
+        rn = ra - (zp_u128)q * rb;  // modulo 2^128; the true value lies in (-rb, 2 rb)
+        if ((zp_i128)rn < 0) {
+          rn += rb;
+          --q;
+        }
         if (rn >= rb) {
           rn -= rb;
-          q = 2;
-          if (rn >= rb) {
-            rn -= rb;
-            q = 3;
-            if (rn >= rb) {
-              q = ra / rb;
-              rn = ra - q * rb;
-            }
-          }
+          ++q;
         }
+      } else {
+        q = (uint64_t)(ra / rb);
+        rn = ra - (zp_u128)q * rb;
       }
-      const zp_i128 tn = ta - (zp_i128)q * tb;
+      const uint64_t tn = ta + q * tb;  // q tb <= |t_{i+1}| < 2^64
       ra = rb;
       rb = rn;
       ta = tb;
       tb = tn;
+      tb_neg = !tb_neg;
     }
-    zp_i128 a = (zp_i128)rb, b = tb;
-    if (b < 0) {
-      a = -a;
-      b = -b;
-    }
-    bool ok = (b > 0) && ((zp_u128)b <= N);
+    zp_i128 a = (zp_i128)rb;
+    const uint64_t b = tb;
+    if (tb_neg) a = -a;
+    bool ok = (b > 0) && (b <= N);
     if (ok) {
       uint64_t g0 = (uint64_t)(a < 0 ? -a : a), g1 = (uint64_t)b;
       while (g1) {

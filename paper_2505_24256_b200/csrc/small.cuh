@@ -1,0 +1,170 @@
+// small.cuh -- one lifting step of a SMALL batch in a single launch (BASELINE.json configs[0]: one function of t = 50
+// terms, B = 11 samples, where the thirteen launches of the general path cost 100 us of launch and dependency latency
+// for 20 ns of arithmetic).  One CTA per function, one lane per node, the whole of PAPER.md section 1-2.2 in order:
+//   (a1) m_i = prod_j y_j^e_ij                                   (L55 eq. (3))
+//   (a2) M(z) = prod_i (z - m_i), product tree in shared memory   (L191)
+//   (a3) q_{l-1} = M_l + m_i q_l;  d = Q_i(m_i);  num_b = sum_l q_l v_{b,l}   (L193-195; deferred sums, L205-209)
+//   (a4) c_{b,i} = num_b / (d [m_i])                              (L196)
+//   (a5) Newton divided differences in x_k, optional monomial expansion   (L17-22 eq. (1))
+// The same exact arithmetic as the general path, so the same (unique) results bit for bit; the host takes this path
+// when F <= ZP_SMALL_MAXF, every t <= ZP_SMALL_MAXT and t B is small enough for one lane per node to be the fast way
+// (zippel_capi.cu: small_ok).
+#pragma once
+#include "kernels.cuh"
+
+#define ZP_SMALL_MAXF 32
+#define ZP_SMALL_MAXT 128
+#define ZP_SMALL_NB 4    // right-hand sides per pass over the quotient chain (accumulators in registers)
+#define ZP_SMALL_MAXG 3  // groups of lanes that share the right-hand sides of a function; one more group builds tables
+
+struct SmallOffs {
+  int64_t o[ZP_SMALL_MAXF + 1];
+};
+
+// CTA = (G + 1) groups of MAXT lanes.  Lane i of group g < G owns node i and the right-hand sides [g per, (g + 1) per):
+// every group runs the quotient chain of its node itself (one modular multiply-add per stage; the chain is the
+// critical path, the dot products ride on it), so the B dot products of a node proceed in G lanes at once.  Group G
+// meanwhile inverts Newton's sample differences (one Fermat power each), which nothing needs before the solve is done.
+__global__ void __launch_bounds__(ZP_SMALL_MAXT*(ZP_SMALL_MAXG + 1))
+k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const uint64_t* __restrict__ anchors,
+             const uint64_t* __restrict__ samples, int B, int G, int s0, const uint64_t* __restrict__ vals, int64_t T_tot,
+             ZpMod k, int basis, uint64_t* __restrict__ out, uint64_t* __restrict__ nodes_out, int32_t* __restrict__ status) {
+  __shared__ uint64_t Y[32 * 16];                  // (y_j^(2^b))~
+  __shared__ uint64_t buf[2][ZP_SMALL_MAXT];       // product tree; then M~_0 .. M~_{t-1}
+  __shared__ uint64_t sInv[64 * 64];               // (1 / (c_j - c_jj))~, jj < j
+  __shared__ uint64_t sC[64];                      // c_j~
+  __shared__ int32_t s_solve, s_newton;
+  extern __shared__ __align__(16) uint64_t cols[];  // [B x MAXT]: column c_{.,i} at cols[b MAXT + i]; then sv
+  constexpr int S = ZP_SMALL_MAXT;
+  const int f = blockIdx.x;
+  const int64_t off = offs.o[f];
+  const int t = (int)(offs.o[f + 1] - off);
+  const int g = threadIdx.x / S, i = threadIdx.x % S;
+  const bool live = i < t;
+  const uint64_t p = k.p;
+  if (threadIdx.x == 0) s_solve = s_newton = ZP_ST_NONE;
+  // ---- the function's values -> shared memory (unit-stride loads), the anchors' power table
+  uint64_t* sv = cols + B * S;  // [B x MAXT]: v_{b,l} at sv[b MAXT + l]
+  for (int b = g; b < B; b += G + 1)
+    if (live) sv[b * S + i] = zp_canon(vals[(int64_t)b * T_tot + off + i], p);
+  if (threadIdx.x < nv) {
+    uint64_t y = to_mont(zp_canon(anchors[threadIdx.x], p), k);
+    for (int b = 0; b < 16; ++b) {
+      Y[threadIdx.x * 16 + b] = y;
+      y = mont_mul(y, y, k);
+    }
+  }
+  __syncthreads();
+  if (g == G) {  // ---- the table group: Newton's inverse differences
+    for (int x = i; x < B * B; x += S) {
+      const int j = x / B, jj = x % B;
+      const uint64_t cj = zp_canon(samples[j], p);
+      if (jj == 0) sC[j] = to_mont(cj, k);
+      if (jj < j) {
+        const uint64_t diff = mod_sub(cj, zp_canon(samples[jj], p), p);
+        if (diff == 0) atomicMin(&s_newton, (int32_t)(((uint32_t)j << 8) | ZP_ST_DUPLICATE_SAMPLE));
+        sInv[x] = mont_inv(to_mont(diff, k), k);
+      }
+    }
+  }
+  // ---- (a1) node of this lane (every solving group computes it: no hand-over)
+  uint64_t mm = 0;  // m_i~
+  if (live && g < G) {
+    const uint16_t* e = exps + (off + i) * nv;
+    mm = k.r1;
+    for (int j = 0; j < nv; ++j) {
+      uint32_t ej = e[j];
+      for (int b = 0; ej; ++b, ej >>= 1)
+        if (ej & 1) mm = mont_mul(mm, Y[j * 16 + b], k);
+    }
+    if (g == 0) {
+      if (nodes_out) nodes_out[off + i] = from_mont(mm, k);
+      buf[0][i] = mod_neg(mm, p);  // (z - m_i)' = -m_i~
+    }
+  }
+  // ---- (a2) product tree (as k_tree_leaf), by group 0; the barriers are the CTA's
+  int cur = 0;
+  for (int a = 1; a < t; a <<= 1) {
+    __syncthreads();
+    if (live && g == 0) {
+      const int base = i & ~(2 * a - 1);
+      const int b = (t - base - a) < a ? (t - base - a) : a;
+      buf[cur ^ 1][i] = (b <= 0) ? buf[cur][i] : tree_merge_coef(buf[cur] + base, a, b, i - base, k);
+    }
+    cur ^= 1;
+  }
+  __syncthreads();
+  const uint64_t* M = buf[cur];  // M~_l, l < t; M_t = 1
+  // ---- (a3) + (a4): the right-hand sides of this group, NB per pass over the chain q_{t-1} = 1, q_{l-1} = M_l + m q_l
+  if (live && g < G) {
+    const int per = (B + G - 1) / G, bA = g * per, bB = (bA + per < B) ? bA + per : B;
+    uint64_t inv = 0;  // (1 / (d [m]))~ after the first pass
+    for (int b0 = bA; b0 < bB; b0 += ZP_SMALL_NB) {
+      const int nb = (bB - b0 < ZP_SMALL_NB) ? bB - b0 : ZP_SMALL_NB;
+      Acc acc[ZP_SMALL_NB];
+#pragma unroll
+      for (int b = 0; b < ZP_SMALL_NB; ++b) acc_zero(acc[b]);
+      uint64_t q = k.r1, d = k.r1;
+      const uint64_t* v[ZP_SMALL_NB];  // rows beyond nb repeat the last one (their sums are dropped): no branch in the loop
+#pragma unroll
+      for (int b = 0; b < ZP_SMALL_NB; ++b) v[b] = sv + (b0 + (b < nb ? b : nb - 1)) * S;
+      for (int l = t - 1; l >= 1; --l) {
+#pragma unroll
+        for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][l]);
+        q = mod_add(M[l], mont_mul(mm, q, k), p);
+        d = mod_add(mont_mul(d, mm, k), q, p);
+      }
+#pragma unroll
+      for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][0]);
+      if (b0 == bA) {
+        const uint64_t dd = s0 ? mont_mul(d, mm, k) : d;
+        if (dd == 0 && g == 0) atomicMin(&s_solve, (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
+        inv = mont_inv(dd, k);
+      }
+#pragma unroll
+      for (int b = 0; b < ZP_SMALL_NB; ++b)
+        if (b < nb)  // sum of Montgomery x plain: redc160 and c160 give the plain sum; plain x Montgomery -> plain
+          cols[(b0 + b) * S + i] = mont_mul(mont_mul(acc_redc160(acc[b], k), k.c160, k), inv, k);
+    }
+  }
+  __syncthreads();  // the columns, sInv, sC, s_newton are complete
+  // ---- (a5) Newton in x_k on this lane's column (shared memory), then the column goes out
+  if (live && g == 0) {
+    uint64_t* col = cols + i;
+    const int D = B - 1;
+    // the steps of one level read the previous level only: four at a time, loads before stores, so that their
+    // products overlap (one warp per scheduler: latency is all there is)
+    for (int l = 1; l <= D; ++l) {
+      int j = D;
+      for (; j - 3 >= l; j -= 4) {
+        const uint64_t v0 = col[j * S], v1 = col[(j - 1) * S], v2 = col[(j - 2) * S], v3 = col[(j - 3) * S], v4 = col[(j - 4) * S];
+        const uint64_t* w = sInv + j * B + (j - l);  // row stride B, same column offset j - l
+        col[j * S] = mont_mul(mod_sub(v0, v1, p), w[0], k);
+        col[(j - 1) * S] = mont_mul(mod_sub(v1, v2, p), w[-B - 1], k);
+        col[(j - 2) * S] = mont_mul(mod_sub(v2, v3, p), w[-2 * B - 2], k);
+        col[(j - 3) * S] = mont_mul(mod_sub(v3, v4, p), w[-3 * B - 3], k);
+      }
+      for (; j >= l; --j) col[j * S] = mont_mul(mod_sub(col[j * S], col[(j - 1) * S], p), sInv[j * B + (j - l)], k);
+    }
+    if (basis == 1)
+      for (int j = D - 1; j >= 0; --j) {
+        const uint64_t cj = sC[j];
+        int x = j;
+        for (; x + 3 < D; x += 4) {
+          const uint64_t v0 = col[x * S], v1 = col[(x + 1) * S], v2 = col[(x + 2) * S], v3 = col[(x + 3) * S], v4 = col[(x + 4) * S];
+          col[x * S] = mod_sub(v0, mont_mul(v1, cj, k), p);
+          col[(x + 1) * S] = mod_sub(v1, mont_mul(v2, cj, k), p);
+          col[(x + 2) * S] = mod_sub(v2, mont_mul(v3, cj, k), p);
+          col[(x + 3) * S] = mod_sub(v3, mont_mul(v4, cj, k), p);
+        }
+        for (; x < D; ++x) col[x * S] = mod_sub(col[x * S], mont_mul(col[(x + 1) * S], cj, k), p);
+      }
+  }
+  __syncthreads();
+  for (int b = g; b < B; b += G + 1)
+    if (live) out[(int64_t)b * T_tot + off + i] = cols[b * S + i];
+  if (threadIdx.x == 0) {
+    const int32_t s = (s_solve != ZP_ST_NONE) ? s_solve : s_newton;
+    status[f] = (s == ZP_ST_NONE) ? 0 : s;
+  }
+}

@@ -10,6 +10,7 @@
 #include "../../include/zippel.h"
 #include "kernels.cuh"
 #include "subq.cuh"
+#include "small.cuh"
 
 namespace {
 
@@ -768,6 +769,35 @@ HostWs carve_host(void* base, int64_t T_tot, int F, int nv, int B, const SqSizes
 // (a1)-(a5) on the functions [f0, f1) of a batch whose arrays are resident in full (row stride T_tot): the
 // kernels index by absolute term offsets, so a chunk is the same launch sequence on shifted offset/status
 // pointers.  The whole batch is the chunk [0, F).
+// Small batches take one fused launch (small.cuh): at most ZP_SMALL_MAXF functions of at most ZP_SMALL_MAXT terms, and
+// little enough work per lane (pipe cycles of the chain, the B dot products and Newton's B^2 / 2 steps) that one lane
+// per node beats the launch and dependency latency of the general path (about 100 us for its thirteen launches).
+inline int small_groups(int B) {  // lanes per node: one per ZP_SMALL_NB right-hand sides, at most ZP_SMALL_MAXG
+  const int g = (B + ZP_SMALL_NB - 1) / ZP_SMALL_NB;
+  return g > ZP_SMALL_MAXG ? ZP_SMALL_MAXG : g;
+}
+bool small_ok(const int64_t* h_offs, int F, int B) {
+  if (F > ZP_SMALL_MAXF) return false;
+  int64_t tmax = 0;
+  for (int f = 0; f < F; ++f) tmax = (h_offs[f + 1] - h_offs[f] > tmax) ? h_offs[f + 1] - h_offs[f] : tmax;
+  if (tmax > ZP_SMALL_MAXT) return false;
+  const int G = small_groups(B), per = (B + G - 1) / G;
+  const int64_t cost = tmax * (18 * (int64_t)per + 108 * ((per + ZP_SMALL_NB - 1) / ZP_SMALL_NB)) + 80 * (int64_t)B * B;
+  return cost <= 50000;
+}
+void lift_small(const int64_t* h_offs, int F, int64_t T_tot, int nv, const uint16_t* exps, const uint64_t* anchors,
+                const uint64_t* samples, int B, int s0, const uint64_t* vals, const ZpMod& k, int basis, uint64_t* out,
+                uint64_t* nodes_out, int32_t* status, cudaStream_t st) {
+  ProfScope prof(ZP_K_NODE_SOLVE, st);
+  SmallOffs so;
+  for (int f = 0; f <= F; ++f) so.o[f] = h_offs[f];  // absolute slots, by value: no upload
+  const size_t smem = 2 * 8 * (size_t)B * ZP_SMALL_MAXT;  // the columns of Newton's recurrence and the function's values
+  cudaFuncSetAttribute(k_lift_small, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 8 * ZP_MAX_B * ZP_SMALL_MAXT);
+  const int G = small_groups(B);
+  ++g_launches, k_lift_small<<<F, ZP_SMALL_MAXT*(G + 1), smem, st>>>(exps, so, nv, anchors, samples, B, G, s0, vals, T_tot, k, basis, out,
+                                                                     nodes_out, status);
+}
+
 void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T_tot, int nv, const uint16_t* exps,
                 const uint64_t* anchors, const uint64_t* samples, int B, int s0, const uint64_t* vals, const ZpMod& k,
                 int basis, uint64_t* out, uint64_t* nodes, int32_t* status, cudaStream_t st) {
@@ -893,6 +923,10 @@ int zippel_lift_step(const uint16_t* exps, const int64_t* h_offsets, int F, int 
   if (!ws_ok(workspace, workspace_bytes, carve(nullptr, T_tot, F, B, 0, sq).bytes)) return ZP_ERR_WORKSPACE;
   const Ws w = carve(workspace, T_tot, F, B, 0, sq);
   cudaStream_t st = (cudaStream_t)stream;
+  if (small_ok(h_offsets, F, B)) {
+    lift_small(h_offsets, F, T_tot, nv, exps, anchors, samples, B, s0, vals, k, basis, out, nodes_out, status, st);
+    return cuda_ok();
+  }
   upload_offsets(w, h_offsets, F, st);
   lift_chunk(w, h_offsets, 0, F, T_tot, nv, exps, anchors, samples, B, s0, vals, k, basis, out,
              nodes_out ? nodes_out : w.nodes, status, st);
@@ -956,8 +990,11 @@ int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int 
     cudaMemcpy2DAsync(h.vals + a, pitch, h_vals + a, pitch, 8 * (size_t)n, (size_t)B, cudaMemcpyHostToDevice, P->s_in);
     cudaEventRecord(P->ev_in[c], P->s_in);
     cudaStreamWaitEvent(st, P->ev_in[c], 0);
-    lift_chunk(w, h_offsets, f0, f1, T_tot, nv, h.exps, h.anchors, h.samples, B, s0, h.vals, k, basis, h.out, w.nodes,
-               h.status, st);
+    if (nch == 1 && small_ok(h_offsets, F, B))
+      lift_small(h_offsets, F, T_tot, nv, h.exps, h.anchors, h.samples, B, s0, h.vals, k, basis, h.out, nullptr, h.status, st);
+    else
+      lift_chunk(w, h_offsets, f0, f1, T_tot, nv, h.exps, h.anchors, h.samples, B, s0, h.vals, k, basis, h.out, w.nodes,
+                 h.status, st);
     cudaEventRecord(P->ev_done[c], st);
     cudaStreamWaitEvent(P->s_out, P->ev_done[c], 0);
     cudaMemcpy2DAsync(h_out + a, pitch, h.out + a, pitch, 8 * (size_t)n, (size_t)B, cudaMemcpyDeviceToHost, P->s_out);

@@ -63,3 +63,25 @@ def test_crt_parity_arbitrary_residues(zp, ref, p1, p2):
     gn, gd, gs = both(zp, ref, r1, r2, p1, p2)
     assert (gs == 0).any()
     assert int(gn[0]) == 0 and int(gd[0]) == 1 and int(gn[1]) == 1 and int(gn[2]) == -1
+
+
+def test_crt_huge_and_borderline_quotients(zp, ref):
+    """The kernel estimates Euclid's quotients in double precision and takes the exact 128-bit division only beyond 2^50:
+    combined values x chosen so that the first quotients m / x are huge (x just above N), sit at the 2^50 switch, or at
+    powers of two where a rounded estimate is off by one -- followed by arbitrary continuations.  == the oracle."""
+    m = P1 * P2
+    N = math.isqrt((m - 1) // 2)
+    xs = [N + 1, N + 2, N + 12345, (1 << 63), (1 << 64) - 1, (1 << 64), (1 << 64) + 1, (1 << 70) + 3, m - 1, m - 2, m // 2, m // 2 + 1,
+          m // 3, m // 3 + 1]
+    for e in (49, 50, 51, 52, 53):  # first quotient about 2^e
+        for d in (-2, -1, 0, 1, 2):
+            xs.append(m // ((1 << e) + d))
+            xs.append(m // ((1 << e) + d) + 1)
+    rng = random.Random(77)
+    for _ in range(300):  # second and later quotients large: x = (m + r) / q-ish with a tiny remainder
+        q = rng.randrange(1 << 40, 1 << 62)
+        xs.append(m // q + rng.randrange(0, 3))
+    xs = [x for x in xs if 0 < x < m]
+    r1 = np.array([x % P1 for x in xs], dtype=np.uint64)
+    r2 = np.array([x % P2 for x in xs], dtype=np.uint64)
+    both(zp, ref, r1, r2, P1, P2)
