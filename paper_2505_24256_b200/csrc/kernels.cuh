@@ -206,7 +206,7 @@ k_solve_table(const uint64_t* __restrict__ Mt, const int64_t* __restrict__ offse
 #ifdef ZP_K3_FORCE_ORIENT
 #define ZP_K3_ORIENT(NB) (ZP_K3_FORCE_ORIENT)
 #else
-#define ZP_K3_ORIENT_MASK 0x1810300u
+#define ZP_K3_ORIENT_MASK 0x1810740u
 #define ZP_K3_ORIENT(NB) ((ZP_K3_ORIENT_MASK >> (NB)) & 1u)
 #endif
 

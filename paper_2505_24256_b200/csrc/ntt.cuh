@@ -27,7 +27,8 @@
 #define ZP_NTT_TAB 4096    // entries per table
 #define ZP_NTT_LOGC 12     // a CTA transforms chunks of 4096 words in shared memory
 #define ZP_NTT_C (1 << ZP_NTT_LOGC)
-#define ZP_NTT_THREADS 256
+#define ZP_NTT_THREADS 256      // lanes per CTA for full grids
+#define ZP_NTT_THREADS_SMALL 512  // for grids that leave SMs idle: one group per lane and round, half the latency
 
 struct NttCtx {
   ZpMod q[3];
@@ -149,15 +150,15 @@ ZP_DEV void ntt_group_inv(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, in
   }
 }
 // all the stages of [lo, hi] on the tile in shared memory (the tile is complete and visible on entry and on exit)
-template <bool INV>
+template <bool INV, int TH>
 ZP_DEV void ntt_tile(uint64_t* sm, int hi, int lo, const ulonglong2* __restrict__ tab, const ZpMod& q) {
 #pragma unroll 1
   for (int r = 0; r < 4; ++r) {
     const int f = INV ? r : 3 - r, sh = 3 * f;
     if (sh > hi || sh + 2 < lo) continue;  // no stage in this field
 #pragma unroll 1
-    for (int g = 0; g < ZP_NTT_C / 8 / ZP_NTT_THREADS; ++g) {
-      const int eb = ntt_gbase(threadIdx.x + ZP_NTT_THREADS * g, sh);
+    for (int g = 0; g < ZP_NTT_C / 8 / TH; ++g) {
+      const int eb = ntt_gbase(threadIdx.x + TH * g, sh);
       ulonglong2 w[8];
       ntt_group_twiddles(w, eb, sh, hi, lo, tab);
       uint64_t x[8];
@@ -181,8 +182,8 @@ ZP_DEV void ntt_tile(uint64_t* sm, int hi, int lo, const ulonglong2* __restrict_
 //                      11 .. 12 - logR.  R <= 512 (rows of G >= 8 words).
 // logRp > 0: the transforms are the rows of parents of length 2^(logn + logRp); row c's element j is twisted by
 // w_parent^(brev(c) j) on load (forward) / by its inverse on store (inverse).
-template <bool INV>
-__global__ void __launch_bounds__(ZP_NTT_THREADS, 4)
+template <bool INV, int TH>
+__global__ void __launch_bounds__(TH, 1024 / TH)
 k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp, NttCtx cx) {
   __shared__ uint64_t sm[ZP_NTT_SMEM];
   const int jp = blockIdx.y;
@@ -210,8 +211,8 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
   const int G1 = (1 << logG) - 1;
   const int ln1 = (1 << logn) - 1;
 #pragma unroll 4
-  for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-    const int e = T + ZP_NTT_THREADS * m;
+  for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+    const int e = T + TH * m;
     const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
     uint64_t v = 0;
     if (off < E) {
@@ -225,10 +226,10 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
   }
   __syncthreads();
   const int hi = logR ? 11 : logn - 1, lo = logR ? 12 - logR : 0;
-  ntt_tile<INV>(sm, hi, lo, INV ? cx.Ui[jp] : cx.U[jp], q);
+  ntt_tile<INV, TH>(sm, hi, lo, INV ? cx.Ui[jp] : cx.U[jp], q);
 #pragma unroll 4
-  for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-    const int e = T + ZP_NTT_THREADS * m;
+  for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+    const int e = T + TH * m;
     const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
     if (off < E) {
       uint64_t v = sm[ntt_pad(e)];
@@ -256,8 +257,8 @@ ZP_DEV uint64_t ntt_canon4(uint64_t b, const ZpMod& q) {  // [0, 4q) -> [0, q)
   b = (b >= 2 * q.p) ? b - 2 * q.p : b;
   return (b >= q.p) ? b - q.p : b;
 }
-template <int MODE>
-__global__ void __launch_bounds__(ZP_NTT_THREADS, 3)
+template <int MODE, int TH>
+__global__ void __launch_bounds__(TH, 768 / TH)
 k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict__ B, int64_t EB, uint64_t* __restrict__ O,
           int64_t EO, int logn, int logRp, int logseg, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1, uint64_t Kq2) {
   extern __shared__ __align__(16) uint64_t ntt_mul_smem[];  // 2 x 32 KB (dynamic: above the 48 KB static limit)
@@ -284,8 +285,8 @@ k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict
 #pragma unroll 1
   for (int which = 0; which < (MODE == 0 ? 2 : 1); ++which) {
 #pragma unroll 4
-    for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-      const int e = T + ZP_NTT_THREADS * m;
+    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+      const int e = T + TH * m;
       uint64_t v = 0;
       if (c0 + e < Edrv) {
         if (MODE == 0) {
@@ -299,10 +300,10 @@ k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict
       sm[ntt_pad(e)] = v;
     }
     __syncthreads();
-    ntt_tile<false>(sm, logn - 1, 0, cx.U[jp], q);
+    ntt_tile<false, TH>(sm, logn - 1, 0, cx.U[jp], q);
     if (which == 0) {
 #pragma unroll 4
-      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) smA[T + ZP_NTT_THREADS * m] = sm[T + ZP_NTT_THREADS * m];  // same swizzle
+      for (int m = 0; m < ZP_NTT_C / TH; ++m) smA[T + TH * m] = sm[T + TH * m];  // same swizzle
       __syncthreads();  // the working tile is reused
     }
   }
@@ -310,30 +311,30 @@ k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict
   for (int side = 0; side < (MODE == 0 ? 1 : 2); ++side) {
     if (MODE == 0) {  // the second operand's transform is in the working tile
 #pragma unroll 4
-      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-        const int se = T + ZP_NTT_THREADS * m;  // any order: the product is position-wise
+      for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+        const int se = T + TH * m;  // any order: the product is position-wise
         sm[se] = mont_mul(mont_mul(smA[se], ntt_canon4(sm[se], q), q), Kq, q);
       }
     } else {  // the sibling's transform at the same positions of its segment: all 16 loads of a lane in flight together
-      uint64_t b[ZP_NTT_C / ZP_NTT_THREADS];
+      uint64_t b[ZP_NTT_C / TH];
 #pragma unroll
-      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-        const int e = T + ZP_NTT_THREADS * m;
+      for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+        const int e = T + TH * m;
         const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
         const uint32_t tsk = (logseg >= ZP_NTT_LOGC) ? t0 : seg % Pu;  // uniform branch: the division only for short segments
         b[m] = (c0 + e < Edrv) ? __ldg(B + (((int64_t)(2 * tsk + 1 - side) << logseg) | pos)) : 0;
       }
 #pragma unroll
-      for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-        const int se = ntt_pad(T + ZP_NTT_THREADS * m);
+      for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+        const int se = ntt_pad(T + TH * m);
         sm[se] = mont_mul(mont_mul(smA[se], ntt_canon4(b[m], q), q), Kq, q);
       }
     }
     __syncthreads();
-    ntt_tile<true>(sm, logn - 1, 0, cx.Ui[jp], q);
+    ntt_tile<true, TH>(sm, logn - 1, 0, cx.Ui[jp], q);
 #pragma unroll 4
-    for (int m = 0; m < ZP_NTT_C / ZP_NTT_THREADS; ++m) {
-      const int e = T + ZP_NTT_THREADS * m;
+    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+      const int e = T + TH * m;
       if (c0 + e >= Edrv) continue;
       uint64_t v = sm[ntt_pad(e)];
       if (logRp) v = ntt_twist<true>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);

@@ -399,16 +399,24 @@ NttPlan ntt_plan(int logn) {
   return pl;
 }
 inline dim3 ntt_grid(int64_t E) { return dim3((unsigned)((E + ZP_NTT_C - 1) / ZP_NTT_C), 3); }
+// grids that do not fill the GPU run 512 lanes per CTA (one group per lane and round: half the latency per tile)
+inline bool ntt_small_grid(int64_t E) { return 3 * ((E + ZP_NTT_C - 1) / ZP_NTT_C) < 2 * (int64_t)sm_count(); }
+template <bool INV>
+void ntt_pass_launch(uint64_t* buf, int64_t E, int logn, int logR, int logRp, const NttCtx& cx, cudaStream_t st) {
+  if (ntt_small_grid(E))
+    ++g_launches, k_ntt_pass<INV, ZP_NTT_THREADS_SMALL><<<ntt_grid(E), ZP_NTT_THREADS_SMALL, 0, st>>>(buf, E, logn, logR, logRp, cx);
+  else
+    ++g_launches, k_ntt_pass<INV, ZP_NTT_THREADS><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, logn, logR, logRp, cx);
+}
 // the strided passes alone, on every segment of `buf` ([3][E] words, segments of 2^logn), in place
 void ntt_strided(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
   const NttPlan pl = ntt_plan(logn);
-  const dim3 g = ntt_grid(E);
   if (!inverse) {
-    if (pl.lr1) ++g_launches, k_ntt_pass<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, pl.lr1, 0, cx);
-    if (pl.lr2) ++g_launches, k_ntt_pass<false><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx);
+    if (pl.lr1) ntt_pass_launch<false>(buf, E, logn, pl.lr1, 0, cx, st);
+    if (pl.lr2) ntt_pass_launch<false>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx, st);
   } else {
-    if (pl.lr2) ++g_launches, k_ntt_pass<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx);
-    if (pl.lr1) ++g_launches, k_ntt_pass<true><<<g, ZP_NTT_THREADS, 0, st>>>(buf, E, logn, pl.lr1, 0, cx);
+    if (pl.lr2) ntt_pass_launch<true>(buf, E, logn - pl.lr1, pl.lr2, pl.lr1, cx, st);
+    if (pl.lr1) ntt_pass_launch<true>(buf, E, logn, pl.lr1, 0, cx, st);
   }
 }
 // complete transforms of every segment, in place (one to three passes)
@@ -416,10 +424,24 @@ void ntt_run(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx,
   const NttPlan pl = ntt_plan(logn);
   if (!inverse) {
     ntt_strided(false, buf, E, logn, cx, st);
-    ++g_launches, k_ntt_pass<false><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, pl.lc, 0, pl.lrp, cx);
+    ntt_pass_launch<false>(buf, E, pl.lc, 0, pl.lrp, cx, st);
   } else {
-    ++g_launches, k_ntt_pass<true><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, pl.lc, 0, pl.lrp, cx);
+    ntt_pass_launch<true>(buf, E, pl.lc, 0, pl.lrp, cx, st);
     ntt_strided(true, buf, E, logn, cx, st);
+  }
+}
+template <int MODE>
+void ntt_mul_launch(int64_t Edrv, const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* O, int64_t EO, int lc,
+                    int lrp, int logn, int64_t P, const NttCtx& cx, const uint64_t (&Kq)[3], cudaStream_t st) {
+  const size_t smem = 16 * ZP_NTT_SMEM;
+  if (ntt_small_grid(Edrv)) {
+    cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL><<<ntt_grid(Edrv), ZP_NTT_THREADS_SMALL, smem, st>>>(A, EA, B, EB, O, EO, lc, lrp, logn, P,
+                                                                                                       cx, Kq[0], Kq[1], Kq[2]);
+  } else {
+    cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS><<<ntt_grid(Edrv), ZP_NTT_THREADS, smem, st>>>(A, EA, B, EB, O, EO, lc, lrp, logn, P, cx, Kq[0],
+                                                                                           Kq[1], Kq[2]);
   }
 }
 // products of segments of 2^logn words (k_ntt_mul): the strided passes on the operands, the fused chunk kernel, the
@@ -431,8 +453,7 @@ void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx&
   uint64_t Kq[3];
   make_kq(logn, Kq);
   ntt_strided(false, X, EX, logn, cx, st);
-  cudaFuncSetAttribute(k_ntt_mul<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * ZP_NTT_SMEM);
-  ++g_launches, k_ntt_mul<0><<<ntt_grid(EO), ZP_NTT_THREADS, 16 * ZP_NTT_SMEM, st>>>(X, EX, nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq[0], Kq[1], Kq[2]);
+  ntt_mul_launch<0>(EO, X, EX, nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq, st);
   ntt_strided(true, O, EO, logn, cx, st);
 }
 //   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds complete
@@ -444,8 +465,7 @@ void ntt_mul_down(uint64_t* Y, int64_t EY, const uint64_t* Xhat, int64_t EX, uin
   uint64_t Kq[3];
   make_kq(logn, Kq);
   ntt_strided(false, Y, EY, logn, cx, st);
-  cudaFuncSetAttribute(k_ntt_mul<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * ZP_NTT_SMEM);
-  ++g_launches, k_ntt_mul<1><<<ntt_grid(EY), ZP_NTT_THREADS, 16 * ZP_NTT_SMEM, st>>>(Y, EY, Xhat, EX, O, EO, pl.lc, pl.lrp, logn, P, cx, Kq[0], Kq[1], Kq[2]);
+  ntt_mul_launch<1>(EY, Y, EY, Xhat, EX, O, EO, pl.lc, pl.lrp, logn, P, cx, Kq, st);
   ntt_strided(true, O, EO, logn, cx, st);
 }
 // the per-call context: host constants + this workspace's tables (built by the first launch of the call)
