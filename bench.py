@@ -178,7 +178,7 @@ def subq_units(t, B):
         P = len(pairs)
         outs = sum(a + b for b in pairs)
         up += P * (3 * ntt(n) + pw(n)) + crt(outs)
-        down += P * 2 * ntt(n) + V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(outs))
+        down += V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(outs))  # the children's transforms are kept from the up-tree
     newton = sum(1.5 * k * k * C_MAC for k in (1 << i for i in range(10)))  # schoolbook base case to x^1024
     kk = SQ_KB
     while kk < t:

@@ -320,12 +320,12 @@ k_node_solve(const uint64_t* __restrict__ nodes, const ulonglong4* __restrict__ 
 
 // ------------------------------------------------------------------------------------------------
 // (a4) batched inversion (Montgomery's trick: "scalar-multiplied by the modular inverse
-// of the polynomial value").  A warp inverts 32 N values with ONE Fermat power: every lane multiplies its N values up
-// (prefix products in registers), the 32 lane products are scanned from both ends with shuffles (10 products per lane),
-// all lanes raise the warp's total to p - 2 together (the same instructions once per warp), and each lane unwinds its
-// own prefix products: 3 N + 12 + 125 / 1 products per lane for N inverses, i.e. about 3 + 137 / N per value against 125
-// for a Fermat power per value.  x[] Montgomery, in place -> inverses; zeros are skipped (left 0) and reported through
-// the returned mask.  Every lane of the warp must call it (full-mask shuffles).
+// of the polynomial value").  A warp inverts 32 N values with ONE modular inversion: every lane multiplies its N values
+// up (prefix products in registers), the 32 lane products are scanned from both ends with shuffles (10 products per
+// lane), all lanes invert the warp's total together (the same argument in every lane: the binary algorithm of
+// modarith.cuh, mont_inv_uniform), and each lane unwinds its own prefix products: about 3 N + 14 products per lane for N
+// inverses against 125 per value for a Fermat power each.  x[] Montgomery, in place -> inverses; zeros are skipped
+// (left 0) and reported through the returned mask.  Every lane of the warp must call it (full-mask shuffles).
 // ------------------------------------------------------------------------------------------------
 ZP_DEV uint64_t shfl_up64(uint64_t v, int o) {
   return ((uint64_t)__shfl_up_sync(0xffffffffu, (uint32_t)(v >> 32), o) << 32) | __shfl_up_sync(0xffffffffu, (uint32_t)v, o);
@@ -355,7 +355,7 @@ ZP_DEV uint32_t warp_batch_inv(uint64_t (&x)[N], const ZpMod& k) {
     below = (lane >= o) ? a : below;
     above = (lane + o < 32) ? b : above;
   }
-  const uint64_t tinv = mont_inv(shfl_idx64(below, 31), k);  // 1 / (product of the whole warp)
+  const uint64_t tinv = mont_inv_uniform(shfl_idx64(below, 31), k);  // 1 / (product of the whole warp): uniform
   const uint64_t lo = shfl_up64(below, 1), hi = shfl_down64(above, 1);
   uint64_t inv = tinv;  // 1 / run = tinv * (lanes below) * (lanes above)
   if (lane > 0) inv = mont_mul(inv, lo, k);

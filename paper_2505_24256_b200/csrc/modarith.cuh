@@ -88,8 +88,42 @@ ZP_DEV uint64_t mont_pow(uint64_t x, uint64_t e, const ZpMod& k) {
   }
   return r;
 }
-// Inverse by Fermat, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.
+// a^-1 mod p for a in [1, p), p odd, gcd(a, p) = 1, by the binary extended Euclidean algorithm: at most 2 x 63
+// halvings and 63 subtractions of plain 64-bit integers (no multiplication), against the 125 dependent Montgomery
+// products of a Fermat power -- a Montgomery product alone is about 160 cycles of latency on sm_100a, and an inversion
+// is latency, not throughput, where it sits alone in a warp (the one inversion of a batched inversion).
+// Invariants: x1 a = u, x2 a = v (mod p).  0 (or a common factor: p not prime) -> 0; callers flag zeros.
+ZP_DEV uint64_t zp_inv_binary(uint64_t a, uint64_t p) {
+  uint64_t u = a, v = p, x1 = 1, x2 = 0;
+  if (a == 0) return 0;
+  for (int guard = 0; guard < 512 && u != 1 && v != 1; ++guard) {
+    if ((u & 1) == 0) {
+      u >>= 1;
+      x1 = (x1 & 1) ? (x1 + p) >> 1 : x1 >> 1;  // x1 + p < 2^64: both below 2^63
+    } else if ((v & 1) == 0) {
+      v >>= 1;
+      x2 = (x2 & 1) ? (x2 + p) >> 1 : x2 >> 1;
+    } else if (u >= v) {
+      u -= v;
+      x1 = (x1 >= x2) ? x1 - x2 : x1 + p - x2;
+      if (u == 0) return 0;  // gcd(a, p) > 1
+    } else {
+      v -= u;
+      x2 = (x2 >= x1) ? x2 - x1 : x2 + p - x1;
+    }
+  }
+  return u == 1 ? x1 : (v == 1 ? x2 : 0);
+}
+// Inverse by Fermat, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.  The form for lanes
+// with DIFFERENT arguments: the same instructions in every lane (the binary algorithm above diverges four ways per
+// iteration: measured 1.5x slower than this in k_newton_prep, k_thiele and k_lift_small).
 ZP_DEV uint64_t mont_inv(uint64_t x, const ZpMod& k) { return mont_pow(x, k.p - 2, k); }
+// The same for an argument that is UNIFORM across the warp (the one inversion of a batched inversion): the binary
+// algorithm, (x^-1)~ = 2^128 / x~ = the plain inverse of x~ times r2 twice (Montgomery products).
+ZP_DEV uint64_t mont_inv_uniform(uint64_t x, const ZpMod& k) {
+  const uint64_t z = zp_inv_binary(x, k.p);
+  return mont_mul(mont_mul(z, k.r2, k), k.r2, k);
+}
 
 // ---- Horner step with Shoup companions (the hot recurrence of (a3): q <- M_l + m q, d <- M'_l + m d) ----
 // For w in [0,p) its companion is w' = floor(w 2^64 / p) < 2^64.  Since w 2^64 - w~ = w' p with

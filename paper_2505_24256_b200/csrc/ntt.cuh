@@ -249,7 +249,8 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
 // operands through the forward stages, multiply, and take the product back through the inverse stages without the
 // transformed operands ever leaving the SM.  The factor 1/n rides on the product (Kq[j] = 2^128 / n mod q_j:
 // mont_mul(mont_mul(a, b), Kq) = a b / n).  A CTA = one chunk of one prime.
-//   MODE 0 (pairs): O segment o = A segment 2o * A segment 2o + 1               (up-tree; Newton; root; B unused)
+//   MODE 0 (pairs): O segment o = A segment 2o * A segment 2o + 1               (up-tree; Newton; root); B != null (= A):
+//                   the complete transforms of the operands are written back over them (kept for MODE 1 later)
 //   MODE 1 (down) : O segments 2 vt + side = A segment vt * B segment 2 (vt mod P) + 1 - side, side = 0, 1, where B holds
 //                   COMPLETE forward transforms (k_ntt_pass): tails x reversed siblings, the siblings' transforms are
 //                   shared by all the vectors of a level.  EA, EB, EO: words per prime of the three buffers.
@@ -259,7 +260,7 @@ ZP_DEV uint64_t ntt_canon4(uint64_t b, const ZpMod& q) {  // [0, 4q) -> [0, q)
 }
 template <int MODE, int TH>
 __global__ void __launch_bounds__(TH, 768 / TH)
-k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict__ B, int64_t EB, uint64_t* __restrict__ O,
+k_ntt_mul(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* __restrict__ O,
           int64_t EO, int logn, int logRp, int logseg, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1, uint64_t Kq2) {
   extern __shared__ __align__(16) uint64_t ntt_mul_smem[];  // 2 x 32 KB (dynamic: above the 48 KB static limit)
   uint64_t *sm = ntt_mul_smem, *smA = ntt_mul_smem + ZP_NTT_SMEM;  // the working tile; the first operand's transform
@@ -301,6 +302,16 @@ k_ntt_mul(const uint64_t* __restrict__ A, int64_t EA, const uint64_t* __restrict
     }
     __syncthreads();
     ntt_tile<false, TH>(sm, logn - 1, 0, cx.U[jp], q);
+    if (MODE == 0 && B != nullptr) {  // keep: the operand's complete transform goes back to where it came from (B = A)
+#pragma unroll 4
+      for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+        const int e = T + TH * m;
+        if (c0 + e < Edrv) {
+          const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+          const_cast<uint64_t*>(A)[((int64_t)(2 * seg + which) << logseg) | pos] = sm[ntt_pad(e)];
+        }
+      }
+    }
     if (which == 0) {
 #pragma unroll 4
       for (int m = 0; m < ZP_NTT_C / TH; ++m) smA[T + TH * m] = sm[T + TH * m];  // same swizzle

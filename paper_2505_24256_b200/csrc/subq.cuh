@@ -28,26 +28,8 @@ struct SqTask {
 };
 
 // ---- (up) ---------------------------------------------------------------------------------------------------------------
-// X[j][2t][i] = A'_i (i < a), X[j][2t+1][i] = B'_i (i < b), zero-padded to n = 2a.  The residues mod p are < 2^63 < 4q:
-// valid lazy inputs for all three primes as they are.
-__global__ void __launch_bounds__(256)
-k_sq_up_prep(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn, uint64_t* __restrict__ X,
-             int64_t EX) {
-  const int64_t n = (int64_t)1 << logn;
-  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t seg = e >> logn, i = e & (n - 1);
-    const SqTask t = tasks[seg >> 1];
-    uint64_t v = 0;
-    if (seg & 1) {
-      if (i < t.b) v = lev[t.base + t.a + i];
-    } else {
-      if (i < t.a) v = lev[t.base + i];
-    }
-    X[e] = v;
-    X[EX + e] = v;
-    X[2 * EX + e] = v;
-  }
-}
+// The product of a pair is taken on the REVERSED children (k_sq_down_prepx below fills X: rev(A') rev(B') = rev(A' B'),
+// degree a + b - 2), because their transforms are what the down-tree needs again: O[t][i] = (A' B')_{a+b-2-i}.
 // C' = A' B' + z^a B' + z^b A'  (Montgomery in, Montgomery out: co carries K = 2^-64)
 __global__ void __launch_bounds__(256)
 k_sq_up_fin(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn,
@@ -57,7 +39,11 @@ k_sq_up_fin(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, 
     const int64_t c = e & (n - 1);
     const SqTask t = tasks[e >> logn];
     if (c >= t.a + t.b) continue;
-    uint64_t r = ntt_crt(O[e], O[EO + e], O[2 * EO + e], cx, co, kp);
+    uint64_t r = 0;
+    if (c <= t.a + t.b - 2) {
+      const int64_t src = e - c + (t.a + t.b - 2 - c);
+      r = ntt_crt(O[src], O[EO + src], O[2 * EO + src], cx, co, kp);
+    }
     if (c >= t.a) r = mod_add(r, lev[t.base + t.a + (c - t.a)], kp.p);
     if (c >= t.b) r = mod_add(r, lev[t.base + (c - t.b)], kp.p);
     nxt[t.base + c] = r;

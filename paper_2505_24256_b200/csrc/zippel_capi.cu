@@ -118,7 +118,7 @@ struct SqRun {
 };
 struct SqSizes {
   bool any = false;
-  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0, maxFns = 0;
+  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0, maxFns = 0, sumXl = 0;
   int maxLev = 0, Vc = 1;
   int64_t thr = 0;  // the threshold the runs were found with (sq_threshold on the whole batch)
 };
@@ -191,18 +191,19 @@ SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
   z.Vc = (int)(vc < 1 ? 1 : (vc > B + 1 ? B + 1 : vc));
   for (const SqRun& r : runs) {
     z.maxLev = r.nlev > z.maxLev ? r.nlev : z.maxLev;
-    int64_t ntasks = 0, leaves = 0;
+    int64_t ntasks = 0, leaves = 0, sumXl = 0;
     for (int l = 0; l < r.nlev; ++l) {
       std::vector<SqTask> pairs, copies;
       sq_level_tasks(h_offs, r, l, &pairs, &copies);
       const int64_t n = (int64_t)2 * ZP_LEAF << l, P = (int64_t)pairs.size();
-      mx(z.maxX, 2 * P * n);
+      sumXl += 2 * P * n;  // the level's transformed (reversed) children stay for the down-tree
       mx(z.maxO, P * n);
       mx(z.maxY, z.Vc * P * n);
       mx(z.maxO, 2 * z.Vc * P * n);
       ntasks += (int64_t)pairs.size() + (int64_t)copies.size();
     }
     mx(z.maxTasks, ntasks);
+    mx(z.sumXl, sumXl);
     int64_t sumK = 0, sumR = 0;  // the functions of a run take the Newton steps and the root products together
     for (int f = r.f0; f < r.f1; ++f) {
       const int64_t t = h_offs[f + 1] - h_offs[f];
@@ -234,7 +235,7 @@ struct Ws {
   SqTask* sq_tasks;
   SqFn* sq_fns;
   int64_t* sq_leafoffs;
-  uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Y, *sq_O;
+  uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Xl, *sq_Y, *sq_O;
   size_t bytes;
 };
 
@@ -275,6 +276,7 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags, const SqSizes& sq =
     w.sq_tailB = (uint64_t*)take(8 * (size_t)(B + 1) * sq.maxT);
     w.sq_alpha = (uint64_t*)take(8 * (size_t)sq.alphaN);
     w.sq_X = (uint64_t*)take(8 * 3 * (size_t)sq.maxX);
+    w.sq_Xl = (uint64_t*)take(8 * 3 * (size_t)sq.sumXl);  // per tree level: the transforms of the reversed children
     w.sq_Y = (uint64_t*)take(8 * 3 * (size_t)sq.maxY);
     w.sq_O = (uint64_t*)take(8 * 3 * (size_t)sq.maxO);
   }
@@ -447,13 +449,14 @@ void ntt_mul_launch(int64_t Edrv, const uint64_t* A, int64_t EA, const uint64_t*
 // products of segments of 2^logn words (k_ntt_mul): the strided passes on the operands, the fused chunk kernel, the
 // strided passes on the product.
 //   pairs: O segment o = X segment 2o * X segment 2o + 1 (EO = EX / 2); X is overwritten by its strided passes
-void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx& cx, cudaStream_t st) {
+//   keep: X ends up holding the COMPLETE forward transforms of its segments (the chunk stages are written back)
+void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx& cx, cudaStream_t st, bool keep = false) {
   const NttPlan pl = ntt_plan(logn);
   const int64_t EO = EX / 2;
   uint64_t Kq[3];
   make_kq(logn, Kq);
   ntt_strided(false, X, EX, logn, cx, st);
-  ntt_mul_launch<0>(EO, X, EX, nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq, st);
+  ntt_mul_launch<0>(EO, X, EX, keep ? X : nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq, st);
   ntt_strided(true, O, EO, logn, cx, st);
 }
 //   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds complete
@@ -521,6 +524,8 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
 
   // (up) leaves, then one product per pair and level
   auto lev = [&](int l) { return w.sq_lev + (size_t)l * T; };
+  std::vector<int64_t> xoff(r.nlev + 1, 0);  // words per prime of the levels below l in sq_Xl
+  for (int l = 0; l < r.nlev; ++l) xoff[l + 1] = xoff[l] + 2 * (int64_t)(copy0[l] - pair0[l]) * ((int64_t)2 * ZP_LEAF << l);
   {
     ProfScope prof(ZP_K_MASTER_POLY, st);
     dim3 g((unsigned)((r.tmax + ZP_LEAF - 1) / ZP_LEAF), grid_y(Fr));
@@ -532,8 +537,11 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       const SqTask* tp = w.sq_tasks + pair0[l];
       if (P) {
         const int64_t EX = 2 * P * n, EO = P * n;
-        ++g_launches, k_sq_up_prep<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_X, EX);
-        ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
+        // the REVERSED children are multiplied (rev(A') rev(B') = rev(A' B')): their transforms are what the down-tree
+        // correlates the tails with, and they are kept for it
+        uint64_t* Xl = w.sq_Xl + 3 * xoff[l];
+        ++g_launches, k_sq_down_prepx<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, Xl, EX);
+        ntt_mul_pairs(Xl, EX, w.sq_O, logn, cx, st, true);
         ++g_launches, k_sq_up_fin<<<sq_blocks(EO), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_O, EO, cx, co1, k, lev(l + 1));
       }
       const int nc = (int)(copy1[l] - copy0[l]);
@@ -592,13 +600,12 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
     const SqTask* tp = w.sq_tasks + pair0[l];
     if (P) {
       const int64_t EX = 2 * P * n;
-      ++g_launches, k_sq_down_prepx<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_X, EX);
-      ntt_run(false, w.sq_X, EX, logn, cx, st);
+      const uint64_t* Xl = w.sq_Xl + 3 * xoff[l];  // the transforms of the reversed children, from the up-tree
       for (int v0 = 0; v0 < V; v0 += w.sq.Vc) {
         const int nv = (V - v0 < w.sq.Vc) ? V - v0 : w.sq.Vc;
         const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
         ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
-        ntt_mul_down(w.sq_Y, EY, w.sq_X, EX, w.sq_O, logn, P, cx, st);
+        ntt_mul_down(w.sq_Y, EY, Xl, EX, w.sq_O, logn, P, cx, st);
         ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
                                                                     nxt + (size_t)v0 * T);
       }

@@ -45,7 +45,7 @@ def test_work_model_of_the_subquadratic_route():
     up = 2 * (3 * ntt(2048) + pw(2048)) + crt(4096) + 1 * (3 * ntt(4096) + pw(4096)) + crt(4096)
     assert parts["up_tree"] == up
     V = 2
-    down = sum(P * 2 * ntt(n) + V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in ((2, 2048), (1, 4096)))
+    down = sum(V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in ((2, 2048), (1, 4096)))
     assert parts["down_tree"] == down
     assert parts["leaves"] == 4 * 1024 * 1024 * (4 + 16 + 2 * 8)
     t19, _ = b.subq_units(1 << 19, 1)
