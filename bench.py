@@ -150,7 +150,7 @@ def sq_threshold(ts, B):
     """csrc/zippel_capi.cu sq_threshold: functions with at least this many terms take the sub-quadratic route."""
     if sum(int(t) for t in ts if int(t) >= 3072) >= 65536:
         return 3072
-    return 3072 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 16384
+    return 3072 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 12288
 C_MONT = 18  # Montgomery product: 8 wide + 2 low
 
 

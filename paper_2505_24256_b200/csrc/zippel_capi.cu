@@ -118,14 +118,14 @@ struct SqRun {
 };
 struct SqSizes {
   bool any = false;
-  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0, maxFns = 0, sumXl = 0;
+  int64_t maxT = 0, alphaN = 0, maxX = 0, maxY = 0, maxO = 0, maxTasks = 0, maxLeaves = 0, maxFns = 0, sumXl = 0, maxO2 = 0;
   int maxLev = 0, Vc = 1;
   int64_t thr = 0;  // the threshold the runs were found with (sq_threshold on the whole batch)
 };
 // Which functions take the sub-quadratic route: those with at least sq_threshold terms.  Measured on B200 (profiles/
 // r02_crossover.md): a batch with enough long functions to fill the GPU crosses over at t = 3072 for every B; a single
-// function (or a few) is bound by the latency of the route's ~170 dependent launches and crosses over later, the later
-// the fewer right-hand sides there are to amortise them (B = 1: 16384, B = 3: 8192, B = 9: 4096, B = 21: 3072).
+// function (or a few) is bound by the latency of the route's ~150 dependent launches and crosses over later, the later
+// the fewer right-hand sides there are to amortise them (B = 1: 12288, B = 3: 8192, B = 9: 4096, B = 21: 3072).
 int64_t sq_threshold(const int64_t* h_offs, int F, int B) {
   if (g_subq_min_t > 0) return g_subq_min_t;
   int64_t sum = 0;
@@ -134,7 +134,7 @@ int64_t sq_threshold(const int64_t* h_offs, int F, int B) {
     if (t >= 3072) sum += t;
   }
   if (sum >= 65536) return 3072;
-  return B >= 16 ? 3072 : B >= 6 ? 4096 : B >= 2 ? 8192 : 16384;
+  return B >= 16 ? 3072 : B >= 6 ? 4096 : B >= 2 ? 8192 : 12288;
 }
 inline bool sq_is_long(int64_t t, int64_t thr) { return t >= thr && t > ZP_LEAF; }
 
@@ -215,7 +215,7 @@ SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
     }
     mx(z.alphaN, sumK);
     mx(z.maxX, 2 * (sumK > sumR ? sumK : sumR));
-    mx(z.maxO, sumK > sumR ? sumK : sumR);
+    mx(z.maxO2, sumK > sumR ? sumK : sumR);
     mx(z.maxFns, r.f1 - r.f0);
     mx(z.maxLeaves, leaves);
   }
@@ -235,7 +235,7 @@ struct Ws {
   SqTask* sq_tasks;
   SqFn* sq_fns;
   int64_t* sq_leafoffs;
-  uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Xl, *sq_Y, *sq_O;
+  uint64_t *sq_lev, *sq_tailA, *sq_tailB, *sq_alpha, *sq_X, *sq_Xl, *sq_Y, *sq_O, *sq_O2;
   size_t bytes;
 };
 
@@ -279,6 +279,7 @@ Ws carve(void* base, int64_t T_tot, int F, int B, int flags, const SqSizes& sq =
     w.sq_Xl = (uint64_t*)take(8 * 3 * (size_t)sq.sumXl);  // per tree level: the transforms of the reversed children
     w.sq_Y = (uint64_t*)take(8 * 3 * (size_t)sq.maxY);
     w.sq_O = (uint64_t*)take(8 * 3 * (size_t)sq.maxO);
+    w.sq_O2 = (uint64_t*)take(8 * 3 * (size_t)sq.maxO2);  // products of the Newton chain (second stream)
   }
   w.bytes = o;
   return w;
@@ -495,6 +496,28 @@ uint64_t* g_sq_dump_out = nullptr;
 #define SQ_DUMP(stage, ptr, words)
 #endif
 
+// second stream of the sub-quadratic route (created once per device, kept for the process; zippel_shutdown destroys
+// it): the Newton iteration for the M' tail runs on it beside the value vectors' down-tree
+struct SqAux {
+  bool ready = false;
+  cudaStream_t s2 = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+};
+SqAux g_sqaux[16];
+SqAux* get_sqaux() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 16) return nullptr;
+  SqAux& A = g_sqaux[dev];
+  if (!A.ready) {
+    if (cudaStreamCreateWithFlags(&A.s2, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&A.ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&A.ev_join, cudaEventDisableTiming) != cudaSuccess)
+      return nullptr;
+    A.ready = true;
+  }
+  return &A;
+}
+
 // (a2)-(a4) for one run of long functions; nodes / vals / coefs point at the run's first slot (row strides ldv, ldc)
 void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun& r, const uint64_t* nodes,
               const uint64_t* vals, int64_t ldv, int B, int s0, const ZpMod& k, uint64_t* coefs, int64_t ldc,
@@ -553,6 +576,11 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   // root tails: rows 0 .. B-1 = the values; row B = rev(M') / rev(M) mod x^t per function
   const int V = B + 1;
   uint64_t *cur = w.sq_tailA, *nxt = w.sq_tailB;
+  // The M' tail needs the power-series inverse of rev(M) (a chain of small dependent launches); the value vectors do
+  // not: their down-tree runs on st while the Newton iteration runs on a second stream, then the M' vector follows.
+  SqAux* aux = get_sqaux();
+  const cudaStream_t sn = aux ? aux->s2 : st;
+  int64_t dump_alpha_off = 0, dump_alpha_t = 0;  // (test hook: the longest function's inverse series)
   ++g_launches, k_sq_load_vals<<<dim3(sq_blocks(T), (unsigned)(B < 64 ? B : 64)), 256, 0, st>>>(vals, ldv, B, T, k, cur, T);
   {
     // the functions of the run, longest first: those still iterating at precision kk (t > kk) are a prefix
@@ -567,57 +595,83 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       ao += kf;
     }
     cudaMemcpyAsync(w.sq_fns, fns.data(), sizeof(SqFn) * fns.size(), cudaMemcpyHostToDevice, st);
+    if (aux) {  // fork: the second stream starts after everything queued on st so far (up-tree, uploads)
+      cudaEventRecord(aux->ev_fork, st);
+      cudaStreamWaitEvent(aux->s2, aux->ev_fork, 0);
+    }
     const uint64_t* top = lev(r.nlev);
-    ++g_launches, k_sq_inv_base<<<(unsigned)Fr, 512, 0, st>>>(top, w.sq_fns, k, w.sq_alpha);
+    ++g_launches, k_sq_inv_base<<<(unsigned)Fr, 512, 0, sn>>>(top, w.sq_fns, k, w.sq_alpha);
     for (int64_t kk = ZP_SQ_KB; kk < r.tmax; kk <<= 1) {  // precision kk -> 2 kk, products of length n = 2 kk
       int64_t nact = 0;
       while (nact < Fr && fns[nact].t > kk) ++nact;
       const int logn = ceil_log2(2 * kk);
       const int64_t n = 2 * kk, EX = 2 * nact * n;
-      ++g_launches, k_sq_newton_prep1<<<sq_blocks(EX), 256, 0, st>>>(top, w.sq_fns, nact, w.sq_alpha, logn, k, w.sq_X);
-      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
-      ++g_launches, k_sq_newton_mid<<<sq_blocks(EX), 256, 0, st>>>(w.sq_O, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha, w.sq_X);
-      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
-      ++g_launches, k_sq_newton_fin<<<sq_blocks(nact * kk), 256, 0, st>>>(w.sq_O, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha);
+      ++g_launches, k_sq_newton_prep1<<<sq_blocks(EX), 256, 0, sn>>>(top, w.sq_fns, nact, w.sq_alpha, logn, k, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
+      ++g_launches, k_sq_newton_mid<<<sq_blocks(EX), 256, 0, sn>>>(w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
+      ++g_launches, k_sq_newton_fin<<<sq_blocks(nact * kk), 256, 0, sn>>>(w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha);
     }
-    SQ_DUMP(2, w.sq_alpha + fns[0].aoff, fns[0].t);
+    dump_alpha_off = fns[0].aoff;
+    dump_alpha_t = fns[0].t;
     for (int g0 = 0; g0 < Fr;) {  // root products: the functions with the same product length n >= 2 t together
       const int logn = ceil_log2(2 * fns[g0].t);
       int g1 = g0;
       while (g1 < Fr && ceil_log2(2 * fns[g1].t) == logn) ++g1;
       const int64_t n = (int64_t)1 << logn, ng = g1 - g0, EX = 2 * ng * n;
-      ++g_launches, k_sq_root_prep<<<sq_blocks(EX), 256, 0, st>>>(top, w.sq_fns + g0, ng, w.sq_alpha, logn, k, w.sq_X);
-      ntt_mul_pairs(w.sq_X, EX, w.sq_O, logn, cx, st);
-      ++g_launches, k_sq_root_fin<<<sq_blocks(ng * n), 256, 0, st>>>(w.sq_O, w.sq_fns + g0, ng, logn, cx, co2, k, cur + (size_t)B * T);
+      ++g_launches, k_sq_root_prep<<<sq_blocks(EX), 256, 0, sn>>>(top, w.sq_fns + g0, ng, w.sq_alpha, logn, k, w.sq_X);
+      ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
+      ++g_launches, k_sq_root_fin<<<sq_blocks(ng * n), 256, 0, sn>>>(w.sq_O2, w.sq_fns + g0, ng, logn, cx, co2, k, cur + (size_t)B * T);
       g0 = g1;
     }
   }
-  SQ_DUMP(3, cur, (size_t)V * T);
-  // (down) level by level, vectors in chunks of Vc
-  for (int l = r.nlev - 1; l >= 0; --l) {
-    const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
-    const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
-    const SqTask* tp = w.sq_tasks + pair0[l];
-    if (P) {
-      const int64_t EX = 2 * P * n;
-      const uint64_t* Xl = w.sq_Xl + 3 * xoff[l];  // the transforms of the reversed children, from the up-tree
-      for (int v0 = 0; v0 < V; v0 += w.sq.Vc) {
-        const int nv = (V - v0 < w.sq.Vc) ? V - v0 : w.sq.Vc;
-        const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
-        ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
-        ntt_mul_down(w.sq_Y, EY, Xl, EX, w.sq_O, logn, P, cx, st);
-        ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(cur + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
-                                                                    nxt + (size_t)v0 * T);
+  // (down) level by level for the vector rows [va, vb), in chunks of Vc; returns with the rows in `cur`'s final buffer
+  auto down = [&](int va, int vb, uint64_t* c, uint64_t* n2) {
+    const int Vr = vb - va;
+    for (int l = r.nlev - 1; l >= 0; --l) {
+      const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
+      const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
+      const SqTask* tp = w.sq_tasks + pair0[l];
+      if (P) {
+        const int64_t EX = 2 * P * n;
+        const uint64_t* Xl = w.sq_Xl + 3 * xoff[l];  // the transforms of the reversed children, from the up-tree
+        for (int v0 = va; v0 < vb; v0 += w.sq.Vc) {
+          const int nv = (vb - v0 < w.sq.Vc) ? vb - v0 : w.sq.Vc;
+          const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
+          ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
+          ntt_mul_down(w.sq_Y, EY, Xl, EX, w.sq_O, logn, P, cx, st);
+          ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
+                                                                      n2 + (size_t)v0 * T);
+        }
       }
+      const int nc = (int)(copy1[l] - copy0[l]);
+      if (nc) {
+        const int ny = nc * Vr;
+        ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(ny < 1024 ? ny : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, c + (size_t)va * T,
+                                                                                             n2 + (size_t)va * T, Vr, T);
+      }
+      uint64_t* tmp = c;
+      c = n2;
+      n2 = tmp;
     }
-    const int nc = (int)(copy1[l] - copy0[l]);
-    if (nc) {
-      const int ny = nc * V;
-      ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(ny < 1024 ? ny : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, cur, nxt, V, T);
-    }
-    uint64_t* tmp = cur;
-    cur = nxt;
-    nxt = tmp;
+    return c;
+  };
+  SQ_DUMP(3, cur, (size_t)B * T);        // (the root tails of the values, before their buffer is reused)
+  uint64_t* fin = down(0, B, cur, nxt);  // the value vectors, beside the Newton chain
+  if (aux) {                             // join: the M' tail is complete
+    cudaEventRecord(aux->ev_join, sn);
+    cudaStreamWaitEvent(st, aux->ev_join, 0);
+  }
+  SQ_DUMP(2, w.sq_alpha + dump_alpha_off, dump_alpha_t);
+#ifdef ZP_TEST_HOOKS
+  if (g_sq_dump_stage == 3 && g_sq_dump_out)  // (and the root tail of M')
+    cudaMemcpyAsync(g_sq_dump_out + (size_t)B * T, cur + (size_t)B * T, 8 * (size_t)T, cudaMemcpyDeviceToDevice, st);
+#endif
+  (void)dump_alpha_off, (void)dump_alpha_t;
+  down(B, V, cur, nxt);  // the M' vector
+  if (fin != cur) {
+    nxt = cur;
+    cur = fin;
   }
   SQ_DUMP(4, cur, (size_t)V * T);
   // (leaf) the synthetic-division dots of (a3) on the leaves as functions, B + 1 right-hand sides, unscaled
@@ -1184,6 +1238,15 @@ int zippel_shutdown(void) {
       cudaEventDestroy(P.ev_done[c]);
     }
     P = Pipe();
+  }
+  for (int dev = 0; dev < 16; ++dev) {
+    SqAux& A = g_sqaux[dev];
+    if (!A.ready) continue;
+    cudaSetDevice(dev);
+    cudaStreamDestroy(A.s2);
+    cudaEventDestroy(A.ev_fork);
+    cudaEventDestroy(A.ev_join);
+    A = SqAux();
   }
   return cuda_ok();
 }
