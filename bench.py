@@ -142,15 +142,15 @@ def load_workload(idx: int, seed_shift: int, F_override):
                                 sh["emax"], sh["B"], with_planted=False)
 
 
-# the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_LEAF, g_subq_min_t)
-SQ_LEAF, SQ_KB = 1024, 1024
+# the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_SQ_LEAF, ZP_SQ_KB)
+SQ_LEAF, SQ_KB = 512, 1024
 
 
 def sq_threshold(ts, B):
     """csrc/zippel_capi.cu sq_threshold: functions with at least this many terms take the sub-quadratic route."""
-    if sum(int(t) for t in ts if int(t) >= 3072) >= 65536:
-        return 3072
-    return 3072 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 12288
+    if sum(int(t) for t in ts if int(t) >= 2048) >= 65536:
+        return 2048
+    return 2048 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 12288
 C_MONT = 18  # Montgomery product: 8 wide + 2 low
 
 
@@ -360,7 +360,7 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
     achieved = ns_ops / (ns_ms * 1e-3) / 1e12
     ns_ops_instr = float(sum(int(t) ** 2 for t in ns_ts)) * (2 * C_MM_INSTR + B * C_MAC_INSTR)  # SURVEY.md 8(d).4 accounting
     if subq:
-        kernel = "sub-quadratic solve after the product tree: tails down the tree (k_ntt_* passes, pointwise, CRT), leaf k_node_solve, k_inv_finish"
+        kernel = "sub-quadratic solve (csrc/subq.cuh): leaf trees, up-tree, Newton chain, tails down the tree (k_ntt_mul, k_ntt_pass, CRT), leaf k_node_solve, k_inv_finish"
         cost = ("W_alg of the sub-quadratic route (bench.py subq_units, DESIGN.md section 12): butterfly = one Shoup product = 16 units, "
                 "pointwise = 2 Montgomery products (36), CRT + reduction = 5 (90), leaves = quadratic node solve with B + 1 right-hand sides")
     elif idx == 5 or (B == 1 and int(min(ts)) >= 4096):

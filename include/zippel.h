@@ -206,7 +206,7 @@ unsigned long long zippel_launch_count(void);
  *   ZP_TUNE_SUBQ_MIN_T: functions with at least this many terms (and more than 1024) take the sub-quadratic route
  *   (three-prime NTT product tree, tails, leaf solves: csrc/subq.cuh) instead of the quadratic
  *   kernels of PAPER.md section 2.2.  Same results bit for bit.  Default 0 = the measured rule:
- *   3072 terms when the batch holds at least 65536 terms in such functions, else 3072 / 4096 / 8192 / 12288 terms for
+ *   2048 terms when the batch holds at least 65536 terms in such functions, else 2048 / 4096 / 8192 / 12288 terms for
  *   B >= 16 / >= 6 / >= 2 / = 1 right-hand sides (a single function is bound by the latency of the route's launches). */
 #define ZP_TUNE_SUBQ_MIN_T 1
 int zippel_set_tuning(int key, int64_t value);

@@ -114,7 +114,7 @@ inline int ceil_log2(int64_t x) {
 struct SqRun {
   int f0, f1;
   int64_t a0, T, tmax;
-  int nlev;  // levels 0 .. nlev; block size at level l = ZP_LEAF << l
+  int nlev;  // levels 0 .. nlev; block size at level l = ZP_SQ_LEAF << l
 };
 struct SqSizes {
   bool any = false;
@@ -123,24 +123,28 @@ struct SqSizes {
   int64_t thr = 0;  // the threshold the runs were found with (sq_threshold on the whole batch)
 };
 // Which functions take the sub-quadratic route: those with at least sq_threshold terms.  Measured on B200 (profiles/
-// r02_crossover.md): a batch with enough long functions to fill the GPU crosses over at t = 3072 for every B; a single
+// r02_crossover.md): a batch with enough long functions to fill the GPU crosses over at t = 2048 for every B; a single
 // function (or a few) is bound by the latency of the route's ~150 dependent launches and crosses over later, the later
-// the fewer right-hand sides there are to amortise them (B = 1: 12288, B = 3: 8192, B = 9: 4096, B = 21: 3072).
+// the fewer right-hand sides there are to amortise them (B = 1: 12288, B = 3: 8192, B = 9: 4096, B = 21: 2048).
 int64_t sq_threshold(const int64_t* h_offs, int F, int B) {
   if (g_subq_min_t > 0) return g_subq_min_t;
   int64_t sum = 0;
   for (int f = 0; f < F; ++f) {
     const int64_t t = h_offs[f + 1] - h_offs[f];
-    if (t >= 3072) sum += t;
+    if (t >= 2048) sum += t;
   }
-  if (sum >= 65536) return 3072;
-  return B >= 16 ? 3072 : B >= 6 ? 4096 : B >= 2 ? 8192 : 12288;
+  if (sum >= 65536) return 2048;
+  return B >= 16 ? 2048 : B >= 6 ? 4096 : B >= 2 ? 8192 : 12288;
 }
+// leaves of the sub-quadratic route: blocks of at most this many nodes are solved by the quadratic kernels (at most ZP_LEAF)
+#ifndef ZP_SQ_LEAF
+#define ZP_SQ_LEAF 512
+#endif
 inline bool sq_is_long(int64_t t, int64_t thr) { return t >= thr && t > ZP_LEAF; }
 
 // pair and copy tasks of level l (children of size a = LEAF << l) for a run; slots relative to the run
 void sq_level_tasks(const int64_t* h_offs, const SqRun& r, int l, std::vector<SqTask>* pairs, std::vector<SqTask>* copies) {
-  const int64_t a = (int64_t)ZP_LEAF << l;
+  const int64_t a = (int64_t)ZP_SQ_LEAF << l;
   for (int f = r.f0; f < r.f1; ++f) {
     const int64_t off = h_offs[f] - r.a0, t = h_offs[f + 1] - h_offs[f];
     int64_t base = 0;
@@ -172,7 +176,7 @@ void sq_find_runs(const int64_t* h_offs, int F, int64_t thr, std::vector<SqRun>*
     r.f1 = f;
     r.a0 = h_offs[r.f0];
     r.T = h_offs[r.f1] - r.a0;
-    r.nlev = ceil_log2((r.tmax + ZP_LEAF - 1) / ZP_LEAF);
+    r.nlev = ceil_log2((r.tmax + ZP_SQ_LEAF - 1) / ZP_SQ_LEAF);
     runs->push_back(r);
   }
 }
@@ -195,7 +199,7 @@ SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
     for (int l = 0; l < r.nlev; ++l) {
       std::vector<SqTask> pairs, copies;
       sq_level_tasks(h_offs, r, l, &pairs, &copies);
-      const int64_t n = (int64_t)2 * ZP_LEAF << l, P = (int64_t)pairs.size();
+      const int64_t n = (int64_t)2 * ZP_SQ_LEAF << l, P = (int64_t)pairs.size();
       sumXl += 2 * P * n;  // the level's transformed (reversed) children stay for the down-tree
       mx(z.maxO, P * n);
       mx(z.maxY, z.Vc * P * n);
@@ -207,7 +211,7 @@ SqSizes sq_sizes(const int64_t* h_offs, int F, int B) {
     int64_t sumK = 0, sumR = 0;  // the functions of a run take the Newton steps and the root products together
     for (int f = r.f0; f < r.f1; ++f) {
       const int64_t t = h_offs[f + 1] - h_offs[f];
-      leaves += (t + ZP_LEAF - 1) / ZP_LEAF;
+      leaves += (t + ZP_SQ_LEAF - 1) / ZP_SQ_LEAF;
       int64_t kf = ZP_SQ_KB;
       while (kf < t) kf <<= 1;
       sumK += kf;                                 // final precision of alpha; Newton's last step: n = kf
@@ -524,6 +528,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
               cudaStream_t st) {
   const int64_t T = r.T;
   const int Fr = r.f1 - r.f0;
+  ProfScope prof(ZP_K_NODE_SOLVE, st);  // the whole route of the run: leaf trees, up-tree, tails, leaves, division
   const CrtOut co0 = make_crt_out(k, 0), co1 = make_crt_out(k, 1), co2 = make_crt_out(k, 2);
   (void)co0;
   // task lists of every level, and the leaf offsets: one upload per array
@@ -538,7 +543,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   }
   std::vector<int64_t> leafoffs;
   for (int f = r.f0; f < r.f1; ++f)
-    for (int64_t x = h_offs[f]; x < h_offs[f + 1]; x += ZP_LEAF) leafoffs.push_back(x - r.a0);
+    for (int64_t x = h_offs[f]; x < h_offs[f + 1]; x += ZP_SQ_LEAF) leafoffs.push_back(x - r.a0);
   leafoffs.push_back(T);
   const int nleaves = (int)leafoffs.size() - 1;
   if (!tasks.empty()) cudaMemcpyAsync(w.sq_tasks, tasks.data(), sizeof(SqTask) * tasks.size(), cudaMemcpyHostToDevice, st);
@@ -548,14 +553,13 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   // (up) leaves, then one product per pair and level
   auto lev = [&](int l) { return w.sq_lev + (size_t)l * T; };
   std::vector<int64_t> xoff(r.nlev + 1, 0);  // words per prime of the levels below l in sq_Xl
-  for (int l = 0; l < r.nlev; ++l) xoff[l + 1] = xoff[l] + 2 * (int64_t)(copy0[l] - pair0[l]) * ((int64_t)2 * ZP_LEAF << l);
+  for (int l = 0; l < r.nlev; ++l) xoff[l + 1] = xoff[l] + 2 * (int64_t)(copy0[l] - pair0[l]) * ((int64_t)2 * ZP_SQ_LEAF << l);
   {
     ProfScope prof(ZP_K_MASTER_POLY, st);
-    dim3 g((unsigned)((r.tmax + ZP_LEAF - 1) / ZP_LEAF), grid_y(Fr));
-    // k_tree_leaf indexes nodes and out by absolute slots: shift both so that the run starts at its own slot 0
-    ++g_launches, k_tree_leaf<<<g, ZP_K2_THREADS, 0, st>>>(nodes - r.a0, d_offs, Fr, k, lev(0) - r.a0);
+    // the leaves as functions of at most ZP_SQ_LEAF nodes (run-local slots): one CTA builds each leaf's polynomial
+    ++g_launches, k_tree_leaf<<<dim3(1, grid_y(nleaves)), ZP_K2_THREADS, 0, st>>>(nodes, w.sq_leafoffs, nleaves, k, lev(0));
     for (int l = 0; l < r.nlev; ++l) {
-      const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
+      const int logn = ceil_log2((int64_t)2 * ZP_SQ_LEAF << l);
       const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
       const SqTask* tp = w.sq_tasks + pair0[l];
       if (P) {
@@ -572,7 +576,6 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
     }
   }
   SQ_DUMP(1, lev(r.nlev), T);
-  ProfScope prof(ZP_K_NODE_SOLVE, st);
   // root tails: rows 0 .. B-1 = the values; row B = rev(M') / rev(M) mod x^t per function
   const int V = B + 1;
   uint64_t *cur = w.sq_tailA, *nxt = w.sq_tailB;
@@ -629,7 +632,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   auto down = [&](int va, int vb, uint64_t* c, uint64_t* n2) {
     const int Vr = vb - va;
     for (int l = r.nlev - 1; l >= 0; --l) {
-      const int logn = ceil_log2((int64_t)2 * ZP_LEAF << l);
+      const int logn = ceil_log2((int64_t)2 * ZP_SQ_LEAF << l);
       const int64_t n = (int64_t)1 << logn, P = (int64_t)(copy0[l] - pair0[l]);
       const SqTask* tp = w.sq_tasks + pair0[l];
       if (P) {
@@ -676,12 +679,12 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
   SQ_DUMP(4, cur, (size_t)V * T);
   // (leaf) the synthetic-division dots of (a3) on the leaves as functions, B + 1 right-hand sides, unscaled
   {
-    dim3 gt((unsigned)((ZP_LEAF + 255) / 256), grid_y(nleaves));
+    dim3 gt((unsigned)((ZP_SQ_LEAF + 255) / 256), grid_y(nleaves));
     ++g_launches, k_solve_table<<<gt, 256, 0, st>>>(lev(0), w.sq_leafoffs, nleaves, k, w.tab, w.R);
     ++g_launches, k_fill_u64<<<sq_blocks(T), 256, 0, st>>>(w.scale, T, k.c224);  // scale = 1: plain numerators out
     const int passes = (V + ZP_NB_MAX - 1) / ZP_NB_MAX;
     const int per = (V + passes - 1) / passes;
-    dim3 g((unsigned)((ZP_LEAF + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(nleaves));
+    dim3 g((unsigned)((ZP_SQ_LEAF + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(nleaves));
     for (int b0 = 0; b0 < V; b0 += per) {
       const int nb = (V - b0 < per) ? (V - b0) : per;
       dispatch_node_solve(nb, g, st, nodes, w.tab, w.sq_leafoffs, nleaves, cur, T, b0, 0, k, w.scale, nxt, nullptr);

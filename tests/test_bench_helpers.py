@@ -34,20 +34,21 @@ def test_work_model_matches_design_md():
 
 def test_work_model_of_the_subquadratic_route():
     """bench.py subq_units counts the plan of csrc/zippel_capi.cu:sq_solve; checked here against the counts written
-    out by hand for t = 4096 (two levels above the 1024-node leaves), B = 1, and for its growth (t log^2 t)."""
+    out by hand for t = 4096 (three levels above the 512-node leaves), B = 1, and for its growth (t log^2 t)."""
     from math import log2
 
     b = load_bench()
     ntt = lambda n: 3 * (n / 2) * log2(n) * 16
     pw = lambda n: 3 * n * 36
     crt = lambda n: n * 90
-    tot, parts = b.subq_units(4096, 1)
-    up = 2 * (3 * ntt(2048) + pw(2048)) + crt(4096) + 1 * (3 * ntt(4096) + pw(4096)) + crt(4096)
+    tot, parts = b.subq_units(4096, 1)  # three levels above the 512-node leaves: (pairs, n) = (4, 1024), (2, 2048), (1, 4096)
+    levels = ((4, 1024), (2, 2048), (1, 4096))
+    up = sum(P * (3 * ntt(n) + pw(n)) + crt(4096) for P, n in levels)
     assert parts["up_tree"] == up
     V = 2
-    down = sum(V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in ((2, 2048), (1, 4096)))
+    down = sum(V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in levels)  # the siblings' transforms are kept
     assert parts["down_tree"] == down
-    assert parts["leaves"] == 4 * 1024 * 1024 * (4 + 16 + 2 * 8)
+    assert parts["leaves"] == 8 * 512 * 512 * (4 + 16 + 2 * 8)
     t19, _ = b.subq_units(1 << 19, 1)
     t20, _ = b.subq_units(1 << 20, 1)
     assert 2.0 < t20 / t19 < 2.3  # quasi-linear
