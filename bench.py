@@ -386,8 +386,8 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
             "unit": "T multiplier-pipe units/s (IMAD = 1, 32x32->64 product = 2)", "frac": achieved / peak,
             # dram__bytes_read.sum + dram__bytes_write.sum of the k_node_solve<21> launch from an ncu --set full capture of
             # the same command; algorithmic 1540 MB.  Only known for the default config; not measured in this run.
-            "traffic": 1556.6e6 if (idx == 2 and not F_override) else None,
-            "traffic_source": "ncu --set full capture of the same command (profiles/r02_final.md: k_node_solve<21> 895.6 MB read + 661.0 MB "
+            "traffic": 1555.9e6 if (idx == 2 and not F_override) else None,
+            "traffic_source": "ncu --set full capture of the same command (profiles/r02_final.md: k_node_solve<21> 895.5 MB read + 660.4 MB "
                               "written), not this run" if (idx == 2 and not F_override) else None,
             "peak_source": "derived (DESIGN.md 5.1): " + peak_how + "; profiles/r01_baseline.md measures IMAD at 63.5 and "
                            "IMAD.WIDE at 31.8 lanes/clk/SM",
