@@ -105,3 +105,20 @@ def test_two_step_chain_on_the_gpu(zp, ref):
     got = {tuple(r): int(c) for r, c in zip(zp.to_host(ne4[:t4].contiguous()).tolist(), zp.to_host(nc4[:t4]).tolist())}
     assert got == terms
     assert int(degs4.cpu().numpy()[0]) == max(k[3] for k in terms)
+
+
+@pytest.mark.parametrize("nv,ts", [(12, [700, 3, 2049, 1]),              # wide rows: the staging buffer is off
+                                   (2, [5, 4096, 1, 1, 2047, 3]),         # odd total: the scalar load path
+                                   (3, None)])                            # thousands of tiny functions per block
+def test_extend_block_boundaries_wide_rows_and_tiny_functions(zp, ref, nv, ts):
+    """The single-pass kernel's corners: functions that start at, just before and just after a 2048-term block, more
+    function starts in one block than lanes, rows too wide for the shared-memory staging, an odd number of terms (rows
+    not 16-byte aligned), sparse and dense coefficients."""
+    if ts is None:
+        r = np.random.Generator(np.random.Philox(key=[10, 977]))
+        ts = [int(x) for x in r.integers(1, 4, 6000)]
+    for dense in (False, True):
+        w = wl.make_box_workload("extb", wl.SEED_BASE + 95 + nv, len(ts), nv, ts, 80, 5, dense=dense)
+        coefs = w.planted.copy()
+        coefs[:, ::7] = 0  # vanished terms scattered over the batch
+        both(zp, ref, w, coefs)
