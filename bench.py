@@ -73,6 +73,8 @@ def parse():
     ap.add_argument("--F", type=int, default=None, help="override the number of functions (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--subq-min-t", type=int, default=None,
+                    help="override the route rule: functions with at least this many terms take the sub-quadratic route (0 = built-in rule)")
     ap.add_argument("--no-extra-legs", action="store_true",
                     help="default config only: skip the C5 and C1 legs attached to the line as \"c5\" and \"c1\"")
     return ap.parse_args()
@@ -142,14 +144,14 @@ def load_workload(idx: int, seed_shift: int, F_override):
                                 sh["emax"], sh["B"], with_planted=False)
 
 
-# the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_SQ_LEAF, ZP_SQ_KB)
-SQ_LEAF, SQ_KB = 512, 1024
+# the sub-quadratic route (csrc/subq.cuh): constants mirrored from csrc (ZP_SQ_LEAF, ZP_SQ_KB, ZP_SQ_BATCH_T)
+SQ_LEAF, SQ_KB, SQ_BATCH_T = 512, 1024, 960
 
 
 def sq_threshold(ts, B):
     """csrc/zippel_capi.cu sq_threshold: functions with at least this many terms take the sub-quadratic route."""
-    if sum(int(t) for t in ts if int(t) >= 2048) >= 65536:
-        return 2048
+    if sum(int(t) for t in ts if int(t) >= SQ_BATCH_T) >= 65536:
+        return SQ_BATCH_T
     return 2048 if B >= 16 else 4096 if B >= 6 else 8192 if B >= 2 else 12288
 C_MONT = 18  # Montgomery product: 8 wide + 2 low
 
@@ -311,7 +313,10 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
         t0 = time.perf_counter()
         e0.record(stream)
         for i in range(K):
-            api.zippel_profile_events(api.K_NODE_SOLVE | (1 << 8), ev_k[i][0], ev_k[i][1])  # 1st node solve of the step
+            # the event hook times one kind of scope per step: the node solve (quadratic route) or the whole
+            # sub-quadratic route on even steps, the leaf solve of the sub-quadratic route on odd steps
+            kind = api.K_LEAF_SOLVE if (subq and i % 2 == 1) else api.K_NODE_SOLVE
+            api.zippel_profile_events(kind | (1 << 8), ev_k[i][0], ev_k[i][1])  # 1st occurrence in the step
             step()
         e1.record(stream)
         torch.cuda.synchronize()
@@ -321,7 +326,12 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
         launches = api.zippel_launch_count() - n0
         clocks = sampler.stop(t0, t1) if sampler else None
         ms = e0.elapsed_time(e1)
-        ns_ms = sum(a.elapsed_time(b) for a, b in ev_k) / K
+        if subq and K >= 2:
+            ns_ms = sum(ev_k[i][0].elapsed_time(ev_k[i][1]) for i in range(0, K, 2)) / len(range(0, K, 2))
+            leaf_ms = sum(ev_k[i][0].elapsed_time(ev_k[i][1]) for i in range(1, K, 2)) / len(range(1, K, 2))
+        else:
+            ns_ms = sum(a.elapsed_time(b) for a, b in ev_k) / K
+            leaf_ms = None
     ms = sharding.max_over_ranks(ms, "cuda")
     ms_per_step = ms / K
     terms = B * T_tot * world
@@ -401,6 +411,25 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
     if subq:
         line["roofline"]["speedup_vs_quadratic_work"] = quad_equiv / total_ops
         line["roofline"]["quadratic_equivalent_frac"] = quad_equiv / (ms_per_step * 1e-3) / 1e12 / peak
+        if leaf_ms:
+            thr = sq_threshold(ts, B)
+            leaf_t2 = float(sum(min(SQ_LEAF, int(t) - x) ** 2 for t in ts if int(t) >= thr for x in range(0, int(t), SQ_LEAF)))
+            leaf_ops = leaf_t2 * (C_MM + (B + 1) * C_MAC)
+            leaf = {"kernel": f"k_node_solve<{B + 1 if B + 1 <= 25 else 'passes'}> on the {SQ_LEAF}-node leaves (B + 1 right-hand sides)",
+                    "ms_per_launch": leaf_ms, "algorithmic_ops_per_launch": leaf_ops, "achieved": leaf_ops / (leaf_ms * 1e-3) / 1e12,
+                    "frac": leaf_ops / (leaf_ms * 1e-3) / 1e12 / peak, "share_of_step": leaf_ms / ms_per_step}
+            if leaf["share_of_step"] >= 0.5:
+                # one kernel holds most of the step: it is the dominant kernel, the route-level figures move aside
+                r = line["roofline"]
+                r["route"] = {"kernel": r["kernel"], "achieved": r["achieved"], "frac": r["frac"], "ms": r["ms_per_launch"],
+                              "algorithmic_ops": r["algorithmic_ops_per_launch"], "algorithmic_cost": r["algorithmic_cost"]}
+                r.update(kernel=leaf["kernel"], achieved=leaf["achieved"], frac=leaf["frac"], ms_per_launch=leaf_ms,
+                         algorithmic_ops_per_launch=leaf_ops, share_of_step=leaf["share_of_step"],
+                         algorithmic_cost="modular multiply-add = 16 units, deferred 64x64 MAC = 8 units; per (node, stage) of a leaf 16 + 8 (B + 1)")
+                if idx == 2 and not F_override:
+                    r["traffic"], r["traffic_source"] = None, None
+            else:
+                line["roofline"]["leaf_solve"] = leaf
     else:
         line["roofline"]["frac_instr_count_10_4"] = ns_ops_instr / (ns_ms * 1e-3) / 1e12 / peak
     return line
@@ -421,6 +450,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
     api.lib()
+    if args.subq_min_t is not None:
+        api.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, args.subq_min_t)
     idx = args.config
     line = run_leg(idx, args.steps, args.warmup, args.F, not args.no_e2e, rank, world, local)
     # the default line carries the other half of north_star's target (the t = 2^19 solve, configs[4]) and the latency

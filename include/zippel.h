@@ -198,6 +198,7 @@ int crt_rational_reconstruct_batch(const uint64_t* r1, const uint64_t* r2, int64
 #define ZP_K_NEWTON 5
 #define ZP_K_POWER_SUMS 6
 #define ZP_K_BALANCE 7
+#define ZP_K_LEAF_SOLVE 8 /* sub-quadratic route: k_node_solve on the leaves (B + 1 right-hand sides) */
 int zippel_profile_events(int kernel, void* ev_start, void* ev_stop);
 /* Number of kernels this library has enqueued in this process so far (bench.py's gpu_launches). */
 unsigned long long zippel_launch_count(void);
@@ -206,8 +207,10 @@ unsigned long long zippel_launch_count(void);
  *   ZP_TUNE_SUBQ_MIN_T: functions with at least this many terms (and more than 1024) take the sub-quadratic route
  *   (three-prime NTT product tree, tails, leaf solves: csrc/subq.cuh) instead of the quadratic
  *   kernels of PAPER.md section 2.2.  Same results bit for bit.  Default 0 = the measured rule:
- *   2048 terms when the batch holds at least 65536 terms in such functions, else 2048 / 4096 / 8192 / 12288 terms for
- *   B >= 16 / >= 6 / >= 2 / = 1 right-hand sides (a single function is bound by the latency of the route's launches). */
+ *   960 terms when the batch holds at least 65536 terms in such functions, else 2048 / 4096 / 8192 / 12288 terms for
+ *   B >= 16 / >= 6 / >= 2 / = 1 right-hand sides (a single function is bound by the latency of the route's launches).
+ *   The route needs more workspace (zippel_workspace_bytes accounts for it: about 1 KB per term and right-hand side
+ *   group for the kept transforms and the tails; BASELINE.json configs[1] takes 4 GB instead of 0.3 GB). */
 #define ZP_TUNE_SUBQ_MIN_T 1
 int zippel_set_tuning(int key, int64_t value);
 

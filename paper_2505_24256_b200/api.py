@@ -34,7 +34,7 @@ EXPORTS = (
 )
 TUNE_SUBQ_MIN_T = 1
 SUBQ_MIN_T_DEFAULT = 0  # g_subq_min_t in csrc/zippel_capi.cu: 0 = the built-in rule (sq_threshold)
-K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE = 1, 2, 3, 5, 6, 7
+K_EVAL_NODES, K_MASTER_POLY, K_NODE_SOLVE, K_NEWTON, K_POWER_SUMS, K_BALANCE, K_LEAF_SOLVE = 1, 2, 3, 5, 6, 7, 8
 
 
 class ZippelError(RuntimeError):

@@ -123,24 +123,26 @@ struct SqSizes {
   int64_t thr = 0;  // the threshold the runs were found with (sq_threshold on the whole batch)
 };
 // Which functions take the sub-quadratic route: those with at least sq_threshold terms.  Measured on B200 (profiles/
-// r02_crossover.md): a batch with enough long functions to fill the GPU crosses over at t = 2048 for every B; a single
-// function (or a few) is bound by the latency of the route's ~150 dependent launches and crosses over later, the later
-// the fewer right-hand sides there are to amortise them (B = 1: 12288, B = 3: 8192, B = 9: 4096, B = 21: 2048).
+// r02_crossover.md): a batch with enough functions to fill the GPU crosses over between t = 800 and t = 1000 for every B
+// (one tree level above two leaves already halves the t^2 work of the leaves); a single function (or a few) is bound by
+// the latency of the route's ~150 dependent launches and crosses over later, the later the fewer right-hand sides
+// there are to amortise them (B = 1: 12288, B = 3: 8192, B = 9: 4096, B = 21: 2048).
+#define ZP_SQ_BATCH_T 960
 int64_t sq_threshold(const int64_t* h_offs, int F, int B) {
   if (g_subq_min_t > 0) return g_subq_min_t;
   int64_t sum = 0;
   for (int f = 0; f < F; ++f) {
     const int64_t t = h_offs[f + 1] - h_offs[f];
-    if (t >= 2048) sum += t;
+    if (t >= ZP_SQ_BATCH_T) sum += t;
   }
-  if (sum >= 65536) return 2048;
+  if (sum >= 65536) return ZP_SQ_BATCH_T;
   return B >= 16 ? 2048 : B >= 6 ? 4096 : B >= 2 ? 8192 : 12288;
 }
 // leaves of the sub-quadratic route: blocks of at most this many nodes are solved by the quadratic kernels (at most ZP_LEAF)
 #ifndef ZP_SQ_LEAF
 #define ZP_SQ_LEAF 512
 #endif
-inline bool sq_is_long(int64_t t, int64_t thr) { return t >= thr && t > ZP_LEAF; }
+inline bool sq_is_long(int64_t t, int64_t thr) { return t >= thr && t > ZP_SQ_LEAF; }
 
 // pair and copy tasks of level l (children of size a = LEAF << l) for a run; slots relative to the run
 void sq_level_tasks(const int64_t* h_offs, const SqRun& r, int l, std::vector<SqTask>* pairs, std::vector<SqTask>* copies) {
@@ -685,6 +687,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
     const int passes = (V + ZP_NB_MAX - 1) / ZP_NB_MAX;
     const int per = (V + passes - 1) / passes;
     dim3 g((unsigned)((ZP_SQ_LEAF + ZP_K3_THREADS - 1) / ZP_K3_THREADS), grid_y(nleaves));
+    ProfScope prof_leaf(ZP_K_LEAF_SOLVE, st);
     for (int b0 = 0; b0 < V; b0 += per) {
       const int nb = (V - b0 < per) ? (V - b0) : per;
       dispatch_node_solve(nb, g, st, nodes, w.tab, w.sq_leafoffs, nleaves, cur, T, b0, 0, k, w.scale, nxt, nullptr);
@@ -1217,7 +1220,7 @@ int crt_rational_reconstruct_batch(const uint64_t* r1, const uint64_t* r2, int64
 unsigned long long zippel_launch_count(void) { return g_launches; }
 
 int zippel_profile_events(int kernel, void* ev_start, void* ev_stop) {
-  if (kernel < 0 || (kernel & 0xff) > 7 || (kernel != 0 && (!ev_start || !ev_stop))) return ZP_ERR_ARG;
+  if (kernel < 0 || (kernel & 0xff) > 8 || (kernel != 0 && (!ev_start || !ev_stop))) return ZP_ERR_ARG;
   g_prof_ordinal = (kernel >> 8) - 1;  // bits 8.. : 0 = every occurrence, n = only the n-th (1-based) after this call
   g_prof_seen = 0;
   kernel &= 0xff;

@@ -18,10 +18,14 @@ def load_bench():
 
 def test_work_model_matches_design_md():
     b = load_bench()
-    ts = [1000] * 4096
+    ts = [900] * 4096  # below the batch threshold of the sub-quadratic route: the quadratic kernels
     total, ns = b.work_model(ts, 21, 4, True, False)
-    assert ns == 4096 * 1000 * 1000 * (16 + 8 * 22)  # one multiply-add + (B + 1) MACs per (node, stage)
+    assert ns == 4096 * 900 * 900 * (16 + 8 * 22)  # one multiply-add + (B + 1) MACs per (node, stage)
     assert total > ns and (total - ns) / ns < 0.05  # tree, Newton, nodes: a few per cent
+    # BASELINE.json configs[1] (t = 1000, 4096 functions) is above it: two 512-node leaves and one tree level per function
+    tot2, ns2 = b.work_model([1000] * 4096, 21, 4, True, False)
+    assert b.sq_threshold([1000] * 4096, 21) == 960 and b.sq_threshold([1000] * 60, 21) == 2048
+    assert ns2 == 4096 * b.subq_units(1000, 21)[0] and ns2 < 0.75 * 4096 * 1000 * 1000 * (16 + 8 * 22)
     _, ns5 = b.work_model([4096], 1, 10, False, False)
     assert ns5 == (1 << 24) * 20  # B = 1 route below the sub-quadratic threshold: two evaluations by MACs + the correlation
     _, ns_small = b.work_model([1000], 1, 10, False, False)

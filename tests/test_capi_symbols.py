@@ -69,7 +69,9 @@ def test_long_skeleton_workspace_and_limits():
     many = np.arange(33, dtype=np.int64) * 5000
     assert not grows(one, 1) and not grows(one, 5) and grows(one, 9) and grows(one, 21)
     assert grows(many, 1) and grows(many, 21)
-    assert not grows(np.arange(4097, dtype=np.int64) * 1000, 21)  # configs[1]: t = 1000 stays on the quadratic kernels
+    assert grows(np.arange(4097, dtype=np.int64) * 1000, 21)      # configs[1]: 4096 functions of t = 1000 take the route,
+    assert not grows(np.arange(4097, dtype=np.int64) * 900, 21)    # functions of 900 terms do not,
+    assert not grows(np.arange(61, dtype=np.int64) * 1000, 21)     # and neither do 60 functions of 1000 (too few to fill the GPU)
     big = np.array([0, 1 << 23], dtype=np.int64)
     assert L.zippel_workspace_bytes(big.ctypes.data, 1, 1, 0) == 0
     ok = np.array([0, (1 << 23) - 1], dtype=np.int64)
