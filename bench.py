@@ -427,7 +427,11 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
                          algorithmic_ops_per_launch=leaf_ops, share_of_step=leaf["share_of_step"],
                          algorithmic_cost="modular multiply-add = 16 units, deferred 64x64 MAC = 8 units; per (node, stage) of a leaf 16 + 8 (B + 1)")
                 if idx == 2 and not F_override:
-                    r["traffic"], r["traffic_source"] = None, None
+                    # DRAM bytes of this launch from the ncu --set full capture of the same command; algorithmic: the B + 1
+                    # tails read and the B + 1 numerator rows written once, 8 (B + 1) T_tot bytes each way (1442 MB)
+                    r["traffic"] = 1613.6e6
+                    r["traffic_source"] = ("ncu --set full capture of the same command (profiles/r02_final.md: k_node_solve<22> "
+                                           "923.3 MB read + 690.2 MB written), not this run")
             else:
                 line["roofline"]["leaf_solve"] = leaf
     else:

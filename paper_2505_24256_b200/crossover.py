@@ -2,7 +2,7 @@
 
     python -m paper_2505_24256_b200.crossover [--out crossover.json]
 
-For F in {1, 64} functions of t terms and B right-hand sides, vandermonde_solve_batch is timed (CUDA events on the
+For F in {1, 64, 4096} functions of t terms and B right-hand sides, vandermonde_solve_batch is timed (CUDA events on the
 launching stream, 3 warm-ups, 10 repetitions) with the route forced either way through zippel_set_tuning, and the
 two results are compared for equality.  The built-in rule (sq_threshold in csrc/zippel_capi.cu, include/zippel.h)
 was read off this table (profiles/r02_crossover.md).
@@ -20,7 +20,7 @@ from . import api, workloads as wl
 
 def run(t, B, F, route, reps=10):
     P = wl.P63
-    api.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 1025 if route == "subq" else (1 << 22))
+    api.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, 513 if route == "subq" else (1 << 22))
     r = np.random.Generator(np.random.Philox(key=[5, t]))
     offs = np.arange(F + 1, dtype=np.int64) * t
     nodes = np.empty(F * t, dtype=np.uint64)
@@ -52,17 +52,18 @@ def main():
     api.lib()
     res = []
     try:
-        for F in (1, 64):
-            for B in (1, 3, 9, 21):
-                for t in (1536, 2048, 3072, 4096, 6144, 8192, 12288, 16384, 32768):
-                    if F * t * B > 1 << 26:
-                        continue
-                    q_ms, oq = run(t, B, F, "quad")
-                    s_ms, os_ = run(t, B, F, "subq")
-                    same = bool((oq == os_).all())
-                    res.append(dict(F=F, B=B, t=t, quad_ms=q_ms, subq_ms=s_ms, same=same))
-                    print(f"F={F} B={B} t={t} quadratic {q_ms:.3f} ms sub-quadratic {s_ms:.3f} ms {'same' if same else 'DIFFERENT'}",
-                          flush=True)
+        cases = [(F, B, t) for F in (1, 64) for B in (1, 3, 9, 21)
+                 for t in (1536, 2048, 3072, 4096, 6144, 8192, 12288, 16384, 32768) if F * t * B <= 1 << 26]
+        # many short functions (BASELINE.json configs[1] is 4096 functions of 1000 terms): the batch threshold
+        cases += [(4096, B, t) for B in (1, 21) for t in (640, 800, 960, 1000, 1280, 1536)]
+        for F, B, t in cases:
+            reps = 10 if F < 4096 else 3
+            q_ms, oq = run(t, B, F, "quad", reps)
+            s_ms, os_ = run(t, B, F, "subq", reps)
+            same = bool((oq == os_).all())
+            res.append(dict(F=F, B=B, t=t, quad_ms=q_ms, subq_ms=s_ms, same=same))
+            print(f"F={F} B={B} t={t} quadratic {q_ms:.3f} ms sub-quadratic {s_ms:.3f} ms {'same' if same else 'DIFFERENT'}",
+                  flush=True)
     finally:
         api.zippel_set_tuning(api.TUNE_SUBQ_MIN_T, api.SUBQ_MIN_T_DEFAULT)
     if a.out:
