@@ -101,11 +101,11 @@ ZP_DEV int ntt_gbase(int gidx, int sh) { return ((gidx >> sh) << (sh + 3)) | (gi
 // the twiddles of the (up to three) stages of the field at bit sh for the group whose first word is eb: slot 4 >> bb ..
 // of stage bb holds its 4 >> bb entries (w[1]: stage 2; w[2..3]: stage 1; w[4..7]: stage 0); stages outside [lo, hi] load
 // nothing.  Issued before the words of the group are read, so that the two latencies overlap.
-ZP_DEV void ntt_group_twiddles(ulonglong2 (&w)[8], int eb, int sh, int hi, int lo, const ulonglong2* __restrict__ tab) {
+ZP_DEV void ntt_group_twiddles(ulonglong2 (&w)[8], int eb, int sh, int hi, int bmax, int lo, const ulonglong2* __restrict__ tab) {
 #pragma unroll
   for (int bb = 2; bb >= 0; --bb) {
     const int b = sh + bb;
-    if (b > hi || b < lo) continue;  // uniform
+    if (b > bmax || b < lo) continue;  // uniform
     const int ls = hi - b, mask = (1 << ls) - 1;
     const int ihi = (eb >> (sh + 3)) << (2 - bb);  // the block bits above the field; j's bits above bb fill the rest
 #pragma unroll
@@ -113,12 +113,12 @@ ZP_DEV void ntt_group_twiddles(ulonglong2 (&w)[8], int eb, int sh, int hi, int l
   }
 }
 // the forward stages of one field on one group (values in [0, 4q), Harvey butterflies)
-ZP_DEV void ntt_group_fwd(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int hi, int lo, const ZpMod& q) {
+ZP_DEV void ntt_group_fwd(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int bmax, int lo, const ZpMod& q) {
   const uint64_t q2 = 2 * q.p;
 #pragma unroll
   for (int bb = 2; bb >= 0; --bb) {
     const int b = sh + bb;
-    if (b > hi || b < lo) continue;  // uniform
+    if (b > bmax || b < lo) continue;  // uniform
 #pragma unroll
     for (int j0 = 0; j0 < 8; ++j0) {
       if (j0 >> bb & 1) continue;
@@ -132,12 +132,12 @@ ZP_DEV void ntt_group_fwd(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, in
   }
 }
 // inverse: values in [0, 2q), Gentleman-Sande butterflies with the inverse twiddles
-ZP_DEV void ntt_group_inv(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int hi, int lo, const ZpMod& q) {
+ZP_DEV void ntt_group_inv(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, int bmax, int lo, const ZpMod& q) {
   const uint64_t q2 = 2 * q.p;
 #pragma unroll
   for (int bb = 0; bb < 3; ++bb) {
     const int b = sh + bb;
-    if (b > hi || b < lo) continue;  // uniform
+    if (b > bmax || b < lo) continue;  // uniform
 #pragma unroll
     for (int j0 = 0; j0 < 8; ++j0) {
       if (j0 >> bb & 1) continue;
@@ -149,23 +149,76 @@ ZP_DEV void ntt_group_inv(uint64_t (&x)[8], const ulonglong2 (&w)[8], int sh, in
     }
   }
 }
-// all the stages of [lo, hi] on the tile in shared memory (the tile is complete and visible on entry and on exit)
+// The stages on the top three bits 11 .. 9 of the tile index run in the registers of the lane that loads (forward) or
+// stores (inverse) the words: lane T moves the words e = T + TH m, so with TH <= 512 those bits are bits of m, the pairs
+// of such a stage are pairs of the lane's own words, and the twiddle depends on m only (the same for every lane).  A
+// lane takes its words eight at a time (those that differ in the bits 11 .. 9 only: e = T + TH h + 512 mm, mm = 0 .. 7,
+// h < 512 / TH).  One round trip through shared memory and one barrier less per tile transform than four rounds there.
+#define ZP_NTT_TOPBIT 9
+template <int TH>
+ZP_DEV int ntt_top_word(int h, int mm) { return threadIdx.x + TH * h + 512 * mm; }
+ZP_DEV void ntt_top_fwd(uint64_t (&x)[8], int hi, int lo, const ulonglong2* __restrict__ U, const ZpMod& q) {
+  const uint64_t q2 = 2 * q.p;
+#pragma unroll
+  for (int bb = 2; bb >= 0; --bb) {
+    const int b = ZP_NTT_TOPBIT + bb;
+    if (b > hi || b < lo) continue;  // uniform
+    const int ls = hi - b, mask = (1 << ls) - 1;
+#pragma unroll
+    for (int k = 0; k < (4 >> bb); ++k) {  // the blocks of this stage among the lane's words
+      const ulonglong2 w = __ldg(U + (1 << ls) + (k & mask));
+#pragma unroll
+      for (int jl = 0; jl < (1 << bb); ++jl) {
+        const int m0 = (k << (bb + 1)) | jl, m1 = m0 | (1 << bb);
+        uint64_t u = x[m0];
+        u = (u >= q2) ? u - q2 : u;
+        const uint64_t v = ntt_mul(x[m1], w, q);
+        x[m0] = u + v;
+        x[m1] = u - v + q2;
+      }
+    }
+  }
+}
+ZP_DEV void ntt_top_inv(uint64_t (&x)[8], int hi, int lo, const ulonglong2* __restrict__ Ui, const ZpMod& q) {
+  const uint64_t q2 = 2 * q.p;
+#pragma unroll
+  for (int bb = 0; bb < 3; ++bb) {
+    const int b = ZP_NTT_TOPBIT + bb;
+    if (b > hi || b < lo) continue;  // uniform
+    const int ls = hi - b, mask = (1 << ls) - 1;
+#pragma unroll
+    for (int k = 0; k < (4 >> bb); ++k) {
+      const ulonglong2 w = __ldg(Ui + (1 << ls) + (k & mask));
+#pragma unroll
+      for (int jl = 0; jl < (1 << bb); ++jl) {
+        const int m0 = (k << (bb + 1)) | jl, m1 = m0 | (1 << bb);
+        const uint64_t u = x[m0], v = x[m1];
+        const uint64_t sum = u + v;
+        x[m0] = (sum >= q2) ? sum - q2 : sum;
+        x[m1] = ntt_mul(u - v + q2, w, q);
+      }
+    }
+  }
+}
+// the stages of [lo, hi] BELOW bit 9 on the tile in shared memory, three per round (the tile is complete and
+// visible on entry and on exit); hi is still the pass's top bit: it fixes the twiddle level of every stage
 template <bool INV, int TH>
 ZP_DEV void ntt_tile(uint64_t* sm, int hi, int lo, const ulonglong2* __restrict__ tab, const ZpMod& q) {
+  const int bmax = hi < ZP_NTT_TOPBIT - 1 ? hi : ZP_NTT_TOPBIT - 1;
 #pragma unroll 1
-  for (int r = 0; r < 4; ++r) {
-    const int f = INV ? r : 3 - r, sh = 3 * f;
-    if (sh > hi || sh + 2 < lo) continue;  // no stage in this field
+  for (int r = 0; r < 3; ++r) {
+    const int f = INV ? r : 2 - r, sh = 3 * f;
+    if (sh > bmax || sh + 2 < lo) continue;  // no stage in this field
 #pragma unroll 1
     for (int g = 0; g < ZP_NTT_C / 8 / TH; ++g) {
       const int eb = ntt_gbase(threadIdx.x + TH * g, sh);
       ulonglong2 w[8];
-      ntt_group_twiddles(w, eb, sh, hi, lo, tab);
+      ntt_group_twiddles(w, eb, sh, hi, bmax, lo, tab);
       uint64_t x[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) x[j] = sm[ntt_pad(eb + (j << sh))];
-      if (INV) ntt_group_inv(x, w, sh, hi, lo, q);
-      else ntt_group_fwd(x, w, sh, hi, lo, q);
+      if (INV) ntt_group_inv(x, w, sh, bmax, lo, q);
+      else ntt_group_fwd(x, w, sh, bmax, lo, q);
 #pragma unroll
       for (int j = 0; j < 8; ++j) sm[ntt_pad(eb + (j << sh))] = x[j];
     }
@@ -210,34 +263,64 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
   }
   const int G1 = (1 << logG) - 1;
   const int ln1 = (1 << logn) - 1;
-#pragma unroll 4
-  for (int m = 0; m < ZP_NTT_C / TH; ++m) {
-    const int e = T + TH * m;
-    const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
-    uint64_t v = 0;
-    if (off < E) {
-      v = g[off];
-      if (!INV && logRp) {
-        const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
-        v = ntt_twist<false>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
-      }
-    }
-    sm[ntt_pad(e)] = v;
-  }
-  __syncthreads();
   const int hi = logR ? 11 : logn - 1, lo = logR ? 12 - logR : 0;
-  ntt_tile<INV, TH>(sm, hi, lo, INV ? cx.Ui[jp] : cx.U[jp], q);
-#pragma unroll 4
-  for (int m = 0; m < ZP_NTT_C / TH; ++m) {
-    const int e = T + TH * m;
-    const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
-    if (off < E) {
-      uint64_t v = sm[ntt_pad(e)];
-      if (INV && logRp) {
-        const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
-        v = ntt_twist<true>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
+  uint64_t x[8];
+  if (!INV) {
+#pragma unroll 1
+    for (int h = 0; h < 512 / TH; ++h) {
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) {
+        const int e = ntt_top_word<TH>(h, mm);
+        const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+        uint64_t v = 0;
+        if (off < E) {
+          v = g[off];
+          if (logRp) {
+            const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
+            v = ntt_twist<false>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
+          }
+        }
+        x[mm] = v;
       }
-      g[off] = v;
+      ntt_top_fwd(x, hi, lo, cx.U[jp], q);
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) sm[ntt_pad(ntt_top_word<TH>(h, mm))] = x[mm];
+    }
+    __syncthreads();
+    ntt_tile<false, TH>(sm, hi, lo, cx.U[jp], q);
+#pragma unroll 4
+    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+      const int e = T + TH * m;
+      const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+      if (off < E) g[off] = sm[ntt_pad(e)];
+    }
+  } else {
+#pragma unroll 4
+    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
+      const int e = T + TH * m;
+      const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+      sm[ntt_pad(e)] = (off < E) ? g[off] : 0;
+    }
+    __syncthreads();
+    ntt_tile<true, TH>(sm, hi, lo, cx.Ui[jp], q);
+#pragma unroll 1
+    for (int h = 0; h < 512 / TH; ++h) {
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) x[mm] = sm[ntt_pad(ntt_top_word<TH>(h, mm))];
+      ntt_top_inv(x, hi, lo, cx.Ui[jp], q);
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) {
+        const int e = ntt_top_word<TH>(h, mm);
+        const int64_t off = base + ((int64_t)(e >> logG) << rowshift) + (e & G1);
+        if (off < E) {
+          uint64_t v = x[mm];
+          if (logRp) {
+            const uint32_t c = (uint32_t)((off >> logn) & ((1 << logRp) - 1)), pos = (uint32_t)(off & ln1);
+            v = ntt_twist<true>(v, (brev_bits(c, logRp) * pos) << (ZP_NTT_LOGMAX - lpar), cx.Tlo[jp], cx.Thi[jp], q);
+          }
+          g[off] = v;
+        }
+      }
     }
   }
 }
@@ -285,20 +368,27 @@ k_ntt_mul(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t
   // the first (and in MODE 0 the second) operand's chunk -> forward stages; the first one's transform is parked in smA
 #pragma unroll 1
   for (int which = 0; which < (MODE == 0 ? 2 : 1); ++which) {
-#pragma unroll 4
-    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
-      const int e = T + TH * m;
-      uint64_t v = 0;
-      if (c0 + e < Edrv) {
-        if (MODE == 0) {
-          const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
-          v = A[((int64_t)(2 * seg + which) << logseg) | pos];
-        } else {
-          v = A[c0 + e];
+#pragma unroll 1
+    for (int h = 0; h < 512 / TH; ++h) {
+      uint64_t x[8];
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) {
+        const int e = ntt_top_word<TH>(h, mm);
+        uint64_t v = 0;
+        if (c0 + e < Edrv) {
+          if (MODE == 0) {
+            const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+            v = A[((int64_t)(2 * seg + which) << logseg) | pos];
+          } else {
+            v = A[c0 + e];
+          }
+          if (logRp) v = ntt_twist<false>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
         }
-        if (logRp) v = ntt_twist<false>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
+        x[mm] = v;
       }
-      sm[ntt_pad(e)] = v;
+      ntt_top_fwd(x, logn - 1, 0, cx.U[jp], q);  // the stages on the bits 11 .. 9, in registers
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) sm[ntt_pad(ntt_top_word<TH>(h, mm))] = x[mm];
     }
     __syncthreads();
     ntt_tile<false, TH>(sm, logn - 1, 0, cx.U[jp], q);
@@ -343,17 +433,24 @@ k_ntt_mul(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t
     }
     __syncthreads();
     ntt_tile<true, TH>(sm, logn - 1, 0, cx.Ui[jp], q);
-#pragma unroll 4
-    for (int m = 0; m < ZP_NTT_C / TH; ++m) {
-      const int e = T + TH * m;
-      if (c0 + e >= Edrv) continue;
-      uint64_t v = sm[ntt_pad(e)];
-      if (logRp) v = ntt_twist<true>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
-      if (MODE == 0) {
-        O[c0 + e] = v;
-      } else {
-        const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
-        O[((int64_t)(2 * seg + side) << logseg) | pos] = v;
+#pragma unroll 1
+    for (int h = 0; h < 512 / TH; ++h) {
+      uint64_t x[8];
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) x[mm] = sm[ntt_pad(ntt_top_word<TH>(h, mm))];
+      ntt_top_inv(x, logn - 1, 0, cx.Ui[jp], q);
+#pragma unroll
+      for (int mm = 0; mm < 8; ++mm) {
+        const int e = ntt_top_word<TH>(h, mm);
+        if (c0 + e >= Edrv) continue;
+        uint64_t v = x[mm];
+        if (logRp) v = ntt_twist<true>(v, (bc * (uint32_t)e) << tsh, Tlo, Thi, q);
+        if (MODE == 0) {
+          O[c0 + e] = v;
+        } else {
+          const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
+          O[((int64_t)(2 * seg + side) << logseg) | pos] = v;
+        }
       }
     }
     __syncthreads();  // MODE 1: the tile is reused by the other side
