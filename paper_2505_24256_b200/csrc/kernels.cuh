@@ -370,6 +370,60 @@ ZP_DEV uint32_t warp_batch_inv(uint64_t (&x)[N], const ZpMod& k) {
   return zero;
 }
 
+// The same over a whole CTA (blockDim.x a multiple of 32, sh = 64 words of shared memory): the warps' totals meet in
+// shared memory and warp 0 runs the one inversion for all of them -- the inversion is ~3000 instructions, as many as a
+// warp spends on streaming ~60 products, so it pays to share it wider where the CTA can wait for it.  Two barriers;
+// every lane of the CTA must call.
+template <int N>
+ZP_DEV uint32_t cta_batch_inv(uint64_t (&x)[N], const ZpMod& k, uint64_t* sh) {
+  uint64_t pre[N];
+  uint64_t run = k.r1;
+  uint32_t zero = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    pre[i] = run;
+    if (x[i] == 0) zero |= 1u << i;
+    else run = mont_mul(run, x[i], k);
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint64_t below = run, above = run;  // products over the lanes <= this one / >= this one
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint64_t a = mont_mul(below, shfl_up64(below, o), k), b = mont_mul(above, shfl_down64(above, o), k);
+    below = (lane >= o) ? a : below;
+    above = (lane + o < 32) ? b : above;
+  }
+  if (lane == 31) sh[warp] = below;  // the warp's total
+  __syncthreads();
+  if (warp == 0) {
+    uint64_t tb = lane < nw ? sh[lane] : k.r1, ta = tb;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint64_t a = mont_mul(tb, shfl_up64(tb, o), k), b = mont_mul(ta, shfl_down64(ta, o), k);
+      tb = (lane >= o) ? a : tb;
+      ta = (lane + o < 32) ? b : ta;
+    }
+    uint64_t winv = mont_inv_uniform(shfl_idx64(tb, 31), k);  // 1 / (product of the whole CTA)
+    const uint64_t lo = shfl_up64(tb, 1), hi = shfl_down64(ta, 1);
+    if (lane > 0) winv = mont_mul(winv, lo, k);
+    if (lane < 31) winv = mont_mul(winv, hi, k);
+    if (lane < nw) sh[32 + lane] = winv;  // 1 / (total of warp `lane`)
+  }
+  __syncthreads();
+  uint64_t inv = sh[32 + warp];
+  const uint64_t lo = shfl_up64(below, 1), hi = shfl_down64(above, 1);
+  if (lane > 0) inv = mont_mul(inv, lo, k);
+  if (lane < 31) inv = mont_mul(inv, hi, k);
+#pragma unroll
+  for (int i = N - 1; i >= 0; --i) {
+    if (zero >> i & 1) continue;
+    const uint64_t xi = x[i];
+    x[i] = mont_mul(inv, pre[i], k);
+    inv = mont_mul(inv, xi, k);
+  }
+  return zero;
+}
+
 // The division that ends every solve: for the slots i of the functions behind `offs` (all pointers at the batch's slot
 // 0, the functions cover the slots [a0, a0 + T)),  d_i = den_i [m_i if s0 = 1]  (den plain) and
 //   APPLY = false:  scale_i = 2^224 / d_i  (plain; the factor k_node_solve multiplies its reduced sums by), in place or not
@@ -783,28 +837,36 @@ __global__ void k_status_finish(const int32_t* pre, const int32_t* solve, const 
 // ------------------------------------------------------------------------------------------------
 // (a6) K6 power sums R_{b,s} = sum_i a_{b,i} m_i^(s+s0)  ("raise base variable
 // values to various powers and substitute them into the polynomial"; strided power tables, A21).
-// CTA = (function f, block of 256 consecutive s); node tiles of 128 in shared memory with the strided power
-// tables  P_i[x] = a_i m_i^(sb0+s0) m_i^x,  H_i[x] = m_i^(16x)   (x < 16):  lane s adds P_i[s & 15] * H_i[s >> 4],
-// a deferred sum over i with no modular product in the inner loop.
+// CTA = (function f, block of 512 consecutive s); node tiles of 64 in shared memory with the strided power
+// tables  P_i[x] = a_i m_i^(sb0+s0) m_i^x (x < 16),  H_i[x] = m_i^(16x) (x < 32):  a_i m_i^(s+s0) = P_i[s & 15] * H_i[s >> 4]
+// for s = sb0 + 16 s2 + s1, a deferred sum over i with no modular product in the inner loop (PAPER.md L205-209,
+// L219-225).  A lane owns a 2 x 2 block of (s1, s2): two 16-byte reads of shared memory serve four multiply-adds
+// (one 8-byte read each would make shared memory, not the multiplier, the limit: two wavefronts per multiply-add).
+// Where the block holds fewer than 512 wanted s (short functions) the lanes left over split the nodes of a tile among
+// groups instead (group g takes the nodes x = g mod ng) and the groups' residues are added at the end.
 // ------------------------------------------------------------------------------------------------
-#define ZP_K6_THREADS 256
-#define ZP_K6_NODES 128
+#define ZP_K6_THREADS 128
+#define ZP_K6_NODES 64
+#define ZP_K6_SBLOCK 512
 __global__ void __launch_bounds__(ZP_K6_THREADS)
 k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ offsets, int F,
              const uint64_t* __restrict__ coef, int64_t T_tot, int B, int s0, ZpMod k, uint64_t* __restrict__ out) {
-  // lane s = sb0 + 16 s2 + s1:  a_i m_i^(s+s0) = [a_i m_i^(sb0+s0) m_i^s1] * [(m_i^16)^s2] = P_i[s1] * H_i[s2],
-  // so with the two 16-entry tables of a node in shared memory the inner loop is one deferred MAC per (s, i)
-  __shared__ uint64_t sP[ZP_K6_NODES * 16];  // Montgomery
-  __shared__ uint64_t sH[ZP_K6_NODES * 16];  // plain
+  __shared__ ulonglong2 sP[ZP_K6_NODES * 8];   // Montgomery: {P_i[2a], P_i[2a+1]} at [i * 8 + a]
+  __shared__ ulonglong2 sH[ZP_K6_NODES * 16];  // plain: {H_i[2c], H_i[2c+1]} at [i * 16 + c]
+  const int a = threadIdx.x & 7;
   for (int f = blockIdx.y; f < F; f += gridDim.y) {
     const int64_t off = offsets[f];
     const int t = (int)(offsets[f + 1] - off);
-    const int sb0 = blockIdx.x * ZP_K6_THREADS;
+    const int sb0 = blockIdx.x * ZP_K6_SBLOCK;
     if (sb0 >= t) continue;
-    const int s = sb0 + threadIdx.x;
+    int cr = 1;  // 32 cr >= the wanted s of this block, a power of two <= 16; ng = 16 / cr groups share the nodes
+    while (32 * cr < t - sb0 && cr < 16) cr <<= 1;
+    const int ng = 16 / cr, c = (threadIdx.x >> 3) & (cr - 1), grp = (threadIdx.x >> 3) / cr;
+    const int ls = 32 * c + 2 * a, s = sb0 + ls;  // this lane: s, s + 1, s + 16, s + 17
     for (int b = 0; b < B; ++b) {
-      Acc acc;
-      acc_zero(acc);
+      Acc acc[4];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) acc_zero(acc[x]);
       for (int i0 = 0; i0 < t; i0 += ZP_K6_NODES) {
         const int n = t - i0 < ZP_K6_NODES ? t - i0 : ZP_K6_NODES;
         __syncthreads();
@@ -812,56 +874,90 @@ k_power_sums(const uint64_t* __restrict__ nodes, const int64_t* __restrict__ off
           const int x = threadIdx.x >> 1, which = threadIdx.x & 1;
           if (x < n) {
             const uint64_t m = to_mont(zp_canon(nodes[off + i0 + x], k.p), k);
+            uint64_t* dst;
+            uint64_t pw, step;
+            int cnt;
             if (which == 0) {
-              const uint64_t a = to_mont(zp_canon(coef[(int64_t)b * T_tot + off + i0 + x], k.p), k);
-              uint64_t pw = mont_mul(a, mont_pow(m, (uint64_t)(sb0 + s0), k), k);
-              for (int e = 0; e < 16; ++e) {
-                sP[x * 16 + e] = pw;
-                pw = mont_mul(pw, m, k);
-              }
+              const uint64_t av = to_mont(zp_canon(coef[(int64_t)b * T_tot + off + i0 + x], k.p), k);
+              const int e0 = sb0 + s0;
+              pw = e0 == 0 ? av : e0 == 1 ? mont_mul(av, m, k) : mont_mul(av, mont_pow(m, (uint64_t)e0, k), k);
+              step = m;
+              dst = reinterpret_cast<uint64_t*>(sP + x * 8);
+              cnt = 16;
             } else {
-              uint64_t m16 = m;
-              for (int e = 0; e < 4; ++e) m16 = mont_mul(m16, m16, k);
-              uint64_t pw = 1 % k.p;  // plain; plain * Montgomery -> plain
-              for (int e = 0; e < 16; ++e) {
-                sH[x * 16 + e] = pw;
-                pw = mont_mul(pw, m16, k);
-              }
+              step = m;
+              for (int e = 0; e < 4; ++e) step = mont_mul(step, step, k);
+              pw = 1 % k.p;  // plain; plain * Montgomery -> plain
+              dst = reinterpret_cast<uint64_t*>(sH + x * 16);
+              cnt = 32;
+            }
+            for (int e = 0; e < cnt; ++e) {
+              dst[e] = pw;
+              pw = mont_mul(pw, step, k);
             }
           }
         }
         __syncthreads();
-        const uint64_t* pP = sP + (threadIdx.x & 15);
-        const uint64_t* pH = sH + (threadIdx.x >> 4);
-        int x = 0;
-        for (; x + 1 < n; x += 2) acc_mac2(acc, pP[x * 16], pH[x * 16], pP[x * 16 + 16], pH[x * 16 + 16]);
-        if (x < n) acc_mac(acc, pP[x * 16], pH[x * 16]);
+        const ulonglong2* pP = sP + a;
+        const ulonglong2* pH = sH + c;
+#pragma unroll 2
+        for (int x = grp; x < n; x += ng) {
+          const ulonglong2 P = pP[x * 8], H = pH[x * 16];
+          acc_mac(acc[0], P.x, H.x);
+          acc_mac(acc[1], P.y, H.x);
+          acc_mac(acc[2], P.x, H.y);
+          acc_mac(acc[3], P.y, H.y);
+        }
       }
-      if (s < t) out[(int64_t)b * T_tot + off + s] = mont_mul(acc_redc160(acc, k), k.c160, k);  // Montgomery * plain sums
+      uint64_t r[4];  // Montgomery * plain sums
+#pragma unroll
+      for (int x = 0; x < 4; ++x) r[x] = mont_mul(acc_redc160(acc[x], k), k.c160, k);
+      if (ng > 1) {  // (uniform) the groups' partial sums meet in shared memory, over the tables
+        uint64_t* red = reinterpret_cast<uint64_t*>(sH);  // [ng][32 cr] = 512 words
+        __syncthreads();
+#pragma unroll
+        for (int x = 0; x < 4; ++x) red[grp * 32 * cr + ls + (x & 1) + 16 * (x >> 1)] = r[x];
+        __syncthreads();
+        if (grp == 0)
+#pragma unroll
+          for (int x = 0; x < 4; ++x)
+            for (int g = 1; g < ng; ++g) r[x] = mod_add(r[x], red[g * 32 * cr + ls + (x & 1) + 16 * (x >> 1)], k.p);
+      }
+      uint64_t* o = out + (int64_t)b * T_tot + off;
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        const int sx = s + (x & 1) + 16 * (x >> 1);
+        if (grp == 0 && sx < t) o[sx] = r[x];
+      }
     }
   }
 }
 
-// (a6) K7 balance: V_{j,s} = u_{j,s} * R_s / u_{0,s}   (eq. (4), readings G3, G20).  HBM stream
-// (16 B bytes per probe); the pivots u_{0,s} are inverted 32 x ZP_BAL_N at a time per warp (warp_batch_inv above).
+// (a6) K7 balance: V_{j,s} = u_{j,s} * R_s / u_{0,s}   (eq. (4), readings G3, G20), in two launches:
+// k_balance_scale: w_s = R_s / u_{0,s} for every slot s, as the plain residue with its Shoup companion; the pivots
+//   u_{0,s} are inverted 256 x ZP_BAL_N at a time per CTA (cta_batch_inv above); u_{0,s} = 0 -> ZP_ST_ZERO_PIVOT, w_s = 0.
+// k_balance_apply: the HBM stream (16 bytes per probe): a CTA takes 256 x ZP_BAL_N slots x ZP_BAL_ROWS rows, the
+//   multiplier of a column stays in registers down its rows, one Shoup product (any 64-bit u in, no canonicalisation
+//   before it) and one conditional subtraction per probe.  The grid is (slot blocks) x (row blocks): enough CTAs for
+//   an even spread over the SMs whatever the batch's shape.
 #define ZP_BAL_N 4
+#define ZP_BAL_ROWS 8
 __global__ void __launch_bounds__(256)
-k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const int64_t* __restrict__ offsets, int F,
-          int64_t T_tot, int B, ZpMod k, uint64_t* __restrict__ V, int32_t* __restrict__ pre) {
-  const int64_t nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  for (int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w * (32 * ZP_BAL_N) < T_tot; w += nwarp) {
-    const int64_t x0 = w * (32 * ZP_BAL_N) + lane;
-    uint64_t sc[ZP_BAL_N];
+k_balance_scale(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const int64_t* __restrict__ offsets, int F,
+                int64_t T_tot, ZpMod k, ulonglong2* __restrict__ sc, int32_t* __restrict__ pre) {
+  __shared__ uint64_t sh[64];
+  for (int64_t c0 = (int64_t)blockIdx.x * (256 * ZP_BAL_N); c0 < T_tot; c0 += (int64_t)gridDim.x * (256 * ZP_BAL_N)) {
+    const int64_t x0 = c0 + threadIdx.x;
+    uint64_t w[ZP_BAL_N];
 #pragma unroll
     for (int y = 0; y < ZP_BAL_N; ++y) {
-      const int64_t x = x0 + 32 * y;
-      sc[y] = (x < T_tot) ? to_mont(zp_canon(u[x], k.p), k) : k.r1;
+      const int64_t x = x0 + 256 * y;
+      w[y] = (x < T_tot) ? to_mont(zp_canon(u[x], k.p), k) : k.r1;
     }
-    const uint32_t zero = warp_batch_inv<ZP_BAL_N>(sc, k);
+    const uint32_t zero = cta_batch_inv<ZP_BAL_N>(w, k, sh);
 #pragma unroll
     for (int y = 0; y < ZP_BAL_N; ++y) {
-      const int64_t x = x0 + 32 * y;
+      const int64_t x = x0 + 256 * y;
       if (x >= T_tot) continue;
       if (zero >> y & 1) {
         int lo = 0, hi = F;  // function of slot x: offsets[lo] <= x < offsets[lo+1]
@@ -870,19 +966,30 @@ k_balance(const uint64_t* __restrict__ u, const uint64_t* __restrict__ R, const 
           if (offsets[mid] <= x) lo = mid; else hi = mid;
         }
         atomicMin(&pre[lo], (int32_t)(((uint32_t)(x - offsets[lo]) << 8) | ZP_ST_ZERO_PIVOT));
+        sc[x] = make_ulonglong2(0, 0);
       } else {
-        sc[y] = mont_mul(to_mont(R[x], k), sc[y], k);  // (R_s / u_{0,s})~
+        const uint64_t wm = mont_mul(to_mont(R[x], k), w[y], k);  // (R_s / u_{0,s})~
+        sc[x] = make_ulonglong2(from_mont(wm, k), shoup_companion(wm, k));
       }
     }
-#pragma unroll 4
-    for (int j = 0; j < B; ++j) {  // (unrolled: the loads of four rows are in flight together)
-      uint64_t v[ZP_BAL_N];
+  }
+}
+__global__ void __launch_bounds__(256)
+k_balance_apply(const uint64_t* __restrict__ u, const ulonglong2* __restrict__ sc, int64_t T_tot, int B, ZpMod k,
+                uint64_t* __restrict__ V) {
+  const int64_t x0 = (int64_t)blockIdx.x * (256 * ZP_BAL_N) + threadIdx.x;
+  const int j0 = blockIdx.y * ZP_BAL_ROWS, j1 = (j0 + ZP_BAL_ROWS < B) ? j0 + ZP_BAL_ROWS : B;
+  ulonglong2 w[ZP_BAL_N];
 #pragma unroll
-      for (int y = 0; y < ZP_BAL_N; ++y) v[y] = (x0 + 32 * y < T_tot) ? __ldcs(u + (int64_t)j * T_tot + x0 + 32 * y) : 0;
+  for (int y = 0; y < ZP_BAL_N; ++y) w[y] = (x0 + 256 * y < T_tot) ? __ldg(sc + x0 + 256 * y) : make_ulonglong2(0, 0);
+#pragma unroll 2
+  for (int j = j0; j < j1; ++j) {  // (unrolled: the loads of two rows, eight words a lane, are in flight together)
+    uint64_t v[ZP_BAL_N];
 #pragma unroll
-      for (int y = 0; y < ZP_BAL_N; ++y)
-        if (x0 + 32 * y < T_tot) V[(int64_t)j * T_tot + x0 + 32 * y] = mont_mul(zp_canon(v[y], k.p), sc[y], k);
-    }
+    for (int y = 0; y < ZP_BAL_N; ++y) v[y] = (x0 + 256 * y < T_tot) ? __ldcs(u + (int64_t)j * T_tot + x0 + 256 * y) : 0;
+#pragma unroll
+    for (int y = 0; y < ZP_BAL_N; ++y)
+      if (x0 + 256 * y < T_tot) __stcs(V + (int64_t)j * T_tot + x0 + 256 * y, shoup_mul(v[y], w[y], k));
   }
 }
 

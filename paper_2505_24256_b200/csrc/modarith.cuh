@@ -88,42 +88,53 @@ ZP_DEV uint64_t mont_pow(uint64_t x, uint64_t e, const ZpMod& k) {
   }
   return r;
 }
-// a^-1 mod p for a in [1, p), p odd, gcd(a, p) = 1, by the binary extended Euclidean algorithm: at most 2 x 63
-// halvings and 63 subtractions of plain 64-bit integers (no multiplication), against the 125 dependent Montgomery
-// products of a Fermat power -- a Montgomery product alone is about 160 cycles of latency on sm_100a, and an inversion
-// is latency, not throughput, where it sits alone in a warp (the one inversion of a batched inversion).
-// Invariants: x1 a = u, x2 a = v (mod p).  0 (or a common factor: p not prime) -> 0; callers flag zeros.
-ZP_DEV uint64_t zp_inv_binary(uint64_t a, uint64_t p) {
-  uint64_t u = a, v = p, x1 = 1, x2 = 0;
+// a^-1 2^k mod p for a in [1, p), p odd, gcd(a, p) = 1 -- the first phase of Kaliski's "almost Montgomery inverse", with
+// the runs of halvings taken at once (count of trailing zeros) and no branch in the loop, so that lanes with different
+// arguments run the same instructions.  Plain 64-bit integers, no multiplication: a Montgomery product is about 160
+// cycles of latency on sm_100a and a Fermat power is 125 of them in a chain; this loop is ~45 iterations (at most
+// 126) of ~30 instructions.  Invariants (u, v odd):  p = u s + v r  (so r + s <= p: nothing overflows),
+// a s = v 2^k,  a r = -u 2^k (mod p).  The loop ends with u = v = gcd(a, p); then a s = 2^k.  62 <= ... k <= 126 for
+// p near 2^63, k >= log2 p in general.  0 or a common factor (p not prime) -> 0; callers flag zeros.
+ZP_DEV uint64_t zp_almost_inv(uint64_t a, uint64_t p, int& kout) {
+  kout = 0;
   if (a == 0) return 0;
-  for (int guard = 0; guard < 512 && u != 1 && v != 1; ++guard) {
-    if ((u & 1) == 0) {
-      u >>= 1;
-      x1 = (x1 & 1) ? (x1 + p) >> 1 : x1 >> 1;  // x1 + p < 2^64: both below 2^63
-    } else if ((v & 1) == 0) {
-      v >>= 1;
-      x2 = (x2 & 1) ? (x2 + p) >> 1 : x2 >> 1;
-    } else if (u >= v) {
-      u -= v;
-      x1 = (x1 >= x2) ? x1 - x2 : x1 + p - x2;
-      if (u == 0) return 0;  // gcd(a, p) > 1
-    } else {
-      v -= u;
-      x2 = (x2 >= x1) ? x2 - x1 : x2 + p - x1;
-    }
+  uint64_t u = p, v = a, r = 0, s = 1;
+  int k = __ffsll((long long)v) - 1;
+  v >>= k;
+  while (u != v) {
+    const bool gt = u > v;
+    const uint64_t d = gt ? u - v : v - u;  // even, non-zero
+    const int z = __ffsll((long long)d) - 1;
+    const uint64_t dz = d >> z, sum = r + s, sh = (gt ? s : r) << z;
+    u = gt ? dz : u;
+    v = gt ? v : dz;
+    r = gt ? sum : sh;
+    s = gt ? sh : sum;
+    k += z;
   }
-  return u == 1 ? x1 : (v == 1 ? x2 : 0);
+  kout = k;
+  return u == 1 ? s : 0;
 }
-// Inverse by Fermat, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.  The form for lanes
-// with DIFFERENT arguments: the same instructions in every lane (the binary algorithm above diverges four ways per
-// iteration: measured 1.5x slower than this in k_newton_prep, k_thiele and k_lift_small).
-ZP_DEV uint64_t mont_inv(uint64_t x, const ZpMod& k) { return mont_pow(x, k.p - 2, k); }
-// The same for an argument that is UNIFORM across the warp (the one inversion of a batched inversion): the binary
-// algorithm, (x^-1)~ = 2^128 / x~ = the plain inverse of x~ times r2 twice (Montgomery products).
-ZP_DEV uint64_t mont_inv_uniform(uint64_t x, const ZpMod& k) {
-  const uint64_t z = zp_inv_binary(x, k.p);
-  return mont_mul(mont_mul(z, k.r2, k), k.r2, k);
+// 2^j mod p, 0 <= j <= 64
+ZP_DEV uint64_t zp_pow2_mod(int j, const ZpMod& k) {
+  if (j == 64) return k.r1;
+  const uint64_t x = 1ull << j;
+  if (x < k.p) return x;
+  return (x - k.p < k.p) ? x - k.p : x % k.p;  // (the division only for p < 2^62)
 }
+// Inverse, x~ -> (x^-1)~ ; 0 -> 0 (callers flag it).  p prime is the caller's contract.  With s = (x~)^-1 2^k from above,
+// (x^-1)~ = 2^128 / x~ = s 2^(128-k):  mont_mul(s, r2) = s 2^64, times 2^e / 2^64 with e = 128 - k in [2, 128].
+ZP_DEV uint64_t mont_inv(uint64_t x, const ZpMod& k) {
+  int kk;
+  const uint64_t s = zp_almost_inv(x, k.p, kk);
+  const int e = 128 - kk;
+  const uint64_t c = (e <= 64) ? zp_pow2_mod(e, k) : mont_mul(zp_pow2_mod(e - 64, k), k.r2, k);  // 2^e mod p
+  return mont_mul(mont_mul(s, k.r2, k), c, k);
+}
+// Inverse by Fermat: kept as the cross-check of the one above (zippel_modarith_selftest)
+ZP_DEV uint64_t mont_inv_fermat(uint64_t x, const ZpMod& k) { return mont_pow(x, k.p - 2, k); }
+// (the argument is uniform across the warp: the one inversion of a batched inversion; same routine)
+ZP_DEV uint64_t mont_inv_uniform(uint64_t x, const ZpMod& k) { return mont_inv(x, k); }
 
 // ---- Horner step with Shoup companions (the hot recurrence of (a3): q <- M_l + m q, d <- M'_l + m d) ----
 // For w in [0,p) its companion is w' = floor(w 2^64 / p) < 2^64.  Since w 2^64 - w~ = w' p with

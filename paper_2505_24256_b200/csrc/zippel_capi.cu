@@ -817,7 +817,7 @@ void run_eval_nodes(const uint16_t* exps, int64_t T_tot, int nv, const uint64_t*
 void run_power_sums(const Ws& w, const uint64_t* nodes, int F, int64_t T_tot, int64_t tmax, const uint64_t* coef,
                     int B, int s0, const ZpMod& k, uint64_t* out, cudaStream_t st) {
   ProfScope prof(ZP_K_POWER_SUMS, st);
-  dim3 g((unsigned)((tmax + ZP_K6_THREADS - 1) / ZP_K6_THREADS), grid_y(F));
+  dim3 g((unsigned)((tmax + ZP_K6_SBLOCK - 1) / ZP_K6_SBLOCK), grid_y(F));
   ++g_launches, k_power_sums<<<g, ZP_K6_THREADS, 0, st>>>(nodes, w.d_offsets, F, coef, T_tot, B, s0, k, out);
 }
 
@@ -1131,11 +1131,14 @@ int balanced_zippel_lift_step(const zp_part* num, const zp_part* den, int F, int
     ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(w.st_pre, F, ZP_ST_NONE);
     run_eval_nodes(q->exps, T_tot[x], nv, anchors, k, w.nodes, st);
     run_power_sums(w, w.nodes, F, T_tot[x], tmax[x], q->skel, 1, s0, k, w.R, st);
-    int64_t blocks = (T_tot[x] + 256 * ZP_BAL_N - 1) / (256 * ZP_BAL_N);
-    if (blocks > sm_count() * 32) blocks = sm_count() * 32;
     {
       ProfScope prof(ZP_K_BALANCE, st);
-      ++g_launches, k_balance<<<(unsigned)blocks, 256, 0, st>>>(q->uvals, w.R, w.d_offsets, F, T_tot[x], B, k, w.V, w.st_pre);
+      const int64_t cb = (T_tot[x] + 256 * ZP_BAL_N - 1) / (256 * ZP_BAL_N);
+      ulonglong2* sc = reinterpret_cast<ulonglong2*>(w.tab);  // free until the solve builds its table
+      ++g_launches, k_balance_scale<<<(unsigned)(cb > sm_count() * 8 ? sm_count() * 8 : cb), 256, 0, st>>>(
+                        q->uvals, w.R, w.d_offsets, F, T_tot[x], k, sc, w.st_pre);
+      const dim3 g((unsigned)cb, (unsigned)((B + ZP_BAL_ROWS - 1) / ZP_BAL_ROWS));  // T_tot < 2^31: cb < 2^21
+      ++g_launches, k_balance_apply<<<g, 256, 0, st>>>(q->uvals, sc, T_tot[x], B, k, w.V);
     }
     run_solve(w, q->h_offsets, w.nodes, F, T_tot[x], tmax[x], w.V, B, s0, k, q->out, st);
     run_newton(w, samples, B, q->out, T_tot[x], T_tot[x], k, basis, q->out, st, true);

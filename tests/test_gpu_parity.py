@@ -508,6 +508,19 @@ def test_balanced_probe_offset_and_ragged_lengths(zp, ref, s0, ragged):
             assert (g[:, sl].astype(object) == w.planted[:, sl].astype(object) * f_scale[f] % p).all()
 
 
+@pytest.mark.parametrize("s0", [0, 1])
+def test_balanced_long_functions_cross_the_power_sum_blocks(zp, ref, s0):
+    """Functions of more than 512 terms: k_power_sums takes the probes s in blocks of 512 (the table of a later block
+    starts at m^(sb0 + s0)), the nodes in tiles of 64, and splits the nodes of a tile among lane groups where the last
+    block is short; k_balance_apply's grid has several slot blocks and row blocks (B = 25 > ZP_BAL_ROWS)."""
+    rw = wl.make_rational_workload("rag4l", wl.SEED_BASE + 47, 4, 6, [1100, 40, 1024, 577], [515, 1025, 3, 640], 24, 25, s0=s0)
+    rw.num.s0 = rw.den.s0 = s0
+    parts, f_scale = balanced_inputs(ref, rw)
+    (wn, wd, wst), (gn, gd, st) = run_balanced_both(zp, ref, rw, parts, s0, 0)
+    assert not wst.any() and (st == wst).all()
+    assert (gn == wn).all() and (gd == wd).all()
+
+
 def test_balanced_zero_pivots_in_a_ragged_batch(zp, ref):
     """Zero pivots u_{0,s} in several functions of a ragged batch, inside and at the ends of a warp's group of the
     batched inversion: status word (smallest probe index) and every other function's output as the oracle's."""
