@@ -24,7 +24,7 @@ struct SmallOffs {
 // CTA = (G + 1) groups of MAXT lanes.  Lane i of group g < G owns node i and the right-hand sides [g per, (g + 1) per):
 // every group runs the quotient chain of its node itself (one modular multiply-add per stage; the chain is the
 // critical path, the dot products ride on it), so the B dot products of a node proceed in G lanes at once.  Group G
-// meanwhile inverts Newton's sample differences (one Fermat power each), which nothing needs before the solve is done.
+// meanwhile inverts Newton's sample differences (one inversion each), which nothing needs before the solve is done.
 __global__ void __launch_bounds__(ZP_SMALL_MAXT*(ZP_SMALL_MAXG + 1))
 k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const uint64_t* __restrict__ anchors,
              const uint64_t* __restrict__ samples, int B, int G, int s0, const uint64_t* __restrict__ vals, int64_t T_tot,
@@ -33,13 +33,18 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
   __shared__ uint64_t buf[2][ZP_SMALL_MAXT];       // product tree; then M~_0 .. M~_{t-1}
   __shared__ uint64_t sInv[64 * 64];               // (1 / (c_j - c_jj))~, jj < j
   __shared__ uint64_t sC[64];                      // c_j~
+  __shared__ ulonglong2 sMt[ZP_SMALL_MAXT];        // {M_l, its Shoup companion}, l < t (plain residues)
   __shared__ int32_t s_solve, s_newton;
   extern __shared__ __align__(16) uint64_t cols[];  // [B x MAXT]: column c_{.,i} at cols[b MAXT + i]; then sv
   constexpr int S = ZP_SMALL_MAXT;
   const int f = blockIdx.x;
   const int64_t off = offs.o[f];
   const int t = (int)(offs.o[f + 1] - off);
-  const int g = threadIdx.x / S, i = threadIdx.x % S;
+  // warp w serves group g = w div 4 and the nodes 32 q .. 32 q + 31 with q = (w + rev(g)) mod 4, rev = the two bits of g
+  // swapped: the four warps of a group sit on the four schedulers (warp w runs on scheduler w mod 4), and the warps
+  // with live lanes (q small when t is) of DIFFERENT groups on different ones (with q = w mod 4 a function of 50 terms
+  // kept its six solving warps on two schedulers)
+  const int g = threadIdx.x / S, i = 32 * (((threadIdx.x >> 5) + ((g & 1) << 1 | (g >> 1 & 1))) & 3) + (threadIdx.x & 31);
   const bool live = i < t;
   const uint64_t p = k.p;
   if (threadIdx.x == 0) s_solve = s_newton = ZP_ST_NONE;
@@ -94,37 +99,47 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
     cur ^= 1;
   }
   __syncthreads();
-  const uint64_t* M = buf[cur];  // M~_l, l < t; M_t = 1
-  // ---- (a3) + (a4): the right-hand sides of this group, NB per pass over the chain q_{t-1} = 1, q_{l-1} = M_l + m q_l
+  if (live && g == 0) {  // M_l as a plain residue with its Shoup companion: the addend of the chain's Horner step
+    const uint64_t Mm = buf[cur][i];
+    sMt[i] = make_ulonglong2(from_mont(Mm, k), shoup_companion(Mm, k));
+  }
+  __syncthreads();
+  // ---- (a3) + (a4): the right-hand sides of this group, NB per pass over the chain q_{t-1} = 1, q_{l-1} = M_l + m q_l.
+  // One warp or two per scheduler run this, so it is the number of instructions on the dependent path that counts:
+  // the chain runs on plain residues with Shoup steps (modarith.cuh: horner_step, lazy in [0, 2p)), d = Q(m) likewise
+  // (d <- d m + q, first pass only), and the dot products take the lazy q as it is (deferred sums, L205-209).
   if (live && g < G) {
     const int per = (B + G - 1) / G, bA = g * per, bB = (bA + per < B) ? bA + per : B;
+    const uint64_t m = from_mont(mm, k), mc = shoup_companion(mm, k);
     uint64_t inv = 0;  // (1 / (d [m]))~ after the first pass
     for (int b0 = bA; b0 < bB; b0 += ZP_SMALL_NB) {
       const int nb = (bB - b0 < ZP_SMALL_NB) ? bB - b0 : ZP_SMALL_NB;
       Acc acc[ZP_SMALL_NB];
 #pragma unroll
       for (int b = 0; b < ZP_SMALL_NB; ++b) acc_zero(acc[b]);
-      uint64_t q = k.r1, d = k.r1;
+      uint64_t q = 1 % p, d = q;  // plain; q lazy in [0, 2p), d in [0, 2p)
       const uint64_t* v[ZP_SMALL_NB];  // rows beyond nb repeat the last one (their sums are dropped): no branch in the loop
 #pragma unroll
       for (int b = 0; b < ZP_SMALL_NB; ++b) v[b] = sv + (b0 + (b < nb ? b : nb - 1)) * S;
       for (int l = t - 1; l >= 1; --l) {
 #pragma unroll
         for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][l]);
-        q = mod_add(M[l], mont_mul(mm, q, k), p);
-        d = mod_add(mont_mul(d, mm, k), q, p);
+        const ulonglong2 Ml = sMt[l];
+        q = horner_step(q, m, mc, Ml.x, Ml.y, k);
+        if (b0 == bA) d = lazy_canon(shoup_mul_lazy(d, m, mc, k), p) + lazy_canon(q, p);  // (uniform over the lane's pass)
       }
 #pragma unroll
       for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][0]);
       if (b0 == bA) {
-        const uint64_t dd = s0 ? mont_mul(d, mm, k) : d;
+        uint64_t dd = to_mont(lazy_canon(d, p), k);
+        if (s0) dd = mont_mul(dd, mm, k);
         if (dd == 0 && g == 0) atomicMin(&s_solve, (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
         inv = mont_inv(dd, k);
       }
 #pragma unroll
       for (int b = 0; b < ZP_SMALL_NB; ++b)
-        if (b < nb)  // sum of Montgomery x plain: redc160 and c160 give the plain sum; plain x Montgomery -> plain
-          cols[(b0 + b) * S + i] = mont_mul(mont_mul(acc_redc160(acc[b], k), k.c160, k), inv, k);
+        if (b < nb)  // sum of plain x plain: redc160 and c224 give the Montgomery form of the sum; x (1/d)~ -> plain
+          cols[(b0 + b) * S + i] = mont_mul(mont_mul(acc_redc160(acc[b], k), k.c224, k), inv, k);
     }
   }
   __syncthreads();  // the columns, sInv, sC, s_newton are complete
