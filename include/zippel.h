@@ -41,6 +41,7 @@ extern "C" {
 #define ZP_ERR_ARG 1       /* null pointer, size <= 0, p even / < 3 / >= 2^63, nv > ZP_MAX_NV, B > ZP_MAX_B */
 #define ZP_ERR_WORKSPACE 2 /* workspace too small or misaligned */
 #define ZP_ERR_CUDA 3      /* launch / configuration error, or no device */
+#define ZP_ERR_SCRATCH_LIMIT 4 /* zippel_extend_skeleton_static: the batch needs more than ZP_STATIC_SCRATCH_BYTES */
 
 /* per-function status codes (low byte of status[f]) */
 #define ZP_ST_DUPLICATE_NODE 16   /* den_i == 0: two terms map to one node (G24); or m_i == 0 with s0 = 1 (G25) */
@@ -174,6 +175,25 @@ int thiele_reconstruct_batch(const uint64_t* points, int T, const uint64_t* vals
 int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs, int B,
                            uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap, int64_t* new_offsets,
                            int32_t* degs, void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same operation for callers that may not allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc) and so have no workspace to pass: the scratch that zippel_extend_skeleton
+ * takes from its workspace (the function offsets and the look-back descriptors of its one-pass scan, k_ext_fused)
+ * lies in a file-scope `static __device__` array of ZP_STATIC_SCRATCH_BYTES bytes inside the library (every GPU that
+ * loads the library holds it until the process exits).  Same arguments without the workspace, same results bit for
+ * bit.  The call allocates nothing: no cudaMalloc / cudaFree / allocating library routine; it enqueues one copy of
+ * h_offsets (read before the call returns), one memset of the descriptors and two kernels on `stream`.
+ *   Limit: 256-byte-rounded 8 (F + 1) bytes of offsets + 8 (ceil(T_tot / 2048) + 1) bytes of descriptors must fit
+ *   ZP_STATIC_SCRATCH_BYTES (e.g. F = 4096 functions of 10^4 terms: 0.2 MB); beyond it the call enqueues nothing and
+ *   returns ZP_ERR_SCRATCH_LIMIT (zippel_strerror names the limit).
+ *   The array is ONE per device and every call uses it: the call clears what must start at zero (the descriptors), but
+ *   two calls that overlap on the GPU (different streams, or threads) race on it -- order them, or give the others
+ *   the workspace variant above.  zippel_static_scratch_bytes() returns the limit. */
+#define ZP_STATIC_SCRATCH_BYTES (1u << 20)
+int zippel_extend_skeleton_static(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs,
+                                  int B, uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap,
+                                  int64_t* new_offsets, int32_t* degs, void* stream);
+size_t zippel_static_scratch_bytes(void);
 
 /* (f4, SURVEY.md section 8 "next") Second prime + CRT + rational reconstruction (the reduction runs
  * over several large primes "fitting into 2^64" and "the final reconstruction to rational numbers is performed as

@@ -19,7 +19,7 @@ import torch
 
 from . import build as _build
 
-ZP_OK, ZP_ERR_ARG, ZP_ERR_WORKSPACE, ZP_ERR_CUDA = 0, 1, 2, 3
+ZP_OK, ZP_ERR_ARG, ZP_ERR_WORKSPACE, ZP_ERR_CUDA, ZP_ERR_SCRATCH_LIMIT = 0, 1, 2, 3, 4
 ST_DUPLICATE_NODE, ST_DUPLICATE_SAMPLE, ST_ZERO_PIVOT = 16, 17, 18
 BASIS_NEWTON, BASIS_MONOMIAL = 0, 1
 WS_BALANCED = 1
@@ -30,7 +30,7 @@ EXPORTS = (
     "newton_interp_batch", "zippel_lift_step", "zippel_power_sums", "balanced_zippel_lift_step",
     "zippel_lift_step_host", "zippel_host_workspace_bytes", "zippel_profile_events",
     "zippel_launch_count", "thiele_reconstruct_batch", "zippel_extend_skeleton", "crt_rational_reconstruct_batch",
-    "zippel_set_tuning", "zippel_shutdown",
+    "zippel_set_tuning", "zippel_shutdown", "zippel_extend_skeleton_static", "zippel_static_scratch_bytes",
 )
 TUNE_SUBQ_MIN_T = 1
 SUBQ_MIN_T_DEFAULT = 0  # g_subq_min_t in csrc/zippel_capi.cu: 0 = the built-in rule (sq_threshold)
@@ -70,6 +70,9 @@ def declare(L: C.CDLL) -> C.CDLL:
     L.thiele_reconstruct_batch.argtypes = [vp, i32, vp, C.c_int64, C.c_int64, u64, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
     L.zippel_extend_skeleton.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp, C.c_size_t, vp]
     L.crt_rational_reconstruct_batch.argtypes = [vp, vp, C.c_int64, u64, u64, vp, vp, vp, vp]
+    L.zippel_extend_skeleton_static.argtypes = [vp, vp, i32, i32, vp, i32, u64, vp, vp, C.c_int64, vp, vp, vp]
+    L.zippel_static_scratch_bytes.argtypes = []
+    L.zippel_static_scratch_bytes.restype = C.c_size_t
     L.zippel_launch_count.restype = C.c_ulonglong
     L.zippel_launch_count.argtypes = []
     L.zippel_set_tuning.argtypes = [i32, i64]
@@ -384,6 +387,29 @@ def zippel_extend_skeleton(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: 
                                             _ptr(no), _ptr(degs), _ptr(workspace), workspace.numel(), _stream(stream)),
                "zippel_extend_skeleton")
         return ne, nc, no, degs
+
+
+def zippel_static_scratch_bytes() -> int:
+    return int(lib().zippel_static_scratch_bytes())
+
+
+def zippel_extend_skeleton_static(exps: torch.Tensor, offsets, coefs: torch.Tensor, p: int, new_exps: torch.Tensor,
+                                  new_coefs: torch.Tensor, new_offsets: torch.Tensor, degs: torch.Tensor, stream=None):
+    """(f1) without a workspace and without any allocation (zippel.h: zippel_extend_skeleton_static): the caller passes
+    the outputs -- new_exps [cap, nv+1] int16, new_coefs [cap] int64, new_offsets [F+1] int64, degs [F] int32, all on
+    the device -- and cap = new_coefs.numel().  The scratch is ONE array per device inside the library: calls that
+    overlap on the GPU race.  Raises ZippelError (code ZP_ERR_SCRATCH_LIMIT) beyond zippel_static_scratch_bytes()."""
+    _need_cuda()
+    with _on(stream):
+        o = _offs(offsets)
+        F, (B, T_tot), nv = len(o) - 1, coefs.shape, exps.shape[1]
+        cap = int(new_coefs.numel())
+        assert new_exps.dtype == torch.int16 and new_exps.is_contiguous() and tuple(new_exps.shape) == (cap, nv + 1)
+        assert new_coefs.dtype == torch.int64 and new_offsets.dtype == torch.int64 and new_offsets.numel() == F + 1
+        assert degs.dtype == torch.int32 and degs.numel() == F
+        _check(lib().zippel_extend_skeleton_static(_ptr(exps), o.ctypes.data, F, nv, _ptr(coefs), B, p, _ptr(new_exps),
+                                                   _ptr(new_coefs), cap, _ptr(new_offsets), _ptr(degs), _stream(stream)),
+               "zippel_extend_skeleton_static")
 
 
 ST_NO_RATIONAL = 21

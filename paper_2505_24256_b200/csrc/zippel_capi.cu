@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/zippel.h"
@@ -938,6 +939,7 @@ const char* zippel_strerror(int code) {
     case ZP_ERR_ARG: return "bad argument";
     case ZP_ERR_WORKSPACE: return "workspace too small or misaligned";
     case ZP_ERR_CUDA: return "CUDA error";
+    case ZP_ERR_SCRATCH_LIMIT: return "batch exceeds the static scratch array (ZP_STATIC_SCRATCH_BYTES = 1 MiB: offsets + scan descriptors)";
     case ZP_ST_DUPLICATE_NODE: return "duplicate (or zero) node";
     case ZP_ST_DUPLICATE_SAMPLE: return "duplicate sample";
     case ZP_ST_ZERO_PIVOT: return "zero pivot in balancing";
@@ -1192,6 +1194,57 @@ int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F
   if (smem > 98304) stage_rows = 0, smem = 0;
   cudaFuncSetAttribute(k_ext_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, 98304);
   ++g_launches, k_ext_fused<<<(unsigned)nb, ZP_K9_THREADS, smem, st>>>(exps, nv, coefs, T_tot, B, w.d_offsets, F, k, desc, nb, new_exps,
+                                                                        new_coefs, cap, new_offsets, degs, stage_rows);
+  return cuda_ok();
+}
+
+// ---- the entry point that allocates nothing (zippel.h: zippel_extend_skeleton_static) ---------------------------------
+// The scratch of k_ext_fused -- [offsets (F + 1) int64, rounded to 256 bytes | descriptors (nb + 1) x 8 bytes] -- in a
+// file-scope device array.  In host code the NAME g_static_scratch is a host-side stand-in, not a device address: the
+// kernels get the address that cudaGetSymbolAddress returns for the CURRENT device, looked up once per device.
+static __device__ __align__(256) unsigned char g_static_scratch[ZP_STATIC_SCRATCH_BYTES];
+static unsigned char* g_static_scratch_ptr[64] = {nullptr};  // per device ordinal
+static std::mutex g_static_scratch_mu;
+static unsigned char* static_scratch() {  // device address on the current device, or nullptr
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lock(g_static_scratch_mu);
+  if (!g_static_scratch_ptr[dev]) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) {
+      cudaGetLastError();  // (clear it: the caller gets ZP_ERR_CUDA)
+      return nullptr;
+    }
+    g_static_scratch_ptr[dev] = static_cast<unsigned char*>(ptr);
+  }
+  return g_static_scratch_ptr[dev];
+}
+size_t zippel_static_scratch_bytes(void) { return ZP_STATIC_SCRATCH_BYTES; }
+
+int zippel_extend_skeleton_static(const uint16_t* exps, const int64_t* h_offsets, int F, int nv, const uint64_t* coefs,
+                                  int B, uint64_t p, uint16_t* new_exps, uint64_t* new_coefs, int64_t cap,
+                                  int64_t* new_offsets, int32_t* degs, void* stream) {
+  ZpMod k;
+  int64_t T_tot, tmax;
+  if (!exps || !coefs || !new_exps || !new_coefs || !new_offsets || !degs || nv <= 0 || nv >= ZP_MAX_NV || B <= 0 ||
+      B > ZP_MAX_B || cap < 0 || !make_mod(p, &k) || !check_offsets(h_offsets, F, &T_tot, &tmax))
+    return ZP_ERR_ARG;
+  const int64_t nb = (T_tot + ZP_K9_BLOCK - 1) / ZP_K9_BLOCK;
+  const size_t offs_bytes = al(sizeof(int64_t) * (size_t)(F + 1)), desc_bytes = 8 * (size_t)(nb + 1);
+  if (offs_bytes + desc_bytes > ZP_STATIC_SCRATCH_BYTES) return ZP_ERR_SCRATCH_LIMIT;
+  unsigned char* base = static_scratch();
+  if (!base) return ZP_ERR_CUDA;
+  int64_t* d_offsets = reinterpret_cast<int64_t*>(base);
+  unsigned long long* desc = reinterpret_cast<unsigned long long*>(base + offs_bytes);
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaMemcpyAsync(d_offsets, h_offsets, sizeof(int64_t) * (size_t)(F + 1), cudaMemcpyHostToDevice, st);
+  ++g_launches, k_fill_i32<<<(F + 255) / 256, 256, 0, st>>>(degs, F, -1);
+  cudaMemsetAsync(desc, 0, desc_bytes, st);  // the array keeps the last call's tickets and flags: they start at zero
+  int stage_rows = ZP_K9_BLOCK + ZP_K9_BLOCK / 4;  // (as zippel_extend_skeleton)
+  size_t smem = (size_t)stage_rows * (8 + 2 * (size_t)(nv + 1)) + 2 * (size_t)nv * ZP_K9_BLOCK + 32;
+  if (smem > 98304) stage_rows = 0, smem = 0;
+  cudaFuncSetAttribute(k_ext_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, 98304);
+  ++g_launches, k_ext_fused<<<(unsigned)nb, ZP_K9_THREADS, smem, st>>>(exps, nv, coefs, T_tot, B, d_offsets, F, k, desc, nb, new_exps,
                                                                         new_coefs, cap, new_offsets, degs, stage_rows);
   return cuda_ok();
 }
