@@ -16,6 +16,8 @@
 #define ZP_SMALL_MAXT 128
 #define ZP_SMALL_NB 4    // right-hand sides per pass over the quotient chain (accumulators in registers)
 #define ZP_SMALL_MAXG 3  // groups of lanes that share the right-hand sides of a function; one more group builds tables
+#define ZP_SMALL_MAXB 25  // Newton's steps per level and lane: (B - 1) / LPC <= ZP_SMALL_OPS (LPC = 4 from B = 9 on, else 2)
+#define ZP_SMALL_OPS 6
 
 struct SmallOffs {
   int64_t o[ZP_SMALL_MAXF + 1];
@@ -24,7 +26,8 @@ struct SmallOffs {
 // CTA = (G + 1) groups of MAXT lanes.  Lane i of group g < G owns node i and the right-hand sides [g per, (g + 1) per):
 // every group runs the quotient chain of its node itself (one modular multiply-add per stage; the chain is the
 // critical path, the dot products ride on it), so the B dot products of a node proceed in G lanes at once.  Group G
-// meanwhile inverts Newton's sample differences (one inversion each), which nothing needs before the solve is done.
+// meanwhile inverts Newton's sample differences and, running the chain once more without dot products, computes the
+// denominators Q_i(m_i) and their inverses, which nothing needs before the columns go out.
 __global__ void __launch_bounds__(ZP_SMALL_MAXT*(ZP_SMALL_MAXG + 1))
 k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const uint64_t* __restrict__ anchors,
              const uint64_t* __restrict__ samples, int B, int G, int s0, const uint64_t* __restrict__ vals, int64_t T_tot,
@@ -34,6 +37,7 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
   __shared__ uint64_t sInv[64 * 64];               // (1 / (c_j - c_jj))~, jj < j
   __shared__ uint64_t sC[64];                      // c_j~
   __shared__ ulonglong2 sMt[ZP_SMALL_MAXT];        // {M_l, its Shoup companion}, l < t (plain residues)
+  __shared__ uint64_t sDinv[ZP_SMALL_MAXT];        // (1 / (Q_i(m_i) [m_i]))~
   __shared__ int32_t s_solve, s_newton;
   extern __shared__ __align__(16) uint64_t cols[];  // [B x MAXT]: column c_{.,i} at cols[b MAXT + i]; then sv
   constexpr int S = ZP_SMALL_MAXT;
@@ -72,9 +76,9 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
       }
     }
   }
-  // ---- (a1) node of this lane (every solving group computes it: no hand-over)
+  // ---- (a1) node of this lane (every group computes it: no hand-over)
   uint64_t mm = 0;  // m_i~
-  if (live && g < G) {
+  if (live) {
     const uint16_t* e = exps + (off + i) * nv;
     mm = k.r1;
     for (int j = 0; j < nv; ++j) {
@@ -104,80 +108,99 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
     sMt[i] = make_ulonglong2(from_mont(Mm, k), shoup_companion(Mm, k));
   }
   __syncthreads();
-  // ---- (a3) + (a4): the right-hand sides of this group, NB per pass over the chain q_{t-1} = 1, q_{l-1} = M_l + m q_l.
+  // ---- (a3): the right-hand sides of this group, NB per pass over the chain q_{t-1} = 1, q_{l-1} = M_l + m q_l.
   // One warp or two per scheduler run this, so it is the number of instructions on the dependent path that counts:
-  // the chain runs on plain residues with Shoup steps (modarith.cuh: horner_step, lazy in [0, 2p)), d = Q(m) likewise
-  // (d <- d m + q, first pass only), and the dot products take the lazy q as it is (deferred sums, L205-209).
-  if (live && g < G) {
-    const int per = (B + G - 1) / G, bA = g * per, bB = (bA + per < B) ? bA + per : B;
+  // the chain runs on plain residues with Shoup steps (modarith.cuh: horner_step, lazy in [0, 2p)) and the dot products
+  // take the lazy q as it is (deferred sums, L205-209).  The columns are stored UNSCALED; the division (a4) by
+  // d = Q(m) [m] commutes with Newton's recurrence (linear in the column) and is applied on the way out.  d and its
+  // inverse are the table group's: the chain once more, without dot products, beside the solving groups.
+  if (live) {
     const uint64_t m = from_mont(mm, k), mc = shoup_companion(mm, k);
-    uint64_t inv = 0;  // (1 / (d [m]))~ after the first pass
-    for (int b0 = bA; b0 < bB; b0 += ZP_SMALL_NB) {
-      const int nb = (bB - b0 < ZP_SMALL_NB) ? bB - b0 : ZP_SMALL_NB;
-      Acc acc[ZP_SMALL_NB];
+    if (g < G) {
+      const int per = (B + G - 1) / G, bA = g * per, bB = (bA + per < B) ? bA + per : B;
+      for (int b0 = bA; b0 < bB; b0 += ZP_SMALL_NB) {
+        const int nb = (bB - b0 < ZP_SMALL_NB) ? bB - b0 : ZP_SMALL_NB;
+        Acc acc[ZP_SMALL_NB];
 #pragma unroll
-      for (int b = 0; b < ZP_SMALL_NB; ++b) acc_zero(acc[b]);
-      uint64_t q = 1 % p, d = q;  // plain; q lazy in [0, 2p), d in [0, 2p)
-      const uint64_t* v[ZP_SMALL_NB];  // rows beyond nb repeat the last one (their sums are dropped): no branch in the loop
+        for (int b = 0; b < ZP_SMALL_NB; ++b) acc_zero(acc[b]);
+        uint64_t q = 1 % p;              // plain, lazy in [0, 2p)
+        const uint64_t* v[ZP_SMALL_NB];  // rows beyond nb repeat the last one (their sums are dropped): no branch in the loop
 #pragma unroll
-      for (int b = 0; b < ZP_SMALL_NB; ++b) v[b] = sv + (b0 + (b < nb ? b : nb - 1)) * S;
+        for (int b = 0; b < ZP_SMALL_NB; ++b) v[b] = sv + (b0 + (b < nb ? b : nb - 1)) * S;
+        for (int l = t - 1; l >= 1; --l) {
+#pragma unroll
+          for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][l]);
+          const ulonglong2 Ml = sMt[l];
+          q = horner_step(q, m, mc, Ml.x, Ml.y, k);
+        }
+#pragma unroll
+        for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][0]);
+#pragma unroll
+        for (int b = 0; b < ZP_SMALL_NB; ++b)
+          if (b < nb)  // sum of plain x plain: redc160, then c224, give the plain sum
+            cols[(b0 + b) * S + i] = mont_mul(acc_redc160(acc[b], k), k.c224, k);
+      }
+    } else {  // d = Q(m) = sum_l q_l m^l by Horner beside the chain: d <- d m + q
+      uint64_t q = 1 % p, d = q;
       for (int l = t - 1; l >= 1; --l) {
-#pragma unroll
-        for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][l]);
         const ulonglong2 Ml = sMt[l];
         q = horner_step(q, m, mc, Ml.x, Ml.y, k);
-        if (b0 == bA) d = lazy_canon(shoup_mul_lazy(d, m, mc, k), p) + lazy_canon(q, p);  // (uniform over the lane's pass)
+        d = lazy_canon(shoup_mul_lazy(d, m, mc, k), p) + lazy_canon(q, p);
       }
-#pragma unroll
-      for (int b = 0; b < ZP_SMALL_NB; ++b) acc_mac(acc[b], q, v[b][0]);
-      if (b0 == bA) {
-        uint64_t dd = to_mont(lazy_canon(d, p), k);
-        if (s0) dd = mont_mul(dd, mm, k);
-        if (dd == 0 && g == 0) atomicMin(&s_solve, (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
-        inv = mont_inv(dd, k);
-      }
-#pragma unroll
-      for (int b = 0; b < ZP_SMALL_NB; ++b)
-        if (b < nb)  // sum of plain x plain: redc160 and c224 give the Montgomery form of the sum; x (1/d)~ -> plain
-          cols[(b0 + b) * S + i] = mont_mul(mont_mul(acc_redc160(acc[b], k), k.c224, k), inv, k);
+      uint64_t dd = to_mont(lazy_canon(d, p), k);
+      if (s0) dd = mont_mul(dd, mm, k);
+      if (dd == 0) atomicMin(&s_solve, (int32_t)(((uint32_t)i << 8) | ZP_ST_DUPLICATE_NODE));
+      sDinv[i] = mont_inv(dd, k);  // (1 / (d [m]))~
     }
   }
-  __syncthreads();  // the columns, sInv, sC, s_newton are complete
-  // ---- (a5) Newton in x_k on this lane's column (shared memory), then the column goes out
-  if (live && g == 0) {
-    uint64_t* col = cols + i;
+  __syncthreads();  // the columns, sDinv, sInv, sC, s_newton are complete
+  // ---- (a5) Newton in x_k on the columns (shared memory), then the columns go out.  The steps of one level (or of one
+  // pass of the expansion) read the previous level only, so they are shared out among LPC = 2 or 4 neighbouring lanes
+  // of a warp per column (all the CTA's lanes work: 128 (G + 1) >= 128 LPC): a lane loads the operands of its (at most
+  // ZP_SMALL_OPS) steps, the warp meets, the lane multiplies and stores, the warp meets again.  The latency of one
+  // Montgomery product per level instead of that of a quarter of the level's products one after another.
+  {
+    const int LPC = (G + 1 >= 4) ? 4 : 2;  // G >= 1
+    const int ci = threadIdx.x / LPC, sub = threadIdx.x % LPC;
+    const bool on = ci < t;
+    uint64_t* col = cols + (on ? ci : 0);
     const int D = B - 1;
-    // the steps of one level read the previous level only: four at a time, loads before stores, so that their
-    // products overlap (one warp per scheduler: latency is all there is)
-    for (int l = 1; l <= D; ++l) {
-      int j = D;
-      for (; j - 3 >= l; j -= 4) {
-        const uint64_t v0 = col[j * S], v1 = col[(j - 1) * S], v2 = col[(j - 2) * S], v3 = col[(j - 3) * S], v4 = col[(j - 4) * S];
-        const uint64_t* w = sInv + j * B + (j - l);  // row stride B, same column offset j - l
-        col[j * S] = mont_mul(mod_sub(v0, v1, p), w[0], k);
-        col[(j - 1) * S] = mont_mul(mod_sub(v1, v2, p), w[-B - 1], k);
-        col[(j - 2) * S] = mont_mul(mod_sub(v2, v3, p), w[-2 * B - 2], k);
-        col[(j - 3) * S] = mont_mul(mod_sub(v3, v4, p), w[-3 * B - 3], k);
+    for (int l = 1; l <= D; ++l) {  // level l: c_j <- (c_j - c_{j-1}) / (x_j - x_{j-l}),  j = D .. l
+      uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
+#pragma unroll
+      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+        const int j = D - sub - LPC * x;
+        if (on && j >= l) a[x] = col[j * S], bb[x] = col[(j - 1) * S];
       }
-      for (; j >= l; --j) col[j * S] = mont_mul(mod_sub(col[j * S], col[(j - 1) * S], p), sInv[j * B + (j - l)], k);
+      __syncwarp();
+#pragma unroll
+      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+        const int j = D - sub - LPC * x;
+        if (on && j >= l) col[j * S] = mont_mul(mod_sub(a[x], bb[x], p), sInv[j * B + (j - l)], k);
+      }
+      __syncwarp();
     }
     if (basis == 1)
-      for (int j = D - 1; j >= 0; --j) {
+      for (int j = D - 1; j >= 0; --j) {  // pass j: a_x <- a_x - c_j a_{x+1},  x = j .. D - 1
         const uint64_t cj = sC[j];
-        int x = j;
-        for (; x + 3 < D; x += 4) {
-          const uint64_t v0 = col[x * S], v1 = col[(x + 1) * S], v2 = col[(x + 2) * S], v3 = col[(x + 3) * S], v4 = col[(x + 4) * S];
-          col[x * S] = mod_sub(v0, mont_mul(v1, cj, k), p);
-          col[(x + 1) * S] = mod_sub(v1, mont_mul(v2, cj, k), p);
-          col[(x + 2) * S] = mod_sub(v2, mont_mul(v3, cj, k), p);
-          col[(x + 3) * S] = mod_sub(v3, mont_mul(v4, cj, k), p);
+        uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
+#pragma unroll
+        for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+          const int e = j + sub + LPC * x;
+          if (on && e < D) a[x] = col[e * S], bb[x] = col[(e + 1) * S];
         }
-        for (; x < D; ++x) col[x * S] = mod_sub(col[x * S], mont_mul(col[(x + 1) * S], cj, k), p);
+        __syncwarp();
+#pragma unroll
+        for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+          const int e = j + sub + LPC * x;
+          if (on && e < D) col[e * S] = mod_sub(a[x], mont_mul(bb[x], cj, k), p);
+        }
+        __syncwarp();
       }
   }
   __syncthreads();
   for (int b = g; b < B; b += G + 1)
-    if (live) out[(int64_t)b * T_tot + off + i] = cols[b * S + i];
+    if (live) out[(int64_t)b * T_tot + off + i] = mont_mul(cols[b * S + i], sDinv[i], k);  // (a4): plain x Montgomery
   if (threadIdx.x == 0) {
     const int32_t s = (s_solve != ZP_ST_NONE) ? s_solve : s_newton;
     status[f] = (s == ZP_ST_NONE) ? 0 : s;

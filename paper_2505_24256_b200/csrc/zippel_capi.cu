@@ -865,7 +865,7 @@ inline int small_groups(int B) {  // lanes per node: one per ZP_SMALL_NB right-h
   return g > ZP_SMALL_MAXG ? ZP_SMALL_MAXG : g;
 }
 bool small_ok(const int64_t* h_offs, int F, int B) {
-  if (F > ZP_SMALL_MAXF) return false;
+  if (F > ZP_SMALL_MAXF || B > ZP_SMALL_MAXB) return false;
   int64_t tmax = 0;
   for (int f = 0; f < F; ++f) tmax = (h_offs[f + 1] - h_offs[f] > tmax) ? h_offs[f + 1] - h_offs[f] : tmax;
   if (tmax > ZP_SMALL_MAXT) return false;

@@ -42,7 +42,7 @@ def both(zp, ref, w, vals, s0, basis):
 
 
 @pytest.mark.parametrize("ts,B,nv", [([50], 11, 2), ([1], 1, 1), ([1, 2, 3, 128, 127, 64, 65, 33], 3, 3), ([128] * 32, 2, 5),
-                                     ([17, 40], 21, 4), ([5], 20, 2)])
+                                     ([17, 40], 21, 4), ([5], 20, 2), ([10, 3], 24, 2), ([100, 31], 8, 3)])
 @pytest.mark.parametrize("s0", [0, 1])
 @pytest.mark.parametrize("basis", [0, 1])
 def test_small_batches_take_one_launch_and_match(zp, ref, ts, B, nv, s0, basis):
