@@ -429,9 +429,9 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
                 if idx == 2 and not F_override:
                     # DRAM bytes of this launch from the ncu --set full capture of the same command; algorithmic: the B + 1
                     # tails read and the B + 1 numerator rows written once, 8 (B + 1) T_tot bytes each way (1442 MB)
-                    r["traffic"] = 1613.6e6
+                    r["traffic"] = 1615.0e6
                     r["traffic_source"] = ("ncu --set full capture of the same command (profiles/r02_final.md: k_node_solve<22> "
-                                           "923.3 MB read + 690.2 MB written), not this run")
+                                           "924.0 MB read + 691.0 MB written), not this run")
             else:
                 line["roofline"]["leaf_solve"] = leaf
     else:
