@@ -336,14 +336,15 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
 //                   the complete transforms of the operands are written back over them (kept for MODE 1 later)
 //   MODE 1 (down) : O segments 2 vt + side = A segment vt * B segment 2 (vt mod P) + 1 - side, side = 0, 1, where B holds
 //                   COMPLETE forward transforms (k_ntt_pass): tails x reversed siblings, the siblings' transforms are
-//                   shared by all the vectors of a level.  EA, EB, EO: words per prime of the three buffers.
+//                   shared by all the vectors of a level.  EA, EB, EO: words per prime of the three buffers; SA: the
+//                   distance between the primes' copies of A.
 ZP_DEV uint64_t ntt_canon4(uint64_t b, const ZpMod& q) {  // [0, 4q) -> [0, q)
   b = (b >= 2 * q.p) ? b - 2 * q.p : b;
   return (b >= q.p) ? b - q.p : b;
 }
 template <int MODE, int TH>
 __global__ void __launch_bounds__(TH, 768 / TH)
-k_ntt_mul(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* __restrict__ O,
+k_ntt_mul(const uint64_t* A, int64_t EA, int64_t SA, const uint64_t* B, int64_t EB, uint64_t* __restrict__ O,
           int64_t EO, int logn, int logRp, int logseg, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1, uint64_t Kq2) {
   extern __shared__ __align__(16) uint64_t ntt_mul_smem[];  // 2 x 32 KB (dynamic: above the 48 KB static limit)
   uint64_t *sm = ntt_mul_smem, *smA = ntt_mul_smem + ZP_NTT_SMEM;  // the working tile; the first operand's transform
@@ -355,7 +356,7 @@ k_ntt_mul(const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t
   const int64_t Edrv = MODE == 0 ? EO : EA;
   const uint32_t segmask = (1u << logseg) - 1;
   const ulonglong2 *Tlo = cx.Tlo[jp], *Thi = cx.Thi[jp];
-  A += (int64_t)jp * EA;
+  A += (int64_t)jp * SA;  // SA = EA, or 0 when the three primes read ONE copy of the operand (residues mod p, MODE 1)
   B += (int64_t)jp * EB;
   O += (int64_t)jp * EO;
   // Segments of at least a chunk (logseg >= 12): the chunk lies in ONE segment, seg0, at the positions pos0 + e, and

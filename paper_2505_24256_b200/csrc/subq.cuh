@@ -80,19 +80,21 @@ k_sq_down_prepx(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tas
     X[2 * EX + e] = v;
   }
 }
-// Y[j][v P + t][i] = tail_{L u R}(P_v)_i, i < a + b
+// Y[j][v P + t][i] = tail_{L u R}(P_v)_i, i < a + b  (copies = 1: one copy serves the three primes, n <= 4096)
 __global__ void __launch_bounds__(256)
 k_sq_down_prepy(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
-                uint64_t* __restrict__ Y, int64_t EY) {
+                uint64_t* __restrict__ Y, int64_t EY, int copies) {
   const int64_t n = (int64_t)1 << logn;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EY; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1);
-    const int64_t v = seg / P;
+    const int64_t v = (int64_t)((uint32_t)seg / (uint32_t)P);  // (segments of a launch: < 2^31)
     const SqTask t = tasks[seg - v * P];
     const uint64_t x = (i < t.a + t.b) ? cur[v * ld + t.base + i] : 0;
     Y[e] = x;
-    Y[EY + e] = x;
-    Y[2 * EY + e] = x;
+    if (copies == 3) {  // the strided passes of a long transform work in place, per prime
+      Y[EY + e] = x;
+      Y[2 * EY + e] = x;
+    }
   }
 }
 // O segment o = (v P + t) 2 + side.  side 0: tail_L_k = c_{k+b} + (rev(B') * c)_{k+b-1}, k < a;
@@ -104,7 +106,7 @@ k_sq_down_fin(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __rest
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t o = e >> logn, k = e & (n - 1);
     const int side = (int)(o & 1);
-    const int64_t vt = o >> 1, v = vt / P;
+    const int64_t vt = o >> 1, v = (int64_t)((uint32_t)vt / (uint32_t)P);
     const SqTask t = tasks[vt - v * P];
     const int64_t len = side ? t.b : t.a, sh = side ? t.a : t.b;  // own length, sibling's length
     if (k >= len) continue;
@@ -200,7 +202,7 @@ k_sq_newton_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, in
                 ZpMod kp, uint64_t* __restrict__ alphas) {
   const int64_t n = (int64_t)1 << logn, k = n >> 1, EO = nact * n;
   for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < nact * k; x += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t s = x / k, i = x - s * k, o = s * n + i;
+    const int64_t s = x >> (logn - 1), i = x - s * k, o = s * n + i;
     alphas[fns[s].aoff + k + i] = mod_neg(ntt_crt(O[o], O[EO + o], O[2 * EO + o], cx, co, kp), kp.p);
   }
 }

@@ -441,16 +441,16 @@ void ntt_run(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx,
   }
 }
 template <int MODE>
-void ntt_mul_launch(int64_t Edrv, const uint64_t* A, int64_t EA, const uint64_t* B, int64_t EB, uint64_t* O, int64_t EO, int lc,
+void ntt_mul_launch(int64_t Edrv, const uint64_t* A, int64_t EA, int64_t SA, const uint64_t* B, int64_t EB, uint64_t* O, int64_t EO, int lc,
                     int lrp, int logn, int64_t P, const NttCtx& cx, const uint64_t (&Kq)[3], cudaStream_t st) {
   const size_t smem = 16 * ZP_NTT_SMEM;
   if (ntt_small_grid(Edrv)) {
     cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL><<<ntt_grid(Edrv), ZP_NTT_THREADS_SMALL, smem, st>>>(A, EA, B, EB, O, EO, lc, lrp, logn, P,
+    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL><<<ntt_grid(Edrv), ZP_NTT_THREADS_SMALL, smem, st>>>(A, EA, SA, B, EB, O, EO, lc, lrp, logn, P,
                                                                                                        cx, Kq[0], Kq[1], Kq[2]);
   } else {
     cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS><<<ntt_grid(Edrv), ZP_NTT_THREADS, smem, st>>>(A, EA, B, EB, O, EO, lc, lrp, logn, P, cx, Kq[0],
+    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS><<<ntt_grid(Edrv), ZP_NTT_THREADS, smem, st>>>(A, EA, SA, B, EB, O, EO, lc, lrp, logn, P, cx, Kq[0],
                                                                                            Kq[1], Kq[2]);
   }
 }
@@ -464,9 +464,11 @@ void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx&
   uint64_t Kq[3];
   make_kq(logn, Kq);
   ntt_strided(false, X, EX, logn, cx, st);
-  ntt_mul_launch<0>(EO, X, EX, keep ? X : nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq, st);
+  ntt_mul_launch<0>(EO, X, EX, EX, keep ? X : nullptr, 0, O, EO, pl.lc, pl.lrp, logn, 1, cx, Kq, st);
   ntt_strided(true, O, EO, logn, cx, st);
 }
+// copies of Y that k_sq_down_prepy writes: one serves the three primes when the transform has no strided pass
+inline int ntt_down_copies(int logn) { return logn <= ZP_NTT_LOGC ? 1 : 3; }
 //   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds complete
 //   transforms (ntt_run); Y is overwritten by its strided passes
 void ntt_mul_down(uint64_t* Y, int64_t EY, const uint64_t* Xhat, int64_t EX, uint64_t* O, int logn, int64_t P, const NttCtx& cx,
@@ -476,7 +478,7 @@ void ntt_mul_down(uint64_t* Y, int64_t EY, const uint64_t* Xhat, int64_t EX, uin
   uint64_t Kq[3];
   make_kq(logn, Kq);
   ntt_strided(false, Y, EY, logn, cx, st);
-  ntt_mul_launch<1>(EY, Y, EY, Xhat, EX, O, EO, pl.lc, pl.lrp, logn, P, cx, Kq, st);
+  ntt_mul_launch<1>(EY, Y, EY, ntt_down_copies(logn) == 1 ? 0 : EY, Xhat, EX, O, EO, pl.lc, pl.lrp, logn, P, cx, Kq, st);
   ntt_strided(true, O, EO, logn, cx, st);
 }
 // the per-call context: host constants + this workspace's tables (built by the first launch of the call)
@@ -644,7 +646,7 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
         for (int v0 = va; v0 < vb; v0 += w.sq.Vc) {
           const int nv = (vb - v0 < w.sq.Vc) ? vb - v0 : w.sq.Vc;
           const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
-          ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY);
+          ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY, ntt_down_copies(logn));
           ntt_mul_down(w.sq_Y, EY, Xl, EX, w.sq_O, logn, P, cx, st);
           ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
                                                                       n2 + (size_t)v0 * T);
