@@ -102,15 +102,15 @@ k_sq_down_prepy(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __re
 __global__ void __launch_bounds__(256)
 k_sq_down_fin(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
               const uint64_t* __restrict__ O, int64_t EO, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ nxt) {
-  const int64_t n = (int64_t)1 << logn;
-  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t o = e >> logn, k = e & (n - 1);
+  const int64_t h = (int64_t)1 << (logn - 1);  // a tail is at most half a segment long (b <= a = n / 2): lanes over (o, k < n / 2)
+  for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < EO / 2; x += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t o = x >> (logn - 1), k = x & (h - 1);
     const int side = (int)(o & 1);
     const int64_t vt = o >> 1, v = (int64_t)((uint32_t)vt / (uint32_t)P);
     const SqTask t = tasks[vt - v * P];
     const int64_t len = side ? t.b : t.a, sh = side ? t.a : t.b;  // own length, sibling's length
     if (k >= len) continue;
-    const int64_t src = e - k + (k + sh - 1);
+    const int64_t src = (o << logn) + (k + sh - 1);
     const uint64_t r = ntt_crt(O[src], O[EO + src], O[2 * EO + src], cx, co, kp);
     const uint64_t* c = cur + v * ld + t.base;
     nxt[v * ld + t.base + (side ? t.a : 0) + k] = mod_add(r, c[k + sh], kp.p);
