@@ -463,12 +463,17 @@ k_inv_finish(const uint64_t* den, const uint64_t* __restrict__ nodes, int s0, in
       }
       atomicMin(&status[lo], (int32_t)(((uint32_t)(i - offs[lo]) << 8) | ZP_ST_DUPLICATE_NODE));
     }
-    if (APPLY) {
-      for (int b = 0; b < B; ++b) out[(int64_t)b * ldo + i] = mont_mul(num[(int64_t)b * ldn + i], d[x], kp);  // plain x Montgomery
-    } else {
-      out[i] = mont_mul(d[x], kp.c224, kp);
-    }
+    if (!APPLY) out[i] = mont_mul(d[x], kp.c224, kp);
   }
+  if (APPLY)
+    for (int b = 0; b < B; ++b) {  // row by row, the warp's eight loads of a row in flight together (num may be out)
+      uint64_t v[ZP_INV_N];
+#pragma unroll
+      for (int x = 0; x < ZP_INV_N; ++x) v[x] = (i0 + 32 * x < iend) ? __ldcs(num + (int64_t)b * ldn + i0 + 32 * x) : 0;
+#pragma unroll
+      for (int x = 0; x < ZP_INV_N; ++x)
+        if (i0 + 32 * x < iend) out[(int64_t)b * ldo + i0 + 32 * x] = mont_mul(v[x], d[x], kp);  // plain x Montgomery
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
