@@ -333,9 +333,10 @@ k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp,
 // transformed operands ever leaving the SM.  The factor 1/n rides on the product (Kq[j] = 2^128 / n mod q_j:
 // mont_mul(mont_mul(a, b), Kq) = a b / n).  A CTA = one chunk of one prime.
 //   MODE 0 (pairs): O segment o = A segment 2o * A segment 2o + 1               (up-tree; Newton; root); B != null (= A):
-//                   the complete transforms of the operands are written back over them (kept for MODE 1 later)
+//                   the complete transforms of the operands, times 2^64 / n (canonical), are written back over them --
+//                   kept for MODE 1 later, whose pointwise product is then ONE Montgomery product per word
 //   MODE 1 (down) : O segments 2 vt + side = A segment vt * B segment 2 (vt mod P) + 1 - side, side = 0, 1, where B holds
-//                   COMPLETE forward transforms (k_ntt_pass): tails x reversed siblings, the siblings' transforms are
+//                   the COMPLETE forward transforms times 2^64 / n that MODE 0 kept: tails x reversed siblings, the siblings' transforms are
 //                   shared by all the vectors of a level.  EA, EB, EO: words per prime of the three buffers; SA: the
 //                   distance between the primes' copies of A.
 ZP_DEV uint64_t ntt_canon4(uint64_t b, const ZpMod& q) {  // [0, 4q) -> [0, q)
@@ -399,7 +400,7 @@ k_ntt_mul(const uint64_t* A, int64_t EA, int64_t SA, const uint64_t* B, int64_t 
         const int e = T + TH * m;
         if (c0 + e < Edrv) {
           const uint32_t seg = seg0 + ((pos0 + e) >> logseg), pos = (pos0 + e) & segmask;
-          const_cast<uint64_t*>(A)[((int64_t)(2 * seg + which) << logseg) | pos] = sm[ntt_pad(e)];
+          const_cast<uint64_t*>(A)[((int64_t)(2 * seg + which) << logseg) | pos] = mont_mul(sm[ntt_pad(e)], Kq, q);  // x 2^64 / n
         }
       }
     }
@@ -429,7 +430,7 @@ k_ntt_mul(const uint64_t* A, int64_t EA, int64_t SA, const uint64_t* B, int64_t 
 #pragma unroll
       for (int m = 0; m < ZP_NTT_C / TH; ++m) {
         const int se = ntt_pad(T + TH * m);
-        sm[se] = mont_mul(mont_mul(smA[se], ntt_canon4(b[m], q), q), Kq, q);
+        sm[se] = mont_mul(smA[se], b[m], q);  // (the kept transform carries 2^64 / n and is canonical)
       }
     }
     __syncthreads();

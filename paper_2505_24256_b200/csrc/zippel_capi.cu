@@ -469,8 +469,8 @@ void ntt_mul_pairs(uint64_t* X, int64_t EX, uint64_t* O, int logn, const NttCtx&
 }
 // copies of Y that k_sq_down_prepy writes: one serves the three primes when the transform has no strided pass
 inline int ntt_down_copies(int logn) { return logn <= ZP_NTT_LOGC ? 1 : 3; }
-//   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds complete
-//   transforms (ntt_run); Y is overwritten by its strided passes
+//   down: O segments 2 vt + side = Y segment vt * Xhat segment 2 (vt mod P) + 1 - side (EO = 2 EY); Xhat holds the complete
+//   transforms times 2^64 / n that ntt_mul_pairs(keep) left; Y is overwritten by its strided passes
 void ntt_mul_down(uint64_t* Y, int64_t EY, const uint64_t* Xhat, int64_t EX, uint64_t* O, int logn, int64_t P, const NttCtx& cx,
                   cudaStream_t st) {
   const NttPlan pl = ntt_plan(logn);
