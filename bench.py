@@ -159,13 +159,15 @@ C_MONT = 18  # Montgomery product: 8 wide + 2 low
 def subq_units(t, B):
     """Algorithmic multiplier-pipe units of the sub-quadratic solve of ONE function of t terms with B right-hand sides,
     counted on the plan csrc/zippel_capi.cu:sq_solve executes: a length-n transform modulo one prime = (n/2) log2 n
-    butterflies of one Shoup product (16 units); a pointwise product = 2 Montgomery products per prime; Garner CRT +
-    reduction modulo p = 5 Montgomery products per coefficient; the leaves are the quadratic node solve with B + 1
+    butterflies of one Shoup product (16 units); a pointwise product = 2 Montgomery products per prime (1 in the
+    down-tree: the factor 1/n rides on the children's transforms, scaled once when the up-tree keeps them); Garner CRT
+    + reduction modulo p = 5 Montgomery products per coefficient; the leaves are the quadratic node solve with B + 1
     right-hand sides.  Returns (total, parts)."""
     from math import ceil, log2
 
     ntt = lambda n: 3 * (n / 2) * log2(n) * C_MM  # three primes
     pw = lambda n: 3 * n * 2 * C_MONT
+    pw1 = lambda n: 3 * n * C_MONT  # one Montgomery product per word and prime
     crt = lambda n: n * 5 * C_MONT
     V = B + 1
     nlev = max(0, ceil(log2(ceil(t / SQ_LEAF))))
@@ -179,8 +181,8 @@ def subq_units(t, B):
             base += 2 * a
         P = len(pairs)
         outs = sum(a + b for b in pairs)
-        up += P * (3 * ntt(n) + pw(n)) + crt(outs)
-        down += V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(outs))  # the children's transforms are kept from the up-tree
+        up += P * (3 * ntt(n) + pw(n) + 2 * pw1(n)) + crt(outs)  # both children's transforms are kept, times 2^64 / n
+        down += V * (P * (3 * ntt(n) + 2 * pw1(n)) + crt(outs))  # tail x the two kept transforms
     newton = sum(1.5 * k * k * C_MAC for k in (1 << i for i in range(10)))  # schoolbook base case to x^1024
     kk = SQ_KB
     while kk < t:
@@ -372,7 +374,7 @@ def run_leg(idx, K, W, F_override, want_e2e, rank, world, local, sample_clocks=T
     if subq:
         kernel = "sub-quadratic solve (csrc/subq.cuh): leaf trees, up-tree, Newton chain, tails down the tree (k_ntt_mul, k_ntt_pass, CRT), leaf k_node_solve, k_inv_finish"
         cost = ("W_alg of the sub-quadratic route (bench.py subq_units, DESIGN.md section 12): butterfly = one Shoup product = 16 units, "
-                "pointwise = 2 Montgomery products (36), CRT + reduction = 5 (90), leaves = quadratic node solve with B + 1 right-hand sides")
+                "pointwise = 2 Montgomery products (36; 1 in the down-tree, the kept transforms carry 1/n), CRT + reduction = 5 (90), leaves = quadratic node solve with B + 1 right-hand sides")
     elif idx == 5 or (B == 1 and int(min(ts)) >= 4096):
         kernel, cost = "k_corr_w + k_node_eval2", "per (node, stage) 8 (2 + 1/2) units: two evaluations by deferred MACs + the correlation"
     else:

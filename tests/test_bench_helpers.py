@@ -47,10 +47,11 @@ def test_work_model_of_the_subquadratic_route():
     crt = lambda n: n * 90
     tot, parts = b.subq_units(4096, 1)  # three levels above the 512-node leaves: (pairs, n) = (4, 1024), (2, 2048), (1, 4096)
     levels = ((4, 1024), (2, 2048), (1, 4096))
-    up = sum(P * (3 * ntt(n) + pw(n)) + crt(4096) for P, n in levels)
+    pw1 = lambda n: 3 * n * 18  # one Montgomery product per word: scaling a kept transform; the down-tree's pointwise product
+    up = sum(P * (3 * ntt(n) + pw(n) + 2 * pw1(n)) + crt(4096) for P, n in levels)
     assert parts["up_tree"] == up
     V = 2
-    down = sum(V * (P * (3 * ntt(n) + 2 * pw(n)) + crt(4096)) for P, n in levels)  # the siblings' transforms are kept
+    down = sum(V * (P * (3 * ntt(n) + 2 * pw1(n)) + crt(4096)) for P, n in levels)  # the siblings' transforms are kept
     assert parts["down_tree"] == down
     assert parts["leaves"] == 8 * 512 * 512 * (4 + 16 + 2 * 8)
     t19, _ = b.subq_units(1 << 19, 1)
