@@ -1048,10 +1048,12 @@ int zippel_lift_step_host(const uint16_t* h_exps, const int64_t* h_offsets, int 
   Pipe* P = get_pipe();
   if (!P) return ZP_ERR_CUDA;
   // chunks of whole functions; small batches go in one piece.  The first and the last chunks are small because the
-  // first H2D copy and the last D2H copy cannot overlap with anything; sizes grow by about 4x (copy time is about a
-  // quarter of kernel time on C2) so that every copy hides behind the previous chunk's kernels.  Measured on C2:
-  // 18 chunks 61.2 ms, 11 chunks 60.1, 7 chunks 59.8, 6 chunks 59.2 per step (device-resident 56.2).
-  static const int kCut64[] = {0, 2, 10, 32, 54, 62, 64};
+  // first H2D copy and the last D2H copy cannot overlap with anything; the sizes grow and shrink by about 4x, so that
+  // the input of chunk c + 1 has arrived (55 GB/s: the whole input of C2 takes 13 ms) when the kernels of chunk c end
+  // and the output of chunk c is out when the kernels of chunk c + 1 end.  A chunk costs about 0.65 ms of its own
+  // (partial waves of the large kernels, some fifty dependent launches of the route), so fewer is better.  Measured on C2
+  // (device-resident 43.9 ms): 7 chunks {2,5,13,24,13,5,2}/64 49.4 ms, 6 chunks {2,8,22,22,8,2}/64 48.7, 5 chunks 48.5.
+  static const int kCut64[] = {0, 3, 16, 48, 61, 64};
   const size_t bytes = 8 * (size_t)T_tot * B;
   int nch = 1;
   int cut[ZP_PIPE_MAX_CHUNKS + 1];
