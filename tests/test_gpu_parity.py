@@ -270,9 +270,12 @@ def test_newton_small_prime_inplace_and_duplicate(zp, ref):
 
 # ------------------------------------------------------------------------------ (a6) power sums
 @pytest.mark.parametrize("s0", [0, 1])
-def test_power_sums_parity(zp, ref, s0):
-    p = P63
-    nodes, offsets, coef = random_solve_case(13, [1, 130, 257, 700], 3, p)
+@pytest.mark.parametrize("ts,p", [([1, 130, 257, 700], P63),
+                                  # around k_power_sums's blocks: 512 probes per CTA, 64 nodes per tile, 32 probes per lane group
+                                  ([511, 512, 513, 64, 65, 31, 33, 1024, 1537, 2], P63),
+                                  ([100, 600, 3], (1 << 61) - 1), ([40, 529], 65537)])
+def test_power_sums_parity(zp, ref, s0, ts, p):
+    nodes, offsets, coef = random_solve_case(13, ts, 3, p)
     want = ref.power_sums(nodes, offsets, coef, p, s0)
     got = zp.zippel_power_sums(zp.to_dev(nodes), offsets, zp.to_dev(coef), p, s0)
     assert (zp.to_host(got) == want).all()
