@@ -62,6 +62,10 @@ ZP_DEV uint64_t mod_sub(uint64_t a, uint64_t b, uint64_t p) {
 ZP_DEV uint64_t mod_neg(uint64_t a, uint64_t p) { return a ? p - a : 0; }
 // input residue -> canonical.  Callers pass canonical residues (reading G22), so the 64-bit division (about a
 // hundred instructions) sits behind a branch that is practically never taken.
+// Programmatic dependent launch (sm_90+): a kernel launched with the "programmatic stream serialization" attribute may
+// become resident while its predecessor in the stream drains; it must not touch global memory before this wait, which
+// returns when the predecessor grid has completed and its writes are visible.  A no-op under a plain launch.
+ZP_DEV void zp_grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 ZP_DEV uint64_t zp_canon(uint64_t x, uint64_t p) { return x < p ? x : x % p; }
 
 // Montgomery product (54 pipe cycles against 62.5 and 59.7 for the two 32-bit-round forms kept in ubench.cuh,

@@ -238,6 +238,7 @@ ZP_DEV void ntt_tile(uint64_t* sm, int hi, int lo, const ulonglong2* __restrict_
 template <bool INV, int TH>
 __global__ void __launch_bounds__(TH, 1024 / TH)
 k_ntt_pass(uint64_t* __restrict__ buf, int64_t E, int logn, int logR, int logRp, NttCtx cx) {
+  zp_grid_dep_wait();
   __shared__ uint64_t sm[ZP_NTT_SMEM];
   const int jp = blockIdx.y;
   const ZpMod q = cx.q[jp];
@@ -347,6 +348,7 @@ template <int MODE, int TH>
 __global__ void __launch_bounds__(TH, 768 / TH)
 k_ntt_mul(const uint64_t* A, int64_t EA, int64_t SA, const uint64_t* B, int64_t EB, uint64_t* __restrict__ O,
           int64_t EO, int logn, int logRp, int logseg, int64_t P, NttCtx cx, uint64_t Kq0, uint64_t Kq1, uint64_t Kq2) {
+  zp_grid_dep_wait();
   extern __shared__ __align__(16) uint64_t ntt_mul_smem[];  // 2 x 32 KB (dynamic: above the 48 KB static limit)
   uint64_t *sm = ntt_mul_smem, *smA = ntt_mul_smem + ZP_NTT_SMEM;  // the working tile; the first operand's transform
   const int jp = blockIdx.y;

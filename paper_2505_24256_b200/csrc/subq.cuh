@@ -34,6 +34,7 @@ struct SqTask {
 __global__ void __launch_bounds__(256)
 k_sq_up_fin(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn,
             const uint64_t* __restrict__ O, int64_t EO, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ nxt) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t c = e & (n - 1);
@@ -53,6 +54,7 @@ k_sq_up_fin(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, 
 __global__ void __launch_bounds__(256)
 k_sq_copy(const SqTask* __restrict__ tasks, int ntasks, const uint64_t* __restrict__ src, uint64_t* __restrict__ dst, int V,
           int64_t ld) {
+  zp_grid_dep_wait();
   for (int x = blockIdx.y; x < ntasks * V; x += gridDim.y) {
     const SqTask t = tasks[x % ntasks];
     const int64_t o = (int64_t)(x / ntasks) * ld + t.base;
@@ -65,6 +67,7 @@ k_sq_copy(const SqTask* __restrict__ tasks, int ntasks, const uint64_t* __restri
 __global__ void __launch_bounds__(256)
 k_sq_down_prepx(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tasks, int64_t P, int logn,
                 uint64_t* __restrict__ X, int64_t EX) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1);
@@ -84,6 +87,7 @@ k_sq_down_prepx(const uint64_t* __restrict__ lev, const SqTask* __restrict__ tas
 __global__ void __launch_bounds__(256)
 k_sq_down_prepy(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
                 uint64_t* __restrict__ Y, int64_t EY, int copies) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EY; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1);
@@ -102,6 +106,7 @@ k_sq_down_prepy(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __re
 __global__ void __launch_bounds__(256)
 k_sq_down_fin(const uint64_t* __restrict__ cur, int64_t ld, const SqTask* __restrict__ tasks, int64_t P, int logn,
               const uint64_t* __restrict__ O, int64_t EO, NttCtx cx, CrtOut co, ZpMod kp, uint64_t* __restrict__ nxt) {
+  zp_grid_dep_wait();
   const int64_t h = (int64_t)1 << (logn - 1);  // a tail is at most half a segment long (b <= a = n / 2): lanes over (o, k < n / 2)
   for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < EO / 2; x += (int64_t)gridDim.x * blockDim.x) {
     const int64_t o = x >> (logn - 1), k = x & (h - 1);
@@ -168,6 +173,7 @@ k_sq_inv_base(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, Zp
 __global__ void __launch_bounds__(256)
 k_sq_newton_prep1(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, int64_t nact, const uint64_t* __restrict__ alphas,
                   int logn, ZpMod kp, uint64_t* __restrict__ X) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn, EX = 2 * nact * n, k = n >> 1;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1);
@@ -183,6 +189,7 @@ k_sq_newton_prep1(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns
 __global__ void __launch_bounds__(256)
 k_sq_newton_mid(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t nact, int logn, NttCtx cx, CrtOut co,
                 ZpMod kp, const uint64_t* __restrict__ alphas, uint64_t* __restrict__ X) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn, k = n >> 1, EX = 2 * nact * n, EO = nact * n;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1), s = seg >> 1;
@@ -200,6 +207,7 @@ k_sq_newton_mid(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, in
 __global__ void __launch_bounds__(256)
 k_sq_newton_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t nact, int logn, NttCtx cx, CrtOut co,
                 ZpMod kp, uint64_t* __restrict__ alphas) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn, k = n >> 1, EO = nact * n;
   for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < nact * k; x += (int64_t)gridDim.x * blockDim.x) {
     const int64_t s = x >> (logn - 1), i = x - s * k, o = s * n + i;
@@ -211,6 +219,7 @@ k_sq_newton_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, in
 __global__ void __launch_bounds__(256)
 k_sq_root_prep(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, int64_t ng, const uint64_t* __restrict__ alphas,
                int logn, ZpMod kp, uint64_t* __restrict__ X) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn, EX = 2 * ng * n;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EX; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t seg = e >> logn, i = e & (n - 1);
@@ -228,6 +237,7 @@ k_sq_root_prep(const uint64_t* __restrict__ top, const SqFn* __restrict__ fns, i
 __global__ void __launch_bounds__(256)
 k_sq_root_fin(const uint64_t* __restrict__ O, const SqFn* __restrict__ fns, int64_t ng, int logn, NttCtx cx, CrtOut co, ZpMod kp,
               uint64_t* __restrict__ tails) {
+  zp_grid_dep_wait();
   const int64_t n = (int64_t)1 << logn, EO = ng * n;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < EO; e += (int64_t)gridDim.x * blockDim.x) {
     const int64_t s = e >> logn, i = e & (n - 1);

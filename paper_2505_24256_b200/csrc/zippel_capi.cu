@@ -392,6 +392,25 @@ inline unsigned sq_blocks(int64_t n, int per = 256) {
   const int64_t cap = (int64_t)sm_count() * 64;
   return (unsigned)(b < 1 ? 1 : (b > cap ? cap : b));
 }
+// The route is a chain of some two hundred dependent launches, many of them a few microseconds long: they are launched
+// with programmatic stream serialization, so that a kernel becomes resident while its predecessor drains (every kernel
+// launched this way starts with zp_grid_dep_wait(), modarith.cuh: the order of the memory operations is that of a plain
+// launch).  g_launches counts them like the others.
+template <typename... P, typename... A>
+inline void launch_dep(void (*kern)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  ++g_launches;
+  cudaLaunchKernelEx(&cfg, kern, static_cast<P>(args)...);
+}
 // Pass plan of a transform of length 2^logn (ntt.cuh): up to two strided passes of lr1 and lr2 stages, then the chunk
 // stages (lc <= 12 of them) on rows that are twisted by their parent's row index (lrp stages above them).
 struct NttPlan {
@@ -414,9 +433,9 @@ inline bool ntt_small_grid(int64_t E) { return 3 * ((E + ZP_NTT_C - 1) / ZP_NTT_
 template <bool INV>
 void ntt_pass_launch(uint64_t* buf, int64_t E, int logn, int logR, int logRp, const NttCtx& cx, cudaStream_t st) {
   if (ntt_small_grid(E))
-    ++g_launches, k_ntt_pass<INV, ZP_NTT_THREADS_SMALL><<<ntt_grid(E), ZP_NTT_THREADS_SMALL, 0, st>>>(buf, E, logn, logR, logRp, cx);
+    launch_dep(k_ntt_pass<INV, ZP_NTT_THREADS_SMALL>, ntt_grid(E), ZP_NTT_THREADS_SMALL, 0, st, buf, E, logn, logR, logRp, cx);
   else
-    ++g_launches, k_ntt_pass<INV, ZP_NTT_THREADS><<<ntt_grid(E), ZP_NTT_THREADS, 0, st>>>(buf, E, logn, logR, logRp, cx);
+    launch_dep(k_ntt_pass<INV, ZP_NTT_THREADS>, ntt_grid(E), ZP_NTT_THREADS, 0, st, buf, E, logn, logR, logRp, cx);
 }
 // the strided passes alone, on every segment of `buf` ([3][E] words, segments of 2^logn), in place
 void ntt_strided(bool inverse, uint64_t* buf, int64_t E, int logn, const NttCtx& cx, cudaStream_t st) {
@@ -446,11 +465,11 @@ void ntt_mul_launch(int64_t Edrv, const uint64_t* A, int64_t EA, int64_t SA, con
   const size_t smem = 16 * ZP_NTT_SMEM;
   if (ntt_small_grid(Edrv)) {
     cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL><<<ntt_grid(Edrv), ZP_NTT_THREADS_SMALL, smem, st>>>(A, EA, SA, B, EB, O, EO, lc, lrp, logn, P,
+    launch_dep(k_ntt_mul<MODE, ZP_NTT_THREADS_SMALL>, ntt_grid(Edrv), ZP_NTT_THREADS_SMALL, smem, st, A, EA, SA, B, EB, O, EO, lc, lrp, logn, P,
                                                                                                        cx, Kq[0], Kq[1], Kq[2]);
   } else {
     cudaFuncSetAttribute(k_ntt_mul<MODE, ZP_NTT_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    ++g_launches, k_ntt_mul<MODE, ZP_NTT_THREADS><<<ntt_grid(Edrv), ZP_NTT_THREADS, smem, st>>>(A, EA, SA, B, EB, O, EO, lc, lrp, logn, P, cx, Kq[0],
+    launch_dep(k_ntt_mul<MODE, ZP_NTT_THREADS>, ntt_grid(Edrv), ZP_NTT_THREADS, smem, st, A, EA, SA, B, EB, O, EO, lc, lrp, logn, P, cx, Kq[0],
                                                                                            Kq[1], Kq[2]);
   }
 }
@@ -572,12 +591,12 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
         // the REVERSED children are multiplied (rev(A') rev(B') = rev(A' B')): their transforms are what the down-tree
         // correlates the tails with, and they are kept for it
         uint64_t* Xl = w.sq_Xl + 3 * xoff[l];
-        ++g_launches, k_sq_down_prepx<<<sq_blocks(EX), 256, 0, st>>>(lev(l), tp, P, logn, Xl, EX);
+        launch_dep(k_sq_down_prepx, sq_blocks(EX), 256, 0, st, lev(l), tp, P, logn, Xl, EX);
         ntt_mul_pairs(Xl, EX, w.sq_O, logn, cx, st, true);
-        ++g_launches, k_sq_up_fin<<<sq_blocks(EO), 256, 0, st>>>(lev(l), tp, P, logn, w.sq_O, EO, cx, co1, k, lev(l + 1));
+        launch_dep(k_sq_up_fin, sq_blocks(EO), 256, 0, st, lev(l), tp, P, logn, w.sq_O, EO, cx, co1, k, lev(l + 1));
       }
       const int nc = (int)(copy1[l] - copy0[l]);
-      if (nc) ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(nc < 1024 ? nc : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, lev(l), lev(l + 1), 1, 0);
+      if (nc) launch_dep(k_sq_copy, dim3(64, (unsigned)(nc < 1024 ? nc : 1024)), 256, 0, st, w.sq_tasks + copy0[l], nc, lev(l), lev(l + 1), 1, 0);
     }
   }
   SQ_DUMP(1, lev(r.nlev), T);
@@ -614,11 +633,11 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       while (nact < Fr && fns[nact].t > kk) ++nact;
       const int logn = ceil_log2(2 * kk);
       const int64_t n = 2 * kk, EX = 2 * nact * n;
-      ++g_launches, k_sq_newton_prep1<<<sq_blocks(EX), 256, 0, sn>>>(top, w.sq_fns, nact, w.sq_alpha, logn, k, w.sq_X);
+      launch_dep(k_sq_newton_prep1, sq_blocks(EX), 256, 0, sn, top, w.sq_fns, nact, w.sq_alpha, logn, k, w.sq_X);
       ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
-      ++g_launches, k_sq_newton_mid<<<sq_blocks(EX), 256, 0, sn>>>(w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha, w.sq_X);
+      launch_dep(k_sq_newton_mid, sq_blocks(EX), 256, 0, sn, w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha, w.sq_X);
       ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
-      ++g_launches, k_sq_newton_fin<<<sq_blocks(nact * kk), 256, 0, sn>>>(w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha);
+      launch_dep(k_sq_newton_fin, sq_blocks(nact * kk), 256, 0, sn, w.sq_O2, w.sq_fns, nact, logn, cx, co1, k, w.sq_alpha);
     }
     dump_alpha_off = fns[0].aoff;
     dump_alpha_t = fns[0].t;
@@ -627,9 +646,9 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
       int g1 = g0;
       while (g1 < Fr && ceil_log2(2 * fns[g1].t) == logn) ++g1;
       const int64_t n = (int64_t)1 << logn, ng = g1 - g0, EX = 2 * ng * n;
-      ++g_launches, k_sq_root_prep<<<sq_blocks(EX), 256, 0, sn>>>(top, w.sq_fns + g0, ng, w.sq_alpha, logn, k, w.sq_X);
+      launch_dep(k_sq_root_prep, sq_blocks(EX), 256, 0, sn, top, w.sq_fns + g0, ng, w.sq_alpha, logn, k, w.sq_X);
       ntt_mul_pairs(w.sq_X, EX, w.sq_O2, logn, cx, sn);
-      ++g_launches, k_sq_root_fin<<<sq_blocks(ng * n), 256, 0, sn>>>(w.sq_O2, w.sq_fns + g0, ng, logn, cx, co2, k, cur + (size_t)B * T);
+      launch_dep(k_sq_root_fin, sq_blocks(ng * n), 256, 0, sn, w.sq_O2, w.sq_fns + g0, ng, logn, cx, co2, k, cur + (size_t)B * T);
       g0 = g1;
     }
   }
@@ -646,16 +665,16 @@ void sq_solve(const Ws& w, const NttCtx& cx, const int64_t* h_offs, const SqRun&
         for (int v0 = va; v0 < vb; v0 += w.sq.Vc) {
           const int nv = (vb - v0 < w.sq.Vc) ? vb - v0 : w.sq.Vc;
           const int64_t EY = (int64_t)nv * P * n, EO = 2 * EY;
-          ++g_launches, k_sq_down_prepy<<<sq_blocks(EY), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY, ntt_down_copies(logn));
+          launch_dep(k_sq_down_prepy, sq_blocks(EY), 256, 0, st, c + (size_t)v0 * T, T, tp, P, logn, w.sq_Y, EY, ntt_down_copies(logn));
           ntt_mul_down(w.sq_Y, EY, Xl, EX, w.sq_O, logn, P, cx, st);
-          ++g_launches, k_sq_down_fin<<<sq_blocks(EO), 256, 0, st>>>(c + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
+          launch_dep(k_sq_down_fin, sq_blocks(EO), 256, 0, st, c + (size_t)v0 * T, T, tp, P, logn, w.sq_O, EO, cx, co1, k,
                                                                       n2 + (size_t)v0 * T);
         }
       }
       const int nc = (int)(copy1[l] - copy0[l]);
       if (nc) {
         const int ny = nc * Vr;
-        ++g_launches, k_sq_copy<<<dim3(64, (unsigned)(ny < 1024 ? ny : 1024)), 256, 0, st>>>(w.sq_tasks + copy0[l], nc, c + (size_t)va * T,
+        launch_dep(k_sq_copy, dim3(64, (unsigned)(ny < 1024 ? ny : 1024)), 256, 0, st, w.sq_tasks + copy0[l], nc, c + (size_t)va * T,
                                                                                              n2 + (size_t)va * T, Vr, T);
       }
       uint64_t* tmp = c;
