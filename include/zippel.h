@@ -183,8 +183,8 @@ int zippel_extend_skeleton(const uint16_t* exps, const int64_t* h_offsets, int F
  * loads the library holds it until the process exits).  Same arguments without the workspace, same results bit for
  * bit.  The call allocates nothing: no cudaMalloc / cudaFree / allocating library routine; it enqueues one copy of
  * h_offsets (read before the call returns), one memset of the descriptors and two kernels on `stream`.
- *   Limit: 256-byte-rounded 8 (F + 1) bytes of offsets + 8 (ceil(T_tot / 2048) + 1) bytes of descriptors must fit
- *   ZP_STATIC_SCRATCH_BYTES (e.g. F = 4096 functions of 10^4 terms: 0.2 MB); beyond it the call enqueues nothing and
+ *   Limit: 256-byte-rounded 8 (F + 1) bytes of offsets + 8 (ceil(T_tot / 1024) + 1) bytes of descriptors must fit
+ *   ZP_STATIC_SCRATCH_BYTES (e.g. F = 4096 functions of 10^4 terms: 0.35 MB); beyond it the call enqueues nothing and
  *   returns ZP_ERR_SCRATCH_LIMIT (zippel_strerror names the limit).
  *   The array is ONE per device and every call uses it: the call clears what must start at zero (the descriptors), but
  *   two calls that overlap on the GPU (different streams, or threads) race on it -- order them, or give the others

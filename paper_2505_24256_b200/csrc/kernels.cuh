@@ -1165,7 +1165,7 @@ k_thiele(const ulonglong2* __restrict__ xd, const ulonglong2* __restrict__ xm, c
 // (f1) skeleton extension between two lifting steps: the pairs (term i,
 // degree d) with a non-zero monomial coefficient become the terms of the next skeleton, in the order i
 // ascending, d ascending.  An HBM-bound stream compaction in ONE pass over the coefficient matrix:
-//   a CTA takes the next block of 256 consecutive terms (a ticket, so that blocks start in index order), reads their
+//   a CTA takes the next block of ZP_K9_BLOCK consecutive terms (a ticket, so that blocks start in index order), reads their
 //   B coefficients (unit-stride rows), keeps a 64-bit mask of the non-zero degrees per term (B <= 64), scans the
 //   popcounts inside the block, obtains the number of rows emitted by all earlier blocks by a decoupled look-back
 //   over the per-block descriptors {flag, count} (flag 1: the block's own count, 2: the inclusive prefix; one 64-bit
@@ -1177,9 +1177,10 @@ k_thiele(const ulonglong2* __restrict__ xd, const ulonglong2* __restrict__ xm, c
 // that emit more rows than that write them directly.
 // ------------------------------------------------------------------------------------------------
 #define ZP_K9_THREADS 256
-#define ZP_K9_ITEMS 8  // consecutive terms per lane: 64 contiguous bytes of every coefficient row
+#define ZP_K9_ITEMS 4  // consecutive terms per lane: 32 contiguous bytes of every coefficient row (with 8 the kernel needs 80
+                       // registers and three CTAs fill an SM; with 4, five do: 0.262 -> 0.238 ms on C2's output; with 2: 0.278)
 #define ZP_K9_BLOCK (ZP_K9_THREADS * ZP_K9_ITEMS)
-__global__ void __launch_bounds__(ZP_K9_THREADS, 3)
+__global__ void __launch_bounds__(ZP_K9_THREADS, 5)
 k_ext_fused(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restrict__ coefs, int64_t T_tot, int B,
             const int64_t* __restrict__ offsets, int F, ZpMod k, unsigned long long* __restrict__ desc, int64_t nb,
             uint16_t* __restrict__ new_exps, uint64_t* __restrict__ new_coefs, int64_t cap, int64_t* __restrict__ new_offsets,
@@ -1191,13 +1192,13 @@ k_ext_fused(const uint16_t* __restrict__ exps, int nv, const uint64_t* __restric
   if (threadIdx.x == 0) s_bid = (int)atomicAdd(desc + nb, 1ull);
   __syncthreads();
   const int64_t bid = s_bid;
-  const int64_t i0 = bid * ZP_K9_BLOCK, i1 = i0 + (int64_t)threadIdx.x * ZP_K9_ITEMS;  // this lane: terms i1 .. i1 + 7
+  const int64_t i0 = bid * ZP_K9_BLOCK, i1 = i0 + (int64_t)threadIdx.x * ZP_K9_ITEMS;  // this lane: terms i1 .. i1 + ITEMS - 1
   // ---- the one pass over the coefficients: masks of the non-zero degrees of the lane's terms
   uint64_t m[ZP_K9_ITEMS], c1[ZP_K9_ITEMS];  // c1: the term's first non-zero coefficient (no second read for it)
 #pragma unroll
   for (int x = 0; x < ZP_K9_ITEMS; ++x) m[x] = c1[x] = 0;
-  if (i1 + ZP_K9_ITEMS <= T_tot && (T_tot & 1) == 0) {  // whole group, rows 16-byte aligned: four 16-byte loads per row
-#pragma unroll 3
+  if (i1 + ZP_K9_ITEMS <= T_tot && (T_tot & 1) == 0) {  // whole group, rows 16-byte aligned: two 16-byte loads per row
+#pragma unroll 4
     for (int d = 0; d < B; ++d) {
       const ulonglong2* src = reinterpret_cast<const ulonglong2*>(coefs + (int64_t)d * T_tot + i1);
       ulonglong2 v[ZP_K9_ITEMS / 2];

@@ -57,9 +57,9 @@ def _same(zp, w, coefs, got, cap):
 
 
 def test_static_scratch_entry_matches_the_workspace_path_on_consecutive_calls(zp):
-    # 41 blocks of 2048 terms, ragged functions, vanished terms and a function of degree < B - 1
+    # 82 blocks of 1024 terms, ragged functions, vanished terms and a function of degree < B - 1
     big = _batch(131, [30000, 1, 2049, 2048, 7, 25000, 26000], 7, 3, [(slice(None), 5), (slice(4, None), slice(30001, 32050))])
-    # 2 blocks: its blocks take the tickets 0, 1 and look back at descriptors the first call left set
+    # 3 blocks: its blocks take the tickets 0 .. 2 and look back at descriptors the first call left set
     small = _batch(132, [2000, 900, 3], 5, 3, [(slice(None), 2001)])
     cap_big, cap_small = big[1].size, small[1].size
     _same(zp, *big, _static(zp, *big, cap_big), cap_big)
@@ -108,7 +108,7 @@ def test_static_scratch_limit_is_a_clear_error(zp):
     torch.cuda.synchronize()
     assert zp.zippel_launch_count() == n0 and int(outs[1][0]) == -7
     # just inside the limit the same shape goes through
-    F = (lim - 256 - 8 * 2) // 8 - 64
+    F = (lim - 256 - 8 * 2) * 1024 // (8 * 1025) - 64  # 8 (F + 1) bytes of offsets + 8 (F / 1024 + 1) of descriptors
     offsets = np.arange(F + 1, dtype=np.int64)
     ne, nc, no, degs = outs[0][:F], outs[1][:F], outs[2][:F + 1], outs[3][:F]
     zp.zippel_extend_skeleton_static(exps[:F], offsets, coefs[:, :F].contiguous(), wl.P63, ne, nc, no, degs)
