@@ -18,10 +18,55 @@
 #define ZP_SMALL_MAXG 3  // groups of lanes that share the right-hand sides of a function; one more group builds tables
 #define ZP_SMALL_MAXB 25  // Newton's steps per level and lane: (B - 1) / LPC <= ZP_SMALL_OPS (LPC = 4 from B = 9 on, else 2)
 #define ZP_SMALL_OPS 6
+#define ZP_SMALL_LB 16   // Newton as a matrix (below): B <= 16 samples and t <= 64 terms
+#define ZP_SMALL_LS 17   // row stride of that matrix in shared memory (odd: the four rows a warp reads lie in different banks)
 
 struct SmallOffs {
   int64_t o[ZP_SMALL_MAXF + 1];
 };
+
+// Newton's recurrence in x_k (and the expansion to monomials, basis = 1) on ONE column of B plain values, shared by LPC
+// = 2 or 4 neighbouring lanes of a warp (sub = this lane's place among them; every lane of the warp calls, `on` says
+// whether the column exists): element j of the column is col[j * stride].  The steps of one level (or of one pass of
+// the expansion) read the previous level only: a lane loads the operands of its (at most ZP_SMALL_OPS) steps, the warp
+// meets, the lane multiplies and stores, the warp meets again -- the latency of one Montgomery product per level.
+ZP_DEV void small_newton_column(uint64_t* col, int stride, int LPC, int sub, bool on, int B, int basis, const uint64_t* sInv,
+                                const uint64_t* sC, const ZpMod& k) {
+  const uint64_t p = k.p;
+  const int D = B - 1;
+  for (int l = 1; l <= D; ++l) {  // level l: c_j <- (c_j - c_{j-1}) / (x_j - x_{j-l}),  j = D .. l
+    uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
+#pragma unroll
+    for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+      const int j = D - sub - LPC * x;
+      if (on && j >= l) a[x] = col[j * stride], bb[x] = col[(j - 1) * stride];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+      const int j = D - sub - LPC * x;
+      if (on && j >= l) col[j * stride] = mont_mul(mod_sub(a[x], bb[x], p), sInv[j * B + (j - l)], k);
+    }
+    __syncwarp();
+  }
+  if (basis == 1)
+    for (int j = D - 1; j >= 0; --j) {  // pass j: a_x <- a_x - c_j a_{x+1},  x = j .. D - 1
+      const uint64_t cj = sC[j];
+      uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
+#pragma unroll
+      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+        const int e = j + sub + LPC * x;
+        if (on && e < D) a[x] = col[e * stride], bb[x] = col[(e + 1) * stride];
+      }
+      __syncwarp();
+#pragma unroll
+      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
+        const int e = j + sub + LPC * x;
+        if (on && e < D) col[e * stride] = mod_sub(a[x], mont_mul(bb[x], cj, k), p);
+      }
+      __syncwarp();
+    }
+}
 
 // CTA = (G + 1) groups of MAXT lanes.  Lane i of group g < G owns node i and the right-hand sides [g per, (g + 1) per):
 // every group runs the quotient chain of its node itself (one modular multiply-add per stage; the chain is the
@@ -38,6 +83,7 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
   __shared__ uint64_t sC[64];                      // c_j~
   __shared__ ulonglong2 sMt[ZP_SMALL_MAXT];        // {M_l, its Shoup companion}, l < t (plain residues)
   __shared__ uint64_t sDinv[ZP_SMALL_MAXT];        // (1 / (Q_i(m_i) [m_i]))~
+  __shared__ uint64_t sL[ZP_SMALL_LB * ZP_SMALL_LS];  // Newton's matrix L[r][e] (plain) at sL[r LS + e]
   __shared__ int32_t s_solve, s_newton;
   extern __shared__ __align__(16) uint64_t cols[];  // [B x MAXT]: column c_{.,i} at cols[b MAXT + i]; then sv
   constexpr int S = ZP_SMALL_MAXT;
@@ -153,50 +199,46 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
       sDinv[i] = mont_inv(dd, k);  // (1 / (d [m]))~
     }
   }
-  __syncthreads();  // the columns, sDinv, sInv, sC, s_newton are complete
-  // ---- (a5) Newton in x_k on the columns (shared memory), then the columns go out.  The steps of one level (or of one
-  // pass of the expansion) read the previous level only, so they are shared out among LPC = 2 or 4 neighbouring lanes
-  // of a warp per column (all the CTA's lanes work: 128 (G + 1) >= 128 LPC): a lane loads the operands of its (at most
-  // ZP_SMALL_OPS) steps, the warp meets, the lane multiplies and stores, the warp meets again.  The latency of one
-  // Montgomery product per level instead of that of a quarter of the level's products one after another.
-  {
+  // Newton's recurrence is linear in a column: out = L col with the B x B matrix L = Newton(identity), which depends on
+  // the samples only.  Where the table group has idle warps (t <= 64: its lanes i >= 64) and the matrix is small
+  // (B <= 16) they compute L beside the solve, four lanes per column of the identity, and the columns of the solve
+  // then take one deferred dot product per output instead of 2 (B - 1) dependent levels.
+  const bool use_L = B <= ZP_SMALL_LB && t <= 64;
+  if (use_L && g == G && i >= 64) {  // (whole warps: i = 32 q + lane)
+    const int ce = (i - 64) >> 2, sub = i & 3;
+    const bool on = ce < B;
+    for (int rr = sub; rr < B; rr += 4)
+      if (on) sL[rr * ZP_SMALL_LS + ce] = (rr == ce) ? 1 % p : 0;
+    __syncwarp();
+    small_newton_column(sL + (on ? ce : 0), ZP_SMALL_LS, 4, sub, on, B, basis, sInv, sC, k);
+  }
+  __syncthreads();  // the columns, sDinv, sInv, sC, s_newton (and L) are complete
+  // ---- (a5) Newton in x_k on the columns (shared memory), then the columns go out
+  if (use_L) {  // out_r = sum_e L[r][e] col[e]: four lanes per column, rows r = sub (mod 4); plain x plain sums (c224)
+    const int ci = threadIdx.x >> 2, sub = threadIdx.x & 3;
+    const bool on = ci < t;  // 32 (G + 1) >= 64 >= t columns
+    uint64_t v[ZP_SMALL_LB];
+#pragma unroll
+    for (int e = 0; e < ZP_SMALL_LB; ++e) v[e] = (on && e < B) ? cols[e * S + ci] : 0;
+    __syncwarp();  // (the four lanes of a column have read it before any of them writes)
+    Acc acc[ZP_SMALL_LB / 4];
+#pragma unroll
+    for (int x = 0; x < ZP_SMALL_LB / 4; ++x) acc_zero(acc[x]);
+#pragma unroll
+    for (int e = 0; e < ZP_SMALL_LB; ++e)
+      if (e < B) {  // (uniform)
+#pragma unroll
+        for (int x = 0; x < ZP_SMALL_LB / 4; ++x)
+          if (sub + 4 * x < B) acc_mac(acc[x], sL[(sub + 4 * x) * ZP_SMALL_LS + e], v[e]);
+      }
+#pragma unroll
+    for (int x = 0; x < ZP_SMALL_LB / 4; ++x)
+      if (on && sub + 4 * x < B) cols[(sub + 4 * x) * S + ci] = mont_mul(acc_redc160(acc[x], k), k.c224, k);
+  } else {  // the recurrence itself, shared among LPC lanes per column (all the CTA's lanes work: 128 (G + 1) >= 128 LPC)
     const int LPC = (G + 1 >= 4) ? 4 : 2;  // G >= 1
     const int ci = threadIdx.x / LPC, sub = threadIdx.x % LPC;
     const bool on = ci < t;
-    uint64_t* col = cols + (on ? ci : 0);
-    const int D = B - 1;
-    for (int l = 1; l <= D; ++l) {  // level l: c_j <- (c_j - c_{j-1}) / (x_j - x_{j-l}),  j = D .. l
-      uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
-#pragma unroll
-      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
-        const int j = D - sub - LPC * x;
-        if (on && j >= l) a[x] = col[j * S], bb[x] = col[(j - 1) * S];
-      }
-      __syncwarp();
-#pragma unroll
-      for (int x = 0; x < ZP_SMALL_OPS; ++x) {
-        const int j = D - sub - LPC * x;
-        if (on && j >= l) col[j * S] = mont_mul(mod_sub(a[x], bb[x], p), sInv[j * B + (j - l)], k);
-      }
-      __syncwarp();
-    }
-    if (basis == 1)
-      for (int j = D - 1; j >= 0; --j) {  // pass j: a_x <- a_x - c_j a_{x+1},  x = j .. D - 1
-        const uint64_t cj = sC[j];
-        uint64_t a[ZP_SMALL_OPS], bb[ZP_SMALL_OPS];
-#pragma unroll
-        for (int x = 0; x < ZP_SMALL_OPS; ++x) {
-          const int e = j + sub + LPC * x;
-          if (on && e < D) a[x] = col[e * S], bb[x] = col[(e + 1) * S];
-        }
-        __syncwarp();
-#pragma unroll
-        for (int x = 0; x < ZP_SMALL_OPS; ++x) {
-          const int e = j + sub + LPC * x;
-          if (on && e < D) col[e * S] = mod_sub(a[x], mont_mul(bb[x], cj, k), p);
-        }
-        __syncwarp();
-      }
+    small_newton_column(cols + (on ? ci : 0), S, LPC, sub, on, B, basis, sInv, sC, k);
   }
   __syncthreads();
   for (int b = g; b < B; b += G + 1)
