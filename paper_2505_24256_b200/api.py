@@ -120,6 +120,15 @@ def _on(stream):
     return contextlib.nullcontext() if stream is None else torch.cuda.stream(stream)
 
 
+_NO_CTX = contextlib.nullcontext()
+
+
+def _on_if_allocating(stream, *buffers):
+    """_on(stream) when the binding has to allocate one of `buffers` (passed as None); nothing to enter when the caller
+    brought them all -- torch's stream context costs more host time than a small lifting step takes on the GPU."""
+    return _on(stream) if any(b is None for b in buffers) else _NO_CTX
+
+
 def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
     if t is None:
         return None
@@ -225,7 +234,7 @@ def zippel_lift_step(exps: torch.Tensor, offsets, anchors: torch.Tensor, samples
                      stream=None):
     """(a1)-(a5): one lifting step; returns (out [B, T_tot], status [F])."""
     _need_cuda()
-    with _on(stream):
+    with _on_if_allocating(stream, out, status, workspace):
         o = _offs(offsets)
         F, B = len(o) - 1, vals.shape[0]
         nv = exps.shape[1]
