@@ -87,6 +87,7 @@ k_lift_small(const uint16_t* __restrict__ exps, SmallOffs offs, int nv, const ui
   __shared__ int32_t s_solve, s_newton;
   extern __shared__ __align__(16) uint64_t cols[];  // [B x MAXT]: column c_{.,i} at cols[b MAXT + i]; then sv
   constexpr int S = ZP_SMALL_MAXT;
+  zp_grid_dep_wait();  // (launched with programmatic stream serialization: lift_small)
   const int f = blockIdx.x;
   const int64_t off = offs.o[f];
   const int t = (int)(offs.o[f + 1] - off);

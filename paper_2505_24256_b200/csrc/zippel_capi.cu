@@ -903,8 +903,9 @@ void lift_small(const int64_t* h_offs, int F, int64_t T_tot, int nv, const uint1
   const size_t smem = 2 * 8 * (size_t)B * ZP_SMALL_MAXT;  // the columns of Newton's recurrence and the function's values
   cudaFuncSetAttribute(k_lift_small, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 8 * ZP_MAX_B * ZP_SMALL_MAXT);
   const int G = small_groups(B);
-  ++g_launches, k_lift_small<<<F, ZP_SMALL_MAXT*(G + 1), smem, st>>>(exps, so, nv, anchors, samples, B, G, s0, vals, T_tot, k, basis, out,
-                                                                     nodes_out, status);
+  // (programmatic stream serialization: in a loop of small lifts the next launch becomes resident while this one drains)
+  launch_dep(k_lift_small, dim3((unsigned)F), dim3(ZP_SMALL_MAXT * (G + 1)), smem, st, exps, so, nv, anchors, samples, B, G, s0, vals,
+             T_tot, k, basis, out, nodes_out, status);
 }
 
 void lift_chunk(const Ws& w, const int64_t* h_offsets, int f0, int f1, int64_t T_tot, int nv, const uint16_t* exps,
